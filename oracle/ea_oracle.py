@@ -1,0 +1,185 @@
+"""ctypes loader for oracle/ea_oracle.c (the CPU oracle; test infrastructure only).
+
+Argument marshalling only: every step of the method is in ea_oracle.c, where
+each function cites the PAPER.md passage it follows.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from pathlib import Path
+
+import numpy as np
+
+_HERE = Path(__file__).resolve().parent
+_SRC = _HERE / "ea_oracle.c"
+_LIB = _HERE / "libea_oracle.so"
+_lib = None
+
+
+def build_oracle(force: bool = False) -> Path:
+    """Compile the oracle with gcc (plain C, -O2, no fast-math)."""
+    if force or not _LIB.exists() or _LIB.stat().st_mtime < _SRC.stat().st_mtime:
+        tmp = _LIB.with_suffix(f".so.tmp{os.getpid()}")
+        subprocess.check_call(
+            ["gcc", "-O2", "-std=c11", "-fPIC", "-shared", "-fno-fast-math", "-ffp-contract=off",
+             "-o", str(tmp), str(_SRC), "-lm"])
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is not None:
+        return _lib
+    build_oracle()
+    lib = C.CDLL(str(_LIB))
+    vp, i32, i64, u64 = C.c_void_p, C.c_int, C.c_int64, C.c_uint64
+    lib.eao_create.restype = vp
+    lib.eao_create.argtypes = [i32, i32, i32, vp, u64, i32]
+    lib.eao_destroy.argtypes = [vp]
+    lib.eao_set_check.argtypes = [vp, i32]
+    lib.eao_check_failures.restype = i64
+    lib.eao_check_failures.argtypes = [vp]
+    lib.eao_set_couplings.restype = i32
+    lib.eao_set_couplings.argtypes = [vp, vp]
+    lib.eao_set_spins.restype = i32
+    lib.eao_set_spins.argtypes = [vp, vp]
+    lib.eao_set_tables.argtypes = [vp, vp, vp]
+    lib.eao_get_tables.argtypes = [vp, vp, vp]
+    lib.eao_sweep.restype = i32
+    lib.eao_sweep.argtypes = [vp, i64, i32]
+    lib.eao_energy.argtypes = [vp, vp]
+    lib.eao_overlap.restype = i32
+    lib.eao_overlap.argtypes = [vp, vp, i32, vp]
+    lib.eao_get_spins.argtypes = [vp, vp]
+    lib.eao_get_spins_by_slot.argtypes = [vp, vp]
+    lib.eao_get_couplings.argtypes = [vp, vp]
+    lib.eao_get_perm.argtypes = [vp, vp, vp]
+    lib.eao_get_energy_by_slot.argtypes = [vp, vp]
+    lib.eao_get_counters.argtypes = [vp, vp, vp, vp]
+    lib.eao_energy_from_scratch.restype = C.c_int32
+    lib.eao_energy_from_scratch.argtypes = [vp, i32, i32]
+    lib.eao_n_sat.restype = i32
+    lib.eao_n_sat.argtypes = [vp, i32, i32, i32]
+    lib.eao_philox4x32_10.argtypes = [C.c_uint32] * 6 + [vp]
+    _lib = lib
+    return lib
+
+
+def philox4x32_10(c0, c1, c2, c3, k0, k1):
+    out = (C.c_uint32 * 4)()
+    _load().eao_philox4x32_10(c0, c1, c2, c3, k0, k1, out)
+    return tuple(int(v) for v in out)
+
+
+def _ptr(a: np.ndarray):
+    return a.ctypes.data_as(C.c_void_p)
+
+
+class Oracle:
+    """One EA problem on the CPU: L^3 sites, R realizations, n_temps replicas each."""
+
+    def __init__(self, L, n_temps, R, betas, seed, r0=0, check=False):
+        self.lib = _load()
+        self.L, self.nT, self.R, self.N = int(L), int(n_temps), int(R), int(L) ** 3
+        b = np.ascontiguousarray(betas, dtype=np.float64)
+        assert b.shape == (self.nT,)
+        self.h = self.lib.eao_create(self.L, self.nT, self.R, _ptr(b), int(seed), int(r0))
+        if not self.h:
+            raise ValueError("eao_create rejected the arguments")
+        if check:
+            self.lib.eao_set_check(self.h, 1)
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.lib.eao_destroy(self.h)
+            self.h = None
+
+    __del__ = close
+
+    def set_check(self, on=True):
+        self.lib.eao_set_check(self.h, int(on))
+
+    def check_failures(self) -> int:
+        return int(self.lib.eao_check_failures(self.h))
+
+    def set_couplings(self, J):
+        J = np.ascontiguousarray(J, dtype=np.int8)
+        assert J.shape == (self.R, 3, self.N)
+        return self.lib.eao_set_couplings(self.h, _ptr(J))
+
+    def set_spins(self, s):
+        s = np.ascontiguousarray(s, dtype=np.int8)
+        assert s.shape == (self.R, self.nT, self.N)
+        return self.lib.eao_set_spins(self.h, _ptr(s))
+
+    def tables(self):
+        acc = np.zeros((self.nT, 7), dtype=np.uint64)
+        swp = np.zeros((max(self.nT - 1, 1), 3 * self.N + 1), dtype=np.uint64)
+        self.lib.eao_get_tables(self.h, _ptr(acc), _ptr(swp))
+        return acc, swp[: self.nT - 1]
+
+    def set_tables(self, acc, swp):
+        acc = np.ascontiguousarray(acc, dtype=np.uint64)
+        swp = np.ascontiguousarray(swp, dtype=np.uint64)
+        assert acc.shape == (self.nT, 7) and swp.shape == (self.nT - 1, 3 * self.N + 1)
+        self.lib.eao_set_tables(self.h, _ptr(acc), _ptr(swp))
+
+    def sweep(self, n_sweeps, swap_interval):
+        rc = self.lib.eao_sweep(self.h, int(n_sweeps), int(swap_interval))
+        if rc != 0:
+            raise ValueError(f"eao_sweep -> {rc}")
+
+    def energy(self):
+        E = np.zeros((self.R, self.nT), dtype=np.int32)
+        self.lib.eao_energy(self.h, _ptr(E))
+        return E
+
+    def energy_by_slot(self):
+        E = np.zeros((self.R, self.nT), dtype=np.int32)
+        self.lib.eao_get_energy_by_slot(self.h, _ptr(E))
+        return E
+
+    def energy_from_scratch(self, r, k) -> int:
+        return int(self.lib.eao_energy_from_scratch(self.h, int(r), int(k)))
+
+    def n_sat(self, k, r, site) -> int:
+        return int(self.lib.eao_n_sat(self.h, int(k), int(r), int(site)))
+
+    def overlap(self, pairs):
+        pairs = np.ascontiguousarray(pairs, dtype=np.int32).reshape(-1, 2)
+        Q = np.zeros((len(pairs), self.nT), dtype=np.int32)
+        rc = self.lib.eao_overlap(self.h, _ptr(pairs), len(pairs), _ptr(Q))
+        if rc != 0:
+            raise ValueError("bad pair")
+        return Q
+
+    def spins(self):
+        s = np.zeros((self.R, self.nT, self.N), dtype=np.int8)
+        self.lib.eao_get_spins(self.h, _ptr(s))
+        return s
+
+    def spins_by_slot(self):
+        s = np.zeros((self.R, self.nT, self.N), dtype=np.int8)
+        self.lib.eao_get_spins_by_slot(self.h, _ptr(s))
+        return s
+
+    def couplings(self):
+        J = np.zeros((self.R, 3, self.N), dtype=np.int8)
+        self.lib.eao_get_couplings(self.h, _ptr(J))
+        return J
+
+    def perm(self):
+        tau = np.zeros((self.R, self.nT), dtype=np.int32)
+        sigma = np.zeros((self.R, self.nT), dtype=np.int32)
+        self.lib.eao_get_perm(self.h, _ptr(tau), _ptr(sigma))
+        return tau, sigma
+
+    def counters(self):
+        g, n = C.c_uint64(), C.c_uint64()
+        st = (C.c_int64 * 4)()
+        self.lib.eao_get_counters(self.h, C.byref(g), C.byref(n), st)
+        return {"sweeps": g.value, "swap_rounds": n.value, "attempts": st[0], "accepted": st[1],
+                "swap_attempts": st[2], "swap_accepted": st[3]}
