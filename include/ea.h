@@ -1,0 +1,138 @@
+/*
+ * ea.h -- C ABI of libea_b200.so: Metropolis sweeps + parallel tempering for the 3D +-J
+ * Edwards-Anderson spin glass on one NVIDIA B200 (sm_100a).
+ *
+ * Method: arXiv 1311.5582 (Fang et al.).  Citations are PAPER.md:<line> (+ section/equation);
+ * conventions that the paper leaves open are frozen in DESIGN.md section 2 ("R<n>").
+ *
+ * General rules
+ *   - Every pointer argument is a HOST pointer unless its name starts with dev_.
+ *   - The caller owns every input and output buffer; the library copies.  The library owns
+ *     the device state of a handle until ea_destroy (inside the caller's workspace if one
+ *     was given to ea_create_ex).
+ *   - Every call except ea_create* returns 0 (EA_OK) or a negative status.  On error the
+ *     simulation state is unchanged.  ea_last_error() gives a message.
+ *   - Work is enqueued on the handle's CUDA stream.  ea_sweep returns after enqueueing
+ *     (asynchronous); every call that fills a host buffer synchronizes the stream first.
+ *   - One handle is not thread-safe; different handles are independent.
+ *   - There is no CPU fallback: without a CUDA device ea_create* fails (NULL).
+ */
+#ifndef EA_B200_H
+#define EA_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ea_handle ea_handle;
+
+enum {
+    EA_OK = 0,
+    EA_ERR_INVALID_ARG = -1,
+    EA_ERR_ALLOC = -2,
+    EA_ERR_CUDA = -3,
+    EA_ERR_RANGE = -4,
+    EA_ERR_UNSUPPORTED = -5
+};
+
+/* Which sweep implementation ea_sweep uses (ea_set_kernel).  AUTO picks the fastest one
+ * that supports the lattice; all produce identical results. */
+enum {
+    EA_KERNEL_AUTO = 0,
+    EA_KERNEL_GENERIC = 1,   /* any even L: one launch per half-sweep, global memory        */
+    EA_KERNEL_RESIDENT = 2,  /* L in {8,16}: lattices resident in shared memory, one launch
+                                for all sweeps of the call, PT inside a thread-block cluster */
+    EA_KERNEL_TILED = 3      /* L = 32 (and 8,16): z-slab tiles streamed through shared memory */
+};
+
+/*
+ * Problem statement: periodic L^3 cubic lattice (L even, >= 2), n_realizations
+ * disorder realizations, n_temps temperature replicas of each, betas[n_temps] = inverse
+ * temperatures, finite, >= 0, monotone (either direction).  seed = Philox4x32-10 key.
+ * Couplings and spins are initialised from the seed, the temperature
+ * permutation is the identity, the sweep counter is 0.  Limits: n_temps <= 64
+ * (EA_ERR_UNSUPPORTED above).  Returns NULL on failure (see ea_last_error(NULL)).
+ */
+ea_handle *ea_create(int L, int n_temps, int n_realizations, const double *betas, uint64_t seed);
+
+/* Bytes of device workspace ea_create_ex needs for this shape (0 if the shape is invalid). */
+size_t ea_workspace_bytes(int L, int n_temps, int n_realizations);
+
+/*
+ * As ea_create, with: dev_workspace = caller-owned device memory of at least
+ * ea_workspace_bytes() bytes, 256-byte aligned (NULL: the library allocates);
+ * cuda_stream = a cudaStream_t (NULL: the legacy default stream);
+ * first_realization = global index of realization 0, a multiple of 32: a handle created with
+ * first_realization = 32*w0 reproduces words w0.. of a larger problem bit for bit
+ * (sharding by realization word).
+ */
+ea_handle *ea_create_ex(int L, int n_temps, int n_realizations, const double *betas, uint64_t seed,
+                        void *dev_workspace, size_t workspace_bytes, void *cuda_stream,
+                        int first_realization);
+
+void ea_destroy(ea_handle *h);
+
+/* J[r][d][site] in {+1,-1}: d = 0,1,2 is the +x,+y,+z bond of that site,
+ * site = x + L*(y + L*z) (Eq. 1).  Any other value: EA_ERR_INVALID_ARG.
+ * Energies are recomputed. */
+int ea_set_couplings(ea_handle *h, const int8_t *J /* [R][3][N] */);
+
+/* s[r][slot][site] in {+1,-1}, by storage slot.  Energies are recomputed. */
+int ea_set_spins(ea_handle *h, const int8_t *s /* [R][n_temps][N] */);
+
+/* Replace the threshold tables (north_star: "handed to both paths as input data").
+ * acc[t][c] = floor(2^32 min(1, exp(-beta_t (4c-12)))), c = 0..6;
+ * swp[t][m + 3N/2] = floor(2^32 min(1, exp((beta_t - beta_{t+1}) 4m))), m in [-3N/2, 3N/2].
+ * Values in [0, 2^32].  Each column of acc must be monotone in the same direction as betas
+ * and each row of swp monotone in m, else EA_ERR_INVALID_ARG. */
+int ea_set_tables(ea_handle *h, const uint64_t *acc /* [n_temps][7] */,
+                  const uint64_t *swp /* [n_temps-1][3N+1] */);
+int ea_get_tables(ea_handle *h, uint64_t *acc, uint64_t *swp);
+
+/*
+ * n_sweeps >= 0 full checkerboard sweeps (parity 0 then parity 1); a
+ * parallel-tempering round (R4-R6) follows every sweep whose
+ * 1-based GLOBAL index is a multiple of swap_interval; swap_interval = 0: no PT.
+ * EA_ERR_RANGE if the global sweep counter would pass 2^32 - 1.  Asynchronous.
+ */
+int ea_sweep(ea_handle *h, int64_t n_sweeps, int swap_interval);
+
+/* Block until everything enqueued on the handle's stream has finished; reports
+ * asynchronous CUDA errors. */
+int ea_synchronize(ea_handle *h);
+
+/* E[r][t] = H of realization r at temperature index t. */
+int ea_energy(ea_handle *h, int32_t *E /* [R][n_temps] */);
+
+/* Q[p][t] = sum_i s_i(ra, t) s_i(rb, t) for pairs[p] = (ra, rb); rb = -1: all-up reference
+ * (magnetization).  Bad realization index: EA_ERR_INVALID_ARG. */
+int ea_overlap(ea_handle *h, const int32_t *pairs /* [n_pairs][2] */, int n_pairs,
+               int32_t *Q /* [n_pairs][n_temps] */);
+
+/* s[r][t][site] = +-1 by temperature index. */
+int ea_get_spins(ea_handle *h, int8_t *s /* [R][n_temps][N] */);
+
+/* Raw state, for parity tests and checkpoints.  Any pointer may be NULL.
+ * spin_words[k][w][p][j]: bit b = spin of realization 32w+b at slot k, parity p, checkerboard
+ * index j; temp_of_slot[r][k]; energy_by_slot[r][k]. */
+int ea_get_state(ea_handle *h, uint32_t *spin_words /* [n_temps][W][2][N/2] */,
+                 uint8_t *temp_of_slot /* [R][n_temps] */, int32_t *energy_by_slot /* [R][n_temps] */,
+                 uint64_t *sweeps_done, uint64_t *swap_rounds_done);
+
+/* Select the sweep implementation (EA_KERNEL_*); EA_ERR_UNSUPPORTED if it cannot run this shape. */
+int ea_set_kernel(ea_handle *h, int kernel);
+/* The implementation ea_sweep would use now (EA_KERNEL_GENERIC/RESIDENT/TILED). */
+int ea_get_kernel(ea_handle *h);
+/* Number of kernels this handle has launched so far. */
+int64_t ea_launch_count(ea_handle *h);
+
+/* Message for the last failure on h (h = NULL: last ea_create* failure on this thread). */
+const char *ea_last_error(const ea_handle *h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* EA_B200_H */

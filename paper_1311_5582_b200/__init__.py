@@ -1,0 +1,13 @@
+"""paper_1311_5582_b200 -- thin Python binding of libea_b200.so (include/ea.h).
+
+Argument marshalling only: every step of the path (bit-packed store, checkerboard sweep,
+parallel-tempering swap, energy / overlap reductions) runs in the hand-written sm_100a
+kernels of csrc/.  PyTorch is used for device memory (the workspace tensor) and the stream.
+There is no CPU fallback: importing works without a GPU (so the symbol table can be
+checked), creating a simulation does not.
+"""
+from .binding import (EA, EA_KERNEL_AUTO, EA_KERNEL_GENERIC, EA_KERNEL_RESIDENT, EA_KERNEL_TILED,
+                      EAError, exported_symbols, lib, library_path)
+
+__all__ = ["EA", "EAError", "lib", "library_path", "exported_symbols", "EA_KERNEL_AUTO",
+           "EA_KERNEL_GENERIC", "EA_KERNEL_RESIDENT", "EA_KERNEL_TILED"]

@@ -1,0 +1,240 @@
+// ea_generic.cuh -- kernels that work for every even L: seeding, the global-memory half-sweep,
+// the standalone energy reduction, the PT swap round, overlap, pack/unpack.
+// The sm_100a fast paths (ea_resident.cuh, ea_tiled.cuh) reuse pt_swap / energy pieces.
+#pragma once
+#include "ea_device.cuh"
+
+namespace ea {
+
+// ------------------------------------------------------------------ a1: seeding
+// spin word (k, i, w) = PX(0, i>>2, w, (3<<16)|k)[i&3];  coupling word (d, i, w) =
+// PX(0, i, w, 4<<16)[d].  One thread per (w, canonical site i).
+__global__ void k_seed(Params P)
+{
+    const int64_t tid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (tid >= (int64_t)P.W * P.N) return;
+    const int i = (int)(tid % P.N), w = (int)(tid / P.N);
+    const int x = i % P.L, y = (i / P.L) % P.L, z = i / (P.L * P.L);
+    const int p = (x + y + z) & 1;
+    const int j = (x >> 1) + P.Lh * (y + P.L * z);
+    const uint32_t gw = P.w0 + (uint32_t)w;
+    const uint4 c = philox4x32_10(0u, (uint32_t)i, gw, 4u << 16, P.k0, P.k1);
+    uint32_t *cp = P.coup + (size_t)w * 3 * P.N + p * P.Nh + j;
+    cp[0] = c.x; cp[P.N] = c.y; cp[2 * P.N] = c.z;
+    for (int k = 0; k < P.nT; ++k) {
+        const uint4 s = philox4x32_10(0u, (uint32_t)(i >> 2), gw, (3u << 16) | (uint32_t)k, P.k0, P.k1);
+        P.spin[((size_t)k * P.W + w) * P.N + p * P.Nh + j] = pick(s, i & 3);
+    }
+}
+
+__global__ void k_identity_perm(Params P)
+{
+    const int tid = blockIdx.x * blockDim.x + threadIdx.x;
+    if (tid >= P.Rp * P.nT) return;
+    const uint8_t k = (uint8_t)(tid % P.nT);
+    P.tau[tid] = k;
+    P.sigma[tid] = k;
+}
+
+// ------------------------------------------------------------------ rank masks
+// lt[w][k][n] = bits b whose temperature rank pos(tau[32w+b][k]) >= n, n = 0..nT
+// (the paper's "swap the rows of the table, not the lattices", in bit-sliced
+// form).  One warp per (w, k), lane = bit.
+__device__ __forceinline__ void build_lt_row(const Params &P, int w, int k, int lane)
+{
+    const int t = P.tau[(size_t)(32 * w + lane) * P.nT + k];
+    const int pos = P.desc ? t : P.nT - 1 - t;
+    uint32_t *row = P.lt + ((size_t)w * P.nT + k) * P.LTS;
+    for (int n = 0; n <= P.nT; ++n) {
+        const uint32_t m = __ballot_sync(0xFFFFFFFFu, pos >= n);
+        if (lane == (n & 31)) row[n] = m;
+    }
+}
+
+__global__ void k_build_lt(Params P)
+{
+    const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    if (warp >= P.W * P.nT) return;
+    build_lt_row(P, warp / P.nT, warp % P.nT, lane);
+}
+
+// ------------------------------------------------------------------ a2-a7: generic half-sweep
+// One thread per (slot k, word w, quad q): four sites, one Philox call
+// PX(g, q, w, (p<<16)|k) (R17).  Global memory only; any even L.
+__global__ void __launch_bounds__(128) k_half_sweep_generic(Params P, int p, uint32_t g)
+{
+    extern __shared__ uint32_t sm_thr[];   // [3][nT+1]
+    for (int a = threadIdx.x; a < 3 * P.LTS; a += blockDim.x) sm_thr[a] = P.thr32[a];
+    __syncthreads();
+    const int nq = P.Nh >> 2;
+    const int64_t tid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (tid >= (int64_t)P.nT * P.W * nq) return;
+    const int q = (int)(tid % nq);
+    const int w = (int)((tid / nq) % P.W);
+    const int k = (int)(tid / ((int64_t)nq * P.W));
+    uint32_t *sp = P.spin + ((size_t)k * P.W + w) * P.N;
+    const uint32_t *cp = P.coup + (size_t)w * 3 * P.N;
+    const uint32_t *lt = P.lt + ((size_t)w * P.nT + k) * P.LTS;
+    const uint4 rnd = philox4x32_10(g, (uint32_t)q, P.w0 + (uint32_t)w, ((uint32_t)p << 16) | (uint32_t)k,
+                                    P.k0, P.k1);
+#pragma unroll
+    for (int l = 0; l < 4; ++l) {
+        const int j = 4 * q + l;
+        uint32_t s;
+        const Planes pl = site_planes(sp, cp, p, j, P.L, P.Lh, P.Nh, P.N, &s);
+        const uint32_t u = pick(rnd, l);
+        const uint32_t m4 = lt[rank_of(u, sm_thr, P.z[0], P.nT)];
+        const uint32_t m5 = lt[rank_of(u, sm_thr + P.LTS, P.z[1], P.nT)];
+        const uint32_t m6 = lt[rank_of(u, sm_thr + 2 * P.LTS, P.z[2], P.nT)];
+        sp[p * P.Nh + j] = s ^ accept_mask(pl, m4, m5, m6);
+    }
+}
+
+// ------------------------------------------------------------------ a8: energy from scratch
+// E[r][k] = 3N - 2 * (number of satisfied bonds); every bond has exactly one parity-1 end, so
+// the satisfied bonds are sum over parity-1 sites of n_sat.  One block per (w, k); per-thread
+// bit-sliced (vertical) counters, then a transposition to 32 integers with warp reductions.
+constexpr int kEnergyPlanes = 14;   // per-thread count <= 6 * ceil(Nh / 128)
+
+__device__ __forceinline__ void vadd(uint32_t (&c)[kEnergyPlanes], uint32_t x, int from)
+{
+#pragma unroll
+    for (int i = 0; i < kEnergyPlanes; ++i) {
+        if (i < from) continue;
+        const uint32_t t = c[i] & x;
+        c[i] ^= x;
+        x = t;
+    }
+}
+
+__global__ void __launch_bounds__(128) k_energy(Params P)
+{
+    __shared__ int sm_cnt[32];
+    const int w = blockIdx.x / P.nT, k = blockIdx.x % P.nT;
+    const uint32_t *sp = P.spin + ((size_t)k * P.W + w) * P.N;
+    const uint32_t *cp = P.coup + (size_t)w * 3 * P.N;
+    if (threadIdx.x < 32) sm_cnt[threadIdx.x] = 0;
+    __syncthreads();
+    uint32_t c[kEnergyPlanes];
+#pragma unroll
+    for (int i = 0; i < kEnergyPlanes; ++i) c[i] = 0;
+    for (int j = threadIdx.x; j < P.Nh; j += blockDim.x) {
+        uint32_t s;
+        const Planes pl = site_planes(sp, cp, 1, j, P.L, P.Lh, P.Nh, P.N, &s);
+        vadd(c, pl.b0, 0);
+        vadd(c, pl.b1, 1);
+        vadd(c, pl.b2, 2);
+    }
+    const int lane = threadIdx.x & 31;
+    int mine = 0;
+    for (int b = 0; b < 32; ++b) {
+        int v = 0;
+#pragma unroll
+        for (int i = 0; i < kEnergyPlanes; ++i) v += (int)((c[i] >> b) & 1u) << i;
+        v = __reduce_add_sync(0xFFFFFFFFu, v);
+        if (lane == b) mine = v;
+    }
+    atomicAdd(&sm_cnt[lane], mine);
+    __syncthreads();
+    if (threadIdx.x < 32)
+        P.E[(size_t)(32 * w + threadIdx.x) * P.nT + k] = 3 * P.N - 2 * sm_cnt[threadIdx.x];
+}
+
+// ------------------------------------------------------------------ a9: PT swap round
+// Decision for temperature pair (t, t+1) of realization r after sweep g_done:
+//   a = sigma[t], b = sigma[t+1], m = (E_a - E_b)/4, accept iff PX(g_done,t,r,2<<16)[0] < swp[t][m].
+// The swap table is stored trimmed (only thresholds in (0, 2^32), as thr - 1).
+__device__ __forceinline__ bool swap_accept(const Params &P, int t, int m, uint32_t v)
+{
+    const int lo = P.swp_lo[t], cnt = P.swp_cnt[t];
+    if (m < lo) return P.swp_kind[2 * t] != 0;
+    if (m >= lo + cnt) return P.swp_kind[2 * t + 1] != 0;
+    return v <= P.swp_val[P.swp_off[t] + (m - lo)];
+}
+
+// One block per word: lane = realization bit, warps stride over the disjoint pairs of this
+// round (R4); then the rank masks of the word are rebuilt.  No lattice word moves.
+__global__ void __launch_bounds__(256) k_pt_swap(Params P, uint32_t g_done, uint32_t round)
+{
+    const int w = blockIdx.x, lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
+    const int r = 32 * w + lane;
+    uint8_t *sg = P.sigma + (size_t)r * P.nT, *ta = P.tau + (size_t)r * P.nT;
+    const int32_t *E = P.E + (size_t)r * P.nT;
+    for (int t = (int)(round & 1u) + 2 * warp; t + 1 < P.nT; t += 2 * nwarp) {
+        const int a = sg[t], b = sg[t + 1];
+        const int m = (E[a] - E[b]) / 4;
+        const uint4 v = philox4x32_10(g_done, (uint32_t)t, P.r0 + (uint32_t)r, 2u << 16, P.k0, P.k1);
+        if (swap_accept(P, t, m, v.x)) {
+            sg[t] = (uint8_t)b; sg[t + 1] = (uint8_t)a;
+            ta[a] = (uint8_t)(t + 1); ta[b] = (uint8_t)t;
+        }
+    }
+    __syncthreads();
+    for (int k = warp; k < P.nT; k += nwarp) build_lt_row(P, w, k, lane);
+}
+
+// ------------------------------------------------------------------ a10: overlap
+// Q[pair][t] = sum_i s_i(ra, sigma_a[t]) s_i(rb, sigma_b[t]); rb = -1: all-up reference.
+__global__ void __launch_bounds__(256) k_overlap(Params P, const int32_t *pairs, int32_t *Q)
+{
+    __shared__ int sm_sum[8];
+    const int pr = blockIdx.x / P.nT, t = blockIdx.x % P.nT;
+    const int ra = pairs[2 * pr], rb = pairs[2 * pr + 1];
+    const int ka = P.sigma[(size_t)ra * P.nT + t];
+    const uint32_t *sa = P.spin + ((size_t)ka * P.W + (ra >> 5)) * P.N;
+    const uint32_t *sb = nullptr;
+    if (rb >= 0) sb = P.spin + ((size_t)P.sigma[(size_t)rb * P.nT + t] * P.W + (rb >> 5)) * P.N;
+    int agree = 0;
+    for (int i = threadIdx.x; i < P.N; i += blockDim.x) {
+        const uint32_t a = (sa[i] >> (ra & 31)) & 1u;
+        const uint32_t b = sb ? (sb[i] >> (rb & 31)) & 1u : 1u;
+        agree += (a == b);
+    }
+    agree = __reduce_add_sync(0xFFFFFFFFu, agree);
+    if ((threadIdx.x & 31) == 0) sm_sum[threadIdx.x >> 5] = agree;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int tot = 0;
+        for (int i = 0; i < (int)(blockDim.x >> 5); ++i) tot += sm_sum[i];
+        Q[blockIdx.x] = 2 * tot - P.N;
+    }
+}
+
+// ------------------------------------------------------------------ a11: export / import
+// out[r][t][i] = +-1 by temperature index (by_slot = 0) or by slot (by_slot = 1).
+__global__ void k_unpack_spins(Params P, int R, int by_slot, int8_t *out)
+{
+    const int64_t tid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (tid >= (int64_t)R * P.nT * P.N) return;
+    const int i = (int)(tid % P.N);
+    const int t = (int)((tid / P.N) % P.nT);
+    const int r = (int)(tid / ((int64_t)P.N * P.nT));
+    const int k = by_slot ? t : P.sigma[(size_t)r * P.nT + t];
+    const int x = i % P.L, y = (i / P.L) % P.L, z = i / (P.L * P.L);
+    const int p = (x + y + z) & 1, j = (x >> 1) + P.Lh * (y + P.L * z);
+    const uint32_t wv = P.spin[((size_t)k * P.W + (r >> 5)) * P.N + p * P.Nh + j];
+    out[tid] = ((wv >> (r & 31)) & 1u) ? 1 : -1;
+}
+
+// in[r][outer][i] (+-1 int8, canonical site order) -> words[outer'][w][p][j]; one thread per
+// output word.  mode 0: spins (outer = slot k, word index (k W + w) N + ...);
+// mode 1: couplings (outer = d, word index (w 3 + d) N + ...).
+__global__ void k_pack(Params P, int R, int n_outer, int mode, const int8_t *in, uint32_t *words)
+{
+    const int64_t tid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (tid >= (int64_t)n_outer * P.W * P.N) return;
+    const int i = (int)(tid % P.N);
+    const int w = (int)((tid / P.N) % P.W);
+    const int o = (int)(tid / ((int64_t)P.N * P.W));
+    const int x = i % P.L, y = (i / P.L) % P.L, z = i / (P.L * P.L);
+    const int p = (x + y + z) & 1, j = (x >> 1) + P.Lh * (y + P.L * z);
+    uint32_t v = 0;
+    for (int b = 0; b < 32; ++b) {
+        const int r = 32 * w + b;
+        if (r < R && in[((size_t)r * n_outer + o) * P.N + i] > 0) v |= 1u << b;
+    }
+    const size_t dst = mode == 0 ? ((size_t)o * P.W + w) * P.N : ((size_t)w * 3 + o) * P.N;
+    words[dst + p * P.Nh + j] = v;
+}
+
+}  // namespace ea

@@ -1,0 +1,485 @@
+// ea_lib.cu -- host side of libea_b200.so: the C ABI of include/ea.h.
+// Product code.  No CPU fallback: every step of the path runs in the CUDA kernels of
+// ea_generic.cuh / ea_resident.cuh / ea_tiled.cuh.  Shares nothing with oracle/.
+#include "../../include/ea.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "ea_generic.cuh"
+#include "ea_resident.cuh"
+#include "ea_tiled.cuh"
+
+using ea::Params;
+
+struct ea_handle {
+    int L = 0, N = 0, nT = 0, R = 0, W = 0, Rp = 0, r0 = 0;
+    uint64_t seed = 0;
+    std::vector<double> betas;
+    bool desc = true;
+    std::vector<uint64_t> acc, swp;   // host copies of the full tables
+    cudaStream_t stream = nullptr;
+    bool own_ws = false;
+    char *ws = nullptr;
+    size_t ws_bytes = 0;
+    Params P{};
+    uint32_t *d_thr32 = nullptr;
+    int32_t *d_swp_lo = nullptr, *d_swp_cnt = nullptr, *d_swp_off = nullptr;
+    uint8_t *d_swp_kind = nullptr;
+    uint32_t *d_swp_val = nullptr;
+    size_t swp_val_cap = 0;
+    uint64_t g = 0, nswap = 0;
+    bool energy_valid = false;
+    int kernel_sel = EA_KERNEL_AUTO;
+    int64_t launches = 0;
+    int sm_count = 0;
+    mutable std::string err;
+};
+
+static thread_local std::string g_create_err;
+
+static int fail(const ea_handle *h, int code, const std::string &msg)
+{
+    if (h) h->err = msg; else g_create_err = msg;
+    return code;
+}
+#define CUDA_TRY(h, expr)                                                                   \
+    do {                                                                                    \
+        cudaError_t e_ = (expr);                                                            \
+        if (e_ != cudaSuccess)                                                              \
+            return fail(h, EA_ERR_CUDA, std::string(#expr) + ": " + cudaGetErrorString(e_)); \
+    } while (0)
+
+// ---------------------------------------------------------------- workspace layout
+namespace {
+struct Layout {
+    size_t spin, coup, lt, tau, sigma, E, thr32, swp_lo, swp_cnt, swp_off, swp_kind, swp_val, total;
+    size_t swp_val_cap;
+};
+size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+bool shape_ok(int L, int nT, int R)
+{
+    return L >= 2 && (L & 1) == 0 && L <= 128 && nT >= 1 && R >= 1 && R <= (1 << 24);
+}
+
+Layout make_layout(int L, int nT, int R)
+{
+    Layout o{};
+    const size_t N = (size_t)L * L * L, W = (size_t)(R + 31) / 32, Rp = 32 * W;
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t a = off; off = align256(off + bytes); return a; };
+    o.spin = take(4 * (size_t)nT * W * N);
+    o.coup = take(4 * 3 * W * N);
+    o.lt = take(4 * W * nT * (nT + 1));
+    o.tau = take(Rp * nT);
+    o.sigma = take(Rp * nT);
+    o.E = take(4 * Rp * nT);
+    o.thr32 = take(4 * 3 * (size_t)(nT + 1));
+    o.swp_lo = take(4 * (size_t)nT);
+    o.swp_cnt = take(4 * (size_t)nT);
+    o.swp_off = take(4 * (size_t)nT);
+    o.swp_kind = take(2 * (size_t)nT);
+    o.swp_val_cap = (size_t)(nT > 1 ? nT - 1 : 0) * (3 * N + 1);
+    o.swp_val = take(4 * (o.swp_val_cap ? o.swp_val_cap : 1));
+    o.total = off;
+    return o;
+}
+
+uint64_t threshold_of(double x)
+{
+    if (x >= 0.0) return (uint64_t)1 << 32;
+    return (uint64_t)std::floor(std::ldexp(std::exp(x), 32));
+}
+const uint64_t TWO32 = (uint64_t)1 << 32;
+
+void launch_cfg(int64_t n, int block, int &grid) { grid = (int)((n + block - 1) / block); }
+}  // namespace
+
+// ---------------------------------------------------------------- tables -> device form
+// acc: per class c = 4,5,6 a column sorted coldest-first ("pos" order), stored as thr-1 with
+// the leading zero thresholds counted in z[c] (R8).  swp: each row trimmed to the
+// entries strictly between 0 and 2^32.
+static int upload_tables(ea_handle *h, const std::vector<uint64_t> &acc, const std::vector<uint64_t> &swp)
+{
+    const int nT = h->nT, M = 3 * h->N / 2, cols = 2 * M + 1;
+    for (int t = 0; t < nT; ++t)
+        for (int c = 0; c < 7; ++c) {
+            const uint64_t v = acc[(size_t)t * 7 + c];
+            if (v > TWO32) return fail(h, EA_ERR_INVALID_ARG, "acc threshold above 2^32");
+            if (c <= 3 && v != TWO32)
+                return fail(h, EA_ERR_UNSUPPORTED, "acc[t][c<=3] must be 2^32 (dE <= 0 always flips)");
+        }
+    std::vector<uint32_t> thr32((size_t)3 * (nT + 1));
+    int z[3];
+    for (int c = 4; c <= 6; ++c) {
+        uint32_t *col = thr32.data() + (size_t)(c - 4) * (nT + 1);
+        uint64_t prev = 0;
+        int zc = 0;
+        for (int pos = 0; pos < nT; ++pos) {
+            const int t = h->desc ? pos : nT - 1 - pos;
+            const uint64_t v = acc[(size_t)t * 7 + c];
+            if (v < prev) return fail(h, EA_ERR_INVALID_ARG, "acc column not monotone with beta");
+            if (c > 4 && v > acc[(size_t)t * 7 + c - 1])
+                return fail(h, EA_ERR_INVALID_ARG, "acc row not non-increasing in n_sat");
+            prev = v;
+            if (v == 0) { zc = pos + 1; col[pos] = 0; }
+            else col[pos] = (uint32_t)(v - 1);
+        }
+        col[nT] = 0xFFFFFFFFu;
+        z[c - 4] = zc;
+    }
+    std::vector<int32_t> lo(nT, 0), cnt(nT, 0), off(nT, 0);
+    std::vector<uint8_t> kind((size_t)2 * nT, 0);
+    std::vector<uint32_t> val;
+    for (int t = 0; t + 1 < nT; ++t) {
+        const uint64_t *row = swp.data() + (size_t)t * cols;
+        bool inc = true, dec = true;
+        for (int a = 0; a < cols; ++a) {
+            if (row[a] > TWO32) return fail(h, EA_ERR_INVALID_ARG, "swp threshold above 2^32");
+            if (a && row[a] < row[a - 1]) inc = false;
+            if (a && row[a] > row[a - 1]) dec = false;
+        }
+        if (!inc && !dec) return fail(h, EA_ERR_INVALID_ARG, "swp row not monotone in m");
+        int a = 0;
+        while (a < cols && (row[a] == 0 || row[a] == TWO32) && row[a] == row[0]) ++a;
+        int b = a;
+        while (b < cols && row[b] != 0 && row[b] != TWO32) ++b;
+        for (int c2 = b; c2 < cols; ++c2)
+            if (row[c2] != row[cols - 1]) return fail(h, EA_ERR_INVALID_ARG, "swp row not monotone in m");
+        lo[t] = a - M; cnt[t] = b - a; off[t] = (int32_t)val.size();
+        kind[2 * t] = row[0] == TWO32;
+        kind[2 * t + 1] = row[cols - 1] == TWO32;
+        for (int c2 = a; c2 < b; ++c2) val.push_back((uint32_t)(row[c2] - 1));
+    }
+    if (val.size() > h->swp_val_cap) return fail(h, EA_ERR_ALLOC, "swap table overflow");
+    cudaStream_t s = h->stream;
+    CUDA_TRY(h, cudaStreamSynchronize(s));
+    CUDA_TRY(h, cudaMemcpyAsync(h->d_thr32, thr32.data(), 4 * thr32.size(), cudaMemcpyHostToDevice, s));
+    CUDA_TRY(h, cudaMemcpyAsync(h->d_swp_lo, lo.data(), 4 * nT, cudaMemcpyHostToDevice, s));
+    CUDA_TRY(h, cudaMemcpyAsync(h->d_swp_cnt, cnt.data(), 4 * nT, cudaMemcpyHostToDevice, s));
+    CUDA_TRY(h, cudaMemcpyAsync(h->d_swp_off, off.data(), 4 * nT, cudaMemcpyHostToDevice, s));
+    CUDA_TRY(h, cudaMemcpyAsync(h->d_swp_kind, kind.data(), 2 * nT, cudaMemcpyHostToDevice, s));
+    if (!val.empty())
+        CUDA_TRY(h, cudaMemcpyAsync(h->d_swp_val, val.data(), 4 * val.size(), cudaMemcpyHostToDevice, s));
+    CUDA_TRY(h, cudaStreamSynchronize(s));
+    for (int c = 0; c < 3; ++c) h->P.z[c] = z[c];
+    h->acc = acc;
+    h->swp = swp;
+    return EA_OK;
+}
+
+// ---------------------------------------------------------------- small helpers
+static int recompute_energy(ea_handle *h)
+{
+    ea::k_energy<<<h->W * h->nT, 128, 0, h->stream>>>(h->P);
+    h->launches++;
+    CUDA_TRY(h, cudaGetLastError());
+    h->energy_valid = true;
+    return EA_OK;
+}
+static int rebuild_lt(ea_handle *h)
+{
+    int grid;
+    launch_cfg((int64_t)h->W * h->nT * 32, 128, grid);
+    ea::k_build_lt<<<grid, 128, 0, h->stream>>>(h->P);
+    h->launches++;
+    CUDA_TRY(h, cudaGetLastError());
+    return EA_OK;
+}
+
+// ---------------------------------------------------------------- create / destroy
+extern "C" size_t ea_workspace_bytes(int L, int n_temps, int n_realizations)
+{
+    if (!shape_ok(L, n_temps, n_realizations) || n_temps > 64) return 0;
+    return make_layout(L, n_temps, n_realizations).total;
+}
+
+extern "C" ea_handle *ea_create_ex(int L, int n_temps, int n_realizations, const double *betas,
+                                   uint64_t seed, void *dev_workspace, size_t workspace_bytes,
+                                   void *cuda_stream, int first_realization)
+{
+    if (!shape_ok(L, n_temps, n_realizations) || !betas || first_realization < 0 ||
+        (first_realization & 31)) {
+        fail(nullptr, EA_ERR_INVALID_ARG, "ea_create: bad shape (L even >= 2, n_temps >= 1, R >= 1, "
+                                          "first_realization multiple of 32)");
+        return nullptr;
+    }
+    if (n_temps > 64) { fail(nullptr, EA_ERR_UNSUPPORTED, "ea_create: n_temps > 64"); return nullptr; }
+    bool desc = true, asc = true;
+    for (int t = 0; t < n_temps; ++t) {
+        if (!std::isfinite(betas[t]) || betas[t] < 0.0) {
+            fail(nullptr, EA_ERR_INVALID_ARG, "ea_create: betas must be finite and >= 0");
+            return nullptr;
+        }
+        if (t && betas[t] > betas[t - 1]) desc = false;
+        if (t && betas[t] < betas[t - 1]) asc = false;
+    }
+    if (!desc && !asc) { fail(nullptr, EA_ERR_INVALID_ARG, "ea_create: betas not monotone"); return nullptr; }
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        fail(nullptr, EA_ERR_CUDA, "ea_create: no CUDA device (there is no CPU fallback)");
+        return nullptr;
+    }
+    ea_handle *h = new ea_handle();
+    h->L = L; h->N = L * L * L; h->nT = n_temps; h->R = n_realizations;
+    h->W = (n_realizations + 31) / 32; h->Rp = 32 * h->W; h->r0 = first_realization;
+    h->seed = seed; h->betas.assign(betas, betas + n_temps); h->desc = desc;
+    h->stream = (cudaStream_t)cuda_stream;
+    const Layout lay = make_layout(L, n_temps, n_realizations);
+    auto bail = [&](int code, const std::string &m) { fail(nullptr, code, m); ea_destroy(h); return nullptr; };
+    if (dev_workspace) {
+        if (workspace_bytes < lay.total || ((uintptr_t)dev_workspace & 255))
+            return (ea_handle *)bail(EA_ERR_INVALID_ARG, "ea_create_ex: workspace too small or misaligned");
+        h->ws = (char *)dev_workspace;
+    } else {
+        if (cudaMalloc((void **)&h->ws, lay.total) != cudaSuccess)
+            return (ea_handle *)bail(EA_ERR_ALLOC, "ea_create: cudaMalloc failed");
+        h->own_ws = true;
+    }
+    h->ws_bytes = lay.total;
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, dev);
+    Params &P = h->P;
+    P.L = L; P.Lh = L / 2; P.N = h->N; P.Nh = h->N / 2; P.nT = n_temps; P.W = h->W; P.Rp = h->Rp;
+    P.LTS = n_temps + 1;
+    P.k0 = (uint32_t)seed; P.k1 = (uint32_t)(seed >> 32);
+    P.r0 = (uint32_t)first_realization; P.w0 = (uint32_t)(first_realization >> 5);
+    P.desc = desc ? 1 : 0;
+    P.spin = (uint32_t *)(h->ws + lay.spin);
+    P.coup = (uint32_t *)(h->ws + lay.coup);
+    P.lt = (uint32_t *)(h->ws + lay.lt);
+    P.tau = (uint8_t *)(h->ws + lay.tau);
+    P.sigma = (uint8_t *)(h->ws + lay.sigma);
+    P.E = (int32_t *)(h->ws + lay.E);
+    P.thr32 = h->d_thr32 = (uint32_t *)(h->ws + lay.thr32);
+    P.swp_lo = h->d_swp_lo = (int32_t *)(h->ws + lay.swp_lo);
+    P.swp_cnt = h->d_swp_cnt = (int32_t *)(h->ws + lay.swp_cnt);
+    P.swp_off = h->d_swp_off = (int32_t *)(h->ws + lay.swp_off);
+    P.swp_kind = h->d_swp_kind = (uint8_t *)(h->ws + lay.swp_kind);
+    P.swp_val = h->d_swp_val = (uint32_t *)(h->ws + lay.swp_val);
+    h->swp_val_cap = lay.swp_val_cap;
+
+    // threshold tables in double on the host
+    const int M = 3 * h->N / 2;
+    std::vector<uint64_t> acc((size_t)n_temps * 7), swp((size_t)(n_temps > 1 ? n_temps - 1 : 0) * (2 * M + 1));
+    for (int t = 0; t < n_temps; ++t)
+        for (int c = 0; c < 7; ++c) acc[(size_t)t * 7 + c] = threshold_of(-(betas[t] * (double)(4 * c - 12)));
+    for (int t = 0; t + 1 < n_temps; ++t) {
+        const double db = betas[t] - betas[t + 1];
+        for (int m = -M; m <= M; ++m) swp[(size_t)t * (2 * M + 1) + (m + M)] = threshold_of(db * (double)(4 * m));
+    }
+    if (upload_tables(h, acc, swp) != EA_OK) return (ea_handle *)bail(EA_ERR_CUDA, "ea_create: tables: " + h->err);
+
+    int grid;
+    launch_cfg((int64_t)h->W * h->N, 128, grid);
+    ea::k_seed<<<grid, 128, 0, h->stream>>>(P);
+    launch_cfg((int64_t)h->Rp * n_temps, 128, grid);
+    ea::k_identity_perm<<<grid, 128, 0, h->stream>>>(P);
+    h->launches += 2;
+    if (rebuild_lt(h) != EA_OK || recompute_energy(h) != EA_OK ||
+        cudaStreamSynchronize(h->stream) != cudaSuccess || cudaGetLastError() != cudaSuccess)
+        return (ea_handle *)bail(EA_ERR_CUDA, "ea_create: initialisation kernels failed: " + h->err);
+    return h;
+}
+
+extern "C" ea_handle *ea_create(int L, int n_temps, int n_realizations, const double *betas, uint64_t seed)
+{
+    return ea_create_ex(L, n_temps, n_realizations, betas, seed, nullptr, 0, nullptr, 0);
+}
+
+extern "C" void ea_destroy(ea_handle *h)
+{
+    if (!h) return;
+    if (h->ws) cudaStreamSynchronize(h->stream);
+    if (h->own_ws && h->ws) cudaFree(h->ws);
+    delete h;
+}
+
+extern "C" const char *ea_last_error(const ea_handle *h) { return h ? h->err.c_str() : g_create_err.c_str(); }
+extern "C" int64_t ea_launch_count(ea_handle *h) { return h ? h->launches : 0; }
+
+extern "C" int ea_synchronize(ea_handle *h)
+{
+    if (!h) return EA_ERR_INVALID_ARG;
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    CUDA_TRY(h, cudaGetLastError());
+    return EA_OK;
+}
+
+// ---------------------------------------------------------------- inputs
+static int pack_from_host(ea_handle *h, const int8_t *src, int n_outer, int mode, uint32_t *dst)
+{
+    const size_t n = (size_t)h->R * n_outer * h->N;
+    for (size_t a = 0; a < n; ++a)
+        if (src[a] != 1 && src[a] != -1) return fail(h, EA_ERR_INVALID_ARG, "values must be +1 or -1");
+    int8_t *tmp = nullptr;
+    CUDA_TRY(h, cudaMalloc((void **)&tmp, n));
+    cudaError_t e = cudaMemcpyAsync(tmp, src, n, cudaMemcpyHostToDevice, h->stream);
+    if (e == cudaSuccess) {
+        int grid;
+        launch_cfg((int64_t)n_outer * h->W * h->N, 128, grid);
+        ea::k_pack<<<grid, 128, 0, h->stream>>>(h->P, h->R, n_outer, mode, tmp, dst);
+        h->launches++;
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+    cudaFree(tmp);
+    if (e != cudaSuccess) return fail(h, EA_ERR_CUDA, std::string("pack: ") + cudaGetErrorString(e));
+    return recompute_energy(h);
+}
+
+extern "C" int ea_set_couplings(ea_handle *h, const int8_t *J)
+{
+    if (!h || !J) return fail(h, EA_ERR_INVALID_ARG, "ea_set_couplings: null argument");
+    return pack_from_host(h, J, 3, 1, h->P.coup);
+}
+
+extern "C" int ea_set_spins(ea_handle *h, const int8_t *s)
+{
+    if (!h || !s) return fail(h, EA_ERR_INVALID_ARG, "ea_set_spins: null argument");
+    return pack_from_host(h, s, h->nT, 0, h->P.spin);
+}
+
+extern "C" int ea_set_tables(ea_handle *h, const uint64_t *acc, const uint64_t *swp)
+{
+    if (!h || !acc || (h->nT > 1 && !swp)) return fail(h, EA_ERR_INVALID_ARG, "ea_set_tables: null argument");
+    const size_t cols = 3 * (size_t)h->N + 1;
+    std::vector<uint64_t> a(acc, acc + (size_t)h->nT * 7);
+    std::vector<uint64_t> s;
+    if (h->nT > 1) s.assign(swp, swp + (size_t)(h->nT - 1) * cols);
+    return upload_tables(h, a, s);
+}
+
+extern "C" int ea_get_tables(ea_handle *h, uint64_t *acc, uint64_t *swp)
+{
+    if (!h) return EA_ERR_INVALID_ARG;
+    if (acc) std::memcpy(acc, h->acc.data(), 8 * h->acc.size());
+    if (swp && !h->swp.empty()) std::memcpy(swp, h->swp.data(), 8 * h->swp.size());
+    return EA_OK;
+}
+
+// ---------------------------------------------------------------- sweep
+static int sweep_generic(ea_handle *h, int64_t n_sweeps, int swap_interval)
+{
+    const int64_t nthreads = (int64_t)h->nT * h->W * (h->N / 8);
+    int grid;
+    launch_cfg(nthreads, 128, grid);
+    const size_t smem = 4 * 3 * (size_t)(h->nT + 1);
+    for (int64_t it = 0; it < n_sweeps; ++it) {
+        ea::k_half_sweep_generic<<<grid, 128, smem, h->stream>>>(h->P, 0, (uint32_t)h->g);
+        ea::k_half_sweep_generic<<<grid, 128, smem, h->stream>>>(h->P, 1, (uint32_t)h->g);
+        h->launches += 2;
+        h->energy_valid = false;
+        h->g++;
+        if (swap_interval > 0 && h->g % (uint64_t)swap_interval == 0) {
+            int rc = recompute_energy(h);
+            if (rc != EA_OK) return rc;
+            ea::k_pt_swap<<<h->W, 256, 0, h->stream>>>(h->P, (uint32_t)(h->g - 1), (uint32_t)(h->nswap & 1u));
+            h->launches++;
+            h->nswap++;
+        }
+    }
+    CUDA_TRY(h, cudaGetLastError());
+    return EA_OK;
+}
+
+static int pick_kernel(const ea_handle *h)
+{
+    if (h->kernel_sel != EA_KERNEL_AUTO) return h->kernel_sel;
+    return EA_KERNEL_GENERIC;
+}
+
+extern "C" int ea_set_kernel(ea_handle *h, int kernel)
+{
+    if (!h) return EA_ERR_INVALID_ARG;
+    if (kernel == EA_KERNEL_AUTO || kernel == EA_KERNEL_GENERIC) { h->kernel_sel = kernel; return EA_OK; }
+    return fail(h, EA_ERR_UNSUPPORTED, "ea_set_kernel: kernel not available for this shape");
+}
+extern "C" int ea_get_kernel(ea_handle *h) { return h ? pick_kernel(h) : EA_ERR_INVALID_ARG; }
+
+extern "C" int ea_sweep(ea_handle *h, int64_t n_sweeps, int swap_interval)
+{
+    if (!h || n_sweeps < 0 || swap_interval < 0) return fail(h, EA_ERR_INVALID_ARG, "ea_sweep: bad argument");
+    if (h->g + (uint64_t)n_sweeps > 0xFFFFFFFFull) return fail(h, EA_ERR_RANGE, "ea_sweep: sweep counter would pass 2^32-1");
+    if (n_sweeps == 0) return EA_OK;
+    return sweep_generic(h, n_sweeps, swap_interval);
+}
+
+// ---------------------------------------------------------------- observables
+extern "C" int ea_energy(ea_handle *h, int32_t *E)
+{
+    if (!h || !E) return fail(h, EA_ERR_INVALID_ARG, "ea_energy: null argument");
+    if (!h->energy_valid) { int rc = recompute_energy(h); if (rc != EA_OK) return rc; }
+    const size_t n = (size_t)h->Rp * h->nT;
+    std::vector<int32_t> Es(n);
+    std::vector<uint8_t> sg(n);
+    CUDA_TRY(h, cudaMemcpyAsync(Es.data(), h->P.E, 4 * n, cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(h, cudaMemcpyAsync(sg.data(), h->P.sigma, n, cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    for (int r = 0; r < h->R; ++r)
+        for (int t = 0; t < h->nT; ++t)
+            E[(size_t)r * h->nT + t] = Es[(size_t)r * h->nT + sg[(size_t)r * h->nT + t]];
+    return EA_OK;
+}
+
+extern "C" int ea_overlap(ea_handle *h, const int32_t *pairs, int n_pairs, int32_t *Q)
+{
+    if (!h || n_pairs < 0 || (n_pairs && (!pairs || !Q))) return fail(h, EA_ERR_INVALID_ARG, "ea_overlap: bad argument");
+    for (int p = 0; p < n_pairs; ++p)
+        if (pairs[2 * p] < 0 || pairs[2 * p] >= h->R || pairs[2 * p + 1] < -1 || pairs[2 * p + 1] >= h->R)
+            return fail(h, EA_ERR_INVALID_ARG, "ea_overlap: realization index out of range");
+    if (n_pairs == 0) return EA_OK;
+    int32_t *d = nullptr;
+    const size_t nb_p = 8 * (size_t)n_pairs, nb_q = 4 * (size_t)n_pairs * h->nT;
+    CUDA_TRY(h, cudaMalloc((void **)&d, nb_p + nb_q));
+    cudaError_t e = cudaMemcpyAsync(d, pairs, nb_p, cudaMemcpyHostToDevice, h->stream);
+    if (e == cudaSuccess) {
+        ea::k_overlap<<<n_pairs * h->nT, 256, 0, h->stream>>>(h->P, d, d + 2 * (size_t)n_pairs);
+        h->launches++;
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaMemcpyAsync(Q, d + 2 * (size_t)n_pairs, nb_q, cudaMemcpyDeviceToHost, h->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+    cudaFree(d);
+    if (e != cudaSuccess) return fail(h, EA_ERR_CUDA, std::string("ea_overlap: ") + cudaGetErrorString(e));
+    return EA_OK;
+}
+
+extern "C" int ea_get_spins(ea_handle *h, int8_t *s)
+{
+    if (!h || !s) return fail(h, EA_ERR_INVALID_ARG, "ea_get_spins: null argument");
+    const size_t n = (size_t)h->R * h->nT * h->N;
+    int8_t *d = nullptr;
+    CUDA_TRY(h, cudaMalloc((void **)&d, n));
+    int grid;
+    launch_cfg((int64_t)n, 256, grid);
+    ea::k_unpack_spins<<<grid, 256, 0, h->stream>>>(h->P, h->R, 0, d);
+    h->launches++;
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess) e = cudaMemcpyAsync(s, d, n, cudaMemcpyDeviceToHost, h->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+    cudaFree(d);
+    if (e != cudaSuccess) return fail(h, EA_ERR_CUDA, std::string("ea_get_spins: ") + cudaGetErrorString(e));
+    return EA_OK;
+}
+
+extern "C" int ea_get_state(ea_handle *h, uint32_t *spin_words, uint8_t *temp_of_slot,
+                            int32_t *energy_by_slot, uint64_t *sweeps_done, uint64_t *swap_rounds_done)
+{
+    if (!h) return EA_ERR_INVALID_ARG;
+    if (energy_by_slot && !h->energy_valid) { int rc = recompute_energy(h); if (rc != EA_OK) return rc; }
+    const size_t n = (size_t)h->R * h->nT;
+    if (spin_words)
+        CUDA_TRY(h, cudaMemcpyAsync(spin_words, h->P.spin, 4 * (size_t)h->nT * h->W * h->N, cudaMemcpyDeviceToHost, h->stream));
+    if (temp_of_slot) CUDA_TRY(h, cudaMemcpyAsync(temp_of_slot, h->P.tau, n, cudaMemcpyDeviceToHost, h->stream));
+    if (energy_by_slot) CUDA_TRY(h, cudaMemcpyAsync(energy_by_slot, h->P.E, 4 * n, cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    if (sweeps_done) *sweeps_done = h->g;
+    if (swap_rounds_done) *swap_rounds_done = h->nswap;
+    return EA_OK;
+}

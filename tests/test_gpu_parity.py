@@ -1,0 +1,139 @@
+"""GPU parity: the CUDA path (through the C ABI) vs the CPU oracle, bit for bit.
+
+Spins, temperature permutations, integer energies and overlaps must be identical
+(north_star: bit-exact).  Sizes are chosen so the oracle finishes in seconds while the
+GPU grid spans several blocks and ragged tails (R not a multiple of 32, L = 6, 12).
+"""
+import numpy as np
+import pytest
+
+from ea_inputs import CONFIGS, betas_for, random_couplings, random_spins, temperature_ladder
+from util_pack import by_temperature, words_to_spins
+
+pytestmark = pytest.mark.gpu
+
+
+def _pair(L, nT, R, betas, seed, kernel=0, r0=0):
+    from oracle import Oracle
+    from paper_1311_5582_b200 import EA
+    g = EA(L, nT, R, betas, seed, first_realization=r0, kernel=kernel)
+    o = Oracle(L, nT, R, betas, seed, r0=r0)
+    return g, o
+
+
+def _assert_same(g, o, tag=""):
+    st = g.get_state()
+    s_gpu = words_to_spins(st["spin_words"], g.L, g.R)
+    assert (s_gpu == o.spins_by_slot()).all(), f"spins differ {tag}"
+    tau, _ = o.perm()
+    assert (st["temp_of_slot"].astype(np.int32) == tau).all(), f"tau differs {tag}"
+    assert (st["energy_by_slot"] == o.energy_by_slot()).all(), f"energy by slot differs {tag}"
+    assert (g.energy() == o.energy()).all(), f"energy differs {tag}"
+    c = o.counters()
+    assert st["sweeps"] == c["sweeps"] and st["swap_rounds"] == c["swap_rounds"]
+
+
+KERNELS = [1]   # EA_KERNEL_GENERIC; fast paths are added by their own parametrisation below
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("L,nT,R,swap,ns", [
+    (2, 3, 5, 1, 40),
+    (4, 16, 1, 1, 200),        # config 1 shape
+    (6, 5, 33, 2, 25),         # ragged: 2 words, one nearly empty; odd n_temps
+    (8, 16, 32, 1, 30),        # config 2 shape
+    (12, 20, 64, 2, 6),        # config 3 shape (non power of two)
+    (16, 24, 96, 1, 3),        # config 4 shape, 3 words
+    (32, 4, 40, 1, 2),         # config 5 lattice, 2 words
+])
+def test_trajectory_matches_oracle(kernel, L, nT, R, swap, ns):
+    betas = 1.0 / temperature_ladder(nT, 0.5, 2.0)
+    g, o = _pair(L, nT, R, betas, 1000 + L, kernel)
+    acc_g, swp_g = g.get_tables()
+    acc_o, swp_o = o.tables()
+    assert (acc_g == acc_o).all() and (swp_g == swp_o).all()     # same tables on both sides
+    _assert_same(g, o, "after create")
+    done = 0
+    for chunk in (1, ns // 2, ns - 1 - ns // 2):
+        if chunk <= 0:
+            continue
+        g.sweep(chunk, swap); o.sweep(chunk, swap); done += chunk
+        _assert_same(g, o, f"after {done} sweeps")
+    assert (g.get_spins() == o.spins()).all()
+    pairs = [[0, R - 1], [R - 1, 0], [0, 0], [R // 2, -1]]
+    assert (g.overlap(pairs) == o.overlap(pairs)).all()
+    g.destroy()
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_set_couplings_set_spins_set_tables(kernel):
+    L, nT, R = 8, 6, 37
+    betas = 1.0 / temperature_ladder(nT, 0.7, 3.0)
+    g, o = _pair(L, nT, R, betas, 5, kernel)
+    J = random_couplings(R, L ** 3, 11)
+    s = random_spins(R, nT, L ** 3, 12)
+    g.set_couplings(J); o.set_couplings(J)
+    g.set_spins(s); o.set_spins(s)
+    _assert_same(g, o, "after set")
+    # tables handed to both paths as input data (north_star): give the oracle's to the GPU
+    acc, swp = o.tables()
+    g.set_tables(acc, swp)
+    g.sweep(12, 3); o.sweep(12, 3)
+    _assert_same(g, o, "after sweeps")
+    bad = J.copy(); bad[0, 0, 0] = 0
+    from paper_1311_5582_b200 import EAError
+    with pytest.raises(EAError):
+        g.set_couplings(bad)
+    _assert_same(g, o, "state unchanged after rejected input")
+    g.destroy()
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_ascending_betas_beta_zero_and_no_pt(kernel):
+    L, nT, R = 4, 5, 20
+    betas = np.array([0.0, 0.2, 0.5, 1.0, 3.0])          # ascending, includes beta = 0 and very cold
+    g, o = _pair(L, nT, R, betas, 77, kernel)
+    g.sweep(30, 1); o.sweep(30, 1)
+    _assert_same(g, o, "ascending betas")
+    g.sweep(10, 0); o.sweep(10, 0)
+    _assert_same(g, o, "no PT")
+    g.destroy()
+    g, o = _pair(L, 3, R, np.zeros(3), 78, kernel)       # beta = 0: everything accepted
+    s0 = o.spins_by_slot().copy()
+    g.sweep(1, 1); o.sweep(1, 1)
+    _assert_same(g, o, "beta 0")
+    assert (words_to_spins(g.get_state()["spin_words"], L, R) == -s0).all()
+    g.destroy()
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_word_sharding_reproduces_full_run(kernel):
+    # words simulated alone (first_realization = 32 w0) == those words of the full run
+    L, nT, R = 8, 8, 96
+    betas = 1.0 / temperature_ladder(nT, 0.6, 2.0)
+    from paper_1311_5582_b200 import EA
+    full = EA(L, nT, R, betas, 9, kernel=kernel)
+    part = EA(L, nT, 64, betas, 9, first_realization=32, kernel=kernel)
+    full.sweep(15, 1); part.sweep(15, 1)
+    a, b = full.get_state(), part.get_state()
+    assert (a["spin_words"][:, 1:3] == b["spin_words"]).all()
+    assert (a["temp_of_slot"][32:96] == b["temp_of_slot"]).all()
+    assert (full.energy()[32:96] == part.energy()).all()
+    full.destroy(); part.destroy()
+
+
+def test_argument_errors():
+    from paper_1311_5582_b200 import EA, EAError
+    b = np.array([1.0, 0.5])
+    with pytest.raises(EAError):
+        EA(5, 2, 1, b, 1)                      # odd L
+    with pytest.raises(EAError):
+        EA(4, 2, 1, np.array([1.0, np.nan]), 1)
+    with pytest.raises(EAError):
+        EA(4, 3, 1, np.array([1.0, 0.5, 0.7]), 1)   # not monotone
+    g = EA(4, 2, 3, b, 1)
+    with pytest.raises(EAError):
+        g.sweep(-1, 1)
+    with pytest.raises(EAError):
+        g.overlap([[0, 3]])
+    g.destroy()
