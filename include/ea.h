@@ -129,6 +129,12 @@ int ea_get_kernel(ea_handle *h);
 /* Number of kernels this handle has launched so far. */
 int64_t ea_launch_count(ea_handle *h);
 
+/* Measurement helper: issue-rate microbenchmark on the current device.
+ * out[0] = LOP3 lane-operations per second (ALU pipe), out[1] = IMAD lane-operations per second
+ * (FMA pipe), out[2] = a 1:1 LOP3/IMAD mix, out[3] = number of SMs.  The roofline denominator
+ * of the sweep kernel is out[0]. */
+int ea_measure_int_peak(void *cuda_stream, double *out /* [4] */);
+
 /* Message for the last failure on h (h = NULL: last ea_create* failure on this thread). */
 const char *ea_last_error(const ea_handle *h);
 

@@ -7,7 +7,7 @@ There is no CPU fallback: importing works without a GPU (so the symbol table can
 checked), creating a simulation does not.
 """
 from .binding import (EA, EA_KERNEL_AUTO, EA_KERNEL_GENERIC, EA_KERNEL_RESIDENT, EA_KERNEL_TILED,
-                      EAError, exported_symbols, lib, library_path)
+                      EAError, exported_symbols, lib, library_path, measure_int_peak)
 
-__all__ = ["EA", "EAError", "lib", "library_path", "exported_symbols", "EA_KERNEL_AUTO",
+__all__ = ["EA", "EAError", "lib", "library_path", "exported_symbols", "measure_int_peak", "EA_KERNEL_AUTO",
            "EA_KERNEL_GENERIC", "EA_KERNEL_RESIDENT", "EA_KERNEL_TILED"]

@@ -16,7 +16,7 @@ _SYMBOLS = [
     "ea_create", "ea_workspace_bytes", "ea_create_ex", "ea_destroy", "ea_set_couplings",
     "ea_set_spins", "ea_set_tables", "ea_get_tables", "ea_sweep", "ea_synchronize", "ea_energy",
     "ea_overlap", "ea_get_spins", "ea_get_state", "ea_set_kernel", "ea_get_kernel",
-    "ea_launch_count", "ea_last_error",
+    "ea_launch_count", "ea_last_error", "ea_measure_int_peak",
 ]
 
 
@@ -65,6 +65,8 @@ def lib():
     l.ea_launch_count.argtypes = [vp]
     l.ea_last_error.restype = C.c_char_p
     l.ea_last_error.argtypes = [vp]
+    l.ea_measure_int_peak.restype = i32
+    l.ea_measure_int_peak.argtypes = [vp, vp]
     _lib = l
     return l
 
@@ -181,3 +183,12 @@ class EA:
 
     def launch_count(self):
         return int(self._l.ea_launch_count(self.h))
+
+
+def measure_int_peak(stream=None):
+    """ea_measure_int_peak: dict of measured integer issue rates (lane-ops/s)."""
+    out = (C.c_double * 4)()
+    rc = lib().ea_measure_int_peak(stream, out)
+    if rc != 0:
+        raise EAError(rc, "ea_measure_int_peak failed")
+    return {"lop3": out[0], "imad": out[1], "mix": out[2], "sms": int(out[3])}

@@ -3,6 +3,7 @@
 // ea_generic.cuh / ea_resident.cuh / ea_tiled.cuh.  Shares nothing with oracle/.
 #include "../../include/ea.h"
 
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -12,6 +13,7 @@
 #include "ea_generic.cuh"
 #include "ea_resident.cuh"
 #include "ea_tiled.cuh"
+#include "ea_peak.cuh"
 
 using ea::Params;
 
@@ -31,6 +33,9 @@ struct ea_handle {
     uint8_t *d_swp_kind = nullptr;
     uint32_t *d_swp_val = nullptr;
     size_t swp_val_cap = 0;
+    uint32_t *d_bucket = nullptr;      // fast rank table (ea_resident.cuh)
+    int n_bucket = 0, key_lo = 0, key_hi = 0, key_shift = 0;
+    bool fast_rank = false;
     uint64_t g = 0, nswap = 0;
     bool energy_valid = false;
     int kernel_sel = EA_KERNEL_AUTO;
@@ -55,8 +60,9 @@ static int fail(const ea_handle *h, int code, const std::string &msg)
 
 // ---------------------------------------------------------------- workspace layout
 namespace {
+constexpr int kMaxBucket = 2048;
 struct Layout {
-    size_t spin, coup, lt, tau, sigma, E, thr32, swp_lo, swp_cnt, swp_off, swp_kind, swp_val, total;
+    size_t spin, coup, lt, tau, sigma, E, thr32, swp_lo, swp_cnt, swp_off, swp_kind, swp_val, bucket, total;
     size_t swp_val_cap;
 };
 size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
@@ -85,6 +91,7 @@ Layout make_layout(int L, int nT, int R)
     o.swp_kind = take(2 * (size_t)nT);
     o.swp_val_cap = (size_t)(nT > 1 ? nT - 1 : 0) * (3 * N + 1);
     o.swp_val = take(4 * (o.swp_val_cap ? o.swp_val_cap : 1));
+    o.bucket = take(4 * (size_t)kMaxBucket);
     o.total = off;
     return o;
 }
@@ -98,6 +105,66 @@ const uint64_t TWO32 = (uint64_t)1 << 32;
 
 void launch_cfg(int64_t n, int block, int &grid) { grid = (int)((n + block - 1) / block); }
 }  // namespace
+
+
+// ---------------------------------------------------------------- fast rank table
+// Buckets of the draw u by its leading bits: key(u) = bits of (float)u (truncating conversion)
+// >> (23 - MB) = exponent and MB mantissa bits.  For every bucket whose u-interval holds at
+// most one threshold per class, the entry stores 4 * rank at the interval's lower edge for the
+// classes n_sat = 4,5,6 (bytes 0,1,2); other buckets (and u < 2^8) carry bit 31 = "use the
+// exact search".  MB is the smallest of 3..6 that leaves < 1e-5 of the draws on the slow path.
+static bool build_bucket_table(const std::vector<uint32_t> &thr32, const int z[3], int nT,
+                               std::vector<uint32_t> &tab, int &key_lo, int &key_hi, int &key_shift)
+{
+    if (nT > 63) return false;
+    const int LOWEXP = 8;
+    uint32_t umax = 0;
+    for (int c = 0; c < 3; ++c)
+        if (z[c] < nT) umax = std::max(umax, thr32[(size_t)c * (nT + 1) + nT - 1]);
+    for (int MB = 3; MB <= 6; ++MB) {
+        auto key_of = [&](uint32_t u) -> int {
+            if (u == 0) return 0;
+            int e = 31;
+            while (!((u >> e) & 1u)) --e;
+            const uint32_t mant = e >= MB ? (u >> (e - MB)) & ((1u << MB) - 1) : (u << (MB - e)) & ((1u << MB) - 1);
+            return ((e + 127) << MB) | (int)mant;
+        };
+        const int klo = key_of(1u << LOWEXP) - 1;
+        const int khi = std::max(key_of(umax) + 1, klo + 1);
+        const int n = khi - klo + 1;
+        if (n > kMaxBucket) continue;
+        std::vector<uint32_t> t((size_t)n);
+        t[0] = 0x80000000u;
+        double slow_mass = std::ldexp(1.0, LOWEXP - 32);
+        for (int K = klo + 1; K < khi; ++K) {
+            const int e = (K >> MB) - 127;
+            const uint64_t m = (uint64_t)(K & ((1 << MB) - 1));
+            const uint64_t lo_u = (((uint64_t)1 << MB) | m) << (e - MB);
+            const uint64_t hi_u = lo_u + ((uint64_t)1 << (e - MB)) - 1;
+            uint32_t entry = 0;
+            bool slow = false;
+            for (int c = 0; c < 3; ++c) {
+                const uint32_t *col = thr32.data() + (size_t)c * (nT + 1);
+                int nlo = z[c], cnt = 0;
+                for (int i = z[c]; i < nT; ++i) {
+                    if ((uint64_t)col[i] < lo_u) nlo = i + 1;
+                    else if ((uint64_t)col[i] < hi_u) ++cnt;
+                }
+                if (cnt > 1) slow = true;
+                entry |= (uint32_t)(4 * nlo) << (8 * c);
+            }
+            if (slow) { entry |= 0x80000000u; slow_mass += (double)(hi_u - lo_u + 1) / 4294967296.0; }
+            t[(size_t)(K - klo)] = entry;
+        }
+        t[(size_t)(khi - klo)] = (uint32_t)(4 * nT) * 0x010101u;
+        if (slow_mass < 1e-5 || MB == 6) {
+            if (slow_mass > 1e-3) return false;
+            tab = t; key_lo = klo; key_hi = khi; key_shift = 23 - MB;
+            return true;
+        }
+    }
+    return false;
+}
 
 // ---------------------------------------------------------------- tables -> device form
 // acc: per class c = 4,5,6 a column sorted coldest-first ("pos" order), stored as thr-1 with
@@ -166,6 +233,15 @@ static int upload_tables(ea_handle *h, const std::vector<uint64_t> &acc, const s
     if (!val.empty())
         CUDA_TRY(h, cudaMemcpyAsync(h->d_swp_val, val.data(), 4 * val.size(), cudaMemcpyHostToDevice, s));
     CUDA_TRY(h, cudaStreamSynchronize(s));
+    {
+        std::vector<uint32_t> tab;
+        h->fast_rank = build_bucket_table(thr32, z, nT, tab, h->key_lo, h->key_hi, h->key_shift);
+        h->n_bucket = h->fast_rank ? (int)tab.size() : 0;
+        if (h->fast_rank) {
+            CUDA_TRY(h, cudaMemcpyAsync(h->d_bucket, tab.data(), 4 * tab.size(), cudaMemcpyHostToDevice, s));
+            CUDA_TRY(h, cudaStreamSynchronize(s));
+        }
+    }
     for (int c = 0; c < 3; ++c) h->P.z[c] = z[c];
     h->acc = acc;
     h->swp = swp;
@@ -263,6 +339,7 @@ extern "C" ea_handle *ea_create_ex(int L, int n_temps, int n_realizations, const
     P.swp_kind = h->d_swp_kind = (uint8_t *)(h->ws + lay.swp_kind);
     P.swp_val = h->d_swp_val = (uint32_t *)(h->ws + lay.swp_val);
     h->swp_val_cap = lay.swp_val_cap;
+    h->d_bucket = (uint32_t *)(h->ws + lay.bucket);
 
     // threshold tables in double on the host
     const int M = 3 * h->N / 2;
@@ -388,9 +465,101 @@ static int sweep_generic(ea_handle *h, int64_t n_sweeps, int swap_interval)
     return EA_OK;
 }
 
+
+// ---------------------------------------------------------------- resident path (L = 8, 16)
+namespace {
+struct ResPlan { bool ok; int C, S, G; size_t smem; };
+
+size_t resident_smem(const ea_handle *h, int S, int NW)
+{
+    const size_t N = (size_t)h->N, nT = (size_t)h->nT, LTS = nT + 1;
+    return 4 * ((size_t)S * N + (size_t)S * LTS + 3 * LTS + (size_t)h->n_bucket + nT * 32 +
+                (size_t)S * ea::kResPlanes * NW) + 64 * nT + 16;
+}
+
+ResPlan plan_resident(const ea_handle *h)
+{
+    ResPlan pl{false, 1, 0, 1, 0};
+    if (h->L != 8 && h->L != 16) return pl;
+    const int NQ = h->N / 8, NW = NQ / 32;
+    const size_t cap = 227 * 1024;
+    int C = 0;
+    for (int c = 1; c <= 8; ++c) {
+        const int S = (h->nT + c - 1) / c;
+        if (resident_smem(h, S, NW) <= cap) { C = c; break; }
+    }
+    if (!C) return pl;
+    // small problems: spread the slots over more SMs (cluster sizes 2, 4, 8)
+    while (C < 8 && (int64_t)h->W * C * 2 <= h->sm_count && (h->nT + 2 * C - 1) / (2 * C) >= 1 && 2 * C <= h->nT)
+        C *= 2;
+    pl.C = C;
+    pl.S = (h->nT + C - 1) / C;
+    pl.G = 1;
+    if (h->L == 8) { pl.G = 8; while (pl.G > 1 && pl.G > pl.S) pl.G >>= 1; }
+    pl.smem = resident_smem(h, pl.S, NW);
+    pl.ok = true;
+    return pl;
+}
+
+template <int L, int G>
+cudaError_t launch_resident_t(const ea_handle *h, const ea::ResArgs &A, const ResPlan &pl, bool fast)
+{
+    auto kern = fast ? ea::k_resident<L, G, true> : ea::k_resident<L, G, false>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem);
+    if (e != cudaSuccess) return e;
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3((unsigned)(h->W * pl.C));
+    cfg.blockDim = dim3((unsigned)(ea::ResGeom<L>::NQ * G));
+    cfg.dynamicSmemBytes = pl.smem;
+    cfg.stream = h->stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = (unsigned)pl.C;
+    at[0].val.clusterDim.y = 1;
+    at[0].val.clusterDim.z = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, A);
+}
+}  // namespace
+
+static int sweep_resident(ea_handle *h, int64_t n_sweeps, int swap_interval)
+{
+    const ResPlan pl = plan_resident(h);
+    if (!pl.ok) return fail(h, EA_ERR_UNSUPPORTED, "resident kernel: shape not supported");
+    int64_t left = n_sweeps;
+    while (left > 0) {
+        const int chunk = (int)std::min<int64_t>(left, 1 << 30);
+        ea::ResArgs A{};
+        A.P = h->P;
+        A.g0 = (uint32_t)h->g;
+        A.n_sweeps = chunk;
+        A.swap_interval = swap_interval;
+        A.nswap0 = (uint32_t)h->nswap;
+        A.C = pl.C; A.S = pl.S;
+        A.bucket = h->d_bucket; A.n_bucket = h->n_bucket;
+        A.key_lo = h->key_lo; A.key_hi = h->key_hi; A.key_shift = h->key_shift;
+        cudaError_t e = cudaErrorInvalidValue;
+        const bool fast = h->fast_rank;
+        if (h->L == 16) e = launch_resident_t<16, 1>(h, A, pl, fast);
+        else if (pl.G == 8) e = launch_resident_t<8, 8>(h, A, pl, fast);
+        else if (pl.G == 4) e = launch_resident_t<8, 4>(h, A, pl, fast);
+        else if (pl.G == 2) e = launch_resident_t<8, 2>(h, A, pl, fast);
+        else e = launch_resident_t<8, 1>(h, A, pl, fast);
+        if (e != cudaSuccess) return fail(h, EA_ERR_CUDA, std::string("resident launch: ") + cudaGetErrorString(e));
+        h->launches++;
+        if (swap_interval > 0) h->nswap += (h->g + (uint64_t)chunk) / (uint64_t)swap_interval - h->g / (uint64_t)swap_interval;
+        h->g += (uint64_t)chunk;
+        left -= chunk;
+    }
+    h->energy_valid = true;
+    return EA_OK;
+}
+
 static int pick_kernel(const ea_handle *h)
 {
     if (h->kernel_sel != EA_KERNEL_AUTO) return h->kernel_sel;
+    if (plan_resident(h).ok) return EA_KERNEL_RESIDENT;
     return EA_KERNEL_GENERIC;
 }
 
@@ -398,6 +567,7 @@ extern "C" int ea_set_kernel(ea_handle *h, int kernel)
 {
     if (!h) return EA_ERR_INVALID_ARG;
     if (kernel == EA_KERNEL_AUTO || kernel == EA_KERNEL_GENERIC) { h->kernel_sel = kernel; return EA_OK; }
+    if (kernel == EA_KERNEL_RESIDENT && plan_resident(h).ok) { h->kernel_sel = kernel; return EA_OK; }
     return fail(h, EA_ERR_UNSUPPORTED, "ea_set_kernel: kernel not available for this shape");
 }
 extern "C" int ea_get_kernel(ea_handle *h) { return h ? pick_kernel(h) : EA_ERR_INVALID_ARG; }
@@ -407,6 +577,7 @@ extern "C" int ea_sweep(ea_handle *h, int64_t n_sweeps, int swap_interval)
     if (!h || n_sweeps < 0 || swap_interval < 0) return fail(h, EA_ERR_INVALID_ARG, "ea_sweep: bad argument");
     if (h->g + (uint64_t)n_sweeps > 0xFFFFFFFFull) return fail(h, EA_ERR_RANGE, "ea_sweep: sweep counter would pass 2^32-1");
     if (n_sweeps == 0) return EA_OK;
+    if (pick_kernel(h) == EA_KERNEL_RESIDENT) return sweep_resident(h, n_sweeps, swap_interval);
     return sweep_generic(h, n_sweeps, swap_interval);
 }
 
@@ -482,4 +653,40 @@ extern "C" int ea_get_state(ea_handle *h, uint32_t *spin_words, uint8_t *temp_of
     if (sweeps_done) *sweeps_done = h->g;
     if (swap_rounds_done) *swap_rounds_done = h->nswap;
     return EA_OK;
+}
+
+// ---------------------------------------------------------------- measurement helper
+extern "C" int ea_measure_int_peak(void *cuda_stream, double *out)
+{
+    if (!out) return EA_ERR_INVALID_ARG;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return EA_ERR_CUDA;
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    uint32_t *d = nullptr;
+    if (cudaMalloc((void **)&d, 256) != cudaSuccess) return EA_ERR_ALLOC;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    const int iters = 4000, blocks = sms * 8, threads = 256;
+    const double lane_ops = (double)blocks * threads * iters * 64.0;
+    for (int mode = 0; mode < 3; ++mode) {
+        float best = 1e30f;
+        for (int rep = 0; rep < 4; ++rep) {
+            cudaEventRecord(e0, s);
+            if (mode == 0) ea::k_int_peak<0><<<blocks, threads, 0, s>>>(d, iters, 0x9E3779B9u, 0x7F4A7C15u);
+            if (mode == 1) ea::k_int_peak<1><<<blocks, threads, 0, s>>>(d, iters, 0x9E3779B9u, 0x7F4A7C15u);
+            if (mode == 2) ea::k_int_peak<2><<<blocks, threads, 0, s>>>(d, iters, 0x9E3779B9u, 0x7F4A7C15u);
+            cudaEventRecord(e1, s);
+            cudaEventSynchronize(e1);
+            float ms = 0.f;
+            cudaEventElapsedTime(&ms, e0, e1);
+            if (rep > 0 && ms < best) best = ms;
+        }
+        out[mode] = lane_ops / (best * 1e-3);
+    }
+    out[3] = (double)sms;
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaError_t e = cudaGetLastError();
+    cudaFree(d);
+    return e == cudaSuccess ? EA_OK : EA_ERR_CUDA;
 }

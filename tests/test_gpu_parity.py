@@ -33,7 +33,12 @@ def _assert_same(g, o, tag=""):
     assert st["sweeps"] == c["sweeps"] and st["swap_rounds"] == c["swap_rounds"]
 
 
-KERNELS = [1]   # EA_KERNEL_GENERIC; fast paths are added by their own parametrisation below
+KERNELS = [1, 2]   # EA_KERNEL_GENERIC, EA_KERNEL_RESIDENT (L = 8, 16 only)
+
+
+def _skip_unsupported(kernel, L):
+    if kernel == 2 and L not in (8, 16):
+        pytest.skip("resident kernel supports L = 8, 16")
 
 
 @pytest.mark.parametrize("kernel", KERNELS)
@@ -45,8 +50,12 @@ KERNELS = [1]   # EA_KERNEL_GENERIC; fast paths are added by their own parametri
     (12, 20, 64, 2, 6),        # config 3 shape (non power of two)
     (16, 24, 96, 1, 3),        # config 4 shape, 3 words
     (32, 4, 40, 1, 2),         # config 5 lattice, 2 words
+    (8, 6, 40, 3, 14),         # cluster with an empty block, swap every 3rd sweep
+    (16, 5, 33, 1, 4),         # odd n_temps, ragged words
+    (8, 33, 20, 1, 8),         # more temperatures than fit one block group
 ])
 def test_trajectory_matches_oracle(kernel, L, nT, R, swap, ns):
+    _skip_unsupported(kernel, L)
     betas = 1.0 / temperature_ladder(nT, 0.5, 2.0)
     g, o = _pair(L, nT, R, betas, 1000 + L, kernel)
     acc_g, swp_g = g.get_tables()
@@ -90,7 +99,7 @@ def test_set_couplings_set_spins_set_tables(kernel):
 
 @pytest.mark.parametrize("kernel", KERNELS)
 def test_ascending_betas_beta_zero_and_no_pt(kernel):
-    L, nT, R = 4, 5, 20
+    L, nT, R = (8 if kernel == 2 else 4), 5, 20
     betas = np.array([0.0, 0.2, 0.5, 1.0, 3.0])          # ascending, includes beta = 0 and very cold
     g, o = _pair(L, nT, R, betas, 77, kernel)
     g.sweep(30, 1); o.sweep(30, 1)
@@ -136,4 +145,27 @@ def test_argument_errors():
         g.sweep(-1, 1)
     with pytest.raises(EAError):
         g.overlap([[0, 3]])
+    g.destroy()
+
+
+def test_kernels_interleave_on_one_handle():
+    # generic and resident kernels continue each other's state exactly
+    L, nT, R = 16, 8, 64
+    betas = 1.0 / temperature_ladder(nT, 0.7, 2.0)
+    g, o = _pair(L, nT, R, betas, 31)
+    for kernel, n, swap in ((2, 3, 1), (1, 2, 1), (2, 4, 2), (1, 1, 0), (2, 2, 1)):
+        g.set_kernel(kernel)
+        assert g.get_kernel() == kernel
+        g.sweep(n, swap); o.sweep(n, swap)
+        _assert_same(g, o, f"kernel {kernel}")
+    g.destroy()
+
+
+def test_auto_picks_resident_for_L16():
+    from paper_1311_5582_b200 import EA
+    g = EA(16, 4, 32, np.array([1.0, 0.9, 0.8, 0.7]), 1)
+    assert g.get_kernel() == 2
+    g.destroy()
+    g = EA(12, 4, 32, np.array([1.0, 0.9, 0.8, 0.7]), 1)
+    assert g.get_kernel() == 1
     g.destroy()
