@@ -1,0 +1,280 @@
+#!/usr/bin/env python
+"""bench.py -- ps per spin-flip attempt (paper Eq. 2) on BASELINE.json's
+headline workload (config 4: L=16, 2048 realizations x 24 temperatures, PT every sweep),
+through the C ABI of libea_b200.so.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--sweeps-per-step 5000]
+  python bench.py --impl reference ...      # the CPU oracle, as it stands, on the host cores
+
+A *step* = `sweeps_per_step` full checkerboard sweeps, each followed by a PT round (config's
+swap_interval), of the whole workload: every row of SURVEY.md section 8(a) on the hot path.
+One JSON line on stdout (rank 0).  Details: DESIGN.md section 8.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+from ea_inputs import CONFIGS, betas_for  # noqa: E402
+
+METRIC = "ps per spin-flip attempt"
+UNIT = "ps/attempt"
+# ALU-pipe (LOP3/IADD/SHF/ISETP/SEL class) lane-operations the method needs per word update
+# (32 attempts), derived in DESIGN.md section 8; Philox's 5 IMAD.WIDE per update run on the
+# FMA pipe and are not counted here.
+ALU_OPS_PER_WORD_UPDATE = 43.0
+PAPER_PS = 33.5   # GTX 580, PT every 10 sweeps: context, another workload
+
+
+def _clock_sampler(stop, out):
+    q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+    dev = os.environ.get("LOCAL_RANK", "0")
+    while not stop.is_set():
+        try:
+            r = subprocess.run(["nvidia-smi", "-i", dev, f"--query-gpu={q}", "--format=csv,noheader,nounits"],
+                               capture_output=True, text=True, timeout=5)
+            if r.returncode == 0 and r.stdout.strip():
+                out.append([x.strip() for x in r.stdout.strip().split(",")])
+        except Exception:
+            pass
+        stop.wait(0.1)
+
+
+def _clock_summary(samples):
+    sm, mx, reasons = [], [], set()
+    names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+    for s in samples:
+        try:
+            sm.append(float(s[1])); mx.append(float(s[2]))
+        except Exception:
+            continue
+        for name, v in zip(names, s[5:9]):
+            if v.lower().startswith("active"):
+                reasons.add(name)
+    if not sm:
+        return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+    return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "reasons": sorted(reasons),
+            "samples": len(sm)}
+
+
+# ------------------------------------------------------------------ CPU oracle legs
+def _oracle_worker(args):
+    L, nT, betas, seed, r0, sweeps, swap = args
+    from oracle import Oracle
+    o = Oracle(L, nT, 32, betas, seed, r0=r0)
+    t = time.perf_counter()
+    o.sweep(sweeps, swap)
+    return time.perf_counter() - t
+
+
+def oracle_sample(cfg, words, sweeps, procs):
+    """Time the oracle, as it stands, on `words` realization words of cfg (one word = 32
+    realizations, all temperatures) for `sweeps` sweeps, `procs` processes (one word each at a
+    time).  Returns (ps per attempt over the wall time, wall seconds)."""
+    import multiprocessing as mp
+    from oracle import build_oracle
+    build_oracle()
+    betas = betas_for(cfg)
+    jobs = [(cfg.L, cfg.n_temps, betas, cfg.seed, 32 * w, sweeps, cfg.swap_interval) for w in range(words)]
+    t = time.perf_counter()
+    if procs == 1:
+        for j in jobs:
+            _oracle_worker(j)
+    else:
+        with mp.get_context("fork").Pool(procs) as pool:
+            pool.map(_oracle_worker, jobs, chunksize=1)
+    wall = time.perf_counter() - t
+    attempts = words * 32 * cfg.n_temps * cfg.N * sweeps
+    return wall * 1e12 / attempts, wall
+
+
+def run_reference(a, cfg):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    cores = len(os.sched_getaffinity(0))
+    words = min(cores, cfg.W)
+    sweeps = max(1, int(1.5e8 / (32 * cfg.n_temps * cfg.N)))      # ~4 s of one core per word
+    for _ in range(a.warmup):
+        oracle_sample(cfg, words, 1, words)
+    vals, walls = [], []
+    for _ in range(a.steps):
+        v, wsec = oracle_sample(cfg, words, sweeps, words)
+        vals.append(v); walls.append(wsec)
+    value = float(np.mean(vals))
+    sample = f"{words} of {cfg.W} words (32 realizations x {cfg.n_temps} temperatures each) x {sweeps} sweeps per step"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": a.gpus,
+        "steps": a.steps, "warmup": a.warmup, "ms_per_step": float(np.mean(walls)) * 1e3,
+        "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "int8 spins / u32 draws",
+        "data": "synthetic", "config": {"workload": cfg.name, "L": cfg.L, "n_temps": cfg.n_temps,
+                                        "realizations": cfg.R, "swap_interval": cfg.swap_interval,
+                                        "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": words, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+# ------------------------------------------------------------------ CUDA arm
+def run_cuda(a, cfg):
+    import torch
+    import torch.distributed as dist
+    from paper_1311_5582_b200 import EA, measure_int_peak
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    betas = betas_for(cfg)
+    sps = a.sweeps_per_step
+    # weak scaling: every rank owns cfg.R realizations; rank r simulates global words r*W..
+    sim = EA(cfg.L, cfg.n_temps, cfg.R, betas, cfg.seed, first_realization=rank * cfg.W * 32)
+    kernel = sim.get_kernel()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
+
+    def flush_l2():
+        flush.add_(1)
+
+    # ---- kernel-resident timing: state in HBM/SMEM, no host buffers
+    for _ in range(a.warmup):
+        sim.sweep(sps, cfg.swap_interval)
+    barrier()
+    samples, stop = [], threading.Event()
+    th = threading.Thread(target=_clock_sampler, args=(stop, samples), daemon=True)
+    th.start()
+    launches0 = sim.launch_count()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(a.steps)]
+    barrier()
+    for e0, e1 in ev:
+        flush_l2()
+        e0.record()
+        sim.sweep(sps, cfg.swap_interval)
+        e1.record()
+    barrier()
+    stop.set(); th.join()
+    launches = sim.launch_count() - launches0
+    step_ms = [e0.elapsed_time(e1) for e0, e1 in ev]
+    total_ms = float(sum(step_ms))
+    if world > 1:
+        t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    attempts_step = cfg.attempts_per_sweep * sps * world
+    value = total_ms * 1e9 / (attempts_step * a.steps)            # ms -> ps
+
+    # ---- end to end through the C ABI with HOST buffers: upload couplings (pinned int8),
+    #      run the step, read the energies back
+    from ea_inputs import random_couplings
+    Jpin = torch.empty((cfg.R, 3, cfg.N), dtype=torch.int8).pin_memory()
+    Jpin.numpy()[...] = random_couplings(cfg.R, cfg.N, 1000 + rank)
+    Jnp = Jpin.numpy()
+    e2e_steps = max(2, min(a.steps, 3))
+    sim.set_couplings(Jnp); sim.sweep(sps, cfg.swap_interval); sim.energy()
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        sim.set_couplings(Jnp)
+        sim.sweep(sps, cfg.swap_interval)
+        E = sim.energy()
+    barrier()
+    e2e_ms = (time.perf_counter() - t0) * 1e3
+    if world > 1:
+        t = torch.tensor([e2e_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_ms = float(t.item())
+    e2e_value = e2e_ms * 1e9 / (attempts_step * e2e_steps)
+    Rp = 32 * cfg.W
+    h2d = int(Jnp.nbytes)
+    d2h = int(Rp * cfg.n_temps * 4 + Rp * cfg.n_temps)            # energies by slot + sigma
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline: the sweep kernel is ALU-pipe bound
+    peak = measure_int_peak(torch.cuda.current_stream().cuda_stream)
+    # resident kernel: one launch per step, so the step time IS the kernel's launch duration;
+    # generic path: the step is sweep + energy + swap launches and the figure is for the step.
+    alu_ops_per_step = ALU_OPS_PER_WORD_UPDATE * cfg.n_temps * cfg.W * cfg.N * sps
+    achieved = alu_ops_per_step / (float(np.mean(step_ms)) * 1e-3)
+    roofline = {"bound": "alu", "achieved": achieved / 1e12, "peak": peak["lop3"] / 1e12, "unit": "Tlaneop/s",
+                "frac": achieved / peak["lop3"], "traffic": None,
+                "note": "ALU-pipe lane-ops: %.0f per word update (DESIGN.md s8) / measured LOP3 issue peak "
+                        "(ea_measure_int_peak, same process); IMAD peak %.2f, LOP3+IMAD mix %.2f Tlaneop/s"
+                        % (ALU_OPS_PER_WORD_UPDATE, peak["imad"] / 1e12, peak["mix"] / 1e12)}
+
+    # ---- CPU oracle on the host cores: bounded sample of the same workload
+    cores = len(os.sched_getaffinity(0))
+    words = min(cores, cfg.W)
+    o_sweeps = max(1, int(4.0e8 / (32 * cfg.n_temps * cfg.N)))     # ~10 s per core
+    cpu_ps, cpu_wall = oracle_sample(cfg, words, o_sweeps, words)
+    sample = f"{words} of {cfg.W} words (32 realizations x {cfg.n_temps} temperatures each) x {o_sweeps} sweeps, {cpu_wall:.1f} s wall"
+
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": a.steps, "warmup": a.warmup,
+        "ms_per_step": total_ms / a.steps, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
+        "dtype": "u32 bit-sliced words (32 realizations each), u32 Philox draws", "data": "synthetic",
+        "config": {"workload": cfg.name, "L": cfg.L, "n_temps": cfg.n_temps, "realizations_per_gpu": cfg.R,
+                   "swap_interval": cfg.swap_interval, "sweeps_per_step": sps, "seed": cfg.seed,
+                   "kernel": {1: "generic", 2: "resident", 3: "tiled"}.get(kernel, str(kernel)),
+                   "l2": "flushed between timed steps (256 MiB write); state is re-read from HBM each step",
+                   "parallelism": f"shard by realization word x{world}, no collective"},
+        "clocks": _clock_summary(samples),
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "ms_per_step": e2e_ms / e2e_steps,
+                "what": "ea_set_couplings(host J, pinned) + ea_sweep + ea_energy(host E) per step"},
+        "gpu_launches": int(launches),
+        "roofline": roofline,
+        "cpu_baseline": {"value": cpu_ps, "unit": UNIT, "cores": words, "kind": "oracle", "sample": sample},
+        "context": {"paper_ps_per_attempt_gtx580": PAPER_PS, "step_ms": step_ms},
+    }
+    print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--config", type=int, default=4)
+    ap.add_argument("--sweeps-per-step", type=int, default=5000)
+    a = ap.parse_args()
+    a.warmup = max(a.warmup, 3) if a.impl == "cuda" else a.warmup
+    cfg = CONFIGS[a.config]
+    if a.impl == "reference":
+        run_reference(a, cfg)
+    else:
+        if int(os.environ.get("LOCAL_RANK", "0")) == 0:
+            from paper_1311_5582_b200.build import build_library
+            build_library()
+        run_cuda(a, cfg)
+
+
+if __name__ == "__main__":
+    main()

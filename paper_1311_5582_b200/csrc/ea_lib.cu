@@ -33,7 +33,7 @@ struct ea_handle {
     uint8_t *d_swp_kind = nullptr;
     uint32_t *d_swp_val = nullptr;
     size_t swp_val_cap = 0;
-    uint32_t *d_bucket = nullptr;      // fast rank table (ea_resident.cuh)
+    uint4 *d_bucket = nullptr;         // fast rank table (ea_resident.cuh), 16 B entries
     int n_bucket = 0, key_lo = 0, key_hi = 0, key_shift = 0;
     bool fast_rank = false;
     uint64_t g = 0, nswap = 0;
@@ -60,7 +60,7 @@ static int fail(const ea_handle *h, int code, const std::string &msg)
 
 // ---------------------------------------------------------------- workspace layout
 namespace {
-constexpr int kMaxBucket = 2048;
+constexpr int kMaxBucket = 1024;
 struct Layout {
     size_t spin, coup, lt, tau, sigma, E, thr32, swp_lo, swp_cnt, swp_off, swp_kind, swp_val, bucket, total;
     size_t swp_val_cap;
@@ -91,7 +91,7 @@ Layout make_layout(int L, int nT, int R)
     o.swp_kind = take(2 * (size_t)nT);
     o.swp_val_cap = (size_t)(nT > 1 ? nT - 1 : 0) * (3 * N + 1);
     o.swp_val = take(4 * (o.swp_val_cap ? o.swp_val_cap : 1));
-    o.bucket = take(4 * (size_t)kMaxBucket);
+    o.bucket = take(16 * (size_t)kMaxBucket);
     o.total = off;
     return o;
 }
@@ -114,7 +114,7 @@ void launch_cfg(int64_t n, int block, int &grid) { grid = (int)((n + block - 1) 
 // classes n_sat = 4,5,6 (bytes 0,1,2); other buckets (and u < 2^8) carry bit 31 = "use the
 // exact search".  MB is the smallest of 3..6 that leaves < 1e-5 of the draws on the slow path.
 static bool build_bucket_table(const std::vector<uint32_t> &thr32, const int z[3], int nT,
-                               std::vector<uint32_t> &tab, int &key_lo, int &key_hi, int &key_shift)
+                               std::vector<uint4> &tab, int &key_lo, int &key_hi, int &key_shift)
 {
     if (nT > 63) return false;
     const int LOWEXP = 8;
@@ -133,30 +133,30 @@ static bool build_bucket_table(const std::vector<uint32_t> &thr32, const int z[3
         const int khi = std::max(key_of(umax) + 1, klo + 1);
         const int n = khi - klo + 1;
         if (n > kMaxBucket) continue;
-        std::vector<uint32_t> t((size_t)n);
-        t[0] = 0x80000000u;
+        std::vector<uint4> t((size_t)n);
+        t[0] = make_uint4(0x80000000u, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu);
         double slow_mass = std::ldexp(1.0, LOWEXP - 32);
         for (int K = klo + 1; K < khi; ++K) {
             const int e = (K >> MB) - 127;
             const uint64_t m = (uint64_t)(K & ((1 << MB) - 1));
             const uint64_t lo_u = (((uint64_t)1 << MB) | m) << (e - MB);
             const uint64_t hi_u = lo_u + ((uint64_t)1 << (e - MB)) - 1;
-            uint32_t entry = 0;
+            uint32_t entry = 0, inb[3] = {0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu};
             bool slow = false;
             for (int c = 0; c < 3; ++c) {
                 const uint32_t *col = thr32.data() + (size_t)c * (nT + 1);
                 int nlo = z[c], cnt = 0;
                 for (int i = z[c]; i < nT; ++i) {
                     if ((uint64_t)col[i] < lo_u) nlo = i + 1;
-                    else if ((uint64_t)col[i] < hi_u) ++cnt;
+                    else if ((uint64_t)col[i] < hi_u) { if (!cnt) inb[c] = col[i]; ++cnt; }
                 }
                 if (cnt > 1) slow = true;
                 entry |= (uint32_t)(4 * nlo) << (8 * c);
             }
             if (slow) { entry |= 0x80000000u; slow_mass += (double)(hi_u - lo_u + 1) / 4294967296.0; }
-            t[(size_t)(K - klo)] = entry;
+            t[(size_t)(K - klo)] = make_uint4(entry, inb[0], inb[1], inb[2]);
         }
-        t[(size_t)(khi - klo)] = (uint32_t)(4 * nT) * 0x010101u;
+        t[(size_t)(khi - klo)] = make_uint4((uint32_t)(4 * nT) * 0x010101u, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu);
         if (slow_mass < 1e-5 || MB == 6) {
             if (slow_mass > 1e-3) return false;
             tab = t; key_lo = klo; key_hi = khi; key_shift = 23 - MB;
@@ -234,11 +234,11 @@ static int upload_tables(ea_handle *h, const std::vector<uint64_t> &acc, const s
         CUDA_TRY(h, cudaMemcpyAsync(h->d_swp_val, val.data(), 4 * val.size(), cudaMemcpyHostToDevice, s));
     CUDA_TRY(h, cudaStreamSynchronize(s));
     {
-        std::vector<uint32_t> tab;
+        std::vector<uint4> tab;
         h->fast_rank = build_bucket_table(thr32, z, nT, tab, h->key_lo, h->key_hi, h->key_shift);
         h->n_bucket = h->fast_rank ? (int)tab.size() : 0;
         if (h->fast_rank) {
-            CUDA_TRY(h, cudaMemcpyAsync(h->d_bucket, tab.data(), 4 * tab.size(), cudaMemcpyHostToDevice, s));
+            CUDA_TRY(h, cudaMemcpyAsync(h->d_bucket, tab.data(), 16 * tab.size(), cudaMemcpyHostToDevice, s));
             CUDA_TRY(h, cudaStreamSynchronize(s));
         }
     }
@@ -339,7 +339,7 @@ extern "C" ea_handle *ea_create_ex(int L, int n_temps, int n_realizations, const
     P.swp_kind = h->d_swp_kind = (uint8_t *)(h->ws + lay.swp_kind);
     P.swp_val = h->d_swp_val = (uint32_t *)(h->ws + lay.swp_val);
     h->swp_val_cap = lay.swp_val_cap;
-    h->d_bucket = (uint32_t *)(h->ws + lay.bucket);
+    h->d_bucket = (uint4 *)(h->ws + lay.bucket);
 
     // threshold tables in double on the host
     const int M = 3 * h->N / 2;
@@ -473,8 +473,10 @@ struct ResPlan { bool ok; int C, S, G; size_t smem; };
 size_t resident_smem(const ea_handle *h, int S, int NW)
 {
     const size_t N = (size_t)h->N, nT = (size_t)h->nT, LTS = nT + 1;
-    return 4 * ((size_t)S * N + (size_t)S * LTS + 3 * LTS + (size_t)h->n_bucket + nT * 32 +
-                (size_t)S * ea::kResPlanes * NW) + 64 * nT + 16;
+    (void)NW;
+    return 16 * (size_t)h->n_bucket +
+           4 * ((size_t)S * N + (size_t)S * LTS + 3 * LTS + 2 * nT * 32 + (size_t)S * 32 + 4 * nT +
+                nT * (size_t)ea::kSwapWin) + 64 * nT + 16;
 }
 
 ResPlan plan_resident(const ea_handle *h)
@@ -539,6 +541,10 @@ static int sweep_resident(ea_handle *h, int64_t n_sweeps, int swap_interval)
         A.C = pl.C; A.S = pl.S;
         A.bucket = h->d_bucket; A.n_bucket = h->n_bucket;
         A.key_lo = h->key_lo; A.key_hi = h->key_hi; A.key_shift = h->key_shift;
+        for (int r = 0; r < 10; ++r) {
+            A.rk[2 * r] = h->P.k0 + (uint32_t)r * 0x9E3779B9u;
+            A.rk[2 * r + 1] = h->P.k1 + (uint32_t)r * 0xBB67AE85u;
+        }
         cudaError_t e = cudaErrorInvalidValue;
         const bool fast = h->fast_rank;
         if (h->L == 16) e = launch_resident_t<16, 1>(h, A, pl, fast);

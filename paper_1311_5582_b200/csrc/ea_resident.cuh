@@ -25,11 +25,31 @@ struct ResArgs {
     int swap_interval;
     uint32_t nswap0;      // swap rounds done before this call
     int C, S;             // cluster size; slots per block (last block may own fewer)
-    const uint32_t *bucket;   // fast rank table (FAST variant), device memory
+    const uint4 *bucket;      // fast rank table (FAST variant), device memory, 16 B entries
+    uint32_t rk[20];          // Philox round keys (k0 + r*0x9E3779B9, k1 + r*0xBB67AE85), r = 0..9
     int n_bucket, key_lo, key_hi, key_shift;
 };
 
 constexpr int kResPlanes = 10;   // planes of a warp's per-slot satisfied-bond count (<= 768)
+
+// Philox4x32-10 with the ten round keys taken from kernel parameters (constant bank): the
+// key schedule costs no instruction in the loop.
+__device__ __forceinline__ uint4 philox_rk(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                           const uint32_t (&rk)[20])
+{
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint64_t p0 = (uint64_t)0xD2511F53u * c0;
+        const uint64_t p1 = (uint64_t)0xCD9E8D57u * c2;
+        const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ rk[2 * r];
+        const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ rk[2 * r + 1];
+        c1 = (uint32_t)p1;
+        c3 = (uint32_t)p0;
+        c0 = n0;
+        c2 = n2;
+    }
+    return make_uint4(c0, c1, c2, c3);
+}
 
 // ------------------------------------------------------------------ small bit-sliced adders
 __device__ __forceinline__ uint32_t mux(uint32_t a, uint32_t b, uint32_t m) { return (a & ~m) | (b & m); }
@@ -82,34 +102,35 @@ __device__ __forceinline__ Planes planes_after(const Planes &p, uint32_t acc)
 }
 
 // ------------------------------------------------------------------ rank of a draw
-// FAST: one look-up keyed by the leading bits of the draw (float exponent + key_shift
-// mantissa bits, truncating conversion) gives the rank at the bucket's lower edge for the
-// three classes; buckets hold at most one threshold per class, so one compare fixes it.
-// Entries with bit 31 set (several thresholds in the bucket, or draw < 2^8) take the exact
-// binary search.
+// FAST: one 128-bit look-up keyed by the leading bits of the draw (float exponent + MB
+// mantissa bits, truncating conversion).  Entry = { 4*rank at the bucket's lower edge for the
+// classes n_sat = 4,5,6 in bytes 0..2, flag in bit 31 ; thr4 ; thr5 ; thr6 } where thr_c is
+// the (threshold - 1) of class c that lies inside the bucket, or 0xFFFFFFFF if there is none.
+// Buckets hold at most one threshold per class, so rank = rank_lo + (thr_c < u).  Entries with
+// bit 31 set (several thresholds of one class in the bucket, or draw < 2^8) take the exact
+// binary search.  The table sits at shared-memory offset 0, so the look-up address is one LEA.
 struct RankCtx {
-    const uint32_t *thr;     // smem [3][LTS]
-    const uint32_t *bucket;  // smem
+    const uint32_t *thr;     // smem [3][LTS]  (exact search only)
+    const uint4 *bucket;     // smem, biased by -key_lo entries
     int LTS, nT, key_lo, key_hi, key_shift;
     int z0, z1, z2;
 };
 
-__device__ __forceinline__ uint32_t bucket_entry(const RankCtx &R, uint32_t u)
+__device__ __forceinline__ uint4 bucket_entry(const RankCtx &R, uint32_t u)
 {
     int key = (int)(__float_as_uint(__uint2float_rz(u)) >> R.key_shift);
-    key = min(max(key, R.key_lo), R.key_hi) - R.key_lo;
-    return R.bucket[key];
+    key = min(max(key, R.key_lo), R.key_hi);
+    return R.bucket[key];          // R.bucket is biased by -key_lo
 }
 
-__device__ __forceinline__ uint32_t accept_fast(const RankCtx &R, const uint32_t *lt, uint32_t u,
-                                                uint32_t e, const Planes &p)
+__device__ __forceinline__ uint32_t accept_fast(const uint32_t *lt, uint32_t u, const uint4 &e,
+                                                const Planes &p)
 {
-    const char *thr = (const char *)R.thr;
     const char *ltb = (const char *)lt;
-    uint32_t n4 = e & 0xFFu, n5 = (e >> 8) & 0xFFu, n6 = (e >> 16) & 0xFFu;   // rank * 4
-    n4 += (*(const uint32_t *)(thr + n4) < u) ? 4u : 0u;
-    n5 += (*(const uint32_t *)(thr + 4 * R.LTS + n5) < u) ? 4u : 0u;
-    n6 += (*(const uint32_t *)(thr + 8 * R.LTS + n6) < u) ? 4u : 0u;
+    uint32_t n4 = e.x & 0xFFu, n5 = __byte_perm(e.x, 0, 0x4441), n6 = __byte_perm(e.x, 0, 0x4442);
+    n4 += (e.y < u) ? 4u : 0u;
+    n5 += (e.z < u) ? 4u : 0u;
+    n6 += (e.w < u) ? 4u : 0u;
     return accept_mask(p, *(const uint32_t *)(ltb + n4), *(const uint32_t *)(ltb + n5),
                        *(const uint32_t *)(ltb + n6));
 }
@@ -140,21 +161,35 @@ struct ResGeom {
     static_assert(Lh % 4 == 0, "resident kernel needs L multiple of 8");
 };
 
-// Update the four sites of quad q (parity p) of one slot's lattice `sp` (smem, [2][Nh]).
-// Returns the post-update n_sat planes of the four sites through `fin` when ENERGY.
-template <int L, bool FAST, bool ENERGY>
-__device__ __forceinline__ void update_quad(uint32_t *sp, const uint32_t *lt, const RankCtx &R,
-                                            const QuadJ &J, int p, int s, int q, int qyp, int qym,
-                                            int qzp, int qzm, const uint4 rnd, Planes (&fin)[4])
+// New spin words of the four sites of quad q (parity p) of one slot's lattice `sp` (smem,
+// [2][Nh]); nothing is stored.  EXACT = false: ranks from the bucket table; *flag collects
+// bit 31 of the entries (set: the caller must redo the quad with EXACT = true).
+template <int L, bool EXACT, bool ENERGY>
+__device__ __forceinline__ uint4 quad_body(const uint32_t *sp, const uint32_t *lt, const RankCtx &R,
+                                           const QuadJ &J, int p, int s, int q, uint32_t offY, uint32_t offZ,
+                                           const uint4 rnd, Planes (&fin)[4], uint32_t *flag)
 {
     using Gm = ResGeom<L>;
-    uint4 *self_p = reinterpret_cast<uint4 *>(sp + p * Gm::Nh);
-    const uint4 *oth = reinterpret_cast<const uint4 *>(sp + (1 - p) * Gm::Nh);
-    const uint4 me = self_p[q];
-    const uint4 v = oth[q];
-    const uint4 yp = oth[qyp], ym = oth[qym], zp = oth[qzp], zm = oth[qzm];
+    // offY / offZ: byte offsets of the +-y / +-z neighbour quads inside a parity array, two
+    // 16-bit halves each (+ in the low half)
+    const char *self_b = reinterpret_cast<const char *>(sp + p * Gm::Nh);
+    const char *oth_b = reinterpret_cast<const char *>(sp + (1 - p) * Gm::Nh);
+    const uint4 me = *reinterpret_cast<const uint4 *>(self_b + 16 * q);
+    const uint4 v = *reinterpret_cast<const uint4 *>(oth_b + 16 * q);
+    const uint4 yp = *reinterpret_cast<const uint4 *>(oth_b + (offY & 0xFFFFu));
+    const uint4 ym = *reinterpret_cast<const uint4 *>(oth_b + (offY >> 16));
+    const uint4 zp = *reinterpret_cast<const uint4 *>(oth_b + (offZ & 0xFFFFu));
+    const uint4 zm = *reinterpret_cast<const uint4 *>(oth_b + (offZ >> 16));
     uint32_t ext = s ? v.x : v.w;
-    if (Gm::QR == 2) ext = __shfl_xor_sync(0xFFFFFFFFu, ext, 1);
+    if (Gm::QR == 2) {
+        if (EXACT) {   // divergent (rare) path: no shuffle, read the neighbour quad's word
+            const int row = q & ~1;
+            ext = s ? reinterpret_cast<const uint32_t *>(oth_b)[4 * (row + ((q + 1) & 1))]
+                    : reinterpret_cast<const uint32_t *>(oth_b)[4 * (row + ((q + 1) & 1)) + 3];
+        } else {
+            ext = __shfl_xor_sync(0xFFFFFFFFu, ext, 1);
+        }
+    }
     uint4 sh;   // the x neighbour that is not index-aligned: x+1 if s, x-1 otherwise
     sh.x = s ? v.y : ext;
     sh.y = s ? v.z : v.x;
@@ -168,33 +203,40 @@ __device__ __forceinline__ void update_quad(uint32_t *sp, const uint32_t *lt, co
     const uint32_t jys[4] = {J.jys.x, J.jys.y, J.jys.z, J.jys.w}, jym[4] = {J.jym.x, J.jym.y, J.jym.z, J.jym.w};
     const uint32_t jzs[4] = {J.jzs.x, J.jzs.y, J.jzs.z, J.jzs.w}, jzm[4] = {J.jzm.x, J.jzm.y, J.jzm.z, J.jzm.w};
     const uint32_t u[4] = {rnd.x, rnd.y, rnd.z, rnd.w};
-    Planes pl[4];
-    uint32_t e[4];
+    uint32_t out[4];
+    uint32_t fl = 0;
 #pragma unroll
     for (int l = 0; l < 4; ++l) {
-        pl[l] = nsat_planes(xor3(m[l], ja[l], va[l]), xor3(m[l], jb[l], vb[l]),
-                            xor3(m[l], jys[l], a_yp[l]), xor3(m[l], jym[l], a_ym[l]),
-                            xor3(m[l], jzs[l], a_zp[l]), xor3(m[l], jzm[l], a_zm[l]));
-        if (FAST) e[l] = bucket_entry(R, u[l]);
-    }
-    uint32_t acc[4];
-    if (FAST) {
-        if ((e[0] | e[1] | e[2] | e[3]) & 0x80000000u) {
-#pragma unroll
-            for (int l = 0; l < 4; ++l) acc[l] = accept_exact(R, lt, u[l], pl[l]);
+        const Planes pl = nsat_planes(xor3(m[l], ja[l], va[l]), xor3(m[l], jb[l], vb[l]),
+                                      xor3(m[l], jys[l], a_yp[l]), xor3(m[l], jym[l], a_ym[l]),
+                                      xor3(m[l], jzs[l], a_zp[l]), xor3(m[l], jzm[l], a_zm[l]));
+        uint32_t acc;
+        if (EXACT) {
+            acc = accept_exact(R, lt, u[l], pl);
         } else {
-#pragma unroll
-            for (int l = 0; l < 4; ++l) acc[l] = accept_fast(R, lt, u[l], e[l], pl[l]);
+            const uint4 e = bucket_entry(R, u[l]);
+            fl |= e.x;
+            acc = accept_fast(lt, u[l], e, pl);
         }
-    } else {
-#pragma unroll
-        for (int l = 0; l < 4; ++l) acc[l] = accept_exact(R, lt, u[l], pl[l]);
+        out[l] = m[l] ^ acc;
+        if (ENERGY) fin[l] = planes_after(pl, acc);
     }
-    self_p[q] = make_uint4(m[0] ^ acc[0], m[1] ^ acc[1], m[2] ^ acc[2], m[3] ^ acc[3]);
-    if (ENERGY) {
-#pragma unroll
-        for (int l = 0; l < 4; ++l) fin[l] = planes_after(pl[l], acc[l]);
-    }
+    if (!EXACT) *flag = fl;
+    return make_uint4(out[0], out[1], out[2], out[3]);
+}
+
+template <int L, bool FAST, bool ENERGY>
+__device__ __forceinline__ void update_quad(uint32_t *sp, const uint32_t *lt, const RankCtx &R,
+                                            const QuadJ &J, int p, int s, int q, uint32_t offY, uint32_t offZ,
+                                            const uint4 rnd, Planes (&fin)[4])
+{
+    using Gm = ResGeom<L>;
+    uint32_t flag = 0x80000000u;
+    uint4 res;
+    if (FAST) res = quad_body<L, false, ENERGY>(sp, lt, R, J, p, s, q, offY, offZ, rnd, fin, &flag);
+    // rare (or !FAST): redo the whole quad from shared memory with the exact search
+    if ((int)flag < 0) res = quad_body<L, true, ENERGY>(sp, lt, R, J, p, s, q, offY, offZ, rnd, fin, &flag);
+    reinterpret_cast<uint4 *>(sp + p * Gm::Nh)[q] = res;
 }
 
 // Couplings of quad q for parity p from global memory ([d][p][j], 3N words per word w).
@@ -285,11 +327,40 @@ __device__ __forceinline__ void warp_sum4(uint32_t (&en)[4][5], int lane, uint32
     }
 }
 
+__device__ __forceinline__ void cluster_arrive()
+{
+    asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void cluster_wait()
+{
+    asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+
+constexpr int kSwapWin = 64;   // swap thresholds for m in [-kSwapWin, -1] are staged in smem
+
+// Turn the warp's 10-plane satisfied-bond count of one slot (all 8 lanes of a group hold the
+// same planes) into integers and add them to the block's per-(slot, bit) accumulators: lane i
+// of the group takes realization bits i, i+8, i+16, i+24 (two 16-bit fields per word; the
+// shift-and-add runs on the FMA pipe).
+__device__ __forceinline__ void add_counts(const uint32_t (&tot)[kResPlanes], int i, int *acc_row)
+{
+    uint32_t lo = 0, hi = 0;
+#pragma unroll
+    for (int j = 0; j < kResPlanes; ++j) {
+        lo += ((tot[j] >> i) & 0x00010001u) * (1u << j);
+        hi += ((tot[j] >> (i + 8)) & 0x00010001u) * (1u << j);
+    }
+    atomicAdd(acc_row + i, (int)(lo & 0xFFFFu));
+    atomicAdd(acc_row + i + 16, (int)(lo >> 16));
+    atomicAdd(acc_row + i + 8, (int)(hi & 0xFFFFu));
+    atomicAdd(acc_row + i + 24, (int)(hi >> 16));
+}
+
 template <int L, int G, bool FAST>
 __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs A)
 {
     using Gm = ResGeom<L>;
-    constexpr int N = Gm::N, NQ = Gm::NQ, QR = Gm::QR, NT = NQ * G, NW = NQ / 32;
+    constexpr int N = Gm::N, NQ = Gm::NQ, QR = Gm::QR, NT = NQ * G;
     extern __shared__ __align__(16) uint32_t smem[];
     const Params &P = A.P;
     const int nT = P.nT, LTS = P.LTS, S = A.S, C = A.C;
@@ -297,16 +368,19 @@ __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs
     const int k0 = rank * S;
     const int nk = max(0, min(S, nT - k0));      // slots owned by this block
     const int tid = threadIdx.x, lane = tid & 31;
-    const int q = tid % NQ, sg = tid / NQ, wq = q >> 5;
+    const int q = tid % NQ, sg = tid / NQ;
 
-    uint32_t *sp = smem;                          // [S][2][Nh]
-    uint32_t *lt = sp + (size_t)S * N;            // [S][LTS]
-    uint32_t *thr = lt + S * LTS;                 // [3][LTS]
-    uint32_t *bucket = thr + 3 * LTS;             // [n_bucket]
-    int32_t *Eall = (int32_t *)(bucket + A.n_bucket);   // [nT][32]
-    uint32_t *wsum = (uint32_t *)(Eall + nT * 32);      // [S][kResPlanes][NW]
-    uint8_t *tau8 = (uint8_t *)(wsum + S * kResPlanes * NW);   // [32][nT]
-    uint8_t *sig8 = tau8 + 32 * nT;                             // [32][nT]
+    // shared memory: the rank table first (fixed offset 0), lattices next (16 B aligned)
+    uint4 *bucket = reinterpret_cast<uint4 *>(smem);                 // [n_bucket] 16 B entries
+    uint32_t *sp = smem + 4 * (size_t)A.n_bucket;                    // [S][2][Nh]
+    uint32_t *lt = sp + (size_t)S * N;                               // [S][LTS]
+    uint32_t *thr = lt + S * LTS;                                    // [3][LTS]
+    int32_t *Eall = (int32_t *)(thr + 3 * LTS);                      // [2][nT][32], by swap-round parity
+    int32_t *Eacc = Eall + 2 * nT * 32;                              // [S][32] satisfied-bond counts
+    int32_t *swm = Eacc + S * 32;                                    // [nT][4]: lo, cnt, off, kinds
+    uint32_t *swwin = (uint32_t *)(swm + 4 * nT);                    // [nT][kSwapWin] thresholds - 1
+    uint8_t *tau8 = (uint8_t *)(swwin + nT * kSwapWin);              // [32][nT]
+    uint8_t *sig8 = tau8 + 32 * nT;                                  // [32][nT]
 
     // ---- load state: lattices of my slots, tables, permutation of my 32 realizations
     for (int k = 0; k < nk; ++k) {
@@ -321,9 +395,16 @@ __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs
         tau8[a] = P.tau[(size_t)32 * w * nT + a];
         sig8[a] = P.sigma[(size_t)32 * w * nT + a];
     }
-    for (int a = tid; a < nT * 32; a += NT) {     // Eall[k][b] <- E[32w+b][k]
-        const int k = a >> 5, b = a & 31;
-        Eall[a] = P.E[(size_t)(32 * w + b) * nT + k];
+    for (int a = tid; a < S * 32; a += NT) Eacc[a] = 0;
+    for (int a = tid; a < 2 * nT * 32; a += NT) Eall[a] = P.E[(size_t)(32 * w + (a & 31)) * nT + ((a >> 5) % nT)];
+    for (int t = tid; t + 1 < nT; t += NT) {
+        swm[4 * t] = P.swp_lo[t]; swm[4 * t + 1] = P.swp_cnt[t]; swm[4 * t + 2] = P.swp_off[t];
+        swm[4 * t + 3] = (int)P.swp_kind[2 * t] | ((int)P.swp_kind[2 * t + 1] << 1);
+    }
+    for (int a = tid; a < (nT - 1) * kSwapWin; a += NT) {   // window m = -kSwapWin + i of row t
+        const int t = a / kSwapWin, m = -kSwapWin + a % kSwapWin;
+        const int lo = P.swp_lo[t], cnt = P.swp_cnt[t];
+        swwin[a] = (m >= lo && m < lo + cnt) ? P.swp_val[P.swp_off[t] + (m - lo)] : 0u;
     }
 
     // ---- per-thread geometry and couplings (registers, both parities)
@@ -334,13 +415,17 @@ __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs
     const uint32_t *cp = P.coup + (size_t)w * 3 * N;
     const QuadJ J0 = load_quad_j<L>(cp, 0, s0, q, qx, qym, qzm);
     const QuadJ J1 = load_quad_j<L>(cp, 1, 1 - s0, q, qx, qym, qzm);
+    uint32_t offY = (uint32_t)(16 * qyp) | ((uint32_t)(16 * qym) << 16);
+    uint32_t offZ = (uint32_t)(16 * qzp) | ((uint32_t)(16 * qzm) << 16);
+    asm volatile("" : "+r"(offY), "+r"(offZ));    // opaque: keep in registers, do not rematerialize
 
     RankCtx R;
-    R.thr = thr; R.bucket = bucket; R.LTS = LTS; R.nT = nT;
+    R.thr = thr; R.bucket = bucket - A.key_lo; R.LTS = LTS; R.nT = nT;
     R.key_lo = A.key_lo; R.key_hi = A.key_hi; R.key_shift = A.key_shift;
     R.z0 = P.z[0]; R.z1 = P.z[1]; R.z2 = P.z[2];
     const uint32_t gw = P.w0 + (uint32_t)w;
-    __syncthreads();
+    cg::cluster_group cl = cg::this_cluster();
+    if (C > 1) cl.sync(); else __syncthreads();   // every block's shared memory is initialised
 
     uint32_t nswap = A.nswap0;
     for (int it = 0; it < A.n_sweeps; ++it) {
@@ -350,100 +435,95 @@ __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs
         Planes fin[4];
         // ---------------- parity 0
         for (int kl = sg; kl < nk; kl += G) {
-            const uint4 rnd = philox4x32_10(g, (uint32_t)q, gw, (uint32_t)(k0 + kl), P.k0, P.k1);
-            update_quad<L, FAST, false>(sp + (size_t)kl * N, lt + kl * LTS, R, J0, 0, s0, q, qyp, qym, qzp,
-                                        qzm, rnd, fin);
+            const uint4 rnd = philox_rk(g, (uint32_t)q, gw, (uint32_t)(k0 + kl), A.rk);
+            update_quad<L, FAST, false>(sp + (size_t)kl * N, lt + kl * LTS, R, J0, 0, s0, q, offY, offZ, rnd, fin);
         }
         __syncthreads();
         // ---------------- parity 1 (+ satisfied-bond count of the finished sweep)
         if (!need_E) {
             for (int kl = sg; kl < nk; kl += G) {
-                const uint4 rnd = philox4x32_10(g, (uint32_t)q, gw, (1u << 16) | (uint32_t)(k0 + kl), P.k0, P.k1);
-                update_quad<L, FAST, false>(sp + (size_t)kl * N, lt + kl * LTS, R, J1, 1, 1 - s0, q, qyp, qym,
-                                            qzp, qzm, rnd, fin);
+                const uint4 rnd = philox_rk(g, (uint32_t)q, gw, (1u << 16) | (uint32_t)(k0 + kl), A.rk);
+                update_quad<L, FAST, false>(sp + (size_t)kl * N, lt + kl * LTS, R, J1, 1, 1 - s0, q, offY, offZ,
+                                            rnd, fin);
             }
-        } else {
-            for (int kb = sg; kb < S; kb += 4 * G) {     // batches of four slots: kb, kb+G, kb+2G, kb+3G
-                uint32_t en[4][5];
+            __syncthreads();
+            continue;
+        }
+        for (int kb = sg; kb < S; kb += 4 * G) {     // batches of four slots: kb, kb+G, kb+2G, kb+3G
+            uint32_t en[4][5];
 #pragma unroll
-                for (int i = 0; i < 4; ++i) {
-                    const int kl = kb + i * G;
-                    if (kl < nk) {
-                        const uint4 rnd = philox4x32_10(g, (uint32_t)q, gw, (1u << 16) | (uint32_t)(k0 + kl),
-                                                        P.k0, P.k1);
-                        update_quad<L, FAST, true>(sp + (size_t)kl * N, lt + kl * LTS, R, J1, 1, 1 - s0, q, qyp,
-                                                   qym, qzp, qzm, rnd, fin);
-                        quad_sum(fin, en[i]);
-                    } else {
+            for (int i = 0; i < 4; ++i) {
+                const int kl = kb + i * G;
+                if (kl < nk) {
+                    const uint4 rnd = philox_rk(g, (uint32_t)q, gw, (1u << 16) | (uint32_t)(k0 + kl), A.rk);
+                    update_quad<L, FAST, true>(sp + (size_t)kl * N, lt + kl * LTS, R, J1, 1, 1 - s0, q, offY,
+                                               offZ, rnd, fin);
+                    quad_sum(fin, en[i]);
+                } else {
 #pragma unroll
-                        for (int j = 0; j < 5; ++j) en[i][j] = 0;
-                    }
+                    for (int j = 0; j < 5; ++j) en[i][j] = 0;
                 }
-                uint32_t tot[kResPlanes];
-                warp_sum4(en, lane, tot);
-                const int i_mine = 2 * (lane >> 4) + ((lane >> 3) & 1);
-                const int kl = kb + i_mine * G;
-                if ((lane & 7) == 0 && kl < nk) {
-#pragma unroll
-                    for (int j = 0; j < kResPlanes; ++j) wsum[(kl * kResPlanes + j) * NW + wq] = tot[j];
-                }
+            }
+            uint32_t tot[kResPlanes];
+            warp_sum4(en, lane, tot);
+            const int i_mine = 2 * (lane >> 4) + ((lane >> 3) & 1);
+            const int kl = kb + i_mine * G;
+            if (kl < nk) add_counts(tot, lane & 7, Eacc + kl * 32);
+        }
+        __syncthreads();
+        // ---- energies of my slots: E = 3N - 2 (satisfied bonds); pushed into every block of
+        //      the cluster (distributed shared memory), buffer chosen by the swap-round parity
+        int32_t *Ebuf = Eall + (nswap & 1u) * nT * 32;
+        for (int a = tid; a < nk * 32; a += NT) {
+            const int e = 3 * N - 2 * Eacc[a];
+            Eacc[a] = 0;
+            const int dst = k0 * 32 + a;
+            if (C > 1) {
+                for (int rr = 0; rr < C; ++rr) cl.map_shared_rank(Ebuf, rr)[dst] = e;
+            } else {
+                Ebuf[dst] = e;
+            }
+        }
+        if (!swap_now) { __syncthreads(); continue; }
+        if (C > 1) { cluster_arrive(); cluster_wait(); } else __syncthreads();
+        // ---- swap round: warp per temperature pair, lane = realization.  Every block of the
+        //      cluster computes all pairs of its word (identical results).
+        const int warp = tid >> 5, nwarp = NT >> 5;
+        for (int t = (int)(nswap & 1u) + 2 * warp; t + 1 < nT; t += 2 * nwarp) {
+            uint8_t *sg_ = sig8 + lane * nT, *ta_ = tau8 + lane * nT;
+            const int sa = sg_[t], sb = sg_[t + 1];
+            const int m = (Ebuf[sa * 32 + lane] - Ebuf[sb * 32 + lane]) / 4;
+            const uint4 v = philox_rk(g, (uint32_t)t, P.r0 + (uint32_t)(32 * w + lane), 2u << 16, A.rk);
+            const int lo = swm[4 * t], cnt = swm[4 * t + 1], kinds = swm[4 * t + 3];
+            bool acc;
+            if (m < lo) acc = kinds & 1;
+            else if (m >= lo + cnt) acc = (kinds >> 1) & 1;
+            else if (m >= -kSwapWin && m < 0) acc = v.x <= swwin[t * kSwapWin + m + kSwapWin];
+            else acc = v.x <= P.swp_val[swm[4 * t + 2] + (m - lo)];
+            if (acc) {
+                sg_[t] = (uint8_t)sb; sg_[t + 1] = (uint8_t)sa;
+                ta_[sa] = (uint8_t)(t + 1); ta_[sb] = (uint8_t)t;
+            }
+        }
+        ++nswap;
+        __syncthreads();
+        for (int kl = warp; kl < nk; kl += nwarp) {   // rank masks of my slots
+            const int t = tau8[lane * nT + k0 + kl];
+            const int pos = P.desc ? t : nT - 1 - t;
+#pragma unroll 8
+            for (int n = 0; n <= nT; ++n) {
+                const uint32_t mk = __ballot_sync(0xFFFFFFFFu, pos >= n);
+                if (lane == (n & 31)) lt[kl * LTS + n] = mk;
             }
         }
         __syncthreads();
-        if (need_E) {
-            // E[k][b] = 3N - 2 * sum over warps and planes of bit b  (thread = (slot, bit))
-            for (int a = tid; a < nk * 32; a += NT) {
-                const int kl = a >> 5, b = a & 31;
-                int cnt = 0;
-                for (int j = 0; j < kResPlanes; ++j) {
-                    int cj = 0;
-                    for (int x = 0; x < NW; ++x) cj += (int)((wsum[(kl * kResPlanes + j) * NW + x] >> b) & 1u);
-                    cnt += cj << j;
-                }
-                Eall[(k0 + kl) * 32 + b] = 3 * N - 2 * cnt;
-            }
-        }
-        if (swap_now) {
-            if (C > 1) {
-                cg::cluster_group cl = cg::this_cluster();
-                cl.sync();                            // every block's energies are in its Eall
-                for (int rr = 0; rr < C; ++rr) {
-                    if (rr == rank) continue;
-                    const int rk0 = rr * S, rnk = max(0, min(S, nT - rk0));
-                    const int32_t *rE = cl.map_shared_rank(Eall, rr);
-                    for (int a = tid; a < rnk * 32; a += NT) Eall[rk0 * 32 + a] = rE[rk0 * 32 + a];
-                }
-                cl.sync();                            // remote reads done before anyone rewrites Eall
-            } else {
-                __syncthreads();
-            }
-            // swap round: warp per temperature pair, lane = realization (every block computes all
-            // pairs of its word redundantly; results are identical)
-            const int warp = tid >> 5, nwarp = NT >> 5;
-            for (int t = (int)(nswap & 1u) + 2 * warp; t + 1 < nT; t += 2 * nwarp) {
-                uint8_t *sg_ = sig8 + lane * nT, *ta_ = tau8 + lane * nT;
-                const int sa = sg_[t], sb = sg_[t + 1];
-                const int m = (Eall[sa * 32 + lane] - Eall[sb * 32 + lane]) / 4;
-                const uint4 v = philox4x32_10(g, (uint32_t)t, P.r0 + (uint32_t)(32 * w + lane), 2u << 16,
-                                              P.k0, P.k1);
-                if (swap_accept(P, t, m, v.x)) {
-                    sg_[t] = (uint8_t)sb; sg_[t + 1] = (uint8_t)sa;
-                    ta_[sa] = (uint8_t)(t + 1); ta_[sb] = (uint8_t)t;
-                }
-            }
-            ++nswap;
-            __syncthreads();
-            for (int kl = warp; kl < nk; kl += nwarp) {   // rank masks of my slots
-                const int t = tau8[lane * nT + k0 + kl];
-                const int pos = P.desc ? t : nT - 1 - t;
-                for (int n = 0; n <= nT; ++n) {
-                    const uint32_t mk = __ballot_sync(0xFFFFFFFFu, pos >= n);
-                    if (lane == (n & 31)) lt[kl * LTS + n] = mk;
-                }
-            }
-            __syncthreads();
-        }
     }
+    // the energies written last are in the buffer selected by the final nswap parity... the
+    // last sweep always computes them; which buffer depends on whether that sweep swapped
+    const bool last_swapped = A.swap_interval > 0 &&
+                              ((uint64_t)A.g0 + (uint64_t)A.n_sweeps) % (uint64_t)A.swap_interval == 0;
+    const int32_t *Elast = Eall + (((last_swapped ? nswap - 1 : nswap) & 1u) * nT * 32);
+    if (C > 1) cl.sync();                         // no block exits while others may still push to it
 
     // ---- write back
     for (int k = 0; k < nk; ++k) {
@@ -451,7 +531,7 @@ __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs
         const uint4 *src = reinterpret_cast<const uint4 *>(sp + (size_t)k * N);
         for (int a = tid; a < N / 4; a += NT) dst[a] = src[a];
         for (int a = tid; a < LTS; a += NT) P.lt[((size_t)w * nT + k0 + k) * LTS + a] = lt[k * LTS + a];
-        for (int a = tid; a < 32; a += NT) P.E[(size_t)(32 * w + a) * nT + k0 + k] = Eall[(k0 + k) * 32 + a];
+        for (int a = tid; a < 32; a += NT) P.E[(size_t)(32 * w + a) * nT + k0 + k] = Elast[(k0 + k) * 32 + a];
     }
     if (rank == 0) {
         for (int a = tid; a < 32 * nT; a += NT) {
