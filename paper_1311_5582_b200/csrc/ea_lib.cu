@@ -33,6 +33,7 @@ struct ea_handle {
     uint8_t *d_swp_kind = nullptr;
     uint32_t *d_swp_val = nullptr;
     size_t swp_val_cap = 0;
+    int32_t *d_Ecnt = nullptr;         // satisfied-bond counters of the tiled path
     uint4 *d_bucket = nullptr;         // fast rank table (ea_resident.cuh), 16 B entries
     int n_bucket = 0, key_lo = 0, key_hi = 0, key_shift = 0;
     bool fast_rank = false;
@@ -62,7 +63,7 @@ static int fail(const ea_handle *h, int code, const std::string &msg)
 namespace {
 constexpr int kMaxBucket = 1024;
 struct Layout {
-    size_t spin, coup, lt, tau, sigma, E, thr32, swp_lo, swp_cnt, swp_off, swp_kind, swp_val, bucket, total;
+    size_t spin, coup, lt, tau, sigma, E, thr32, swp_lo, swp_cnt, swp_off, swp_kind, swp_val, bucket, ecnt, total;
     size_t swp_val_cap;
 };
 size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
@@ -92,6 +93,7 @@ Layout make_layout(int L, int nT, int R)
     o.swp_val_cap = (size_t)(nT > 1 ? nT - 1 : 0) * (3 * N + 1);
     o.swp_val = take(4 * (o.swp_val_cap ? o.swp_val_cap : 1));
     o.bucket = take(16 * (size_t)kMaxBucket);
+    o.ecnt = take(4 * Rp * nT);
     o.total = off;
     return o;
 }
@@ -340,6 +342,7 @@ extern "C" ea_handle *ea_create_ex(int L, int n_temps, int n_realizations, const
     P.swp_val = h->d_swp_val = (uint32_t *)(h->ws + lay.swp_val);
     h->swp_val_cap = lay.swp_val_cap;
     h->d_bucket = (uint4 *)(h->ws + lay.bucket);
+    h->d_Ecnt = (int32_t *)(h->ws + lay.ecnt);
 
     // threshold tables in double on the host
     const int M = 3 * h->N / 2;
@@ -358,6 +361,7 @@ extern "C" ea_handle *ea_create_ex(int L, int n_temps, int n_realizations, const
     launch_cfg((int64_t)h->Rp * n_temps, 128, grid);
     ea::k_identity_perm<<<grid, 128, 0, h->stream>>>(P);
     h->launches += 2;
+    cudaMemsetAsync(h->d_Ecnt, 0, 4 * (size_t)h->Rp * n_temps, h->stream);
     if (rebuild_lt(h) != EA_OK || recompute_energy(h) != EA_OK ||
         cudaStreamSynchronize(h->stream) != cudaSuccess || cudaGetLastError() != cudaSuccess)
         return (ea_handle *)bail(EA_ERR_CUDA, "ea_create: initialisation kernels failed: " + h->err);
@@ -562,10 +566,94 @@ static int sweep_resident(ea_handle *h, int64_t n_sweeps, int swap_interval)
     return EA_OK;
 }
 
+// ---------------------------------------------------------------- tiled path (L = 16, 32, 64)
+namespace {
+struct TilePlan { bool ok; int SK, nkg; size_t smem; int nthr, nslab; };
+
+TilePlan plan_tiled(const ea_handle *h)
+{
+    TilePlan pl{false, 0, 0, 0, 0, 0};
+    if (h->L != 16 && h->L != 32 && h->L != 64) return pl;
+    const int qpp = (h->L / 8) * h->L;
+    int zs = 512 / qpp; if (zs < 1) zs = 1; if (zs > h->L) zs = h->L;
+    pl.nthr = qpp * zs; pl.nslab = h->L / zs;
+    // slots per block: amortise the per-block set-up (couplings, tables: ~2.5 slot-times)
+    // against wave quantisation on sm_count SMs (one 512-thread block per SM)
+    double best = -1.0;
+    const int nT4 = (h->nT + 3) / 4 * 4;
+    for (int sk = 4; sk <= nT4; sk += 4) {
+        const int nkg = (h->nT + sk - 1) / sk;
+        const int64_t blocks = (int64_t)h->W * pl.nslab * nkg;
+        const int64_t waves = (blocks + h->sm_count - 1) / h->sm_count;
+        const double eff = (double)blocks / (double)(waves * h->sm_count) * (double)sk / ((double)sk + 2.5);
+        if (eff > best) { best = eff; pl.SK = sk; pl.nkg = nkg; }
+    }
+    const size_t LTS = (size_t)h->nT + 1;
+    pl.smem = 16 * (size_t)h->n_bucket + 4 * ((size_t)pl.SK * LTS + 3 * LTS + (size_t)pl.SK * 32) + 16;
+    pl.ok = pl.smem <= 200 * 1024;
+    return pl;
+}
+
+template <int L>
+cudaError_t launch_tiled_t(const ea_handle *h, const ea::TiledArgs &A, const TilePlan &pl, bool fast, bool energy)
+{
+    void (*kern)(const ea::TiledArgs);
+    if (fast) kern = energy ? ea::k_tiled_half<L, true, true> : ea::k_tiled_half<L, true, false>;
+    else kern = energy ? ea::k_tiled_half<L, false, true> : ea::k_tiled_half<L, false, false>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem);
+    if (e != cudaSuccess) return e;
+    kern<<<h->W * pl.nslab * pl.nkg, pl.nthr, pl.smem, h->stream>>>(A);
+    return cudaGetLastError();
+}
+}  // namespace
+
+static int sweep_tiled(ea_handle *h, int64_t n_sweeps, int swap_interval)
+{
+    const TilePlan pl = plan_tiled(h);
+    if (!pl.ok) return fail(h, EA_ERR_UNSUPPORTED, "tiled kernel: shape not supported");
+    ea::TiledArgs A{};
+    A.P = h->P; A.SK = pl.SK; A.n_kgroups = pl.nkg; A.Ecnt = h->d_Ecnt;
+    A.bucket = h->d_bucket; A.n_bucket = h->n_bucket;
+    A.key_lo = h->key_lo; A.key_hi = h->key_hi; A.key_shift = h->key_shift;
+    for (int r = 0; r < 10; ++r) {
+        A.rk[2 * r] = h->P.k0 + (uint32_t)r * 0x9E3779B9u;
+        A.rk[2 * r + 1] = h->P.k1 + (uint32_t)r * 0xBB67AE85u;
+    }
+    const bool fast = h->fast_rank;
+    for (int64_t it = 0; it < n_sweeps; ++it) {
+        const bool swap_now = swap_interval > 0 && (h->g + 1) % (uint64_t)swap_interval == 0;
+        A.g = (uint32_t)h->g;
+        for (int p = 0; p < 2; ++p) {
+            A.parity = p;
+            const bool energy = p == 1 && swap_now;
+            cudaError_t e = cudaErrorInvalidValue;
+            if (h->L == 16) e = launch_tiled_t<16>(h, A, pl, fast, energy);
+            else if (h->L == 32) e = launch_tiled_t<32>(h, A, pl, fast, energy);
+            else e = launch_tiled_t<64>(h, A, pl, fast, energy);
+            if (e != cudaSuccess) return fail(h, EA_ERR_CUDA, std::string("tiled launch: ") + cudaGetErrorString(e));
+            h->launches++;
+        }
+        h->energy_valid = false;
+        h->g++;
+        if (swap_now) {
+            int grid;
+            launch_cfg((int64_t)h->Rp * h->nT, 256, grid);
+            ea::k_tiled_finish<<<grid, 256, 0, h->stream>>>(h->P, h->d_Ecnt);
+            ea::k_pt_swap<<<h->W, 256, 0, h->stream>>>(h->P, (uint32_t)(h->g - 1), (uint32_t)(h->nswap & 1u));
+            h->launches += 2;
+            h->nswap++;
+            h->energy_valid = true;
+        }
+    }
+    CUDA_TRY(h, cudaGetLastError());
+    return EA_OK;
+}
+
 static int pick_kernel(const ea_handle *h)
 {
     if (h->kernel_sel != EA_KERNEL_AUTO) return h->kernel_sel;
     if (plan_resident(h).ok) return EA_KERNEL_RESIDENT;
+    if (plan_tiled(h).ok) return EA_KERNEL_TILED;
     return EA_KERNEL_GENERIC;
 }
 
@@ -574,6 +662,7 @@ extern "C" int ea_set_kernel(ea_handle *h, int kernel)
     if (!h) return EA_ERR_INVALID_ARG;
     if (kernel == EA_KERNEL_AUTO || kernel == EA_KERNEL_GENERIC) { h->kernel_sel = kernel; return EA_OK; }
     if (kernel == EA_KERNEL_RESIDENT && plan_resident(h).ok) { h->kernel_sel = kernel; return EA_OK; }
+    if (kernel == EA_KERNEL_TILED && plan_tiled(h).ok) { h->kernel_sel = kernel; return EA_OK; }
     return fail(h, EA_ERR_UNSUPPORTED, "ea_set_kernel: kernel not available for this shape");
 }
 extern "C" int ea_get_kernel(ea_handle *h) { return h ? pick_kernel(h) : EA_ERR_INVALID_ARG; }
@@ -584,6 +673,7 @@ extern "C" int ea_sweep(ea_handle *h, int64_t n_sweeps, int swap_interval)
     if (h->g + (uint64_t)n_sweeps > 0xFFFFFFFFull) return fail(h, EA_ERR_RANGE, "ea_sweep: sweep counter would pass 2^32-1");
     if (n_sweeps == 0) return EA_OK;
     if (pick_kernel(h) == EA_KERNEL_RESIDENT) return sweep_resident(h, n_sweeps, swap_interval);
+    if (pick_kernel(h) == EA_KERNEL_TILED) return sweep_tiled(h, n_sweeps, swap_interval);
     return sweep_generic(h, n_sweeps, swap_interval);
 }
 

@@ -158,7 +158,7 @@ struct QuadJ {
 template <int L>
 struct ResGeom {
     static constexpr int Lh = L / 2, N = L * L * L, Nh = N / 2, NQ = Nh / 4, QR = Lh / 4;
-    static_assert(Lh % 4 == 0, "resident kernel needs L multiple of 8");
+    static_assert(Lh % 4 == 0 && (QR & (QR - 1)) == 0 && QR <= 8, "needs L in {8,16,32,64}");
 };
 
 // New spin words of the four sites of quad q (parity p) of one slot's lattice `sp` (smem,
@@ -166,28 +166,29 @@ struct ResGeom {
 // bit 31 of the entries (set: the caller must redo the quad with EXACT = true).
 template <int L, bool EXACT, bool ENERGY>
 __device__ __forceinline__ uint4 quad_body(const uint32_t *sp, const uint32_t *lt, const RankCtx &R,
-                                           const QuadJ &J, int p, int s, int q, uint32_t offY, uint32_t offZ,
-                                           const uint4 rnd, Planes (&fin)[4], uint32_t *flag)
+                                           const QuadJ &J, int p, int s, int q, uint32_t oyp, uint32_t oym,
+                                           uint32_t ozp, uint32_t ozm, const uint4 rnd, Planes (&fin)[4],
+                                           uint32_t *flag)
 {
     using Gm = ResGeom<L>;
-    // offY / offZ: byte offsets of the +-y / +-z neighbour quads inside a parity array, two
-    // 16-bit halves each (+ in the low half)
+    // oyp..ozm: byte offsets of the +-y / +-z neighbour quads inside a parity array
     const char *self_b = reinterpret_cast<const char *>(sp + p * Gm::Nh);
     const char *oth_b = reinterpret_cast<const char *>(sp + (1 - p) * Gm::Nh);
     const uint4 me = *reinterpret_cast<const uint4 *>(self_b + 16 * q);
     const uint4 v = *reinterpret_cast<const uint4 *>(oth_b + 16 * q);
-    const uint4 yp = *reinterpret_cast<const uint4 *>(oth_b + (offY & 0xFFFFu));
-    const uint4 ym = *reinterpret_cast<const uint4 *>(oth_b + (offY >> 16));
-    const uint4 zp = *reinterpret_cast<const uint4 *>(oth_b + (offZ & 0xFFFFu));
-    const uint4 zm = *reinterpret_cast<const uint4 *>(oth_b + (offZ >> 16));
+    const uint4 yp = *reinterpret_cast<const uint4 *>(oth_b + oyp);
+    const uint4 ym = *reinterpret_cast<const uint4 *>(oth_b + oym);
+    const uint4 zp = *reinterpret_cast<const uint4 *>(oth_b + ozp);
+    const uint4 zm = *reinterpret_cast<const uint4 *>(oth_b + ozm);
     uint32_t ext = s ? v.x : v.w;
-    if (Gm::QR == 2) {
+    if (Gm::QR > 1) {
+        // the word beyond the quad comes from the next (s) / previous (!s) quad of the row
+        const int qx = q & (Gm::QR - 1);
+        const int qn = (q - qx) + ((qx + (s ? 1 : Gm::QR - 1)) & (Gm::QR - 1));
         if (EXACT) {   // divergent (rare) path: no shuffle, read the neighbour quad's word
-            const int row = q & ~1;
-            ext = s ? reinterpret_cast<const uint32_t *>(oth_b)[4 * (row + ((q + 1) & 1))]
-                    : reinterpret_cast<const uint32_t *>(oth_b)[4 * (row + ((q + 1) & 1)) + 3];
+            ext = reinterpret_cast<const uint32_t *>(oth_b)[4 * qn + (s ? 0 : 3)];
         } else {
-            ext = __shfl_xor_sync(0xFFFFFFFFu, ext, 1);
+            ext = __shfl_sync(0xFFFFFFFFu, ext, qn & 31);
         }
     }
     uint4 sh;   // the x neighbour that is not index-aligned: x+1 if s, x-1 otherwise
@@ -226,17 +227,37 @@ __device__ __forceinline__ uint4 quad_body(const uint32_t *sp, const uint32_t *l
 }
 
 template <int L, bool FAST, bool ENERGY>
-__device__ __forceinline__ void update_quad(uint32_t *sp, const uint32_t *lt, const RankCtx &R,
-                                            const QuadJ &J, int p, int s, int q, uint32_t offY, uint32_t offZ,
-                                            const uint4 rnd, Planes (&fin)[4])
+__device__ __forceinline__ void update_quad_off(uint32_t *sp, const uint32_t *lt, const RankCtx &R,
+                                                const QuadJ &J, int p, int s, int q, uint32_t oyp,
+                                                uint32_t oym, uint32_t ozp, uint32_t ozm, const uint4 rnd,
+                                                Planes (&fin)[4])
 {
     using Gm = ResGeom<L>;
     uint32_t flag = 0x80000000u;
     uint4 res;
-    if (FAST) res = quad_body<L, false, ENERGY>(sp, lt, R, J, p, s, q, offY, offZ, rnd, fin, &flag);
-    // rare (or !FAST): redo the whole quad from shared memory with the exact search
-    if ((int)flag < 0) res = quad_body<L, true, ENERGY>(sp, lt, R, J, p, s, q, offY, offZ, rnd, fin, &flag);
+    if (FAST) res = quad_body<L, false, ENERGY>(sp, lt, R, J, p, s, q, oyp, oym, ozp, ozm, rnd, fin, &flag);
+    // rare (or !FAST): redo the whole quad from memory with the exact search
+    if ((int)flag < 0) res = quad_body<L, true, ENERGY>(sp, lt, R, J, p, s, q, oyp, oym, ozp, ozm, rnd, fin, &flag);
     reinterpret_cast<uint4 *>(sp + p * Gm::Nh)[q] = res;
+}
+
+// resident kernel: neighbour offsets packed two per register (16-bit halves, + in the low half)
+template <int L, bool FAST, bool ENERGY>
+__device__ __forceinline__ void update_quad(uint32_t *sp, const uint32_t *lt, const RankCtx &R,
+                                            const QuadJ &J, int p, int s, int q, uint32_t offY, uint32_t offZ,
+                                            const uint4 rnd, Planes (&fin)[4])
+{
+    update_quad_off<L, FAST, ENERGY>(sp, lt, R, J, p, s, q, offY & 0xFFFFu, offY >> 16, offZ & 0xFFFFu,
+                                     offZ >> 16, rnd, fin);
+}
+
+// tiled kernel: neighbour quad indices
+template <int L, bool FAST, bool ENERGY>
+__device__ __forceinline__ void update_quad_wide(uint32_t *sp, const uint32_t *lt, const RankCtx &R,
+                                                 const QuadJ &J, int p, int s, int q, int qyp, int qym,
+                                                 int qzp, int qzm, const uint4 rnd, Planes (&fin)[4])
+{
+    update_quad_off<L, FAST, ENERGY>(sp, lt, R, J, p, s, q, 16u * qyp, 16u * qym, 16u * qzp, 16u * qzm, rnd, fin);
 }
 
 // Couplings of quad q for parity p from global memory ([d][p][j], 3N words per word w).

@@ -33,12 +33,14 @@ def _assert_same(g, o, tag=""):
     assert st["sweeps"] == c["sweeps"] and st["swap_rounds"] == c["swap_rounds"]
 
 
-KERNELS = [1, 2]   # EA_KERNEL_GENERIC, EA_KERNEL_RESIDENT (L = 8, 16 only)
+KERNELS = [1, 2, 3]   # EA_KERNEL_GENERIC, EA_KERNEL_RESIDENT (L = 8, 16), EA_KERNEL_TILED (L = 16, 32, 64)
 
 
 def _skip_unsupported(kernel, L):
     if kernel == 2 and L not in (8, 16):
         pytest.skip("resident kernel supports L = 8, 16")
+    if kernel == 3 and L not in (16, 32, 64):
+        pytest.skip("tiled kernel supports L = 16, 32, 64")
 
 
 @pytest.mark.parametrize("kernel", KERNELS)
@@ -50,6 +52,7 @@ def _skip_unsupported(kernel, L):
     (12, 20, 64, 2, 6),        # config 3 shape (non power of two)
     (16, 24, 96, 1, 3),        # config 4 shape, 3 words
     (32, 4, 40, 1, 2),         # config 5 lattice, 2 words
+    (32, 10, 33, 2, 3),        # L = 32, slot groups with a ragged tail
     (8, 6, 40, 3, 14),         # cluster with an empty block, swap every 3rd sweep
     (16, 5, 33, 1, 4),         # odd n_temps, ragged words
     (8, 33, 20, 1, 8),         # more temperatures than fit one block group
@@ -76,7 +79,7 @@ def test_trajectory_matches_oracle(kernel, L, nT, R, swap, ns):
 
 @pytest.mark.parametrize("kernel", KERNELS)
 def test_set_couplings_set_spins_set_tables(kernel):
-    L, nT, R = 8, 6, 37
+    L, nT, R = (16 if kernel == 3 else 8), 6, 37
     betas = 1.0 / temperature_ladder(nT, 0.7, 3.0)
     g, o = _pair(L, nT, R, betas, 5, kernel)
     J = random_couplings(R, L ** 3, 11)
@@ -99,7 +102,7 @@ def test_set_couplings_set_spins_set_tables(kernel):
 
 @pytest.mark.parametrize("kernel", KERNELS)
 def test_ascending_betas_beta_zero_and_no_pt(kernel):
-    L, nT, R = (8 if kernel == 2 else 4), 5, 20
+    L, nT, R = {1: 4, 2: 8, 3: 16}[kernel], 5, 20
     betas = np.array([0.0, 0.2, 0.5, 1.0, 3.0])          # ascending, includes beta = 0 and very cold
     g, o = _pair(L, nT, R, betas, 77, kernel)
     g.sweep(30, 1); o.sweep(30, 1)
@@ -118,7 +121,7 @@ def test_ascending_betas_beta_zero_and_no_pt(kernel):
 @pytest.mark.parametrize("kernel", KERNELS)
 def test_word_sharding_reproduces_full_run(kernel):
     # words simulated alone (first_realization = 32 w0) == those words of the full run
-    L, nT, R = 8, 8, 96
+    L, nT, R = (16 if kernel == 3 else 8), 8, 96
     betas = 1.0 / temperature_ladder(nT, 0.6, 2.0)
     from paper_1311_5582_b200 import EA
     full = EA(L, nT, R, betas, 9, kernel=kernel)
@@ -153,7 +156,7 @@ def test_kernels_interleave_on_one_handle():
     L, nT, R = 16, 8, 64
     betas = 1.0 / temperature_ladder(nT, 0.7, 2.0)
     g, o = _pair(L, nT, R, betas, 31)
-    for kernel, n, swap in ((2, 3, 1), (1, 2, 1), (2, 4, 2), (1, 1, 0), (2, 2, 1)):
+    for kernel, n, swap in ((2, 3, 1), (1, 2, 1), (3, 3, 1), (2, 4, 2), (1, 1, 0), (3, 2, 2), (2, 2, 1)):
         g.set_kernel(kernel)
         assert g.get_kernel() == kernel
         g.sweep(n, swap); o.sweep(n, swap)
@@ -168,4 +171,7 @@ def test_auto_picks_resident_for_L16():
     g.destroy()
     g = EA(12, 4, 32, np.array([1.0, 0.9, 0.8, 0.7]), 1)
     assert g.get_kernel() == 1
+    g.destroy()
+    g = EA(32, 4, 32, np.array([1.0, 0.9, 0.8, 0.7]), 1)
+    assert g.get_kernel() == 3
     g.destroy()
