@@ -128,6 +128,26 @@ def run_reference(a, cfg):
     }))
 
 
+# ------------------------------------------------------------------ multi-GPU plumbing
+def shard_first_realization(rank, realizations_per_rank):
+    """Weak scaling by realization word: rank r owns global realizations [r*R, (r+1)*R), R a
+    multiple of 32 per rank except possibly the last word (counters are keyed by the GLOBAL word
+    index, so the union of the ranks equals one big single-process run)."""
+    words = (realizations_per_rank + 31) // 32
+    return rank * words * 32
+
+
+def max_over_ranks(ms, world, device="cuda"):
+    """Timing of a multi-rank run = the slowest rank (all-reduce MAX)."""
+    if world == 1:
+        return float(ms)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
 # ------------------------------------------------------------------ CUDA arm
 def run_cuda(a, cfg):
     import torch
@@ -150,7 +170,7 @@ def run_cuda(a, cfg):
     betas = betas_for(cfg)
     sps = a.sweeps_per_step
     # weak scaling: every rank owns cfg.R realizations; rank r simulates global words r*W..
-    sim = EA(cfg.L, cfg.n_temps, cfg.R, betas, cfg.seed, first_realization=rank * cfg.W * 32)
+    sim = EA(cfg.L, cfg.n_temps, cfg.R, betas, cfg.seed, first_realization=shard_first_realization(rank, cfg.R))
     kernel = sim.get_kernel()
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
 
@@ -176,11 +196,7 @@ def run_cuda(a, cfg):
     stop.set(); th.join()
     launches = sim.launch_count() - launches0
     step_ms = [e0.elapsed_time(e1) for e0, e1 in ev]
-    total_ms = float(sum(step_ms))
-    if world > 1:
-        t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = max_over_ranks(float(sum(step_ms)), world)
     attempts_step = cfg.attempts_per_sweep * sps * world
     value = total_ms * 1e9 / (attempts_step * a.steps)            # ms -> ps
 
@@ -199,11 +215,7 @@ def run_cuda(a, cfg):
         sim.sweep(sps, cfg.swap_interval)
         E = sim.energy()
     barrier()
-    e2e_ms = (time.perf_counter() - t0) * 1e3
-    if world > 1:
-        t = torch.tensor([e2e_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_ms = float(t.item())
+    e2e_ms = max_over_ranks((time.perf_counter() - t0) * 1e3, world)
     e2e_value = e2e_ms * 1e9 / (attempts_step * e2e_steps)
     Rp = 32 * cfg.W
     h2d = int(Jnp.nbytes)

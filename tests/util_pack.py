@@ -24,3 +24,28 @@ def by_temperature(arr_by_slot, tau):
     sigma = np.argsort(tau, axis=1)
     idx = sigma.reshape(sigma.shape + (1,) * (arr_by_slot.ndim - 2))
     return np.take_along_axis(arr_by_slot, idx, axis=1)
+
+
+def spins_to_words(s, L):
+    """s[r][k][site] in +-1 (by slot) -> words[k][w][p][j] (uint32), padding bits 0."""
+    R, nT, N = s.shape
+    W = (R + 31) // 32
+    p, j = checkerboard_maps(L)
+    bits = np.zeros((W * 32, nT, N), dtype=np.uint32)
+    bits[:R] = (s > 0)
+    bits = bits.reshape(W, 32, nT, N)
+    per_site = (bits << np.arange(32, dtype=np.uint32)[None, :, None, None]).sum(axis=1, dtype=np.uint32)  # [w][k][site]
+    words = np.zeros((nT, W, 2, N // 2), dtype=np.uint32)
+    words[:, :, p, j] = per_site.transpose(1, 0, 2)
+    return words
+
+
+def word_digest(spin_words_w, tau_w, E_w):
+    """sha256 over one realization word: spin_words[:, w] ([nT][2][N/2] uint32), temp_of_slot and
+    energy_by_slot of its 32 realizations ([32][nT])."""
+    import hashlib
+    h = hashlib.sha256()
+    h.update(np.ascontiguousarray(spin_words_w, dtype=np.uint32).tobytes())
+    h.update(np.ascontiguousarray(tau_w, dtype=np.uint8).tobytes())
+    h.update(np.ascontiguousarray(E_w, dtype=np.int32).tobytes())
+    return h.hexdigest()
