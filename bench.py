@@ -34,6 +34,10 @@ UNIT = "ps/attempt"
 # FMA pipe and are not counted here.
 ALU_OPS_PER_WORD_UPDATE = 43.0
 PAPER_PS = 33.5   # GTX 580, PT every 10 sweeps: context, another workload
+# DRAM bytes (read + write) of ONE launch of the dominant kernel, from the committed ncu
+# --set full capture (profiles/r01_ncu_resident_cfg4.txt): the state is read once per launch
+# whatever the number of sweeps; the write-back stays in L2.
+NCU_DRAM_BYTES_PER_LAUNCH = {4: 28.87e6}
 
 
 def _clock_sampler(stop, out):
@@ -233,7 +237,7 @@ def run_cuda(a, cfg):
     alu_ops_per_step = ALU_OPS_PER_WORD_UPDATE * cfg.n_temps * cfg.W * cfg.N * sps
     achieved = alu_ops_per_step / (float(np.mean(step_ms)) * 1e-3)
     roofline = {"bound": "alu", "achieved": achieved / 1e12, "peak": peak["lop3"] / 1e12, "unit": "Tlaneop/s",
-                "frac": achieved / peak["lop3"], "traffic": None,
+                "frac": achieved / peak["lop3"], "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(a.config),
                 "note": "ALU-pipe lane-ops: %.0f per word update (DESIGN.md s8) / measured LOP3 issue peak "
                         "(ea_measure_int_peak, same process); IMAD peak %.2f, LOP3+IMAD mix %.2f Tlaneop/s"
                         % (ALU_OPS_PER_WORD_UPDATE, peak["imad"] / 1e12, peak["mix"] / 1e12)}
