@@ -63,11 +63,17 @@ __device__ __forceinline__ uint32_t pick(const uint4 &v, int lane)
 // (bit = 1: satisfied) are summed per bit lane into three planes n_sat = b0 + 2 b1 + 4 b2
 // by a carry-save adder: two full adders, a half adder, a full adder (8 LOP3).
 // ---------------------------------------------------------------------------------
-__device__ __forceinline__ uint32_t xor3(uint32_t a, uint32_t b, uint32_t c) { return a ^ b ^ c; }
-__device__ __forceinline__ uint32_t maj3(uint32_t a, uint32_t b, uint32_t c)
+// One LOP3 each, pinned with inline PTX so that ptxas keeps the 14-instruction form
+// (6 bonds + 8 adder) instead of re-deriving the adder on J ^ s_nb (17-18 LOP3).
+template <int LUT>
+__device__ __forceinline__ uint32_t lop3(uint32_t a, uint32_t b, uint32_t c)
 {
-    return (a & b) | (c & (a | b));
+    uint32_t d;
+    asm("lop3.b32 %0, %1, %2, %3, %4;" : "=r"(d) : "r"(a), "r"(b), "r"(c), "n"(LUT));
+    return d;
 }
+__device__ __forceinline__ uint32_t xor3(uint32_t a, uint32_t b, uint32_t c) { return lop3<0x96>(a, b, c); }
+__device__ __forceinline__ uint32_t maj3(uint32_t a, uint32_t b, uint32_t c) { return lop3<0xE8>(a, b, c); }
 
 struct Planes { uint32_t b0, b1, b2; };
 

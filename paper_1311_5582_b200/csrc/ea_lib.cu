@@ -35,7 +35,8 @@ struct ea_handle {
     size_t swp_val_cap = 0;
     int32_t *d_Ecnt = nullptr;         // satisfied-bond counters of the tiled path
     uint4 *d_bucket = nullptr;         // fast rank table (ea_resident.cuh), 16 B entries
-    int n_bucket = 0, key_lo = 0, key_hi = 0, key_shift = 0;
+    int n_bucket = 0, key_lo = 0, key_shift = 0;
+    uchar4 *d_trip = nullptr;          // [3 nT + 1] combined rank -> (n4, n5, n6)
     bool fast_rank = false;
     uint64_t g = 0, nswap = 0;
     bool energy_valid = false;
@@ -63,7 +64,7 @@ static int fail(const ea_handle *h, int code, const std::string &msg)
 namespace {
 constexpr int kMaxBucket = 1024;
 struct Layout {
-    size_t spin, coup, lt, tau, sigma, E, thr32, swp_lo, swp_cnt, swp_off, swp_kind, swp_val, bucket, ecnt, total;
+    size_t spin, coup, lt, tau, sigma, E, thr32, swp_lo, swp_cnt, swp_off, swp_kind, swp_val, bucket, trip, ecnt, total;
     size_t swp_val_cap;
 };
 size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
@@ -93,6 +94,7 @@ Layout make_layout(int L, int nT, int R)
     o.swp_val_cap = (size_t)(nT > 1 ? nT - 1 : 0) * (3 * N + 1);
     o.swp_val = take(4 * (o.swp_val_cap ? o.swp_val_cap : 1));
     o.bucket = take(16 * (size_t)kMaxBucket);
+    o.trip = take(4 * (3 * (size_t)nT + 2));
     o.ecnt = take(4 * Rp * nT);
     o.total = off;
     return o;
@@ -111,18 +113,31 @@ void launch_cfg(int64_t n, int block, int &grid) { grid = (int)((n + block - 1) 
 
 // ---------------------------------------------------------------- fast rank table
 // Buckets of the draw u by its leading bits: key(u) = bits of (float)u (truncating conversion)
-// >> (23 - MB) = exponent and MB mantissa bits.  For every bucket whose u-interval holds at
-// most one threshold per class, the entry stores 4 * rank at the interval's lower edge for the
-// classes n_sat = 4,5,6 (bytes 0,1,2); other buckets (and u < 2^8) carry bit 31 = "use the
-// exact search".  MB is the smallest of 3..6 that leaves < 1e-5 of the draws on the slow path.
+// >> (23 - MB) = exponent and MB mantissa bits; table index = max(key - key_lo, 0), covering
+// every u up to 2^32 - 1.  Entry = { 16 * (n4 + n5 + n6 at the bucket's lower edge), thr4, thr5,
+// thr6 }: n_c = number of class-c thresholds <= the lower edge, thr_c = the class-c
+// (threshold - 1) inside the bucket or 0xFFFFFFFF.  Buckets holding several thresholds of one
+// class, and all u < 2^8 (index 0), point at row 3 nT + 1 of the mask tables = "use the exact
+// search".  MB is the smallest of 3..6 that leaves < 1e-5 of the draws on the slow path.
+// trip[n] = the triple (n4, n5, n6) whose sum is n (unique: each n_c is monotone in u).
 static bool build_bucket_table(const std::vector<uint32_t> &thr32, const int z[3], int nT,
-                               std::vector<uint4> &tab, int &key_lo, int &key_hi, int &key_shift)
+                               std::vector<uint4> &tab, std::vector<uchar4> &trip, int &key_lo, int &key_shift)
 {
-    if (nT > 63) return false;
-    const int LOWEXP = 8;
-    uint32_t umax = 0;
+    auto rank_c = [&](int c, uint64_t u) {   // n_c(u) = z_c + #{i >= z_c : thr32[c][i] < u}
+        int n = z[c];
+        for (int i = z[c]; i < nT; ++i) if ((uint64_t)thr32[(size_t)c * (nT + 1) + i] < u) n = i + 1;
+        return n;
+    };
+    trip.assign((size_t)3 * nT + 1, make_uchar4((unsigned char)nT, (unsigned char)nT, (unsigned char)nT, 0));
+    auto note = [&](uint64_t u) {
+        const int a = rank_c(0, u), b = rank_c(1, u), c = rank_c(2, u);
+        trip[(size_t)(a + b + c)] = make_uchar4((unsigned char)a, (unsigned char)b, (unsigned char)c, 0);
+    };
+    note(0);
     for (int c = 0; c < 3; ++c)
-        if (z[c] < nT) umax = std::max(umax, thr32[(size_t)c * (nT + 1) + nT - 1]);
+        for (int i = z[c]; i < nT; ++i) note((uint64_t)thr32[(size_t)c * (nT + 1) + i] + 1);
+    const int LOWEXP = 8;
+    const uint32_t slow_row = 16u * (uint32_t)(3 * nT + 1);
     for (int MB = 3; MB <= 6; ++MB) {
         auto key_of = [&](uint32_t u) -> int {
             if (u == 0) return 0;
@@ -132,18 +147,18 @@ static bool build_bucket_table(const std::vector<uint32_t> &thr32, const int z[3
             return ((e + 127) << MB) | (int)mant;
         };
         const int klo = key_of(1u << LOWEXP) - 1;
-        const int khi = std::max(key_of(umax) + 1, klo + 1);
+        const int khi = key_of(0xFFFFFFFFu);
         const int n = khi - klo + 1;
         if (n > kMaxBucket) continue;
         std::vector<uint4> t((size_t)n);
-        t[0] = make_uint4(0x80000000u, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu);
+        t[0] = make_uint4(slow_row, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu);
         double slow_mass = std::ldexp(1.0, LOWEXP - 32);
-        for (int K = klo + 1; K < khi; ++K) {
+        for (int K = klo + 1; K <= khi; ++K) {
             const int e = (K >> MB) - 127;
             const uint64_t m = (uint64_t)(K & ((1 << MB) - 1));
             const uint64_t lo_u = (((uint64_t)1 << MB) | m) << (e - MB);
             const uint64_t hi_u = lo_u + ((uint64_t)1 << (e - MB)) - 1;
-            uint32_t entry = 0, inb[3] = {0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu};
+            uint32_t nsum = 0, inb[3] = {0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu};
             bool slow = false;
             for (int c = 0; c < 3; ++c) {
                 const uint32_t *col = thr32.data() + (size_t)c * (nT + 1);
@@ -153,15 +168,18 @@ static bool build_bucket_table(const std::vector<uint32_t> &thr32, const int z[3
                     else if ((uint64_t)col[i] < hi_u) { if (!cnt) inb[c] = col[i]; ++cnt; }
                 }
                 if (cnt > 1) slow = true;
-                entry |= (uint32_t)(4 * nlo) << (8 * c);
+                nsum += (uint32_t)nlo;
             }
-            if (slow) { entry |= 0x80000000u; slow_mass += (double)(hi_u - lo_u + 1) / 4294967296.0; }
-            t[(size_t)(K - klo)] = make_uint4(entry, inb[0], inb[1], inb[2]);
+            if (slow) {
+                slow_mass += (double)(hi_u - lo_u + 1) / 4294967296.0;
+                t[(size_t)(K - klo)] = make_uint4(slow_row, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu);
+            } else {
+                t[(size_t)(K - klo)] = make_uint4(16u * nsum, inb[0], inb[1], inb[2]);
+            }
         }
-        t[(size_t)(khi - klo)] = make_uint4((uint32_t)(4 * nT) * 0x010101u, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu);
         if (slow_mass < 1e-5 || MB == 6) {
             if (slow_mass > 1e-3) return false;
-            tab = t; key_lo = klo; key_hi = khi; key_shift = 23 - MB;
+            tab = t; key_lo = klo; key_shift = 23 - MB;
             return true;
         }
     }
@@ -237,12 +255,13 @@ static int upload_tables(ea_handle *h, const std::vector<uint64_t> &acc, const s
     CUDA_TRY(h, cudaStreamSynchronize(s));
     {
         std::vector<uint4> tab;
-        h->fast_rank = build_bucket_table(thr32, z, nT, tab, h->key_lo, h->key_hi, h->key_shift);
+        std::vector<uchar4> trip;
+        h->fast_rank = build_bucket_table(thr32, z, nT, tab, trip, h->key_lo, h->key_shift);
         h->n_bucket = h->fast_rank ? (int)tab.size() : 0;
-        if (h->fast_rank) {
+        CUDA_TRY(h, cudaMemcpyAsync(h->d_trip, trip.data(), 4 * trip.size(), cudaMemcpyHostToDevice, s));
+        if (h->fast_rank)
             CUDA_TRY(h, cudaMemcpyAsync(h->d_bucket, tab.data(), 16 * tab.size(), cudaMemcpyHostToDevice, s));
-            CUDA_TRY(h, cudaStreamSynchronize(s));
-        }
+        CUDA_TRY(h, cudaStreamSynchronize(s));
     }
     for (int c = 0; c < 3; ++c) h->P.z[c] = z[c];
     h->acc = acc;
@@ -342,6 +361,7 @@ extern "C" ea_handle *ea_create_ex(int L, int n_temps, int n_realizations, const
     P.swp_val = h->d_swp_val = (uint32_t *)(h->ws + lay.swp_val);
     h->swp_val_cap = lay.swp_val_cap;
     h->d_bucket = (uint4 *)(h->ws + lay.bucket);
+    h->d_trip = (uchar4 *)(h->ws + lay.trip);
     h->d_Ecnt = (int32_t *)(h->ws + lay.ecnt);
 
     // threshold tables in double on the host
@@ -472,27 +492,26 @@ static int sweep_generic(ea_handle *h, int64_t n_sweeps, int swap_interval)
 
 // ---------------------------------------------------------------- resident path (L = 8, 16)
 namespace {
-struct ResPlan { bool ok; int C, S, G; size_t smem; };
+struct ResPlan { bool ok; int C, S, G, swap_win; size_t smem; };
 
-size_t resident_smem(const ea_handle *h, int S, int NW)
+// shared memory of k_resident without the swap-threshold window (layout: ea_resident.cuh)
+size_t resident_smem(const ea_handle *h, int S)
 {
-    const size_t N = (size_t)h->N, nT = (size_t)h->nT, LTS = nT + 1;
-    (void)NW;
-    return 16 * (size_t)h->n_bucket +
-           4 * ((size_t)S * N + (size_t)S * LTS + 3 * LTS + 2 * nT * 32 + (size_t)S * 32 + 4 * nT +
-                nT * (size_t)ea::kSwapWin) + 64 * nT + 16;
+    const size_t N = (size_t)h->N, nT = (size_t)h->nT, LTS = nT + 1, MTS = 3 * nT + 2;
+    return 16 * (size_t)h->n_bucket + 4 * (size_t)S * N + 16 * (size_t)S * MTS +
+           4 * ((size_t)S * LTS + 3 * LTS + MTS + (size_t)S * 32 + 4 * nT) +
+           2 * (2 * nT * 32) + 64 * nT + 16;
 }
 
 ResPlan plan_resident(const ea_handle *h)
 {
-    ResPlan pl{false, 1, 0, 1, 0};
+    ResPlan pl{false, 1, 0, 1, 0, 0};
     if (h->L != 8 && h->L != 16) return pl;
-    const int NQ = h->N / 8, NW = NQ / 32;
     const size_t cap = 227 * 1024;
     int C = 0;
     for (int c = 1; c <= 8; ++c) {
         const int S = (h->nT + c - 1) / c;
-        if (resident_smem(h, S, NW) <= cap) { C = c; break; }
+        if (resident_smem(h, S) <= cap) { C = c; break; }
     }
     if (!C) return pl;
     // small problems: spread the slots over more SMs (cluster sizes 2, 4, 8)
@@ -502,7 +521,10 @@ ResPlan plan_resident(const ea_handle *h)
     pl.S = (h->nT + C - 1) / C;
     pl.G = 1;
     if (h->L == 8) { pl.G = 8; while (pl.G > 1 && pl.G > pl.S) pl.G >>= 1; }
-    pl.smem = resident_smem(h, pl.S, NW);
+    // the swap-threshold window takes what is left, up to 128 entries per temperature pair
+    const size_t base = resident_smem(h, pl.S);
+    pl.swap_win = (int)std::min<size_t>(128, (cap - base) / (4 * (size_t)h->nT));
+    pl.smem = base + 4 * (size_t)h->nT * pl.swap_win;
     pl.ok = true;
     return pl;
 }
@@ -543,8 +565,9 @@ static int sweep_resident(ea_handle *h, int64_t n_sweeps, int swap_interval)
         A.swap_interval = swap_interval;
         A.nswap0 = (uint32_t)h->nswap;
         A.C = pl.C; A.S = pl.S;
-        A.bucket = h->d_bucket; A.n_bucket = h->n_bucket;
-        A.key_lo = h->key_lo; A.key_hi = h->key_hi; A.key_shift = h->key_shift;
+        A.bucket = h->d_bucket; A.n_bucket = h->n_bucket; A.trip = h->d_trip;
+        A.key_lo = h->key_lo; A.key_shift = h->key_shift; A.swap_win = pl.swap_win;
+        A.ones = 0xFFFFFFFFu; A.c48 = 48u; A.cm16 = (uint32_t)-16;
         for (int r = 0; r < 10; ++r) {
             A.rk[2 * r] = h->P.k0 + (uint32_t)r * 0x9E3779B9u;
             A.rk[2 * r + 1] = h->P.k1 + (uint32_t)r * 0xBB67AE85u;
@@ -589,7 +612,9 @@ TilePlan plan_tiled(const ea_handle *h)
         if (eff > best) { best = eff; pl.SK = sk; pl.nkg = nkg; }
     }
     const size_t LTS = (size_t)h->nT + 1;
-    pl.smem = 16 * (size_t)h->n_bucket + 4 * ((size_t)pl.SK * LTS + 3 * LTS + (size_t)pl.SK * 32) + 16;
+    const size_t MTS = 3 * (size_t)h->nT + 2;
+    pl.smem = 16 * (size_t)h->n_bucket + 16 * (size_t)pl.SK * MTS +
+              4 * ((size_t)pl.SK * LTS + 3 * LTS + MTS + (size_t)pl.SK * 32) + 16;
     pl.ok = pl.smem <= 200 * 1024;
     return pl;
 }
@@ -613,8 +638,9 @@ static int sweep_tiled(ea_handle *h, int64_t n_sweeps, int swap_interval)
     if (!pl.ok) return fail(h, EA_ERR_UNSUPPORTED, "tiled kernel: shape not supported");
     ea::TiledArgs A{};
     A.P = h->P; A.SK = pl.SK; A.n_kgroups = pl.nkg; A.Ecnt = h->d_Ecnt;
-    A.bucket = h->d_bucket; A.n_bucket = h->n_bucket;
-    A.key_lo = h->key_lo; A.key_hi = h->key_hi; A.key_shift = h->key_shift;
+    A.bucket = h->d_bucket; A.n_bucket = h->n_bucket; A.trip = h->d_trip;
+    A.key_lo = h->key_lo; A.key_shift = h->key_shift;
+    A.ones = 0xFFFFFFFFu; A.c48 = 48u; A.cm16 = (uint32_t)-16;
     for (int r = 0; r < 10; ++r) {
         A.rk[2 * r] = h->P.k0 + (uint32_t)r * 0x9E3779B9u;
         A.rk[2 * r + 1] = h->P.k1 + (uint32_t)r * 0xBB67AE85u;

@@ -26,9 +26,23 @@ struct ResArgs {
     uint32_t nswap0;      // swap rounds done before this call
     int C, S;             // cluster size; slots per block (last block may own fewer)
     const uint4 *bucket;      // fast rank table (FAST variant), device memory, 16 B entries
+    const uchar4 *trip;       // [3 nT + 1] (n4, n5, n6) of every combined rank
     uint32_t rk[20];          // Philox round keys (k0 + r*0x9E3779B9, k1 + r*0xBB67AE85), r = 0..9
-    int n_bucket, key_lo, key_hi, key_shift;
+    int n_bucket, key_lo, key_shift;
+    int swap_win;             // swap thresholds for m in [-swap_win, -1] are staged in smem
+    uint32_t ones, c48, cm16; // 0xFFFFFFFF, 48, (uint32_t)-16: see RankCtx
 };
+
+// Mask table of one slot from its rank masks (one warp): row n = { lt[n4], lt[n5], lt[n6], 0 },
+// n = 0 .. 3 nT; row 3 nT + 1 = slow-path marker.
+__device__ __forceinline__ void build_mt(uint4 *mt, const uint32_t *lt, const uchar4 *trip, int nT, int lane)
+{
+    for (int n = lane; n <= 3 * nT; n += 32) {
+        const uchar4 t = trip[n];
+        mt[n] = make_uint4(lt[t.x], lt[t.y], lt[t.z], 0u);
+    }
+    if (lane == 0) mt[3 * nT + 1] = make_uint4(0u, 0u, 0u, 0x80000000u);
+}
 
 constexpr int kResPlanes = 10;   // planes of a warp's per-slot satisfied-bond count (<= 768)
 
@@ -103,36 +117,50 @@ __device__ __forceinline__ Planes planes_after(const Planes &p, uint32_t acc)
 
 // ------------------------------------------------------------------ rank of a draw
 // FAST: one 128-bit look-up keyed by the leading bits of the draw (float exponent + MB
-// mantissa bits, truncating conversion).  Entry = { 4*rank at the bucket's lower edge for the
-// classes n_sat = 4,5,6 in bytes 0..2, flag in bit 31 ; thr4 ; thr5 ; thr6 } where thr_c is
-// the (threshold - 1) of class c that lies inside the bucket, or 0xFFFFFFFF if there is none.
-// Buckets hold at most one threshold per class, so rank = rank_lo + (thr_c < u).  Entries with
-// bit 31 set (several thresholds of one class in the bucket, or draw < 2^8) take the exact
-// binary search.  The table sits at shared-memory offset 0, so the look-up address is one LEA.
+// mantissa bits, truncating conversion), then one 128-bit look-up of the three accept masks.
+//   bucket entry = { 16 * (n4 + n5 + n6 at the bucket's lower edge), thr4, thr5, thr6 }
+// where n_c = number of class-c thresholds <= the lower edge and thr_c = the (threshold - 1)
+// of class c inside the bucket, or 0xFFFFFFFF if there is none (at most one per class).
+// The COMBINED rank n = n4 + n5 + n6 of the draw is the lower-edge value plus (thr_c < u) for
+// the three classes.  As u grows the triple (n4, n5, n6) only ever changes at a threshold, so
+// n determines the triple: the per-slot mask table `mt` (3 nT + 2 rows of 16 bytes, rebuilt
+// after every swap round) holds in row n the three rank masks { lt[n4], lt[n5], lt[n6], 0 }.
+// Buckets with several thresholds of one class, and draws < 2^8, point at the last row, whose
+// fourth word is 0x80000000: the caller then redoes the quad with the exact binary search.
+// The three compares run on the FMA pipe: hi32(u * (2^32-1) + thr) = u - (thr < u).
 struct RankCtx {
     const uint32_t *thr;     // smem [3][LTS]  (exact search only)
-    const uint4 *bucket;     // smem, biased by -key_lo entries
-    int LTS, nT, key_lo, key_hi, key_shift;
+    const uint4 *bucket;     // smem
+    int LTS, nT, key_lo, key_shift;
     int z0, z1, z2;
+    uint32_t ones, c48, cm16;   // 0xFFFFFFFF, 48, -16 from kernel parameters (opaque to ptxas,
+                                // so the multiply-adds stay IMADs on the FMA pipe)
 };
 
-__device__ __forceinline__ uint4 bucket_entry(const RankCtx &R, uint32_t u)
+__device__ __forceinline__ uint32_t hi_mad(uint32_t u, uint32_t m, uint32_t t)
 {
-    int key = (int)(__float_as_uint(__uint2float_rz(u)) >> R.key_shift);
-    key = min(max(key, R.key_lo), R.key_hi);
-    return R.bucket[key];          // R.bucket is biased by -key_lo
+    uint64_t x;
+    asm("mad.wide.u32 %0, %1, %2, %3;" : "=l"(x) : "r"(u), "r"(m), "l"((uint64_t)t));
+    return (uint32_t)(x >> 32);
+}
+__device__ __forceinline__ uint32_t mad_lo(uint32_t a, uint32_t b, uint32_t c)
+{
+    uint32_t d;
+    asm("mad.lo.u32 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(c));
+    return d;
 }
 
-__device__ __forceinline__ uint32_t accept_fast(const uint32_t *lt, uint32_t u, const uint4 &e,
-                                                const Planes &p)
+// accept mask of one site from the mask table `mt` of its slot; *flag |= row.w
+__device__ __forceinline__ uint32_t accept_fast(const RankCtx &R, const uint4 *mt, uint32_t u,
+                                                const Planes &p, uint32_t *flag)
 {
-    const char *ltb = (const char *)lt;
-    uint32_t n4 = e.x & 0xFFu, n5 = __byte_perm(e.x, 0, 0x4441), n6 = __byte_perm(e.x, 0, 0x4442);
-    n4 += (e.y < u) ? 4u : 0u;
-    n5 += (e.z < u) ? 4u : 0u;
-    n6 += (e.w < u) ? 4u : 0u;
-    return accept_mask(p, *(const uint32_t *)(ltb + n4), *(const uint32_t *)(ltb + n5),
-                       *(const uint32_t *)(ltb + n6));
+    const int key = (int)(__float_as_uint(__uint2float_rz(u)) >> R.key_shift);
+    const uint4 e = R.bucket[max(key - R.key_lo, 0)];
+    const uint32_t d = hi_mad(u, R.ones, e.y) + hi_mad(u, R.ones, e.z) + hi_mad(u, R.ones, e.w);
+    const uint32_t off = mad_lo(d, R.cm16, mad_lo(u, R.c48, e.x));   // e.x + 16 * (3u - d)
+    const uint4 row = *reinterpret_cast<const uint4 *>(reinterpret_cast<const char *>(mt) + off);
+    *flag |= row.w;
+    return accept_mask(p, row.x, row.y, row.z);
 }
 
 __device__ __forceinline__ uint32_t accept_exact(const RankCtx &R, const uint32_t *lt, uint32_t u,
@@ -165,7 +193,7 @@ struct ResGeom {
 // [2][Nh]); nothing is stored.  EXACT = false: ranks from the bucket table; *flag collects
 // bit 31 of the entries (set: the caller must redo the quad with EXACT = true).
 template <int L, bool EXACT, bool ENERGY>
-__device__ __forceinline__ uint4 quad_body(const uint32_t *sp, const uint32_t *lt, const RankCtx &R,
+__device__ __forceinline__ uint4 quad_body(const uint32_t *sp, const uint32_t *lt, const uint4 *mt, const RankCtx &R,
                                            const QuadJ &J, int p, int s, int q, uint32_t oyp, uint32_t oym,
                                            uint32_t ozp, uint32_t ozm, const uint4 rnd, Planes (&fin)[4],
                                            uint32_t *flag)
@@ -212,13 +240,8 @@ __device__ __forceinline__ uint4 quad_body(const uint32_t *sp, const uint32_t *l
                                       xor3(m[l], jys[l], a_yp[l]), xor3(m[l], jym[l], a_ym[l]),
                                       xor3(m[l], jzs[l], a_zp[l]), xor3(m[l], jzm[l], a_zm[l]));
         uint32_t acc;
-        if (EXACT) {
-            acc = accept_exact(R, lt, u[l], pl);
-        } else {
-            const uint4 e = bucket_entry(R, u[l]);
-            fl |= e.x;
-            acc = accept_fast(lt, u[l], e, pl);
-        }
+        if (EXACT) acc = accept_exact(R, lt, u[l], pl);
+        else acc = accept_fast(R, mt, u[l], pl, &fl);
         out[l] = m[l] ^ acc;
         if (ENERGY) fin[l] = planes_after(pl, acc);
     }
@@ -227,7 +250,7 @@ __device__ __forceinline__ uint4 quad_body(const uint32_t *sp, const uint32_t *l
 }
 
 template <int L, bool FAST, bool ENERGY>
-__device__ __forceinline__ void update_quad_off(uint32_t *sp, const uint32_t *lt, const RankCtx &R,
+__device__ __forceinline__ void update_quad_off(uint32_t *sp, const uint32_t *lt, const uint4 *mt, const RankCtx &R,
                                                 const QuadJ &J, int p, int s, int q, uint32_t oyp,
                                                 uint32_t oym, uint32_t ozp, uint32_t ozm, const uint4 rnd,
                                                 Planes (&fin)[4])
@@ -235,29 +258,29 @@ __device__ __forceinline__ void update_quad_off(uint32_t *sp, const uint32_t *lt
     using Gm = ResGeom<L>;
     uint32_t flag = 0x80000000u;
     uint4 res;
-    if (FAST) res = quad_body<L, false, ENERGY>(sp, lt, R, J, p, s, q, oyp, oym, ozp, ozm, rnd, fin, &flag);
+    if (FAST) res = quad_body<L, false, ENERGY>(sp, lt, mt, R, J, p, s, q, oyp, oym, ozp, ozm, rnd, fin, &flag);
     // rare (or !FAST): redo the whole quad from memory with the exact search
-    if ((int)flag < 0) res = quad_body<L, true, ENERGY>(sp, lt, R, J, p, s, q, oyp, oym, ozp, ozm, rnd, fin, &flag);
+    if ((int)flag < 0) res = quad_body<L, true, ENERGY>(sp, lt, mt, R, J, p, s, q, oyp, oym, ozp, ozm, rnd, fin, &flag);
     reinterpret_cast<uint4 *>(sp + p * Gm::Nh)[q] = res;
 }
 
 // resident kernel: neighbour offsets packed two per register (16-bit halves, + in the low half)
 template <int L, bool FAST, bool ENERGY>
-__device__ __forceinline__ void update_quad(uint32_t *sp, const uint32_t *lt, const RankCtx &R,
+__device__ __forceinline__ void update_quad(uint32_t *sp, const uint32_t *lt, const uint4 *mt, const RankCtx &R,
                                             const QuadJ &J, int p, int s, int q, uint32_t offY, uint32_t offZ,
                                             const uint4 rnd, Planes (&fin)[4])
 {
-    update_quad_off<L, FAST, ENERGY>(sp, lt, R, J, p, s, q, offY & 0xFFFFu, offY >> 16, offZ & 0xFFFFu,
+    update_quad_off<L, FAST, ENERGY>(sp, lt, mt, R, J, p, s, q, offY & 0xFFFFu, offY >> 16, offZ & 0xFFFFu,
                                      offZ >> 16, rnd, fin);
 }
 
 // tiled kernel: neighbour quad indices
 template <int L, bool FAST, bool ENERGY>
-__device__ __forceinline__ void update_quad_wide(uint32_t *sp, const uint32_t *lt, const RankCtx &R,
+__device__ __forceinline__ void update_quad_wide(uint32_t *sp, const uint32_t *lt, const uint4 *mt, const RankCtx &R,
                                                  const QuadJ &J, int p, int s, int q, int qyp, int qym,
                                                  int qzp, int qzm, const uint4 rnd, Planes (&fin)[4])
 {
-    update_quad_off<L, FAST, ENERGY>(sp, lt, R, J, p, s, q, 16u * qyp, 16u * qym, 16u * qzp, 16u * qzm, rnd, fin);
+    update_quad_off<L, FAST, ENERGY>(sp, lt, mt, R, J, p, s, q, 16u * qyp, 16u * qym, 16u * qzp, 16u * qzm, rnd, fin);
 }
 
 // Couplings of quad q for parity p from global memory ([d][p][j], 3N words per word w).
@@ -357,7 +380,6 @@ __device__ __forceinline__ void cluster_wait()
     asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
 
-constexpr int kSwapWin = 64;   // swap thresholds for m in [-kSwapWin, -1] are staged in smem
 
 // Turn the warp's 10-plane satisfied-bond count of one slot (all 8 lanes of a group hold the
 // same planes) into integers and add them to the block's per-(slot, bit) accumulators: lane i
@@ -392,15 +414,18 @@ __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs
     const int q = tid % NQ, sg = tid / NQ;
 
     // shared memory: the rank table first (fixed offset 0), lattices next (16 B aligned)
+    const int MTS = 3 * nT + 2, SW = A.swap_win;
     uint4 *bucket = reinterpret_cast<uint4 *>(smem);                 // [n_bucket] 16 B entries
     uint32_t *sp = smem + 4 * (size_t)A.n_bucket;                    // [S][2][Nh]
-    uint32_t *lt = sp + (size_t)S * N;                               // [S][LTS]
+    uint4 *mt = reinterpret_cast<uint4 *>(sp + (size_t)S * N);       // [S][MTS] mask tables
+    uint32_t *lt = reinterpret_cast<uint32_t *>(mt + (size_t)S * MTS);   // [S][LTS]
     uint32_t *thr = lt + S * LTS;                                    // [3][LTS]
-    int32_t *Eall = (int32_t *)(thr + 3 * LTS);                      // [2][nT][32], by swap-round parity
-    int32_t *Eacc = Eall + 2 * nT * 32;                              // [S][32] satisfied-bond counts
+    uchar4 *trip = reinterpret_cast<uchar4 *>(thr + 3 * LTS);        // [MTS]
+    int32_t *Eacc = (int32_t *)(trip + MTS);                         // [S][32] satisfied-bond counts
     int32_t *swm = Eacc + S * 32;                                    // [nT][4]: lo, cnt, off, kinds
-    uint32_t *swwin = (uint32_t *)(swm + 4 * nT);                    // [nT][kSwapWin] thresholds - 1
-    uint8_t *tau8 = (uint8_t *)(swwin + nT * kSwapWin);              // [32][nT]
+    uint32_t *swwin = (uint32_t *)(swm + 4 * nT);                    // [nT][SW] thresholds - 1
+    int16_t *Eall = (int16_t *)(swwin + nT * SW);                    // [2][nT][32], by swap-round parity
+    uint8_t *tau8 = (uint8_t *)(Eall + 2 * nT * 32);                 // [32][nT]
     uint8_t *sig8 = tau8 + 32 * nT;                                  // [32][nT]
 
     // ---- load state: lattices of my slots, tables, permutation of my 32 realizations
@@ -417,13 +442,15 @@ __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs
         sig8[a] = P.sigma[(size_t)32 * w * nT + a];
     }
     for (int a = tid; a < S * 32; a += NT) Eacc[a] = 0;
-    for (int a = tid; a < 2 * nT * 32; a += NT) Eall[a] = P.E[(size_t)(32 * w + (a & 31)) * nT + ((a >> 5) % nT)];
+    for (int a = tid; a < 2 * nT * 32; a += NT)
+        Eall[a] = (int16_t)P.E[(size_t)(32 * w + (a & 31)) * nT + ((a >> 5) % nT)];   // |E| <= 3N <= 12288
+    for (int a = tid; a < MTS - 1; a += NT) trip[a] = A.trip[a];
     for (int t = tid; t + 1 < nT; t += NT) {
         swm[4 * t] = P.swp_lo[t]; swm[4 * t + 1] = P.swp_cnt[t]; swm[4 * t + 2] = P.swp_off[t];
         swm[4 * t + 3] = (int)P.swp_kind[2 * t] | ((int)P.swp_kind[2 * t + 1] << 1);
     }
-    for (int a = tid; a < (nT - 1) * kSwapWin; a += NT) {   // window m = -kSwapWin + i of row t
-        const int t = a / kSwapWin, m = -kSwapWin + a % kSwapWin;
+    for (int a = tid; a < (nT - 1) * SW; a += NT) {         // window m = -SW + i of row t
+        const int t = a / SW, m = -SW + a % SW;
         const int lo = P.swp_lo[t], cnt = P.swp_cnt[t];
         swwin[a] = (m >= lo && m < lo + cnt) ? P.swp_val[P.swp_off[t] + (m - lo)] : 0u;
     }
@@ -441,11 +468,14 @@ __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs
     asm volatile("" : "+r"(offY), "+r"(offZ));    // opaque: keep in registers, do not rematerialize
 
     RankCtx R;
-    R.thr = thr; R.bucket = bucket - A.key_lo; R.LTS = LTS; R.nT = nT;
-    R.key_lo = A.key_lo; R.key_hi = A.key_hi; R.key_shift = A.key_shift;
+    R.thr = thr; R.bucket = bucket; R.LTS = LTS; R.nT = nT;
+    R.key_lo = A.key_lo; R.key_shift = A.key_shift;
     R.z0 = P.z[0]; R.z1 = P.z[1]; R.z2 = P.z[2];
+    R.ones = A.ones; R.c48 = A.c48; R.cm16 = A.cm16;
     const uint32_t gw = P.w0 + (uint32_t)w;
     cg::cluster_group cl = cg::this_cluster();
+    __syncthreads();
+    for (int kl = tid >> 5; kl < nk; kl += NT >> 5) build_mt(mt + (size_t)kl * MTS, lt + kl * LTS, trip, nT, lane);
     if (C > 1) cl.sync(); else __syncthreads();   // every block's shared memory is initialised
 
     uint32_t nswap = A.nswap0;
@@ -457,14 +487,14 @@ __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs
         // ---------------- parity 0
         for (int kl = sg; kl < nk; kl += G) {
             const uint4 rnd = philox_rk(g, (uint32_t)q, gw, (uint32_t)(k0 + kl), A.rk);
-            update_quad<L, FAST, false>(sp + (size_t)kl * N, lt + kl * LTS, R, J0, 0, s0, q, offY, offZ, rnd, fin);
+            update_quad<L, FAST, false>(sp + (size_t)kl * N, lt + kl * LTS, mt + (size_t)kl * MTS, R, J0, 0, s0, q, offY, offZ, rnd, fin);
         }
         __syncthreads();
         // ---------------- parity 1 (+ satisfied-bond count of the finished sweep)
         if (!need_E) {
             for (int kl = sg; kl < nk; kl += G) {
                 const uint4 rnd = philox_rk(g, (uint32_t)q, gw, (1u << 16) | (uint32_t)(k0 + kl), A.rk);
-                update_quad<L, FAST, false>(sp + (size_t)kl * N, lt + kl * LTS, R, J1, 1, 1 - s0, q, offY, offZ,
+                update_quad<L, FAST, false>(sp + (size_t)kl * N, lt + kl * LTS, mt + (size_t)kl * MTS, R, J1, 1, 1 - s0, q, offY, offZ,
                                             rnd, fin);
             }
             __syncthreads();
@@ -477,7 +507,7 @@ __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs
                 const int kl = kb + i * G;
                 if (kl < nk) {
                     const uint4 rnd = philox_rk(g, (uint32_t)q, gw, (1u << 16) | (uint32_t)(k0 + kl), A.rk);
-                    update_quad<L, FAST, true>(sp + (size_t)kl * N, lt + kl * LTS, R, J1, 1, 1 - s0, q, offY,
+                    update_quad<L, FAST, true>(sp + (size_t)kl * N, lt + kl * LTS, mt + (size_t)kl * MTS, R, J1, 1, 1 - s0, q, offY,
                                                offZ, rnd, fin);
                     quad_sum(fin, en[i]);
                 } else {
@@ -494,15 +524,15 @@ __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs
         __syncthreads();
         // ---- energies of my slots: E = 3N - 2 (satisfied bonds); pushed into every block of
         //      the cluster (distributed shared memory), buffer chosen by the swap-round parity
-        int32_t *Ebuf = Eall + (nswap & 1u) * nT * 32;
+        int16_t *Ebuf = Eall + (nswap & 1u) * nT * 32;
         for (int a = tid; a < nk * 32; a += NT) {
             const int e = 3 * N - 2 * Eacc[a];
             Eacc[a] = 0;
             const int dst = k0 * 32 + a;
             if (C > 1) {
-                for (int rr = 0; rr < C; ++rr) cl.map_shared_rank(Ebuf, rr)[dst] = e;
+                for (int rr = 0; rr < C; ++rr) cl.map_shared_rank(Ebuf, rr)[dst] = (int16_t)e;
             } else {
-                Ebuf[dst] = e;
+                Ebuf[dst] = (int16_t)e;
             }
         }
         if (!swap_now) { __syncthreads(); continue; }
@@ -513,13 +543,13 @@ __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs
         for (int t = (int)(nswap & 1u) + 2 * warp; t + 1 < nT; t += 2 * nwarp) {
             uint8_t *sg_ = sig8 + lane * nT, *ta_ = tau8 + lane * nT;
             const int sa = sg_[t], sb = sg_[t + 1];
-            const int m = (Ebuf[sa * 32 + lane] - Ebuf[sb * 32 + lane]) / 4;
+            const int m = ((int)Ebuf[sa * 32 + lane] - (int)Ebuf[sb * 32 + lane]) / 4;
             const uint4 v = philox_rk(g, (uint32_t)t, P.r0 + (uint32_t)(32 * w + lane), 2u << 16, A.rk);
             const int lo = swm[4 * t], cnt = swm[4 * t + 1], kinds = swm[4 * t + 3];
             bool acc;
             if (m < lo) acc = kinds & 1;
             else if (m >= lo + cnt) acc = (kinds >> 1) & 1;
-            else if (m >= -kSwapWin && m < 0) acc = v.x <= swwin[t * kSwapWin + m + kSwapWin];
+            else if (m >= -SW && m < 0) acc = v.x <= swwin[t * SW + m + SW];
             else acc = v.x <= P.swp_val[swm[4 * t + 2] + (m - lo)];
             if (acc) {
                 sg_[t] = (uint8_t)sb; sg_[t + 1] = (uint8_t)sa;
@@ -536,6 +566,8 @@ __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs
                 const uint32_t mk = __ballot_sync(0xFFFFFFFFu, pos >= n);
                 if (lane == (n & 31)) lt[kl * LTS + n] = mk;
             }
+            __syncwarp();
+            build_mt(mt + (size_t)kl * MTS, lt + kl * LTS, trip, nT, lane);
         }
         __syncthreads();
     }
@@ -543,7 +575,7 @@ __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs
     // last sweep always computes them; which buffer depends on whether that sweep swapped
     const bool last_swapped = A.swap_interval > 0 &&
                               ((uint64_t)A.g0 + (uint64_t)A.n_sweeps) % (uint64_t)A.swap_interval == 0;
-    const int32_t *Elast = Eall + (((last_swapped ? nswap - 1 : nswap) & 1u) * nT * 32);
+    const int16_t *Elast = Eall + (((last_swapped ? nswap - 1 : nswap) & 1u) * nT * 32);
     if (C > 1) cl.sync();                         // no block exits while others may still push to it
 
     // ---- write back

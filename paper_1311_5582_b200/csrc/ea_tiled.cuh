@@ -22,7 +22,9 @@ struct TiledArgs {
     int n_kgroups;           // ceil(nT / SK)
     int32_t *Ecnt;           // [Rp][nT] satisfied-bond counters (ENERGY pass), zeroed by k_tiled_finish
     const uint4 *bucket;
-    int n_bucket, key_lo, key_hi, key_shift;
+    const uchar4 *trip;      // [3 nT + 1] (n4, n5, n6) of every combined rank
+    int n_bucket, key_lo, key_shift;
+    uint32_t ones, c48, cm16;
     uint32_t rk[20];
 };
 
@@ -54,14 +56,18 @@ __global__ void __launch_bounds__(TileGeom<L>::NTHR, 1) k_tiled_half(const Tiled
     const int tid = threadIdx.x, lane = tid & 31;
     const int q = slab * NT + tid;                // quad index inside a parity array
 
+    const int MTS = 3 * nT + 2;
     uint4 *bucket = reinterpret_cast<uint4 *>(smem);               // [n_bucket]
-    uint32_t *lt = smem + 4 * (size_t)A.n_bucket;                  // [SK][LTS]
+    uint4 *mt = bucket + A.n_bucket;                               // [SK][MTS] mask tables
+    uint32_t *lt = reinterpret_cast<uint32_t *>(mt + (size_t)SK * MTS);   // [SK][LTS]
     uint32_t *thr = lt + SK * LTS;                                 // [3][LTS]
-    int32_t *Eacc = (int32_t *)(thr + 3 * LTS);                    // [SK][32]
+    uchar4 *trip = reinterpret_cast<uchar4 *>(thr + 3 * LTS);      // [MTS]
+    int32_t *Eacc = (int32_t *)(trip + MTS);                       // [SK][32]
 
     for (int a = tid; a < A.n_bucket; a += NT) bucket[a] = A.bucket[a];
     for (int a = tid; a < nk * LTS; a += NT) lt[a] = P.lt[((size_t)w * nT + k0) * LTS + a];
     for (int a = tid; a < 3 * LTS; a += NT) thr[a] = P.thr32[a];
+    for (int a = tid; a < MTS - 1; a += NT) trip[a] = A.trip[a];
     if (ENERGY) for (int a = tid; a < SK * 32; a += NT) Eacc[a] = 0;
 
     const int qx = q % QR, y = (q / QR) % L, z = q / (QR * L);
@@ -71,19 +77,24 @@ __global__ void __launch_bounds__(TileGeom<L>::NTHR, 1) k_tiled_half(const Tiled
     const QuadJ J = load_quad_j<L>(P.coup + (size_t)w * 3 * N, p, s, q, qx, qym, qzm);
     // neighbour byte offsets do not fit 16 bits for L = 32, 64: pass quad indices * 16 directly
     RankCtx R;
-    R.thr = thr; R.bucket = bucket - A.key_lo; R.LTS = LTS; R.nT = nT;
-    R.key_lo = A.key_lo; R.key_hi = A.key_hi; R.key_shift = A.key_shift;
+    R.thr = thr; R.bucket = bucket; R.LTS = LTS; R.nT = nT;
+    R.key_lo = A.key_lo; R.key_shift = A.key_shift;
     R.z0 = P.z[0]; R.z1 = P.z[1]; R.z2 = P.z[2];
+    R.ones = A.ones; R.c48 = A.c48; R.cm16 = A.cm16;
     const uint32_t gw = P.w0 + (uint32_t)w;
     const uint32_t c3 = (uint32_t)p << 16;
     __syncthreads();
+    if (FAST) {
+        for (int kl = tid >> 5; kl < nk; kl += NT >> 5) build_mt(mt + (size_t)kl * MTS, lt + kl * LTS, trip, nT, lane);
+        __syncthreads();
+    }
 
     Planes fin[4];
     if (!ENERGY) {
         for (int kl = 0; kl < nk; ++kl) {
             uint32_t *sp = P.spin + ((size_t)(k0 + kl) * P.W + w) * N;
             const uint4 rnd = philox_rk(A.g, (uint32_t)q, gw, c3 | (uint32_t)(k0 + kl), A.rk);
-            update_quad_wide<L, FAST, false>(sp, lt + kl * LTS, R, J, p, s, q, qyp, qym, qzp, qzm, rnd, fin);
+            update_quad_wide<L, FAST, false>(sp, lt + kl * LTS, mt + (size_t)kl * MTS, R, J, p, s, q, qyp, qym, qzp, qzm, rnd, fin);
         }
     }
     for (int kb = 0; ENERGY && kb < SK; kb += 4) {
@@ -94,7 +105,7 @@ __global__ void __launch_bounds__(TileGeom<L>::NTHR, 1) k_tiled_half(const Tiled
             if (kl < nk) {
                 uint32_t *sp = P.spin + ((size_t)(k0 + kl) * P.W + w) * N;
                 const uint4 rnd = philox_rk(A.g, (uint32_t)q, gw, c3 | (uint32_t)(k0 + kl), A.rk);
-                update_quad_wide<L, FAST, true>(sp, lt + kl * LTS, R, J, p, s, q, qyp, qym, qzp, qzm, rnd, fin);
+                update_quad_wide<L, FAST, true>(sp, lt + kl * LTS, mt + (size_t)kl * MTS, R, J, p, s, q, qyp, qym, qzp, qzm, rnd, fin);
                 quad_sum(fin, en[i]);
             } else {
 #pragma unroll
