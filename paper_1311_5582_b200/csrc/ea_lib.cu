@@ -179,6 +179,13 @@ static bool build_bucket_table(const std::vector<uint32_t> &thr32, const int z[3
         }
         if (slow_mass < 1e-5 || MB == 6) {
             if (slow_mass > 1e-3) return false;
+            // entries above the largest threshold are identical: keep one (the kernels clamp)
+            size_t keep = t.size();
+            while (keep > 1 && t[keep - 2].x == t[keep - 1].x && t[keep - 2].y == 0xFFFFFFFFu &&
+                   t[keep - 2].z == 0xFFFFFFFFu && t[keep - 2].w == 0xFFFFFFFFu &&
+                   t[keep - 1].y == 0xFFFFFFFFu && t[keep - 1].z == 0xFFFFFFFFu && t[keep - 1].w == 0xFFFFFFFFu)
+                --keep;
+            t.resize(keep);
             tab = t; key_lo = klo; key_shift = 23 - MB;
             return true;
         }
@@ -567,7 +574,7 @@ static int sweep_resident(ea_handle *h, int64_t n_sweeps, int swap_interval)
         A.C = pl.C; A.S = pl.S;
         A.bucket = h->d_bucket; A.n_bucket = h->n_bucket; A.trip = h->d_trip;
         A.key_lo = h->key_lo; A.key_shift = h->key_shift; A.swap_win = pl.swap_win;
-        A.ones = 0xFFFFFFFFu; A.c48 = 48u; A.cm16 = (uint32_t)-16;
+        A.ones = 0xFFFFFFFFu; A.c48 = 48u; A.cm16 = (uint32_t)-16; A.c16 = 16u;
         for (int r = 0; r < 10; ++r) {
             A.rk[2 * r] = h->P.k0 + (uint32_t)r * 0x9E3779B9u;
             A.rk[2 * r + 1] = h->P.k1 + (uint32_t)r * 0xBB67AE85u;
@@ -640,7 +647,7 @@ static int sweep_tiled(ea_handle *h, int64_t n_sweeps, int swap_interval)
     A.P = h->P; A.SK = pl.SK; A.n_kgroups = pl.nkg; A.Ecnt = h->d_Ecnt;
     A.bucket = h->d_bucket; A.n_bucket = h->n_bucket; A.trip = h->d_trip;
     A.key_lo = h->key_lo; A.key_shift = h->key_shift;
-    A.ones = 0xFFFFFFFFu; A.c48 = 48u; A.cm16 = (uint32_t)-16;
+    A.ones = 0xFFFFFFFFu; A.c48 = 48u; A.cm16 = (uint32_t)-16; A.c16 = 16u;
     for (int r = 0; r < 10; ++r) {
         A.rk[2 * r] = h->P.k0 + (uint32_t)r * 0x9E3779B9u;
         A.rk[2 * r + 1] = h->P.k1 + (uint32_t)r * 0xBB67AE85u;

@@ -30,7 +30,7 @@ struct ResArgs {
     uint32_t rk[20];          // Philox round keys (k0 + r*0x9E3779B9, k1 + r*0xBB67AE85), r = 0..9
     int n_bucket, key_lo, key_shift;
     int swap_win;             // swap thresholds for m in [-swap_win, -1] are staged in smem
-    uint32_t ones, c48, cm16; // 0xFFFFFFFF, 48, (uint32_t)-16: see RankCtx
+    uint32_t ones, c48, cm16, c16; // 0xFFFFFFFF, 48, (uint32_t)-16, 16: see RankCtx
 };
 
 // Mask table of one slot from its rank masks (one warp): row n = { lt[n4], lt[n5], lt[n6], 0 },
@@ -131,10 +131,10 @@ __device__ __forceinline__ Planes planes_after(const Planes &p, uint32_t acc)
 struct RankCtx {
     const uint32_t *thr;     // smem [3][LTS]  (exact search only)
     const uint4 *bucket;     // smem
-    int LTS, nT, key_lo, key_shift;
+    int LTS, nT, key_lo, key_top, key_shift;   // table index = min(max(key - key_lo, 0), key_top)
     int z0, z1, z2;
-    uint32_t ones, c48, cm16;   // 0xFFFFFFFF, 48, -16 from kernel parameters (opaque to ptxas,
-                                // so the multiply-adds stay IMADs on the FMA pipe)
+    uint32_t ones, c48, cm16, c16;   // 0xFFFFFFFF, 48, -16, 16 from kernel parameters (opaque to
+                                     // ptxas, so the multiply-adds stay IMADs on the FMA pipe)
 };
 
 __device__ __forceinline__ uint32_t hi_mad(uint32_t u, uint32_t m, uint32_t t)
@@ -155,7 +155,10 @@ __device__ __forceinline__ uint32_t accept_fast(const RankCtx &R, const uint4 *m
                                                 const Planes &p, uint32_t *flag)
 {
     const int key = (int)(__float_as_uint(__uint2float_rz(u)) >> R.key_shift);
-    const uint4 e = R.bucket[max(key - R.key_lo, 0)];
+    // every bucket above the largest threshold holds the same entry: clamping keeps the 86 % of
+    // the draws that land there on ONE shared-memory address (broadcast, no bank conflicts)
+    const uint32_t boff = mad_lo((uint32_t)min(max(key - R.key_lo, 0), R.key_top), R.c16, 0u);
+    const uint4 e = *reinterpret_cast<const uint4 *>(reinterpret_cast<const char *>(R.bucket) + boff);
     const uint32_t d = hi_mad(u, R.ones, e.y) + hi_mad(u, R.ones, e.z) + hi_mad(u, R.ones, e.w);
     const uint32_t off = mad_lo(d, R.cm16, mad_lo(u, R.c48, e.x));   // e.x + 16 * (3u - d)
     const uint4 row = *reinterpret_cast<const uint4 *>(reinterpret_cast<const char *>(mt) + off);
@@ -192,7 +195,7 @@ struct ResGeom {
 // New spin words of the four sites of quad q (parity p) of one slot's lattice `sp` (smem,
 // [2][Nh]); nothing is stored.  EXACT = false: ranks from the bucket table; *flag collects
 // bit 31 of the entries (set: the caller must redo the quad with EXACT = true).
-template <int L, bool EXACT, bool ENERGY>
+template <int L, bool EXACT, bool ENERGY, bool UNIS>
 __device__ __forceinline__ uint4 quad_body(const uint32_t *sp, const uint32_t *lt, const uint4 *mt, const RankCtx &R,
                                            const QuadJ &J, int p, int s, int q, uint32_t oyp, uint32_t oym,
                                            uint32_t ozp, uint32_t ozm, const uint4 rnd, Planes (&fin)[4],
@@ -208,27 +211,45 @@ __device__ __forceinline__ uint4 quad_body(const uint32_t *sp, const uint32_t *l
     const uint4 ym = *reinterpret_cast<const uint4 *>(oth_b + oym);
     const uint4 zp = *reinterpret_cast<const uint4 *>(oth_b + ozp);
     const uint4 zm = *reinterpret_cast<const uint4 *>(oth_b + ozm);
-    uint32_t ext = s ? v.x : v.w;
-    if (Gm::QR > 1) {
-        // the word beyond the quad comes from the next (s) / previous (!s) quad of the row
-        const int qx = q & (Gm::QR - 1);
-        const int qn = (q - qx) + ((qx + (s ? 1 : Gm::QR - 1)) & (Gm::QR - 1));
-        if (EXACT) {   // divergent (rare) path: no shuffle, read the neighbour quad's word
-            ext = reinterpret_cast<const uint32_t *>(oth_b)[4 * qn + (s ? 0 : 3)];
-        } else {
-            ext = __shfl_sync(0xFFFFFFFFu, ext, qn & 31);
-        }
-    }
-    uint4 sh;   // the x neighbour that is not index-aligned: x+1 if s, x-1 otherwise
-    sh.x = s ? v.y : ext;
-    sh.y = s ? v.z : v.x;
-    sh.z = s ? v.w : v.y;
-    sh.w = s ? ext : v.z;
     const uint32_t m[4] = {me.x, me.y, me.z, me.w};
-    const uint32_t va[4] = {v.x, v.y, v.z, v.w}, vb[4] = {sh.x, sh.y, sh.z, sh.w};
+    const uint32_t jb[4] = {J.jb.x, J.jb.y, J.jb.z, J.jb.w};
+    // x neighbour that is not index-aligned: x+1 if s, x-1 otherwise; the word beyond the quad
+    // (ext) comes from the next (s) / previous (!s) quad of the row
+    uint32_t eb[4];
+    const int qx = q & (Gm::QR - 1);
+    if (UNIS && !EXACT) {
+        // s is warp-uniform (diagonal thread mapping of the resident kernel): a branch instead
+        // of five selects; quads of a row sit in adjacent lanes
+        const int lane = threadIdx.x & 31;
+        const int ln = (lane & ~(Gm::QR - 1)) | ((lane + (s ? 1 : Gm::QR - 1)) & (Gm::QR - 1));
+        if (s) {
+            const uint32_t ext = Gm::QR > 1 ? __shfl_sync(0xFFFFFFFFu, v.x, ln) : v.x;
+            eb[0] = xor3(m[0], jb[0], v.y); eb[1] = xor3(m[1], jb[1], v.z);
+            eb[2] = xor3(m[2], jb[2], v.w); eb[3] = xor3(m[3], jb[3], ext);
+        } else {
+            const uint32_t ext = Gm::QR > 1 ? __shfl_sync(0xFFFFFFFFu, v.w, ln) : v.w;
+            eb[0] = xor3(m[0], jb[0], ext); eb[1] = xor3(m[1], jb[1], v.x);
+            eb[2] = xor3(m[2], jb[2], v.y); eb[3] = xor3(m[3], jb[3], v.z);
+        }
+    } else {
+        uint32_t ext = s ? v.x : v.w;
+        if (Gm::QR > 1) {
+            if (EXACT) {   // divergent (rare) path: no shuffle, read the neighbour quad's word
+                const int qn = (q - qx) + ((qx + (s ? 1 : Gm::QR - 1)) & (Gm::QR - 1));
+                ext = reinterpret_cast<const uint32_t *>(oth_b)[4 * qn + (s ? 0 : 3)];
+            } else {
+                const int lane = threadIdx.x & 31;
+                const int ln = (lane & ~(Gm::QR - 1)) | ((lane + (s ? 1 : Gm::QR - 1)) & (Gm::QR - 1));
+                ext = __shfl_sync(0xFFFFFFFFu, ext, ln);
+            }
+        }
+        eb[0] = xor3(m[0], jb[0], s ? v.y : ext); eb[1] = xor3(m[1], jb[1], s ? v.z : v.x);
+        eb[2] = xor3(m[2], jb[2], s ? v.w : v.y); eb[3] = xor3(m[3], jb[3], s ? ext : v.z);
+    }
+    const uint32_t va[4] = {v.x, v.y, v.z, v.w};
     const uint32_t a_yp[4] = {yp.x, yp.y, yp.z, yp.w}, a_ym[4] = {ym.x, ym.y, ym.z, ym.w};
     const uint32_t a_zp[4] = {zp.x, zp.y, zp.z, zp.w}, a_zm[4] = {zm.x, zm.y, zm.z, zm.w};
-    const uint32_t ja[4] = {J.ja.x, J.ja.y, J.ja.z, J.ja.w}, jb[4] = {J.jb.x, J.jb.y, J.jb.z, J.jb.w};
+    const uint32_t ja[4] = {J.ja.x, J.ja.y, J.ja.z, J.ja.w};
     const uint32_t jys[4] = {J.jys.x, J.jys.y, J.jys.z, J.jys.w}, jym[4] = {J.jym.x, J.jym.y, J.jym.z, J.jym.w};
     const uint32_t jzs[4] = {J.jzs.x, J.jzs.y, J.jzs.z, J.jzs.w}, jzm[4] = {J.jzm.x, J.jzm.y, J.jzm.z, J.jzm.w};
     const uint32_t u[4] = {rnd.x, rnd.y, rnd.z, rnd.w};
@@ -236,7 +257,7 @@ __device__ __forceinline__ uint4 quad_body(const uint32_t *sp, const uint32_t *l
     uint32_t fl = 0;
 #pragma unroll
     for (int l = 0; l < 4; ++l) {
-        const Planes pl = nsat_planes(xor3(m[l], ja[l], va[l]), xor3(m[l], jb[l], vb[l]),
+        const Planes pl = nsat_planes(xor3(m[l], ja[l], va[l]), eb[l],
                                       xor3(m[l], jys[l], a_yp[l]), xor3(m[l], jym[l], a_ym[l]),
                                       xor3(m[l], jzs[l], a_zp[l]), xor3(m[l], jzm[l], a_zm[l]));
         uint32_t acc;
@@ -249,7 +270,7 @@ __device__ __forceinline__ uint4 quad_body(const uint32_t *sp, const uint32_t *l
     return make_uint4(out[0], out[1], out[2], out[3]);
 }
 
-template <int L, bool FAST, bool ENERGY>
+template <int L, bool FAST, bool ENERGY, bool UNIS>
 __device__ __forceinline__ void update_quad_off(uint32_t *sp, const uint32_t *lt, const uint4 *mt, const RankCtx &R,
                                                 const QuadJ &J, int p, int s, int q, uint32_t oyp,
                                                 uint32_t oym, uint32_t ozp, uint32_t ozm, const uint4 rnd,
@@ -258,9 +279,9 @@ __device__ __forceinline__ void update_quad_off(uint32_t *sp, const uint32_t *lt
     using Gm = ResGeom<L>;
     uint32_t flag = 0x80000000u;
     uint4 res;
-    if (FAST) res = quad_body<L, false, ENERGY>(sp, lt, mt, R, J, p, s, q, oyp, oym, ozp, ozm, rnd, fin, &flag);
+    if (FAST) res = quad_body<L, false, ENERGY, UNIS>(sp, lt, mt, R, J, p, s, q, oyp, oym, ozp, ozm, rnd, fin, &flag);
     // rare (or !FAST): redo the whole quad from memory with the exact search
-    if ((int)flag < 0) res = quad_body<L, true, ENERGY>(sp, lt, mt, R, J, p, s, q, oyp, oym, ozp, ozm, rnd, fin, &flag);
+    if ((int)flag < 0) res = quad_body<L, true, ENERGY, UNIS>(sp, lt, mt, R, J, p, s, q, oyp, oym, ozp, ozm, rnd, fin, &flag);
     reinterpret_cast<uint4 *>(sp + p * Gm::Nh)[q] = res;
 }
 
@@ -270,7 +291,7 @@ __device__ __forceinline__ void update_quad(uint32_t *sp, const uint32_t *lt, co
                                             const QuadJ &J, int p, int s, int q, uint32_t offY, uint32_t offZ,
                                             const uint4 rnd, Planes (&fin)[4])
 {
-    update_quad_off<L, FAST, ENERGY>(sp, lt, mt, R, J, p, s, q, offY & 0xFFFFu, offY >> 16, offZ & 0xFFFFu,
+    update_quad_off<L, FAST, ENERGY, true>(sp, lt, mt, R, J, p, s, q, offY & 0xFFFFu, offY >> 16, offZ & 0xFFFFu,
                                      offZ >> 16, rnd, fin);
 }
 
@@ -280,7 +301,7 @@ __device__ __forceinline__ void update_quad_wide(uint32_t *sp, const uint32_t *l
                                                  const QuadJ &J, int p, int s, int q, int qyp, int qym,
                                                  int qzp, int qzm, const uint4 rnd, Planes (&fin)[4])
 {
-    update_quad_off<L, FAST, ENERGY>(sp, lt, mt, R, J, p, s, q, 16u * qyp, 16u * qym, 16u * qzp, 16u * qzm, rnd, fin);
+    update_quad_off<L, FAST, ENERGY, false>(sp, lt, mt, R, J, p, s, q, 16u * qyp, 16u * qym, 16u * qzp, 16u * qzm, rnd, fin);
 }
 
 // Couplings of quad q for parity p from global memory ([d][p][j], 3N words per word w).
@@ -411,7 +432,16 @@ __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs
     const int k0 = rank * S;
     const int nk = max(0, min(S, nT - k0));      // slots owned by this block
     const int tid = threadIdx.x, lane = tid & 31;
-    const int q = tid % NQ, sg = tid / NQ;
+    const int sg = tid / NQ;
+    // Diagonal thread mapping: a warp owns whole diagonals y - z = d (mod L) of one parity of d,
+    // so s = (y + z + p) & 1 = (d + p) & 1 is warp-uniform, and a quarter-warp's consecutive
+    // rows (y+1, z+1) are (L+1) rows apart in memory: its 128-bit accesses hit all 32 banks once.
+    constexpr int RW = 32 / QR, DW = RW / L;                       // rows, diagonals per warp
+    static_assert(RW % L == 0 && DW >= 1, "a warp must hold whole diagonals (L = 8, 16)");
+    const int lw = (tid % NQ) >> 5, rr = lane / QR;
+    const int dq = (lw & 1) + 2 * ((lw >> 1) * DW + rr / L);       // my diagonal
+    const int z = rr % L, y = (z + dq) % L, qx = lane % QR;
+    const int q = qx + QR * (y + L * z);
 
     // shared memory: the rank table first (fixed offset 0), lattices next (16 B aligned)
     const int MTS = 3 * nT + 2, SW = A.swap_win;
@@ -456,10 +486,9 @@ __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs
     }
 
     // ---- per-thread geometry and couplings (registers, both parities)
-    const int qx = q % QR, y = (q / QR) % L, z = q / (QR * L);
     const int qyp = qx + QR * (wrap_inc(y, L) + L * z), qym = qx + QR * (wrap_dec(y, L) + L * z);
     const int qzp = qx + QR * (y + L * wrap_inc(z, L)), qzm = qx + QR * (y + L * wrap_dec(z, L));
-    const int s0 = (y + z) & 1;                   // s for parity 0; parity 1 uses 1 - s0
+    const int s0 = __shfl_sync(0xFFFFFFFFu, (y + z) & 1, 0);   // warp-uniform; parity 1 uses 1 - s0
     const uint32_t *cp = P.coup + (size_t)w * 3 * N;
     const QuadJ J0 = load_quad_j<L>(cp, 0, s0, q, qx, qym, qzm);
     const QuadJ J1 = load_quad_j<L>(cp, 1, 1 - s0, q, qx, qym, qzm);
@@ -469,9 +498,9 @@ __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs
 
     RankCtx R;
     R.thr = thr; R.bucket = bucket; R.LTS = LTS; R.nT = nT;
-    R.key_lo = A.key_lo; R.key_shift = A.key_shift;
+    R.key_lo = A.key_lo; R.key_top = A.n_bucket - 1; R.key_shift = A.key_shift;
     R.z0 = P.z[0]; R.z1 = P.z[1]; R.z2 = P.z[2];
-    R.ones = A.ones; R.c48 = A.c48; R.cm16 = A.cm16;
+    R.ones = A.ones; R.c48 = A.c48; R.cm16 = A.cm16; R.c16 = A.c16;
     const uint32_t gw = P.w0 + (uint32_t)w;
     cg::cluster_group cl = cg::this_cluster();
     __syncthreads();

@@ -24,7 +24,7 @@ struct TiledArgs {
     const uint4 *bucket;
     const uchar4 *trip;      // [3 nT + 1] (n4, n5, n6) of every combined rank
     int n_bucket, key_lo, key_shift;
-    uint32_t ones, c48, cm16;
+    uint32_t ones, c48, cm16, c16;
     uint32_t rk[20];
 };
 
@@ -78,9 +78,9 @@ __global__ void __launch_bounds__(TileGeom<L>::NTHR, 1) k_tiled_half(const Tiled
     // neighbour byte offsets do not fit 16 bits for L = 32, 64: pass quad indices * 16 directly
     RankCtx R;
     R.thr = thr; R.bucket = bucket; R.LTS = LTS; R.nT = nT;
-    R.key_lo = A.key_lo; R.key_shift = A.key_shift;
+    R.key_lo = A.key_lo; R.key_top = A.n_bucket - 1; R.key_shift = A.key_shift;
     R.z0 = P.z[0]; R.z1 = P.z[1]; R.z2 = P.z[2];
-    R.ones = A.ones; R.c48 = A.c48; R.cm16 = A.cm16;
+    R.ones = A.ones; R.c48 = A.c48; R.cm16 = A.cm16; R.c16 = A.c16;
     const uint32_t gw = P.w0 + (uint32_t)w;
     const uint32_t c3 = (uint32_t)p << 16;
     __syncthreads();
