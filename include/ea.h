@@ -45,7 +45,11 @@ enum {
     EA_KERNEL_GENERIC = 1,   /* any even L: one launch per half-sweep, global memory        */
     EA_KERNEL_RESIDENT = 2,  /* L in {8,16}: lattices resident in shared memory, one launch
                                 for all sweeps of the call, PT inside a thread-block cluster */
-    EA_KERNEL_TILED = 3      /* L = 32 (and 8,16): z-slab tiles streamed through shared memory */
+    EA_KERNEL_TILED = 3,     /* L = 16, 32, 64: z-slab tiles, one launch per half-sweep, lattice
+                                read in place from global memory (L1/L2)                     */
+    EA_KERNEL_STREAM = 4     /* L = 32, 64: one persistent cooperative launch for all sweeps; z-slab
+                                tiles streamed through shared memory by TMA bulk copies, two
+                                grid-wide barriers per sweep, PT decided redundantly per block */
 };
 
 /*
@@ -124,7 +128,7 @@ int ea_get_state(ea_handle *h, uint32_t *spin_words /* [n_temps][W][2][N/2] */,
 
 /* Select the sweep implementation (EA_KERNEL_*); EA_ERR_UNSUPPORTED if it cannot run this shape. */
 int ea_set_kernel(ea_handle *h, int kernel);
-/* The implementation ea_sweep would use now (EA_KERNEL_GENERIC/RESIDENT/TILED). */
+/* The implementation ea_sweep would use now (EA_KERNEL_GENERIC/RESIDENT/TILED/STREAM). */
 int ea_get_kernel(ea_handle *h);
 /* Number of kernels this handle has launched so far. */
 int64_t ea_launch_count(ea_handle *h);

@@ -6,8 +6,8 @@ kernels of csrc/.  PyTorch is used for device memory (the workspace tensor) and 
 There is no CPU fallback: importing works without a GPU (so the symbol table can be
 checked), creating a simulation does not.
 """
-from .binding import (EA, EA_KERNEL_AUTO, EA_KERNEL_GENERIC, EA_KERNEL_RESIDENT, EA_KERNEL_TILED,
+from .binding import (EA, EA_KERNEL_AUTO, EA_KERNEL_GENERIC, EA_KERNEL_RESIDENT, EA_KERNEL_TILED, EA_KERNEL_STREAM,
                       EAError, exported_symbols, lib, library_path, measure_int_peak)
 
 __all__ = ["EA", "EAError", "lib", "library_path", "exported_symbols", "measure_int_peak", "EA_KERNEL_AUTO",
-           "EA_KERNEL_GENERIC", "EA_KERNEL_RESIDENT", "EA_KERNEL_TILED"]
+           "EA_KERNEL_GENERIC", "EA_KERNEL_RESIDENT", "EA_KERNEL_TILED", "EA_KERNEL_STREAM"]

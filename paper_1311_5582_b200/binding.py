@@ -10,7 +10,7 @@ _PKG = Path(__file__).resolve().parent
 _LIB_PATH = _PKG / "libea_b200.so"
 _lib = None
 
-EA_KERNEL_AUTO, EA_KERNEL_GENERIC, EA_KERNEL_RESIDENT, EA_KERNEL_TILED = 0, 1, 2, 3
+EA_KERNEL_AUTO, EA_KERNEL_GENERIC, EA_KERNEL_RESIDENT, EA_KERNEL_TILED, EA_KERNEL_STREAM = 0, 1, 2, 3, 4
 
 _SYMBOLS = [
     "ea_create", "ea_workspace_bytes", "ea_create_ex", "ea_destroy", "ea_set_couplings",

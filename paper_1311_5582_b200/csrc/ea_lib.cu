@@ -13,6 +13,7 @@
 #include "ea_generic.cuh"
 #include "ea_resident.cuh"
 #include "ea_tiled.cuh"
+#include "ea_stream.cuh"
 #include "ea_peak.cuh"
 
 using ea::Params;
@@ -95,7 +96,7 @@ Layout make_layout(int L, int nT, int R)
     o.swp_val = take(4 * (o.swp_val_cap ? o.swp_val_cap : 1));
     o.bucket = take(16 * (size_t)kMaxBucket);
     o.trip = take(4 * (3 * (size_t)nT + 2));
-    o.ecnt = take(4 * Rp * nT);
+    o.ecnt = take(2 * 4 * Rp * nT);      // double-buffered by the streaming kernel
     o.total = off;
     return o;
 }
@@ -388,7 +389,7 @@ extern "C" ea_handle *ea_create_ex(int L, int n_temps, int n_realizations, const
     launch_cfg((int64_t)h->Rp * n_temps, 128, grid);
     ea::k_identity_perm<<<grid, 128, 0, h->stream>>>(P);
     h->launches += 2;
-    cudaMemsetAsync(h->d_Ecnt, 0, 4 * (size_t)h->Rp * n_temps, h->stream);
+    cudaMemsetAsync(h->d_Ecnt, 0, 2 * 4 * (size_t)h->Rp * n_temps, h->stream);
     if (rebuild_lt(h) != EA_OK || recompute_energy(h) != EA_OK ||
         cudaStreamSynchronize(h->stream) != cudaSuccess || cudaGetLastError() != cudaSuccess)
         return (ea_handle *)bail(EA_ERR_CUDA, "ea_create: initialisation kernels failed: " + h->err);
@@ -682,10 +683,97 @@ static int sweep_tiled(ea_handle *h, int64_t n_sweeps, int swap_interval)
     return EA_OK;
 }
 
+// ---------------------------------------------------------------- streaming path (L = 32, 64)
+namespace {
+struct StreamPlan { bool ok; int grid, MS, MW; size_t smem; };
+
+template <int L>
+StreamPlan plan_stream_t(const ea_handle *h)
+{
+    using Sg = ea::StreamGeom<L>;
+    StreamPlan pl{false, 0, 0, 0, 0};
+    const long long T = (long long)h->W * Sg::NSLAB * h->nT;
+    if (T >= (1ll << 31)) return pl;
+    pl.grid = (int)std::min<long long>(h->sm_count, T);
+    pl.MS = (int)((T + pl.grid - 1) / pl.grid);
+    const long long per_w = (long long)Sg::NSLAB * h->nT;
+    pl.MW = (int)((pl.MS + per_w - 2) / per_w) + 1;
+    const size_t nT = (size_t)h->nT, LTS = nT + 1, MTS = 3 * nT + 2;
+    pl.smem = 64 + 16 * (size_t)h->n_bucket + (size_t)Sg::NS * Sg::NB * Sg::BUF_BYTES + 16 * (size_t)pl.MS * MTS +
+              4 * ((size_t)pl.MS * LTS + 3 * LTS + MTS + 2 * Sg::NB * 32) + 2 * (size_t)pl.MW * 32 * nT + 16;
+    pl.ok = pl.smem <= 227 * 1024;
+    return pl;
+}
+
+StreamPlan plan_stream(const ea_handle *h)
+{
+    int coop = 0, dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
+    if (!coop) return StreamPlan{false, 0, 0, 0, 0};
+    if (h->L == 32) return plan_stream_t<32>(h);
+    if (h->L == 64) return plan_stream_t<64>(h);
+    return StreamPlan{false, 0, 0, 0, 0};
+}
+
+template <int L>
+cudaError_t launch_stream_t(const ea_handle *h, ea::StreamArgs &A, const StreamPlan &pl, bool fast)
+{
+    void (*kern)(const ea::StreamArgs) = fast ? ea::k_stream<L, true> : ea::k_stream<L, false>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem);
+    if (e != cudaSuccess) return e;
+    int per_sm = 0;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, ea::StreamGeom<L>::NTHR, pl.smem);
+    if (e != cudaSuccess) return e;
+    if (per_sm < 1 || (long long)per_sm * h->sm_count < pl.grid) return cudaErrorCooperativeLaunchTooLarge;
+    void *args[] = {(void *)&A};
+    return cudaLaunchCooperativeKernel((const void *)kern, dim3((unsigned)pl.grid), dim3(ea::StreamGeom<L>::NTHR),
+                                       args, pl.smem, h->stream);
+}
+}  // namespace
+
+static int sweep_stream(ea_handle *h, int64_t n_sweeps, int swap_interval)
+{
+    const StreamPlan pl = plan_stream(h);
+    if (!pl.ok) return fail(h, EA_ERR_UNSUPPORTED, "stream kernel: shape not supported");
+    int64_t left = n_sweeps;
+    while (left > 0) {
+        const int chunk = (int)std::min<int64_t>(left, 1 << 30);
+        ea::StreamArgs A{};
+        A.P = h->P;
+        A.g0 = (uint32_t)h->g;
+        A.n_sweeps = chunk;
+        A.swap_interval = swap_interval;
+        A.nswap0 = (uint32_t)h->nswap;
+        A.Ecnt = h->d_Ecnt;
+        A.bucket = h->d_bucket; A.n_bucket = h->n_bucket; A.trip = h->d_trip;
+        A.key_lo = h->key_lo; A.key_shift = h->key_shift;
+        A.ones = 0xFFFFFFFFu; A.c48 = 48u; A.cm16 = (uint32_t)-16; A.c16 = 16u;
+        A.MS = pl.MS; A.MW = pl.MW;
+        for (int r = 0; r < 10; ++r) {
+            A.rk[2 * r] = h->P.k0 + (uint32_t)r * 0x9E3779B9u;
+            A.rk[2 * r + 1] = h->P.k1 + (uint32_t)r * 0xBB67AE85u;
+        }
+        CUDA_TRY(h, cudaMemsetAsync(h->d_Ecnt, 0, 2 * 4 * (size_t)h->Rp * h->nT, h->stream));
+        const cudaError_t e = h->L == 32 ? launch_stream_t<32>(h, A, pl, h->fast_rank)
+                                         : launch_stream_t<64>(h, A, pl, h->fast_rank);
+        if (e != cudaSuccess) return fail(h, EA_ERR_CUDA, std::string("stream launch: ") + cudaGetErrorString(e));
+        h->launches++;
+        if (swap_interval > 0) h->nswap += (h->g + (uint64_t)chunk) / (uint64_t)swap_interval - h->g / (uint64_t)swap_interval;
+        h->g += (uint64_t)chunk;
+        left -= chunk;
+    }
+    // the tiled path expects its counters cleared
+    CUDA_TRY(h, cudaMemsetAsync(h->d_Ecnt, 0, 2 * 4 * (size_t)h->Rp * h->nT, h->stream));
+    h->energy_valid = true;
+    return EA_OK;
+}
+
 static int pick_kernel(const ea_handle *h)
 {
     if (h->kernel_sel != EA_KERNEL_AUTO) return h->kernel_sel;
     if (plan_resident(h).ok) return EA_KERNEL_RESIDENT;
+    if (plan_stream(h).ok) return EA_KERNEL_STREAM;
     if (plan_tiled(h).ok) return EA_KERNEL_TILED;
     return EA_KERNEL_GENERIC;
 }
@@ -696,6 +784,7 @@ extern "C" int ea_set_kernel(ea_handle *h, int kernel)
     if (kernel == EA_KERNEL_AUTO || kernel == EA_KERNEL_GENERIC) { h->kernel_sel = kernel; return EA_OK; }
     if (kernel == EA_KERNEL_RESIDENT && plan_resident(h).ok) { h->kernel_sel = kernel; return EA_OK; }
     if (kernel == EA_KERNEL_TILED && plan_tiled(h).ok) { h->kernel_sel = kernel; return EA_OK; }
+    if (kernel == EA_KERNEL_STREAM && plan_stream(h).ok) { h->kernel_sel = kernel; return EA_OK; }
     return fail(h, EA_ERR_UNSUPPORTED, "ea_set_kernel: kernel not available for this shape");
 }
 extern "C" int ea_get_kernel(ea_handle *h) { return h ? pick_kernel(h) : EA_ERR_INVALID_ARG; }
@@ -707,6 +796,7 @@ extern "C" int ea_sweep(ea_handle *h, int64_t n_sweeps, int swap_interval)
     if (n_sweeps == 0) return EA_OK;
     if (pick_kernel(h) == EA_KERNEL_RESIDENT) return sweep_resident(h, n_sweeps, swap_interval);
     if (pick_kernel(h) == EA_KERNEL_TILED) return sweep_tiled(h, n_sweeps, swap_interval);
+    if (pick_kernel(h) == EA_KERNEL_STREAM) return sweep_stream(h, n_sweeps, swap_interval);
     return sweep_generic(h, n_sweeps, swap_interval);
 }
 

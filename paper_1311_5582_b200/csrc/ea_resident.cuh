@@ -196,17 +196,17 @@ struct ResGeom {
 // [2][Nh]); nothing is stored.  EXACT = false: ranks from the bucket table; *flag collects
 // bit 31 of the entries (set: the caller must redo the quad with EXACT = true).
 template <int L, bool EXACT, bool ENERGY, bool UNIS>
-__device__ __forceinline__ uint4 quad_body(const uint32_t *sp, const uint32_t *lt, const uint4 *mt, const RankCtx &R,
-                                           const QuadJ &J, int p, int s, int q, uint32_t oyp, uint32_t oym,
-                                           uint32_t ozp, uint32_t ozm, const uint4 rnd, Planes (&fin)[4],
+__device__ __forceinline__ uint4 quad_core(const char *self_q, const char *oth_b, uint32_t ov, uint32_t oyp,
+                                           uint32_t oym, uint32_t ozp, uint32_t ozm, int qx,
+                                           const uint32_t *lt, const uint4 *mt, const RankCtx &R,
+                                           const QuadJ &J, int s, const uint4 rnd, Planes (&fin)[4],
                                            uint32_t *flag)
 {
     using Gm = ResGeom<L>;
-    // oyp..ozm: byte offsets of the +-y / +-z neighbour quads inside a parity array
-    const char *self_b = reinterpret_cast<const char *>(sp + p * Gm::Nh);
-    const char *oth_b = reinterpret_cast<const char *>(sp + (1 - p) * Gm::Nh);
-    const uint4 me = *reinterpret_cast<const uint4 *>(self_b + 16 * q);
-    const uint4 v = *reinterpret_cast<const uint4 *>(oth_b + 16 * q);
+    // self_q: address of the quad's own four words; oth_b: base of the other parity's words;
+    // ov, oyp..ozm: byte offsets in oth_b of the index-aligned quad and of the +-y / +-z quads
+    const uint4 me = *reinterpret_cast<const uint4 *>(self_q);
+    const uint4 v = *reinterpret_cast<const uint4 *>(oth_b + ov);
     const uint4 yp = *reinterpret_cast<const uint4 *>(oth_b + oyp);
     const uint4 ym = *reinterpret_cast<const uint4 *>(oth_b + oym);
     const uint4 zp = *reinterpret_cast<const uint4 *>(oth_b + ozp);
@@ -216,7 +216,6 @@ __device__ __forceinline__ uint4 quad_body(const uint32_t *sp, const uint32_t *l
     // x neighbour that is not index-aligned: x+1 if s, x-1 otherwise; the word beyond the quad
     // (ext) comes from the next (s) / previous (!s) quad of the row
     uint32_t eb[4];
-    const int qx = q & (Gm::QR - 1);
     if (UNIS && !EXACT) {
         // s is warp-uniform (diagonal thread mapping of the resident kernel): a branch instead
         // of five selects; quads of a row sit in adjacent lanes
@@ -235,8 +234,8 @@ __device__ __forceinline__ uint4 quad_body(const uint32_t *sp, const uint32_t *l
         uint32_t ext = s ? v.x : v.w;
         if (Gm::QR > 1) {
             if (EXACT) {   // divergent (rare) path: no shuffle, read the neighbour quad's word
-                const int qn = (q - qx) + ((qx + (s ? 1 : Gm::QR - 1)) & (Gm::QR - 1));
-                ext = reinterpret_cast<const uint32_t *>(oth_b)[4 * qn + (s ? 0 : 3)];
+                const uint32_t on = ov - 16u * qx + 16u * ((qx + (s ? 1 : Gm::QR - 1)) & (Gm::QR - 1));
+                ext = *reinterpret_cast<const uint32_t *>(oth_b + on + (s ? 0 : 12));
             } else {
                 const int lane = threadIdx.x & 31;
                 const int ln = (lane & ~(Gm::QR - 1)) | ((lane + (s ? 1 : Gm::QR - 1)) & (Gm::QR - 1));
@@ -270,6 +269,22 @@ __device__ __forceinline__ uint4 quad_body(const uint32_t *sp, const uint32_t *l
     return make_uint4(out[0], out[1], out[2], out[3]);
 }
 
+// New words of a quad (nothing is stored): fast rank path first; rare (or !FAST): the whole
+// quad again from memory with the exact search.
+template <int L, bool FAST, bool ENERGY, bool UNIS>
+__device__ __forceinline__ uint4 update_quad_mem(const char *self_q, const char *oth_b, uint32_t ov,
+                                                 uint32_t oyp, uint32_t oym, uint32_t ozp, uint32_t ozm, int qx,
+                                                 const uint32_t *lt, const uint4 *mt, const RankCtx &R,
+                                                 const QuadJ &J, int s, const uint4 rnd, Planes (&fin)[4])
+{
+    uint32_t flag = 0x80000000u;
+    uint4 res;
+    if (FAST) res = quad_core<L, false, ENERGY, UNIS>(self_q, oth_b, ov, oyp, oym, ozp, ozm, qx, lt, mt, R, J, s, rnd, fin, &flag);
+    if ((int)flag < 0) res = quad_core<L, true, ENERGY, UNIS>(self_q, oth_b, ov, oyp, oym, ozp, ozm, qx, lt, mt, R, J, s, rnd, fin, &flag);
+    return res;
+}
+
+// lattice `sp` = [2][Nh] words (resident and tiled kernels): update quad q of parity p in place
 template <int L, bool FAST, bool ENERGY, bool UNIS>
 __device__ __forceinline__ void update_quad_off(uint32_t *sp, const uint32_t *lt, const uint4 *mt, const RankCtx &R,
                                                 const QuadJ &J, int p, int s, int q, uint32_t oyp,
@@ -277,12 +292,11 @@ __device__ __forceinline__ void update_quad_off(uint32_t *sp, const uint32_t *lt
                                                 Planes (&fin)[4])
 {
     using Gm = ResGeom<L>;
-    uint32_t flag = 0x80000000u;
-    uint4 res;
-    if (FAST) res = quad_body<L, false, ENERGY, UNIS>(sp, lt, mt, R, J, p, s, q, oyp, oym, ozp, ozm, rnd, fin, &flag);
-    // rare (or !FAST): redo the whole quad from memory with the exact search
-    if ((int)flag < 0) res = quad_body<L, true, ENERGY, UNIS>(sp, lt, mt, R, J, p, s, q, oyp, oym, ozp, ozm, rnd, fin, &flag);
-    reinterpret_cast<uint4 *>(sp + p * Gm::Nh)[q] = res;
+    char *self_q = reinterpret_cast<char *>(sp + p * Gm::Nh) + 16 * q;
+    const char *oth_b = reinterpret_cast<const char *>(sp + (1 - p) * Gm::Nh);
+    const uint4 res = update_quad_mem<L, FAST, ENERGY, UNIS>(self_q, oth_b, 16u * q, oyp, oym, ozp, ozm,
+                                                             q & (Gm::QR - 1), lt, mt, R, J, s, rnd, fin);
+    *reinterpret_cast<uint4 *>(self_q) = res;
 }
 
 // resident kernel: neighbour offsets packed two per register (16-bit halves, + in the low half)

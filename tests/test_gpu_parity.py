@@ -33,7 +33,7 @@ def _assert_same(g, o, tag=""):
     assert st["sweeps"] == c["sweeps"] and st["swap_rounds"] == c["swap_rounds"]
 
 
-KERNELS = [1, 2, 3]   # EA_KERNEL_GENERIC, EA_KERNEL_RESIDENT (L = 8, 16), EA_KERNEL_TILED (L = 16, 32, 64)
+KERNELS = [1, 2, 3, 4]   # GENERIC, RESIDENT (L = 8, 16), TILED (L = 16, 32, 64), STREAM (L = 32, 64)
 
 
 def _skip_unsupported(kernel, L):
@@ -41,6 +41,8 @@ def _skip_unsupported(kernel, L):
         pytest.skip("resident kernel supports L = 8, 16")
     if kernel == 3 and L not in (16, 32, 64):
         pytest.skip("tiled kernel supports L = 16, 32, 64")
+    if kernel == 4 and L not in (32, 64):
+        pytest.skip("stream kernel supports L = 32, 64")
 
 
 @pytest.mark.parametrize("kernel", KERNELS)
