@@ -6,6 +6,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <string>
 #include <vector>
@@ -685,13 +686,13 @@ static int sweep_tiled(ea_handle *h, int64_t n_sweeps, int swap_interval)
 
 // ---------------------------------------------------------------- streaming path (L = 32, 64)
 namespace {
-struct StreamPlan { bool ok; int grid, MS, MW; size_t smem; };
+struct StreamPlan { bool ok; int grid, MS, MW, swap_win; size_t smem, esm_off, batch_off; };
 
 template <int L>
 StreamPlan plan_stream_t(const ea_handle *h)
 {
     using Sg = ea::StreamGeom<L>;
-    StreamPlan pl{false, 0, 0, 0, 0};
+    StreamPlan pl{false, 0, 0, 0, 0, 0, 0, 0};
     const long long T = (long long)h->W * Sg::NSLAB * h->nT;
     if (T >= (1ll << 31)) return pl;
     pl.grid = (int)std::min<long long>(h->sm_count, T);
@@ -699,9 +700,16 @@ StreamPlan plan_stream_t(const ea_handle *h)
     const long long per_w = (long long)Sg::NSLAB * h->nT;
     pl.MW = (int)((pl.MS + per_w - 2) / per_w) + 1;
     const size_t nT = (size_t)h->nT, LTS = nT + 1, MTS = 3 * nT + 2;
-    pl.smem = 64 + 16 * (size_t)h->n_bucket + (size_t)Sg::NS * Sg::NB * Sg::BUF_BYTES + 16 * (size_t)pl.MS * MTS +
-              4 * ((size_t)pl.MS * LTS + 3 * LTS + MTS + 2 * Sg::NB * 32) + 2 * (size_t)pl.MW * 32 * nT + 16;
-    pl.ok = pl.smem <= 227 * 1024;
+    size_t base = 64 + 16 * (size_t)h->n_bucket + (size_t)Sg::NS * Sg::NB * Sg::BUF_BYTES + 16 * (size_t)pl.MS * MTS +
+                  4 * ((size_t)pl.MS * LTS + 3 * LTS + MTS + 2 * Sg::NB * 32) + 2 * (size_t)pl.MW * 32 * nT;
+    pl.esm_off = (base + 15) & ~(size_t)15;
+    pl.batch_off = pl.esm_off + 4 * (size_t)pl.MW * 32 * nT;
+    base = pl.batch_off + 16 * (size_t)pl.MS;
+    const size_t cap = 227 * 1024;
+    if (base > cap) return pl;
+    pl.swap_win = (int)std::min<size_t>(128, (cap - base) / (4 * nT));
+    pl.smem = base + 4 * nT * (size_t)pl.swap_win;
+    pl.ok = pl.MS < 65536;
     return pl;
 }
 
@@ -710,10 +718,10 @@ StreamPlan plan_stream(const ea_handle *h)
     int coop = 0, dev = 0;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
-    if (!coop) return StreamPlan{false, 0, 0, 0, 0};
+    if (!coop) return StreamPlan{false, 0, 0, 0, 0, 0, 0, 0};
     if (h->L == 32) return plan_stream_t<32>(h);
     if (h->L == 64) return plan_stream_t<64>(h);
-    return StreamPlan{false, 0, 0, 0, 0};
+    return StreamPlan{false, 0, 0, 0, 0, 0, 0, 0};
 }
 
 template <int L>
@@ -749,14 +757,29 @@ static int sweep_stream(ea_handle *h, int64_t n_sweeps, int swap_interval)
         A.bucket = h->d_bucket; A.n_bucket = h->n_bucket; A.trip = h->d_trip;
         A.key_lo = h->key_lo; A.key_shift = h->key_shift;
         A.ones = 0xFFFFFFFFu; A.c48 = 48u; A.cm16 = (uint32_t)-16; A.c16 = 16u;
-        A.MS = pl.MS; A.MW = pl.MW;
+        A.MS = pl.MS; A.MW = pl.MW; A.swap_win = pl.swap_win; A.esm_off = (int)pl.esm_off; A.batch_off = (int)pl.batch_off;
         for (int r = 0; r < 10; ++r) {
             A.rk[2 * r] = h->P.k0 + (uint32_t)r * 0x9E3779B9u;
             A.rk[2 * r + 1] = h->P.k1 + (uint32_t)r * 0xBB67AE85u;
         }
+        // debug aid: EA_STREAM_TRACE=<file> dumps per-block phase time stamps of the first 8 sweeps
+        const char *trace_path = std::getenv("EA_STREAM_TRACE");
+        unsigned long long *d_trace = nullptr;
+        const size_t trace_n = (size_t)pl.grid * 64 + 512;
+        if (trace_path && cudaMalloc((void **)&d_trace, 8 * trace_n) == cudaSuccess) {
+            cudaMemsetAsync(d_trace, 0, 8 * trace_n, h->stream);
+            A.trace = d_trace;
+        }
         CUDA_TRY(h, cudaMemsetAsync(h->d_Ecnt, 0, 2 * 4 * (size_t)h->Rp * h->nT, h->stream));
         const cudaError_t e = h->L == 32 ? launch_stream_t<32>(h, A, pl, h->fast_rank)
                                          : launch_stream_t<64>(h, A, pl, h->fast_rank);
+        if (d_trace) {
+            std::vector<unsigned long long> tr(trace_n);
+            cudaMemcpyAsync(tr.data(), d_trace, 8 * trace_n, cudaMemcpyDeviceToHost, h->stream);
+            cudaStreamSynchronize(h->stream);
+            if (FILE *f = std::fopen(trace_path, "wb")) { std::fwrite(tr.data(), 8, trace_n, f); std::fclose(f); }
+            cudaFree(d_trace);
+        }
         if (e != cudaSuccess) return fail(h, EA_ERR_CUDA, std::string("stream launch: ") + cudaGetErrorString(e));
         h->launches++;
         if (swap_interval > 0) h->nswap += (h->g + (uint64_t)chunk) / (uint64_t)swap_interval - h->g / (uint64_t)swap_interval;

@@ -37,7 +37,30 @@ struct StreamArgs {
     uint32_t rk[20];
     int MS;                  // most items one block can get = ceil(items / grid)
     int MW;                  // most words one block can meet
+    int swap_win;            // swap thresholds for m in [-swap_win, -1] are staged in smem
+    int esm_off;             // byte offset (16 B aligned) of the swap-phase staging area in smem
+    int batch_off;           // byte offset (16 B aligned) of the batch list in smem
+    unsigned long long *trace;   // debug (EA_STREAM_TRACE): [block][8 sweeps][8] globaltimer stamps, or null
 };
+
+__device__ __forceinline__ void trace_stamp(const StreamArgs &A, int it, int slot)
+{
+    if (A.trace && threadIdx.x == 0 && it < 8) {
+        unsigned long long t;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+        A.trace[((size_t)blockIdx.x * 8 + it) * 8 + slot] = t;
+    }
+}
+
+// debug: per-batch stamps of block 7 in sweep index 3 (threads 0 and 32)
+__device__ __forceinline__ void trace_detail(const StreamArgs &A, uint32_t it, int p, int bi, int what)
+{
+    if (A.trace && blockIdx.x == 7 && it == 3 && bi < 8 && (threadIdx.x == 0 || threadIdx.x == 32)) {
+        unsigned long long t;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+        A.trace[(size_t)gridDim.x * 64 + (((threadIdx.x >> 5) * 2 + p) * 8 + bi) * 8 + what] = t;
+    }
+}
 
 template <int L>
 struct StreamGeom {
@@ -86,14 +109,26 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t by
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }
 
 
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+
+// One batch = up to NB consecutive slots of one (word, slab) group; the block's batch list is
+// fixed for the whole launch and sits in shared memory.
+struct StreamBatch { int pos, cnt, w, slab; };
+
 // Per-block constants of the streaming kernel.
 template <int L>
 struct StreamCtx {
     int i0, i1;                  // my items [i0, i1), item = (w * NSLAB + slab) * nT + k
+    int nb;                      // my batches
     int nT, LTS, MTS;
     int tid, lane, qx, y, zl;
     uint32_t ov, oyp, oym, ozp, ozm;   // byte offsets inside the other-parity buffer
-    uint64_t *mbar;
+    uint64_t *full;              // [NS]: tiles landed
+    int *done;                   // [NS]: warps that have finished with the stage
+    const StreamBatch *batch;
     unsigned char *bufs;
     uint4 *mt;
     uint32_t *lt;
@@ -101,71 +136,116 @@ struct StreamCtx {
     RankCtx R;
 };
 
-// One half-sweep (parity p) over the block's items.  ENERGY: also count the satisfied bonds of
-// the updated (parity-1) sites into A.Ecnt[ebuf].
-template <int L, bool FAST, bool ENERGY>
-__device__ __forceinline__ void stream_half(const StreamArgs &A, const StreamCtx<L> &C, int p, uint32_t g,
-                                            uint32_t &phase, int ebuf)
+// TMA bulk loads of batch b into ring stage st, issued by the lanes of the producer warp in
+// parallel (lane = 3 * slot + piece): per slot the slab's own-parity words (contiguous) and the
+// other parity's planes z0-1 .. z0+ZS (periodic wrap = 2 pieces).
+template <int L>
+__device__ __forceinline__ void stream_issue(const StreamArgs &A, const StreamCtx<L> &C, int p, int b, int st)
 {
     using Gm = ResGeom<L>;
     using Sg = StreamGeom<L>;
-    constexpr int N = Gm::N, Nh = Gm::Nh, QR = Gm::QR, QPP = Sg::QPP, ZS = Sg::ZS, NT = Sg::NTHR;
+    constexpr int N = Gm::N, Nh = Gm::Nh, QPP = Sg::QPP, ZS = Sg::ZS, NT = Sg::NTHR, NB = Sg::NB;
+    constexpr uint32_t PLB = QPP * 16;       // bytes per plane and parity
+    const Params &P = A.P;
+    const StreamBatch B = C.batch[b];
+    const int k0 = B.pos % C.nT, z0 = B.slab * ZS;
+    if (C.lane == 0) mbar_expect_tx(&C.full[st], (uint32_t)(B.cnt * Sg::BUF_BYTES));
+    __syncwarp();
+    const int i = C.lane / 3, piece = C.lane % 3;
+    if (i < B.cnt) {
+        const uint32_t *base = P.spin + ((size_t)(k0 + i) * P.W + B.w) * N;
+        unsigned char *dst = C.bufs + (size_t)(st * NB + i) * Sg::BUF_BYTES;
+        const uint32_t *ob = base + (1 - p) * Nh;
+        unsigned char *od = dst + Sg::OWN_BYTES;
+        const void *src;
+        uint32_t bytes;
+        if (piece == 0) {
+            src = base + p * Nh + (size_t)B.slab * NT * 4; bytes = Sg::OWN_BYTES;
+        } else if (z0 == 0) {
+            if (piece == 1) { dst = od; src = ob + (size_t)(L - 1) * QPP * 4; bytes = PLB; }
+            else { dst = od + PLB; src = ob; bytes = (ZS + 1) * PLB; }
+        } else if (z0 + ZS == L) {
+            if (piece == 1) { dst = od; src = ob + (size_t)(z0 - 1) * QPP * 4; bytes = (ZS + 1) * PLB; }
+            else { dst = od + (ZS + 1) * PLB; src = ob; bytes = PLB; }
+        } else {
+            dst = od; src = ob + (size_t)(z0 - 1) * QPP * 4; bytes = piece == 1 ? (ZS + 2) * PLB : 0u;
+        }
+        if (bytes) bulk_g2s(dst, src, bytes, &C.full[st]);
+    }
+}
+
+// Warp 0, start of a half-sweep: the first NS batches.  The proxy fence orders the previous
+// phase's global stores (made visible by the grid barrier) before the asynchronous-proxy reads.
+template <int L>
+__device__ __forceinline__ void stream_prime(const StreamArgs &A, const StreamCtx<L> &C, int p)
+{
+    fence_proxy_async();
+    for (int b = 0; b < StreamGeom<L>::NS && b < C.nb; ++b) stream_issue<L>(A, C, p, b, b);
+}
+
+// End of a batch for one warp.  The LAST warp to get here (shared counter) owns the stage: it
+// flushes the batch's satisfied-bond counters (ENERGY) to the global counters and refills the
+// stage with batch b + NS.  No block-wide barrier: the other warps are already on the next stage.
+template <int L, bool ENERGY>
+__device__ __forceinline__ void stream_batch_done(const StreamArgs &A, const StreamCtx<L> &C, int p, int b, int ebuf)
+{
+    using Sg = StreamGeom<L>;
+    constexpr int NB = Sg::NB, NS = Sg::NS, NW = Sg::NTHR / 32;
+    const Params &P = A.P;
+    const int st = b % NS;
+    __threadfence_block();
+    __syncwarp();
+    int last = 0;
+    if (C.lane == 0) last = atomicAdd(&C.done[st], 1) == NW - 1;
+    last = __shfl_sync(0xFFFFFFFFu, last, 0);
+    if (!last) return;
+    if (C.lane == 0) C.done[st] = 0;
+    __threadfence_block();
+    if (ENERGY) {
+        const StreamBatch B = C.batch[b];
+        const int k0 = B.pos % C.nT;
+        int32_t *acc = C.Eacc + (b & 1) * NB * 32;
+        for (int a = C.lane; a < B.cnt * 32; a += 32) {
+            const int v = acc[a];
+            acc[a] = 0;
+            atomicAdd(A.Ecnt + (size_t)ebuf * P.Rp * C.nT + (size_t)(32 * B.w + (a & 31)) * C.nT + k0 + (a >> 5), v);
+        }
+        __syncwarp();
+    }
+    if (b + NS < C.nb) stream_issue<L>(A, C, p, b + NS, st);
+}
+
+// One half-sweep (parity p) over the block's batches; the first NS are in flight (stream_prime).
+// ENERGY: also count the satisfied bonds of the updated (parity-1) sites.
+template <int L, bool FAST, bool ENERGY>
+__device__ __forceinline__ void stream_consume(const StreamArgs &A, const StreamCtx<L> &C, int p, uint32_t g,
+                                               uint32_t &phase, int ebuf)
+{
+    using Gm = ResGeom<L>;
+    using Sg = StreamGeom<L>;
+    constexpr int N = Gm::N, Nh = Gm::Nh, QR = Gm::QR, ZS = Sg::ZS, NT = Sg::NTHR;
     constexpr int NB = Sg::NB, NS = Sg::NS, NSLAB = Sg::NSLAB;
     const Params &P = A.P;
     const int nT = C.nT, tid = C.tid;
-
-    auto batch_count = [&](int pos) { return min(min(NB, C.i1 - pos), nT - pos % nT); };
-    // TMA bulk loads of one batch into ring stage st (one thread): per slot the slab's own-parity
-    // words (contiguous) and the other parity's planes z0-1 .. z0+ZS (periodic wrap = 2 pieces)
-    auto issue = [&](int pos, int st) {
-        const int cnt = batch_count(pos);
-        const int k0 = pos % nT, grp = pos / nT, slab = grp % NSLAB, w = grp / NSLAB;
-        const int z0 = slab * ZS;
-        fence_proxy_async();
-        mbar_expect_tx(&C.mbar[st], (uint32_t)(cnt * Sg::BUF_BYTES));
-        for (int i = 0; i < cnt; ++i) {
-            const uint32_t *base = P.spin + ((size_t)(k0 + i) * P.W + w) * N;
-            unsigned char *dst = C.bufs + (size_t)(st * NB + i) * Sg::BUF_BYTES;
-            bulk_g2s(dst, base + p * Nh + (size_t)slab * NT * 4, Sg::OWN_BYTES, &C.mbar[st]);
-            const uint32_t *ob = base + (1 - p) * Nh;
-            unsigned char *od = dst + Sg::OWN_BYTES;
-            constexpr int PLB = QPP * 16;       // bytes per plane and parity
-            if (z0 == 0) {
-                bulk_g2s(od, ob + (size_t)(L - 1) * QPP * 4, PLB, &C.mbar[st]);
-                bulk_g2s(od + PLB, ob, (ZS + 1) * PLB, &C.mbar[st]);
-            } else if (z0 + ZS == L) {
-                bulk_g2s(od, ob + (size_t)(z0 - 1) * QPP * 4, (ZS + 1) * PLB, &C.mbar[st]);
-                bulk_g2s(od + (ZS + 1) * PLB, ob, PLB, &C.mbar[st]);
-            } else {
-                bulk_g2s(od, ob + (size_t)(z0 - 1) * QPP * 4, (ZS + 2) * PLB, &C.mbar[st]);
-            }
-        }
-    };
-
-    int ld_pos = C.i0;
-    for (int st = 0; st < NS && ld_pos < C.i1; ++st) {
-        if (tid == 0) issue(ld_pos, st);
-        ld_pos += batch_count(ld_pos);
-    }
     int cur_grp = -1, s = 0, q = 0;
     QuadJ J;
     Planes fin[4];
-    int bi = 0;
-    for (int pos = C.i0; pos < C.i1; ++bi) {
-        const int cnt = batch_count(pos), st = bi % NS;
-        const int k0 = pos % nT, grp = pos / nT, slab = grp % NSLAB, w = grp / NSLAB;
+    for (int b = 0; b < C.nb; ++b) {
+        const StreamBatch B = C.batch[b];
+        const int cnt = B.cnt, st = b % NS, pos = B.pos, w = B.w;
+        const int k0 = pos % nT, grp = w * NSLAB + B.slab;
         if (grp != cur_grp) {        // couplings of my quad for this (word, slab) and parity
             cur_grp = grp;
-            const int z = slab * ZS + C.zl;
+            const int z = B.slab * ZS + C.zl;
             s = (C.y + z + p) & 1;
-            q = slab * NT + tid;
+            q = B.slab * NT + tid;
             const int qym = C.qx + QR * (wrap_dec(C.y, L) + L * z);
             const int qzm = C.qx + QR * (C.y + L * wrap_dec(z, L));
             J = load_quad_j<L>(P.coup + (size_t)w * 3 * N, p, s, q, C.qx, qym, qzm);
         }
         const uint32_t gw = P.w0 + (uint32_t)w;
         const uint32_t c3 = (uint32_t)p << 16;
-        mbar_wait(&C.mbar[st], (phase >> st) & 1u);
+        mbar_wait(&C.full[st], (phase >> st) & 1u);
         phase ^= 1u << st;
         const unsigned char *stage = C.bufs + (size_t)(st * NB) * Sg::BUF_BYTES;
         if (!ENERGY) {
@@ -199,22 +279,9 @@ __device__ __forceinline__ void stream_half(const StreamArgs &A, const StreamCtx
             uint32_t tot[kResPlanes];
             warp_sum4(en, C.lane, tot);
             const int i_mine = 2 * (C.lane >> 4) + ((C.lane >> 3) & 1);
-            if (i_mine < cnt) add_counts(tot, C.lane & 7, C.Eacc + ((bi & 1) * NB + i_mine) * 32);
+            if (i_mine < cnt) add_counts(tot, C.lane & 7, C.Eacc + ((b & 1) * NB + i_mine) * 32);
         }
-        __syncthreads();             // the stage is free; this batch's shared counters are complete
-        if (ld_pos < C.i1) {
-            if (tid == 0) issue(ld_pos, st);
-            ld_pos += batch_count(ld_pos);
-        }
-        if (ENERGY) {
-            int32_t *acc = C.Eacc + (bi & 1) * NB * 32;
-            for (int a = tid; a < cnt * 32; a += NT) {
-                const int v = acc[a];
-                acc[a] = 0;
-                atomicAdd(A.Ecnt + (size_t)ebuf * P.Rp * nT + (size_t)(32 * w + (a & 31)) * nT + k0 + (a >> 5), v);
-            }
-        }
-        pos += cnt;
+        stream_batch_done<L, ENERGY>(A, C, p, b, ebuf);
     }
 }
 
@@ -231,6 +298,7 @@ __global__ void __launch_bounds__(StreamGeom<L>::NTHR, 1) k_stream(const StreamA
     const Params &P = A.P;
     const int nT = P.nT, LTS = P.LTS, MTS = 3 * nT + 2, MS = A.MS, MW = A.MW;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarp = NT >> 5;
+    constexpr int NTA = NT;
     cg::grid_group grid = cg::this_grid();
 
     StreamCtx<L> C;
@@ -241,7 +309,7 @@ __global__ void __launch_bounds__(StreamGeom<L>::NTHR, 1) k_stream(const StreamA
     const int w_first = C.i0 / per_w, nwt = (C.i1 - 1) / per_w - w_first + 1;   // words I meet (<= MW)
 
     // shared memory
-    uint64_t *mbar = reinterpret_cast<uint64_t *>(smraw);                        // [NS], 64 B reserved
+    uint64_t *mbar = reinterpret_cast<uint64_t *>(smraw);                        // full[NS], done[NS], nb: 64 B reserved
     uint4 *bucket = reinterpret_cast<uint4 *>(smraw + 64);                       // [n_bucket]
     unsigned char *bufs = reinterpret_cast<unsigned char *>(bucket + A.n_bucket);   // [NS][NB][BUF_BYTES]
     uint4 *mt = reinterpret_cast<uint4 *>(bufs + (size_t)NS * NB * Sg::BUF_BYTES);  // [MS][MTS]
@@ -251,18 +319,35 @@ __global__ void __launch_bounds__(StreamGeom<L>::NTHR, 1) k_stream(const StreamA
     int32_t *Eacc = reinterpret_cast<int32_t *>(trip + MTS);                     // [2][NB][32]
     uint8_t *tau8 = reinterpret_cast<uint8_t *>(Eacc + 2 * NB * 32);             // [MW][32][nT]
     uint8_t *sig8 = tau8 + (size_t)MW * 32 * nT;                                 // [MW][32][nT]
+    const int SW = A.swap_win;
+    int32_t *Esm = reinterpret_cast<int32_t *>(smraw + A.esm_off);               // [MW][32][nT] bond counts
+    StreamBatch *batch = reinterpret_cast<StreamBatch *>(smraw + A.batch_off);   // [MS]
+    uint32_t *swwin = reinterpret_cast<uint32_t *>(batch + MS);                  // [nT][SW] thresholds - 1
 
-    for (int a = tid; a < A.n_bucket; a += NT) bucket[a] = A.bucket[a];
-    for (int a = tid; a < 3 * LTS; a += NT) thr[a] = P.thr32[a];
-    for (int a = tid; a < MTS - 1; a += NT) trip[a] = A.trip[a];
-    for (int a = tid; a < 2 * NB * 32; a += NT) Eacc[a] = 0;
-    for (int a = tid; a < nwt * 32 * nT; a += NT) {
+    for (int a = tid; a < A.n_bucket; a += NTA) bucket[a] = A.bucket[a];
+    for (int a = tid; a < 3 * LTS; a += NTA) thr[a] = P.thr32[a];
+    for (int a = tid; a < MTS - 1; a += NTA) trip[a] = A.trip[a];
+    for (int a = tid; a < (nT - 1) * SW; a += NTA) {         // window m = -SW + i of row t
+        const int t = a / SW, m = -SW + a % SW;
+        const int lo = P.swp_lo[t], cn = P.swp_cnt[t];
+        swwin[a] = (m >= lo && m < lo + cn) ? P.swp_val[P.swp_off[t] + (m - lo)] : 0u;
+    }
+    for (int a = tid; a < 2 * NB * 32; a += NTA) Eacc[a] = 0;
+    for (int a = tid; a < nwt * 32 * nT; a += NTA) {
         tau8[a] = P.tau[(size_t)32 * w_first * nT + a];
         sig8[a] = P.sigma[(size_t)32 * w_first * nT + a];
     }
     if (tid == 0) {
-        for (int i = 0; i < NS; ++i) mbar_init(&mbar[i], 1);
+        for (int i = 0; i < NS; ++i) { mbar_init(&mbar[i], 1); reinterpret_cast<int *>(mbar + NS)[i] = 0; }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        // my batch list: up to NB consecutive slots of one (word, slab) group each
+        int nb = 0;
+        for (int pos = C.i0; pos < C.i1; ++nb) {
+            const int cnt = min(min(NB, C.i1 - pos), nT - pos % nT), grp = pos / nT;
+            batch[nb] = StreamBatch{pos, cnt, grp / NSLAB, grp % NSLAB};
+            pos += cnt;
+        }
+        *reinterpret_cast<int *>(smraw + 48) = nb;
     }
     __syncthreads();
 
@@ -284,7 +369,7 @@ __global__ void __launch_bounds__(StreamGeom<L>::NTHR, 1) k_stream(const StreamA
 
     C.nT = nT; C.LTS = LTS; C.MTS = MTS;
     C.tid = tid; C.lane = lane;
-    C.qx = tid % QR; C.y = (tid / QR) % L; C.zl = tid / QPP;
+    C.qx = tid % QR; C.y = (tid / QR) % L; C.zl = (tid / QPP) % Sg::ZS;   // (producer lanes: unused)
     {
         const int row = QR * C.y + C.qx;
         C.ov = 16u * (uint32_t)((C.zl + 1) * QPP + row);
@@ -293,7 +378,8 @@ __global__ void __launch_bounds__(StreamGeom<L>::NTHR, 1) k_stream(const StreamA
         C.ozp = 16u * (uint32_t)((C.zl + 2) * QPP + row);
         C.ozm = 16u * (uint32_t)(C.zl * QPP + row);
     }
-    C.mbar = mbar; C.bufs = bufs; C.mt = mt; C.lt = lt; C.Eacc = Eacc;
+    C.full = mbar; C.done = reinterpret_cast<int *>(mbar + NS); C.batch = batch; C.bufs = bufs; C.mt = mt; C.lt = lt; C.Eacc = Eacc;
+    C.nb = *reinterpret_cast<const int *>(smraw + 48);
     C.R.thr = thr; C.R.bucket = bucket; C.R.LTS = LTS; C.R.nT = nT;
     C.R.key_lo = A.key_lo; C.R.key_top = A.n_bucket - 1; C.R.key_shift = A.key_shift;
     C.R.z0 = P.z[0]; C.R.z1 = P.z[1]; C.R.z2 = P.z[2];
@@ -302,36 +388,51 @@ __global__ void __launch_bounds__(StreamGeom<L>::NTHR, 1) k_stream(const StreamA
 
     uint32_t nswap = A.nswap0, phase = 0;
     int ebuf = 0;
+    if (warp == 0) stream_prime<L>(A, C, 0);
+    auto bar_compute = [&]() { __syncthreads(); };
     for (int it = 0; it < A.n_sweeps; ++it) {
         const uint32_t g = A.g0 + (uint32_t)it;
         const bool swap_now = A.swap_interval > 0 && ((uint64_t)g + 1) % (uint64_t)A.swap_interval == 0;
         const bool need_E = swap_now || it == A.n_sweeps - 1;
-        stream_half<L, FAST, false>(A, C, 0, g, phase, ebuf);
+        trace_stamp(A, it, 0);
+        stream_consume<L, FAST, false>(A, C, 0, g, phase, ebuf);
+        trace_stamp(A, it, 1);
         grid.sync();
-        if (need_E) stream_half<L, FAST, true>(A, C, 1, g, phase, ebuf);
-        else stream_half<L, FAST, false>(A, C, 1, g, phase, ebuf);
+        if (warp == 0) stream_prime<L>(A, C, 1);
+        trace_stamp(A, it, 2);
+        if (need_E) stream_consume<L, FAST, true>(A, C, 1, g, phase, ebuf);
+        else stream_consume<L, FAST, false>(A, C, 1, g, phase, ebuf);
+        trace_stamp(A, it, 3);
         grid.sync();
+        // the next sweep's first tiles fly while the swap decisions are taken
+        if (warp == 0 && it + 1 < A.n_sweeps) stream_prime<L>(A, C, 0);
+        trace_stamp(A, it, 4);
         if (!need_E) continue;
         const int32_t *cnt = A.Ecnt + (size_t)ebuf * P.Rp * nT;     // satisfied bonds by [r][k]
+        for (int a = tid; a < nwt * 32 * nT; a += NT) Esm[a] = __ldcg(cnt + (size_t)32 * w_first * nT + a);
+        bar_compute();
         if (swap_now) {
             // swap round: warp per temperature pair, lane = realization; every block that works
             // on a word takes the same decisions.  E_a - E_b = -2 (c_a - c_b).
             for (int wl = 0; wl < nwt; ++wl) {
                 const int r = 32 * (w_first + wl) + lane;
                 uint8_t *sg_ = sig8 + (size_t)(wl * 32 + lane) * nT, *ta_ = tau8 + (size_t)(wl * 32 + lane) * nT;
+                const int32_t *er = Esm + (size_t)(wl * 32 + lane) * nT;
                 for (int t = (int)(nswap & 1u) + 2 * warp; t + 1 < nT; t += 2 * nwarp) {
                     const int sa = sg_[t], sb = sg_[t + 1];
-                    const int ca = __ldcg(cnt + (size_t)r * nT + sa), cb = __ldcg(cnt + (size_t)r * nT + sb);
-                    const int m = (cb - ca) / 2;
+                    const int m = (er[sb] - er[sa]) / 2;
                     const uint4 v = philox_rk(g, (uint32_t)t, P.r0 + (uint32_t)r, 2u << 16, A.rk);
-                    if (swap_accept(P, t, m, v.x)) {
+                    const bool acc = (m >= -SW && m < 0 && m >= P.swp_lo[t] && m < P.swp_lo[t] + P.swp_cnt[t])
+                                         ? v.x <= swwin[t * SW + m + SW]
+                                         : swap_accept(P, t, m, v.x);
+                    if (acc) {
                         sg_[t] = (uint8_t)sb; sg_[t + 1] = (uint8_t)sa;
                         ta_[sa] = (uint8_t)(t + 1); ta_[sb] = (uint8_t)t;
                     }
                 }
             }
             ++nswap;
-            __syncthreads();
+            bar_compute();
             rebuild_tables();
         }
         // the block that owns item (w, slab 0, slot 0) keeps the word's global state
@@ -341,7 +442,7 @@ __global__ void __launch_bounds__(StreamGeom<L>::NTHR, 1) k_stream(const StreamA
             if (it == A.n_sweeps - 1) {
                 for (int a = tid; a < 32 * nT; a += NT) {
                     const size_t idx = (size_t)32 * w * nT + a;
-                    P.E[idx] = 3 * N - 2 * __ldcg(cnt + idx);
+                    P.E[idx] = 3 * N - 2 * Esm[(size_t)wl * 32 * nT + a];
                     P.tau[idx] = tau8[(size_t)wl * 32 * nT + a];
                     P.sigma[idx] = sig8[(size_t)wl * 32 * nT + a];
                 }
@@ -359,7 +460,8 @@ __global__ void __launch_bounds__(StreamGeom<L>::NTHR, 1) k_stream(const StreamA
             }
         }
         ebuf ^= 1;
-        __syncthreads();
+        bar_compute();
+        trace_stamp(A, it, 5);
     }
 }
 
