@@ -97,7 +97,7 @@ Layout make_layout(int L, int nT, int R)
     o.swp_val = take(4 * (o.swp_val_cap ? o.swp_val_cap : 1));
     o.bucket = take(16 * (size_t)kMaxBucket);
     o.trip = take(4 * (3 * (size_t)nT + 2));
-    o.ecnt = take(2 * 4 * Rp * nT);      // double-buffered by the streaming kernel
+    o.ecnt = take(2 * 4 * Rp * nT + 256);      // double-buffered by the streaming kernel; + its grid barrier word
     o.total = off;
     return o;
 }
@@ -390,7 +390,7 @@ extern "C" ea_handle *ea_create_ex(int L, int n_temps, int n_realizations, const
     launch_cfg((int64_t)h->Rp * n_temps, 128, grid);
     ea::k_identity_perm<<<grid, 128, 0, h->stream>>>(P);
     h->launches += 2;
-    cudaMemsetAsync(h->d_Ecnt, 0, 2 * 4 * (size_t)h->Rp * n_temps, h->stream);
+    cudaMemsetAsync(h->d_Ecnt, 0, 2 * 4 * (size_t)h->Rp * n_temps + 256, h->stream);
     if (rebuild_lt(h) != EA_OK || recompute_energy(h) != EA_OK ||
         cudaStreamSynchronize(h->stream) != cudaSuccess || cudaGetLastError() != cudaSuccess)
         return (ea_handle *)bail(EA_ERR_CUDA, "ea_create: initialisation kernels failed: " + h->err);
@@ -704,7 +704,7 @@ StreamPlan plan_stream_t(const ea_handle *h)
                   4 * ((size_t)pl.MS * LTS + 3 * LTS + MTS + 2 * Sg::NB * 32) + 2 * (size_t)pl.MW * 32 * nT;
     pl.esm_off = (base + 15) & ~(size_t)15;
     pl.batch_off = pl.esm_off + 4 * (size_t)pl.MW * 32 * nT;
-    base = pl.batch_off + 16 * (size_t)pl.MS;
+    base = pl.batch_off + 16 * (size_t)pl.MS + 8 * nT;
     const size_t cap = 227 * 1024;
     if (base > cap) return pl;
     pl.swap_win = (int)std::min<size_t>(128, (cap - base) / (4 * nT));
@@ -754,6 +754,7 @@ static int sweep_stream(ea_handle *h, int64_t n_sweeps, int swap_interval)
         A.swap_interval = swap_interval;
         A.nswap0 = (uint32_t)h->nswap;
         A.Ecnt = h->d_Ecnt;
+        A.gbar = (unsigned int *)(h->d_Ecnt + 2 * (size_t)h->Rp * h->nT);
         A.bucket = h->d_bucket; A.n_bucket = h->n_bucket; A.trip = h->d_trip;
         A.key_lo = h->key_lo; A.key_shift = h->key_shift;
         A.ones = 0xFFFFFFFFu; A.c48 = 48u; A.cm16 = (uint32_t)-16; A.c16 = 16u;
@@ -765,7 +766,7 @@ static int sweep_stream(ea_handle *h, int64_t n_sweeps, int swap_interval)
         // debug aid: EA_STREAM_TRACE=<file> dumps per-block phase time stamps of the first 8 sweeps
         const char *trace_path = std::getenv("EA_STREAM_TRACE");
         unsigned long long *d_trace = nullptr;
-        const size_t trace_n = (size_t)pl.grid * 64 + 512;
+        const size_t trace_n = (size_t)pl.grid * 64 + (size_t)pl.grid * 64;
         if (trace_path && cudaMalloc((void **)&d_trace, 8 * trace_n) == cudaSuccess) {
             cudaMemsetAsync(d_trace, 0, 8 * trace_n, h->stream);
             A.trace = d_trace;

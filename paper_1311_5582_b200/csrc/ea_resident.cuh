@@ -406,6 +406,48 @@ __device__ __forceinline__ void warp_sum4(uint32_t (&en)[4][5], int lane, uint32
     }
 }
 
+// Two-slot variant (fewer live registers): lanes 0-15 end up with the 10-plane sum over the warp
+// of slot 0, lanes 16-31 with that of slot 1.
+__device__ __forceinline__ void warp_sum2(uint32_t (&en)[2][5], int lane, uint32_t (&out)[kResPlanes])
+{
+    const uint32_t hi16 = (lane & 16) ? 0xFFFFFFFFu : 0u;
+    uint32_t a[6];
+    {
+        uint32_t keep[5], got[5];
+#pragma unroll
+        for (int i = 0; i < 5; ++i) {
+            keep[i] = mux(en[0][i], en[1][i], hi16);
+            got[i] = __shfl_xor_sync(0xFFFFFFFFu, mux(en[1][i], en[0][i], hi16), 16);
+        }
+        vsum<5>(keep, got, a);
+    }
+    uint32_t b[7], c[8], d[9];
+    {
+        uint32_t got[6];
+#pragma unroll
+        for (int i = 0; i < 6; ++i) got[i] = __shfl_xor_sync(0xFFFFFFFFu, a[i], 8);
+        vsum<6>(a, got, b);
+    }
+    {
+        uint32_t got[7];
+#pragma unroll
+        for (int i = 0; i < 7; ++i) got[i] = __shfl_xor_sync(0xFFFFFFFFu, b[i], 4);
+        vsum<7>(b, got, c);
+    }
+    {
+        uint32_t got[8];
+#pragma unroll
+        for (int i = 0; i < 8; ++i) got[i] = __shfl_xor_sync(0xFFFFFFFFu, c[i], 2);
+        vsum<8>(c, got, d);
+    }
+    {
+        uint32_t got[9];
+#pragma unroll
+        for (int i = 0; i < 9; ++i) got[i] = __shfl_xor_sync(0xFFFFFFFFu, d[i], 1);
+        vsum<9>(d, got, out);
+    }
+}
+
 __device__ __forceinline__ void cluster_arrive()
 {
     asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");

@@ -40,6 +40,7 @@ struct StreamArgs {
     int swap_win;            // swap thresholds for m in [-swap_win, -1] are staged in smem
     int esm_off;             // byte offset (16 B aligned) of the swap-phase staging area in smem
     int batch_off;           // byte offset (16 B aligned) of the batch list in smem
+    unsigned int *gbar;      // grid barrier word (zero before the first launch; self-resetting)
     unsigned long long *trace;   // debug (EA_STREAM_TRACE): [block][8 sweeps][8] globaltimer stamps, or null
 };
 
@@ -52,13 +53,14 @@ __device__ __forceinline__ void trace_stamp(const StreamArgs &A, int it, int slo
     }
 }
 
-// debug: per-batch stamps of block 7 in sweep index 3 (threads 0 and 32)
+// debug: stamps of every warp, parity 1, batch 0, sweep index 3, every block (what < 4)
 __device__ __forceinline__ void trace_detail(const StreamArgs &A, uint32_t it, int p, int bi, int what)
 {
-    if (A.trace && blockIdx.x == 7 && it == 3 && bi < 8 && (threadIdx.x == 0 || threadIdx.x == 32)) {
+    const int w = threadIdx.x >> 5;
+    if (A.trace && it == 3 && p == 1 && bi == 0 && (threadIdx.x & 31) == 0 && what < 4) {
         unsigned long long t;
         asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
-        A.trace[(size_t)gridDim.x * 64 + (((threadIdx.x >> 5) * 2 + p) * 8 + bi) * 8 + what] = t;
+        A.trace[(size_t)gridDim.x * 64 + ((size_t)blockIdx.x * 16 + w) * 4 + what] = t;
     }
 }
 
@@ -106,7 +108,7 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t by
                  "l"(src), "r"(bytes), "r"(smem_u32(bar))
                  : "memory");
 }
-__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.global;" ::: "memory"); }
 
 
 __device__ __forceinline__ void mbar_arrive(uint64_t *bar)
@@ -174,34 +176,32 @@ __device__ __forceinline__ void stream_issue(const StreamArgs &A, const StreamCt
     }
 }
 
-// Warp 0, start of a half-sweep: the first NS batches.  The proxy fence orders the previous
+// Start of a half-sweep: the first NS batches, one per warp.  The proxy fence orders the previous
 // phase's global stores (made visible by the grid barrier) before the asynchronous-proxy reads.
 template <int L>
 __device__ __forceinline__ void stream_prime(const StreamArgs &A, const StreamCtx<L> &C, int p)
 {
+    const int b = StreamGeom<L>::NTHR / 32 - 1 - (C.tid >> 5);   // the highest warps issue (scheduler priority)
+    if (b >= StreamGeom<L>::NS || b >= C.nb) return;
     fence_proxy_async();
-    for (int b = 0; b < StreamGeom<L>::NS && b < C.nb; ++b) stream_issue<L>(A, C, p, b, b);
+    stream_issue<L>(A, C, p, b, b);
 }
 
-// End of a batch for one warp.  The LAST warp to get here (shared counter) owns the stage: it
-// flushes the batch's satisfied-bond counters (ENERGY) to the global counters and refills the
-// stage with batch b + NS.  No block-wide barrier: the other warps are already on the next stage.
+// End of a batch: block barrier (the stage is free, the batch's shared counters are complete),
+// then the HIGHEST warp refills the stage with batch b + NS and the next-highest one flushes the
+// satisfied-bond counters (ENERGY) to the global counters.  The warp scheduler serves high warp
+// ids first, so these two catch up with the others at once; a low warp in that role would run
+// alone afterwards and stretch every batch.
 template <int L, bool ENERGY>
 __device__ __forceinline__ void stream_batch_done(const StreamArgs &A, const StreamCtx<L> &C, int p, int b, int ebuf)
 {
     using Sg = StreamGeom<L>;
     constexpr int NB = Sg::NB, NS = Sg::NS, NW = Sg::NTHR / 32;
     const Params &P = A.P;
-    const int st = b % NS;
-    __threadfence_block();
-    __syncwarp();
-    int last = 0;
-    if (C.lane == 0) last = atomicAdd(&C.done[st], 1) == NW - 1;
-    last = __shfl_sync(0xFFFFFFFFu, last, 0);
-    if (!last) return;
-    if (C.lane == 0) C.done[st] = 0;
-    __threadfence_block();
-    if (ENERGY) {
+    const int warp = C.tid >> 5;
+    __syncthreads();
+    if (warp == NW - 1 && b + NS < C.nb) stream_issue<L>(A, C, p, b + NS, b % NS);
+    if (ENERGY && warp == NW - 2) {
         const StreamBatch B = C.batch[b];
         const int k0 = B.pos % C.nT;
         int32_t *acc = C.Eacc + (b & 1) * NB * 32;
@@ -210,9 +210,7 @@ __device__ __forceinline__ void stream_batch_done(const StreamArgs &A, const Str
             acc[a] = 0;
             atomicAdd(A.Ecnt + (size_t)ebuf * P.Rp * C.nT + (size_t)(32 * B.w + (a & 31)) * C.nT + k0 + (a >> 5), v);
         }
-        __syncwarp();
     }
-    if (b + NS < C.nb) stream_issue<L>(A, C, p, b + NS, st);
 }
 
 // One half-sweep (parity p) over the block's batches; the first NS are in flight (stream_prime).
@@ -231,6 +229,7 @@ __device__ __forceinline__ void stream_consume(const StreamArgs &A, const Stream
     QuadJ J;
     Planes fin[4];
     for (int b = 0; b < C.nb; ++b) {
+        __syncwarp();
         const StreamBatch B = C.batch[b];
         const int cnt = B.cnt, st = b % NS, pos = B.pos, w = B.w;
         const int k0 = pos % nT, grp = w * NSLAB + B.slab;
@@ -245,8 +244,10 @@ __device__ __forceinline__ void stream_consume(const StreamArgs &A, const Stream
         }
         const uint32_t gw = P.w0 + (uint32_t)w;
         const uint32_t c3 = (uint32_t)p << 16;
+        trace_detail(A, g - A.g0, p, b, 0);
         mbar_wait(&C.full[st], (phase >> st) & 1u);
         phase ^= 1u << st;
+        trace_detail(A, g - A.g0, p, b, 1);
         const unsigned char *stage = C.bufs + (size_t)(st * NB) * Sg::BUF_BYTES;
         if (!ENERGY) {
             for (int i = 0; i < cnt; ++i) {
@@ -259,33 +260,61 @@ __device__ __forceinline__ void stream_consume(const StreamArgs &A, const Stream
                 reinterpret_cast<uint4 *>(P.spin + ((size_t)(k0 + i) * P.W + w) * N + p * Nh)[q] = res;
             }
         } else {
-            uint32_t en[4][5];
+            for (int i0 = 0; i0 < cnt; i0 += 2) {      // pairs of slots: few live registers
+                uint32_t en[2][5];
 #pragma unroll
-            for (int i = 0; i < 4; ++i) {
-                if (i < cnt) {
-                    const int li = pos + i - C.i0;
-                    const char *buf = reinterpret_cast<const char *>(stage + (size_t)i * Sg::BUF_BYTES);
-                    const uint4 rnd = philox_rk(g, (uint32_t)q, gw, c3 | (uint32_t)(k0 + i), A.rk);
-                    const uint4 res = update_quad_mem<L, FAST, true, false>(
-                        buf + 16 * tid, buf + Sg::OWN_BYTES, C.ov, C.oyp, C.oym, C.ozp, C.ozm, C.qx,
-                        C.lt + li * C.LTS, C.mt + (size_t)li * C.MTS, C.R, J, s, rnd, fin);
-                    reinterpret_cast<uint4 *>(P.spin + ((size_t)(k0 + i) * P.W + w) * N + p * Nh)[q] = res;
-                    quad_sum(fin, en[i]);
-                } else {
+                for (int h = 0; h < 2; ++h) {
+                    const int i = i0 + h;
+                    if (i < cnt) {
+                        const int li = pos + i - C.i0;
+                        const char *buf = reinterpret_cast<const char *>(stage + (size_t)i * Sg::BUF_BYTES);
+                        const uint4 rnd = philox_rk(g, (uint32_t)q, gw, c3 | (uint32_t)(k0 + i), A.rk);
+                        const uint4 res = update_quad_mem<L, FAST, true, false>(
+                            buf + 16 * tid, buf + Sg::OWN_BYTES, C.ov, C.oyp, C.oym, C.ozp, C.ozm, C.qx,
+                            C.lt + li * C.LTS, C.mt + (size_t)li * C.MTS, C.R, J, s, rnd, fin);
+                        reinterpret_cast<uint4 *>(P.spin + ((size_t)(k0 + i) * P.W + w) * N + p * Nh)[q] = res;
+                        quad_sum(fin, en[h]);
+                        trace_detail(A, g - A.g0, p, b, 4 + i);
+                    } else {
 #pragma unroll
-                    for (int j = 0; j < 5; ++j) en[i][j] = 0;
+                        for (int j = 0; j < 5; ++j) en[h][j] = 0;
+                    }
                 }
+                uint32_t tot[kResPlanes];
+                warp_sum2(en, C.lane, tot);
+                const int i_mine = i0 + (C.lane >> 4);
+                if (i_mine < cnt && !(C.lane & 8)) add_counts(tot, C.lane & 7, C.Eacc + ((b & 1) * NB + i_mine) * 32);
             }
-            uint32_t tot[kResPlanes];
-            warp_sum4(en, C.lane, tot);
-            const int i_mine = 2 * (C.lane >> 4) + ((C.lane >> 3) & 1);
-            if (i_mine < cnt) add_counts(tot, C.lane & 7, C.Eacc + ((b & 1) * NB + i_mine) * 32);
         }
+        trace_detail(A, g - A.g0, p, b, 2);
         stream_batch_done<L, ENERGY>(A, C, p, b, ebuf);
+        trace_detail(A, g - A.g0, p, b, 3);
     }
 }
 
 namespace cg = cooperative_groups;
+
+// Grid-wide barrier of a cooperative launch (all blocks co-resident).  Same scheme as
+// cooperative_groups::grid_group::sync (block 0 adds 0x80000000 - (G - 1), the others 1; bit 31
+// flips when everybody has arrived), but the block's LAST warp waits, all lanes together.  With
+// thread 0 as the lone waiter (the library version) warp 0 ran the following batch 2.5 times
+// slower than the other warps (measured; the warp scheduler serves high warp ids first).
+__device__ __forceinline__ void stream_grid_sync(unsigned int *bar)
+{
+    __syncthreads();
+    if (threadIdx.x >= blockDim.x - 32) {        // the whole last warp waits: no divergence inside it
+        unsigned int old = 0;
+        if ((threadIdx.x & 31) == 0) {
+            const unsigned int add = blockIdx.x == 0 ? 0x80000000u - (gridDim.x - 1) : 1u;
+            __threadfence();
+            old = atomicAdd(bar, add);
+        }
+        old = __shfl_sync(0xFFFFFFFFu, old, 0);
+        while ((((old ^ *reinterpret_cast<volatile unsigned int *>(bar)) & 0x80000000u) == 0u)) { }
+        __threadfence();
+    }
+    __syncthreads();
+}
 
 template <int L, bool FAST>
 __global__ void __launch_bounds__(StreamGeom<L>::NTHR, 1) k_stream(const StreamArgs A)
@@ -299,7 +328,6 @@ __global__ void __launch_bounds__(StreamGeom<L>::NTHR, 1) k_stream(const StreamA
     const int nT = P.nT, LTS = P.LTS, MTS = 3 * nT + 2, MS = A.MS, MW = A.MW;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarp = NT >> 5;
     constexpr int NTA = NT;
-    cg::grid_group grid = cg::this_grid();
 
     StreamCtx<L> C;
     const long long T = (long long)P.W * NSLAB * nT;
@@ -323,6 +351,8 @@ __global__ void __launch_bounds__(StreamGeom<L>::NTHR, 1) k_stream(const StreamA
     int32_t *Esm = reinterpret_cast<int32_t *>(smraw + A.esm_off);               // [MW][32][nT] bond counts
     StreamBatch *batch = reinterpret_cast<StreamBatch *>(smraw + A.batch_off);   // [MS]
     uint32_t *swwin = reinterpret_cast<uint32_t *>(batch + MS);                  // [nT][SW] thresholds - 1
+    int *swlo = reinterpret_cast<int *>(swwin + (size_t)nT * SW);                // [nT] first m of the stored range
+    int *swhi = swlo + nT;                                                       // [nT] one past its last m
 
     for (int a = tid; a < A.n_bucket; a += NTA) bucket[a] = A.bucket[a];
     for (int a = tid; a < 3 * LTS; a += NTA) thr[a] = P.thr32[a];
@@ -332,6 +362,7 @@ __global__ void __launch_bounds__(StreamGeom<L>::NTHR, 1) k_stream(const StreamA
         const int lo = P.swp_lo[t], cn = P.swp_cnt[t];
         swwin[a] = (m >= lo && m < lo + cn) ? P.swp_val[P.swp_off[t] + (m - lo)] : 0u;
     }
+    for (int t = tid; t + 1 < nT; t += NTA) { swlo[t] = P.swp_lo[t]; swhi[t] = P.swp_lo[t] + P.swp_cnt[t]; }
     for (int a = tid; a < 2 * NB * 32; a += NTA) Eacc[a] = 0;
     for (int a = tid; a < nwt * 32 * nT; a += NTA) {
         tau8[a] = P.tau[(size_t)32 * w_first * nT + a];
@@ -388,7 +419,7 @@ __global__ void __launch_bounds__(StreamGeom<L>::NTHR, 1) k_stream(const StreamA
 
     uint32_t nswap = A.nswap0, phase = 0;
     int ebuf = 0;
-    if (warp == 0) stream_prime<L>(A, C, 0);
+    stream_prime<L>(A, C, 0);
     auto bar_compute = [&]() { __syncthreads(); };
     for (int it = 0; it < A.n_sweeps; ++it) {
         const uint32_t g = A.g0 + (uint32_t)it;
@@ -397,15 +428,17 @@ __global__ void __launch_bounds__(StreamGeom<L>::NTHR, 1) k_stream(const StreamA
         trace_stamp(A, it, 0);
         stream_consume<L, FAST, false>(A, C, 0, g, phase, ebuf);
         trace_stamp(A, it, 1);
-        grid.sync();
-        if (warp == 0) stream_prime<L>(A, C, 1);
+        stream_grid_sync(A.gbar);
+        __syncwarp();   // thread 0 spins inside grid.sync: make its warp converge again before the hot loop
+        stream_prime<L>(A, C, 1);
         trace_stamp(A, it, 2);
         if (need_E) stream_consume<L, FAST, true>(A, C, 1, g, phase, ebuf);
         else stream_consume<L, FAST, false>(A, C, 1, g, phase, ebuf);
         trace_stamp(A, it, 3);
-        grid.sync();
+        stream_grid_sync(A.gbar);
+        __syncwarp();   // thread 0 spins inside grid.sync: make its warp converge again before the hot loop
         // the next sweep's first tiles fly while the swap decisions are taken
-        if (warp == 0 && it + 1 < A.n_sweeps) stream_prime<L>(A, C, 0);
+        if (it + 1 < A.n_sweeps) stream_prime<L>(A, C, 0);
         trace_stamp(A, it, 4);
         if (!need_E) continue;
         const int32_t *cnt = A.Ecnt + (size_t)ebuf * P.Rp * nT;     // satisfied bonds by [r][k]
@@ -422,7 +455,7 @@ __global__ void __launch_bounds__(StreamGeom<L>::NTHR, 1) k_stream(const StreamA
                     const int sa = sg_[t], sb = sg_[t + 1];
                     const int m = (er[sb] - er[sa]) / 2;
                     const uint4 v = philox_rk(g, (uint32_t)t, P.r0 + (uint32_t)r, 2u << 16, A.rk);
-                    const bool acc = (m >= -SW && m < 0 && m >= P.swp_lo[t] && m < P.swp_lo[t] + P.swp_cnt[t])
+                    const bool acc = (m >= -SW && m < 0 && m >= swlo[t] && m < swhi[t])
                                          ? v.x <= swwin[t * SW + m + SW]
                                          : swap_accept(P, t, m, v.x);
                     if (acc) {
