@@ -120,7 +120,9 @@ void launch_cfg(int64_t n, int block, int &grid) { grid = (int)((n + block - 1) 
 // thr6 }: n_c = number of class-c thresholds <= the lower edge, thr_c = the class-c
 // (threshold - 1) inside the bucket or 0xFFFFFFFF.  Buckets holding several thresholds of one
 // class, and all u < 2^8 (index 0), point at row 3 nT + 1 of the mask tables = "use the exact
-// search".  MB is the smallest of 3..6 that leaves < 1e-5 of the draws on the slow path.
+// search".  MB is the smallest of 3..6 that leaves < 1e-5 of the draws on the slow path.  (Measured
+// on config 4: a finer table removes the slow quads, worth 5 %, but spreads the look-ups over more
+// shared-memory banks, which costs 6 %.)
 // trip[n] = the triple (n4, n5, n6) whose sum is n (unique: each n_c is monotone in u).
 static bool build_bucket_table(const std::vector<uint32_t> &thr32, const int z[3], int nT,
                                std::vector<uint4> &tab, std::vector<uchar4> &trip, int &key_lo, int &key_shift)

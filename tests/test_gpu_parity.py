@@ -81,7 +81,7 @@ def test_trajectory_matches_oracle(kernel, L, nT, R, swap, ns):
 
 @pytest.mark.parametrize("kernel", KERNELS)
 def test_set_couplings_set_spins_set_tables(kernel):
-    L, nT, R = (16 if kernel == 3 else 8), 6, 37
+    L, nT, R = {1: 8, 2: 8, 3: 16, 4: 32}[kernel], 6, 37
     betas = 1.0 / temperature_ladder(nT, 0.7, 3.0)
     g, o = _pair(L, nT, R, betas, 5, kernel)
     J = random_couplings(R, L ** 3, 11)
@@ -104,7 +104,7 @@ def test_set_couplings_set_spins_set_tables(kernel):
 
 @pytest.mark.parametrize("kernel", KERNELS)
 def test_ascending_betas_beta_zero_and_no_pt(kernel):
-    L, nT, R = {1: 4, 2: 8, 3: 16}[kernel], 5, 20
+    L, nT, R = {1: 4, 2: 8, 3: 16, 4: 32}[kernel], 5, 20
     betas = np.array([0.0, 0.2, 0.5, 1.0, 3.0])          # ascending, includes beta = 0 and very cold
     g, o = _pair(L, nT, R, betas, 77, kernel)
     g.sweep(30, 1); o.sweep(30, 1)
@@ -123,7 +123,7 @@ def test_ascending_betas_beta_zero_and_no_pt(kernel):
 @pytest.mark.parametrize("kernel", KERNELS)
 def test_word_sharding_reproduces_full_run(kernel):
     # words simulated alone (first_realization = 32 w0) == those words of the full run
-    L, nT, R = (16 if kernel == 3 else 8), 8, 96
+    L, nT, R = {1: 8, 2: 8, 3: 16, 4: 32}[kernel], 8, 96
     betas = 1.0 / temperature_ladder(nT, 0.6, 2.0)
     from paper_1311_5582_b200 import EA
     full = EA(L, nT, R, betas, 9, kernel=kernel)
@@ -166,6 +166,20 @@ def test_kernels_interleave_on_one_handle():
     g.destroy()
 
 
+def test_stream_and_tiled_interleave_on_one_handle():
+    # L = 32: the persistent streaming kernel, the tiled kernel and the generic one continue each
+    # other's state exactly (also with sweeps that are not followed by a swap round)
+    L, nT, R = 32, 6, 40
+    betas = 1.0 / temperature_ladder(nT, 0.9, 2.0)
+    g, o = _pair(L, nT, R, betas, 32)
+    for kernel, n, swap in ((4, 3, 1), (3, 2, 1), (4, 3, 2), (1, 1, 1), (4, 2, 0), (4, 1, 1)):
+        g.set_kernel(kernel)
+        assert g.get_kernel() == kernel
+        g.sweep(n, swap); o.sweep(n, swap)
+        _assert_same(g, o, f"kernel {kernel}")
+    g.destroy()
+
+
 def test_auto_picks_resident_for_L16():
     from paper_1311_5582_b200 import EA
     g = EA(16, 4, 32, np.array([1.0, 0.9, 0.8, 0.7]), 1)
@@ -175,5 +189,5 @@ def test_auto_picks_resident_for_L16():
     assert g.get_kernel() == 1
     g.destroy()
     g = EA(32, 4, 32, np.array([1.0, 0.9, 0.8, 0.7]), 1)
-    assert g.get_kernel() == 3
+    assert g.get_kernel() == 4
     g.destroy()
