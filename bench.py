@@ -29,15 +29,17 @@ from ea_inputs import CONFIGS, betas_for  # noqa: E402
 
 METRIC = "ps per spin-flip attempt"
 UNIT = "ps/attempt"
-# ALU-pipe (LOP3/IADD/SHF/ISETP/SEL class) lane-operations the method needs per word update
-# (32 attempts), derived in DESIGN.md section 8; Philox's 5 IMAD.WIDE per update run on the
-# FMA pipe and are not counted here.
-ALU_OPS_PER_WORD_UPDATE = 43.0
+# ALU-pipe (LOP3/IADD/SHF/ISETP class) lane-operations the method needs per word update
+# (32 attempts), derived in DESIGN.md section 8: 30 on every update + 15.5 on parity-1 updates
+# (energy).  Philox's multiplies and the table addressing run on the FMA pipe and are not
+# counted; the kernels execute ~47 ALU instructions per update (profiles/).
+ALU_OPS_PER_WORD_UPDATE = 38.0
 PAPER_PS = 33.5   # GTX 580, PT every 10 sweeps: context, another workload
 # DRAM bytes (read + write) of ONE launch of the dominant kernel, from the committed ncu
 # --set full capture (profiles/r01_ncu_resident_cfg4.txt): the state is read once per launch
 # whatever the number of sweeps; the write-back stays in L2.
 NCU_DRAM_BYTES_PER_LAUNCH = {4: 28.87e6}
+NCU_ALU_PIPE_BUSY = {4: "86 %"}
 
 
 def _clock_sampler(stop, out):
@@ -239,8 +241,22 @@ def run_cuda(a, cfg):
     roofline = {"bound": "alu", "achieved": achieved / 1e12, "peak": peak["lop3"] / 1e12, "unit": "Tlaneop/s",
                 "frac": achieved / peak["lop3"], "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(a.config),
                 "note": "ALU-pipe lane-ops: %.0f per word update (DESIGN.md s8) / measured LOP3 issue peak "
-                        "(ea_measure_int_peak, same process); IMAD peak %.2f, LOP3+IMAD mix %.2f Tlaneop/s"
-                        % (ALU_OPS_PER_WORD_UPDATE, peak["imad"] / 1e12, peak["mix"] / 1e12)}
+                        "(ea_measure_int_peak, same process); IMAD peak %.2f, LOP3+IMAD mix %.2f Tlaneop/s; "
+                        "ncu: ALU pipe %s busy on the occupied SMs (profiles/)"
+                        % (ALU_OPS_PER_WORD_UPDATE, peak["imad"] / 1e12, peak["mix"] / 1e12,
+                           NCU_ALU_PIPE_BUSY.get(a.config, "n/a"))}
+    if kernel == 4:
+        # streaming kernel: algorithmic bytes = per half-sweep and item, tile read (own parity 8 KiB +
+        # other parity with halo 12 KiB at L = 32) + own parity written back; the state fits L2, so
+        # this is L2 traffic and the HBM figure is context, not the bound
+        zs = 512 // ((cfg.L // 8) * cfg.L)
+        tile = 512 * 16 + (zs + 2) * (cfg.L // 8) * cfg.L * 16 + 512 * 16
+        bytes_step = 2.0 * tile * cfg.n_temps * cfg.W * (cfg.L // zs) * sps
+        hbm = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"] if os.path.exists(
+            os.path.join(ROOT, "MEASURED_PEAKS.json")) else 6650.0
+        roofline["hbm_view"] = {"algorithmic_GBps": bytes_step / (float(np.mean(step_ms)) * 1e-3) / 1e9,
+                                "peak_GBps": hbm, "frac": bytes_step / (float(np.mean(step_ms)) * 1e-3) / 1e9 / hbm,
+                                "note": "tile bytes streamed per sweep / time; served by L2 (state 35 MiB < 126 MB)"}
 
     # ---- CPU oracle on the host cores: bounded sample of the same workload
     cores = len(os.sched_getaffinity(0))
@@ -255,7 +271,7 @@ def run_cuda(a, cfg):
         "dtype": "u32 bit-sliced words (32 realizations each), u32 Philox draws", "data": "synthetic",
         "config": {"workload": cfg.name, "L": cfg.L, "n_temps": cfg.n_temps, "realizations_per_gpu": cfg.R,
                    "swap_interval": cfg.swap_interval, "sweeps_per_step": sps, "seed": cfg.seed,
-                   "kernel": {1: "generic", 2: "resident", 3: "tiled"}.get(kernel, str(kernel)),
+                   "kernel": {1: "generic", 2: "resident", 3: "tiled", 4: "stream"}.get(kernel, str(kernel)),
                    "l2": "flushed between timed steps (256 MiB write); state is re-read from HBM each step",
                    "parallelism": f"shard by realization word x{world}, no collective"},
         "clocks": _clock_summary(samples),

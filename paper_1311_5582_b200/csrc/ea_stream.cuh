@@ -13,8 +13,11 @@
 // sweep separate the half-sweeps (two consecutive stages).  Energies: satisfied
 // bonds of the parity-1 pass -> per-block shared atomics -> global counters; after the second
 // barrier every block takes the parallel-tempering decisions of the words it works on
-// (identical in every block: same counters, same Philox draws) and rebuilds its mask tables.
-// No lattice word moves in a swap.
+// (identical in every block: same counters, same Philox draws) and rebuilds its mask tables,
+// while the first tiles of the next sweep are already in flight.  No lattice word moves in a
+// swap.  Scheduling notes (measured, profiles/): the warp scheduler serves high
+// warp ids first, so the block's HIGHEST warps issue the TMA copies, flush the counters and wait
+// on the grid barrier; with warp 0 in those roles every batch waited for it.
 #pragma once
 #include <cooperative_groups.h>
 
@@ -111,11 +114,6 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t by
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.global;" ::: "memory"); }
 
 
-__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
-{
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-
 // One batch = up to NB consecutive slots of one (word, slab) group; the block's batch list is
 // fixed for the whole launch and sits in shared memory.
 struct StreamBatch { int pos, cnt, w, slab; };
@@ -129,7 +127,6 @@ struct StreamCtx {
     int tid, lane, qx, y, zl;
     uint32_t ov, oyp, oym, ozp, ozm;   // byte offsets inside the other-parity buffer
     uint64_t *full;              // [NS]: tiles landed
-    int *done;                   // [NS]: warps that have finished with the stage
     const StreamBatch *batch;
     unsigned char *bufs;
     uint4 *mt;
@@ -138,7 +135,7 @@ struct StreamCtx {
     RankCtx R;
 };
 
-// TMA bulk loads of batch b into ring stage st, issued by the lanes of the producer warp in
+// TMA bulk loads of batch b into ring stage st, issued by the lanes of one warp in
 // parallel (lane = 3 * slot + piece): per slot the slab's own-parity words (contiguous) and the
 // other parity's planes z0-1 .. z0+ZS (periodic wrap = 2 pieces).
 template <int L>
@@ -337,7 +334,7 @@ __global__ void __launch_bounds__(StreamGeom<L>::NTHR, 1) k_stream(const StreamA
     const int w_first = C.i0 / per_w, nwt = (C.i1 - 1) / per_w - w_first + 1;   // words I meet (<= MW)
 
     // shared memory
-    uint64_t *mbar = reinterpret_cast<uint64_t *>(smraw);                        // full[NS], done[NS], nb: 64 B reserved
+    uint64_t *mbar = reinterpret_cast<uint64_t *>(smraw);                        // full[NS], number of batches: 64 B reserved
     uint4 *bucket = reinterpret_cast<uint4 *>(smraw + 64);                       // [n_bucket]
     unsigned char *bufs = reinterpret_cast<unsigned char *>(bucket + A.n_bucket);   // [NS][NB][BUF_BYTES]
     uint4 *mt = reinterpret_cast<uint4 *>(bufs + (size_t)NS * NB * Sg::BUF_BYTES);  // [MS][MTS]
@@ -369,7 +366,7 @@ __global__ void __launch_bounds__(StreamGeom<L>::NTHR, 1) k_stream(const StreamA
         sig8[a] = P.sigma[(size_t)32 * w_first * nT + a];
     }
     if (tid == 0) {
-        for (int i = 0; i < NS; ++i) { mbar_init(&mbar[i], 1); reinterpret_cast<int *>(mbar + NS)[i] = 0; }
+        for (int i = 0; i < NS; ++i) mbar_init(&mbar[i], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         // my batch list: up to NB consecutive slots of one (word, slab) group each
         int nb = 0;
@@ -400,7 +397,7 @@ __global__ void __launch_bounds__(StreamGeom<L>::NTHR, 1) k_stream(const StreamA
 
     C.nT = nT; C.LTS = LTS; C.MTS = MTS;
     C.tid = tid; C.lane = lane;
-    C.qx = tid % QR; C.y = (tid / QR) % L; C.zl = (tid / QPP) % Sg::ZS;   // (producer lanes: unused)
+    C.qx = tid % QR; C.y = (tid / QR) % L; C.zl = tid / QPP;
     {
         const int row = QR * C.y + C.qx;
         C.ov = 16u * (uint32_t)((C.zl + 1) * QPP + row);
@@ -409,7 +406,7 @@ __global__ void __launch_bounds__(StreamGeom<L>::NTHR, 1) k_stream(const StreamA
         C.ozp = 16u * (uint32_t)((C.zl + 2) * QPP + row);
         C.ozm = 16u * (uint32_t)(C.zl * QPP + row);
     }
-    C.full = mbar; C.done = reinterpret_cast<int *>(mbar + NS); C.batch = batch; C.bufs = bufs; C.mt = mt; C.lt = lt; C.Eacc = Eacc;
+    C.full = mbar; C.batch = batch; C.bufs = bufs; C.mt = mt; C.lt = lt; C.Eacc = Eacc;
     C.nb = *reinterpret_cast<const int *>(smraw + 48);
     C.R.thr = thr; C.R.bucket = bucket; C.R.LTS = LTS; C.R.nT = nT;
     C.R.key_lo = A.key_lo; C.R.key_top = A.n_bucket - 1; C.R.key_shift = A.key_shift;
