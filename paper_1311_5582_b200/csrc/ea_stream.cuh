@@ -251,7 +251,7 @@ __device__ __forceinline__ void stream_consume(const StreamArgs &A, const Stream
                 const int li = pos + i - C.i0;
                 const char *buf = reinterpret_cast<const char *>(stage + (size_t)i * Sg::BUF_BYTES);
                 const uint4 rnd = philox_rk(g, (uint32_t)q, gw, c3 | (uint32_t)(k0 + i), A.rk);
-                const uint4 res = update_quad_mem<L, FAST, false, false>(
+                const uint4 res = update_quad_mem<L, FAST, false, false, false>(
                     buf + 16 * tid, buf + Sg::OWN_BYTES, C.ov, C.oyp, C.oym, C.ozp, C.ozm, C.qx, C.lt + li * C.LTS,
                     C.mt + (size_t)li * C.MTS, C.R, J, s, rnd, fin);
                 reinterpret_cast<uint4 *>(P.spin + ((size_t)(k0 + i) * P.W + w) * N + p * Nh)[q] = res;
@@ -266,7 +266,7 @@ __device__ __forceinline__ void stream_consume(const StreamArgs &A, const Stream
                         const int li = pos + i - C.i0;
                         const char *buf = reinterpret_cast<const char *>(stage + (size_t)i * Sg::BUF_BYTES);
                         const uint4 rnd = philox_rk(g, (uint32_t)q, gw, c3 | (uint32_t)(k0 + i), A.rk);
-                        const uint4 res = update_quad_mem<L, FAST, true, false>(
+                        const uint4 res = update_quad_mem<L, FAST, true, false, false>(
                             buf + 16 * tid, buf + Sg::OWN_BYTES, C.ov, C.oyp, C.oym, C.ozp, C.ozm, C.qx,
                             C.lt + li * C.LTS, C.mt + (size_t)li * C.MTS, C.R, J, s, rnd, fin);
                         reinterpret_cast<uint4 *>(P.spin + ((size_t)(k0 + i) * P.W + w) * N + p * Nh)[q] = res;
