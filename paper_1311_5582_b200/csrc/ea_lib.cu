@@ -520,7 +520,7 @@ ResPlan plan_resident(const ea_handle *h)
     if (h->L != 8 && h->L != 16) return pl;
     const size_t cap = 227 * 1024;
     int C = 0;
-    for (int c = 1; c <= 8; ++c) {
+    for (int c = 1; c <= 8; c *= 2) {            // cluster sizes 1, 2, 4, 8 (others fail to launch)
         const int S = (h->nT + c - 1) / c;
         if (resident_smem(h, S) <= cap) { C = c; break; }
     }
@@ -768,7 +768,7 @@ static int sweep_stream(ea_handle *h, int64_t n_sweeps, int swap_interval)
         // debug aid: EA_STREAM_TRACE=<file> dumps per-block phase time stamps of the first 8 sweeps
         const char *trace_path = std::getenv("EA_STREAM_TRACE");
         unsigned long long *d_trace = nullptr;
-        const size_t trace_n = (size_t)pl.grid * 64 + (size_t)pl.grid * 64;
+        const size_t trace_n = (size_t)pl.grid * 64;
         if (trace_path && cudaMalloc((void **)&d_trace, 8 * trace_n) == cudaSuccess) {
             cudaMemsetAsync(d_trace, 0, 8 * trace_n, h->stream);
             A.trace = d_trace;

@@ -44,7 +44,7 @@ struct StreamArgs {
     int esm_off;             // byte offset (16 B aligned) of the swap-phase staging area in smem
     int batch_off;           // byte offset (16 B aligned) of the batch list in smem
     unsigned int *gbar;      // grid barrier word (zero before the first launch; self-resetting)
-    unsigned long long *trace;   // debug (EA_STREAM_TRACE): [block][8 sweeps][8] globaltimer stamps, or null
+    unsigned long long *trace;   // debug (EA_STREAM_TRACE): [block][8 sweeps][8] globaltimer stamps of the phases, or null
 };
 
 __device__ __forceinline__ void trace_stamp(const StreamArgs &A, int it, int slot)
@@ -53,17 +53,6 @@ __device__ __forceinline__ void trace_stamp(const StreamArgs &A, int it, int slo
         unsigned long long t;
         asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
         A.trace[((size_t)blockIdx.x * 8 + it) * 8 + slot] = t;
-    }
-}
-
-// debug: stamps of every warp, parity 1, batch 0, sweep index 3, every block (what < 4)
-__device__ __forceinline__ void trace_detail(const StreamArgs &A, uint32_t it, int p, int bi, int what)
-{
-    const int w = threadIdx.x >> 5;
-    if (A.trace && it == 3 && p == 1 && bi == 0 && (threadIdx.x & 31) == 0 && what < 4) {
-        unsigned long long t;
-        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
-        A.trace[(size_t)gridDim.x * 64 + ((size_t)blockIdx.x * 16 + w) * 4 + what] = t;
     }
 }
 
@@ -241,10 +230,8 @@ __device__ __forceinline__ void stream_consume(const StreamArgs &A, const Stream
         }
         const uint32_t gw = P.w0 + (uint32_t)w;
         const uint32_t c3 = (uint32_t)p << 16;
-        trace_detail(A, g - A.g0, p, b, 0);
         mbar_wait(&C.full[st], (phase >> st) & 1u);
         phase ^= 1u << st;
-        trace_detail(A, g - A.g0, p, b, 1);
         const unsigned char *stage = C.bufs + (size_t)(st * NB) * Sg::BUF_BYTES;
         if (!ENERGY) {
             for (int i = 0; i < cnt; ++i) {
@@ -271,7 +258,6 @@ __device__ __forceinline__ void stream_consume(const StreamArgs &A, const Stream
                             C.lt + li * C.LTS, C.mt + (size_t)li * C.MTS, C.R, J, s, rnd, fin);
                         reinterpret_cast<uint4 *>(P.spin + ((size_t)(k0 + i) * P.W + w) * N + p * Nh)[q] = res;
                         quad_sum(fin, en[h]);
-                        trace_detail(A, g - A.g0, p, b, 4 + i);
                     } else {
 #pragma unroll
                         for (int j = 0; j < 5; ++j) en[h][j] = 0;
@@ -283,9 +269,7 @@ __device__ __forceinline__ void stream_consume(const StreamArgs &A, const Stream
                 if (i_mine < cnt && !(C.lane & 8)) add_counts(tot, C.lane & 7, C.Eacc + ((b & 1) * NB + i_mine) * 32);
             }
         }
-        trace_detail(A, g - A.g0, p, b, 2);
         stream_batch_done<L, ENERGY>(A, C, p, b, ebuf);
-        trace_detail(A, g - A.g0, p, b, 3);
     }
 }
 

@@ -58,6 +58,9 @@ def _skip_unsupported(kernel, L):
     (8, 6, 40, 3, 14),         # cluster with an empty block, swap every 3rd sweep
     (16, 5, 33, 1, 4),         # odd n_temps, ragged words
     (8, 33, 20, 1, 8),         # more temperatures than fit one block group
+    (64, 3, 33, 1, 2),         # L = 64: one-plane slabs in the streaming kernel, odd n_temps
+    (32, 64, 32, 1, 2),        # the most temperatures the library takes
+    (16, 64, 5, 2, 3),         # 64 temperatures in the resident kernel (cluster of 8)
 ])
 def test_trajectory_matches_oracle(kernel, L, nT, R, swap, ns):
     _skip_unsupported(kernel, L)
