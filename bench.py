@@ -113,7 +113,7 @@ def run_reference(a, cfg):
     cores = len(os.sched_getaffinity(0))
     words = min(cores, cfg.W)
     sweeps = max(1, int(1.5e8 / (32 * cfg.n_temps * cfg.N)))      # ~4 s of one core per word
-    for _ in range(a.warmup):
+    for _ in range(max(a.warmup, 1)):           # at least once: builds the oracle, starts the pool
         oracle_sample(cfg, words, 1, words)
     vals, walls = [], []
     for _ in range(a.steps):
