@@ -773,7 +773,8 @@ static int sweep_stream(ea_handle *h, int64_t n_sweeps, int swap_interval)
             cudaMemsetAsync(d_trace, 0, 8 * trace_n, h->stream);
             A.trace = d_trace;
         }
-        CUDA_TRY(h, cudaMemsetAsync(h->d_Ecnt, 0, 2 * 4 * (size_t)h->Rp * h->nT, h->stream));
+        // counters and the grid-barrier word start from zero in every launch
+        CUDA_TRY(h, cudaMemsetAsync(h->d_Ecnt, 0, 2 * 4 * (size_t)h->Rp * h->nT + 256, h->stream));
         const cudaError_t e = h->L == 32 ? launch_stream_t<32>(h, A, pl, h->fast_rank)
                                          : launch_stream_t<64>(h, A, pl, h->fast_rank);
         if (d_trace) {
@@ -782,6 +783,12 @@ static int sweep_stream(ea_handle *h, int64_t n_sweeps, int swap_interval)
             cudaStreamSynchronize(h->stream);
             if (FILE *f = std::fopen(trace_path, "wb")) { std::fwrite(tr.data(), 8, trace_n, f); std::fclose(f); }
             cudaFree(d_trace);
+        }
+        if (e == cudaErrorCooperativeLaunchTooLarge && h->kernel_sel == EA_KERNEL_AUTO) {
+            // the SMs are not all free (another context holds some): same result, one launch per
+            // half-sweep instead of one cooperative launch
+            cudaGetLastError();
+            return sweep_tiled(h, left, swap_interval);
         }
         if (e != cudaSuccess) return fail(h, EA_ERR_CUDA, std::string("stream launch: ") + cudaGetErrorString(e));
         h->launches++;
