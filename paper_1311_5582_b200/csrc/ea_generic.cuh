@@ -219,7 +219,8 @@ __global__ void k_unpack_spins(Params P, int R, int by_slot, int8_t *out)
 // in[r][outer][i] (+-1 int8, canonical site order) -> words[outer'][w][p][j]; one thread per
 // output word.  mode 0: spins (outer = slot k, word index (k W + w) N + ...);
 // mode 1: couplings (outer = d, word index (w 3 + d) N + ...).
-__global__ void k_pack(Params P, int R, int n_outer, int mode, const int8_t *in, uint32_t *words)
+// *bad is set if any input value is neither +1 nor -1 (the caller then discards `words`).
+__global__ void k_pack(Params P, int R, int n_outer, int mode, const int8_t *in, uint32_t *words, int *bad)
 {
     const int64_t tid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (tid >= (int64_t)n_outer * P.W * P.N) return;
@@ -229,10 +230,15 @@ __global__ void k_pack(Params P, int R, int n_outer, int mode, const int8_t *in,
     const int x = i % P.L, y = (i / P.L) % P.L, z = i / (P.L * P.L);
     const int p = (x + y + z) & 1, j = (x >> 1) + P.Lh * (y + P.L * z);
     uint32_t v = 0;
+    bool wrong = false;
     for (int b = 0; b < 32; ++b) {
         const int r = 32 * w + b;
-        if (r < R && in[((size_t)r * n_outer + o) * P.N + i] > 0) v |= 1u << b;
+        if (r >= R) break;
+        const int8_t v8 = in[((size_t)r * n_outer + o) * P.N + i];
+        wrong |= (v8 != 1 && v8 != -1);
+        if (v8 > 0) v |= 1u << b;
     }
+    if (wrong) *bad = 1;
     const size_t dst = mode == 0 ? ((size_t)o * P.W + w) * P.N : ((size_t)w * 3 + o) * P.N;
     words[dst + p * P.Nh + j] = v;
 }

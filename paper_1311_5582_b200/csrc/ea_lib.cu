@@ -424,24 +424,36 @@ extern "C" int ea_synchronize(ea_handle *h)
 }
 
 // ---------------------------------------------------------------- inputs
+// Host +-1 array -> packed words.  The values are checked on the device while they are packed into
+// a scratch copy; the handle's array is replaced only if all of them are valid (state unchanged on
+// error), so the host never walks the input.
 static int pack_from_host(ea_handle *h, const int8_t *src, int n_outer, int mode, uint32_t *dst)
 {
     const size_t n = (size_t)h->R * n_outer * h->N;
-    for (size_t a = 0; a < n; ++a)
-        if (src[a] != 1 && src[a] != -1) return fail(h, EA_ERR_INVALID_ARG, "values must be +1 or -1");
-    int8_t *tmp = nullptr;
-    CUDA_TRY(h, cudaMalloc((void **)&tmp, n));
+    const size_t nw = (size_t)n_outer * h->W * h->N;
+    const size_t off_w = (n + 255) & ~(size_t)255, off_f = off_w + 4 * nw;
+    char *tmp = nullptr;
+    CUDA_TRY(h, cudaMalloc((void **)&tmp, off_f + 256));
+    int bad = 0;
     cudaError_t e = cudaMemcpyAsync(tmp, src, n, cudaMemcpyHostToDevice, h->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(tmp + off_f, 0, 4, h->stream);
     if (e == cudaSuccess) {
         int grid;
-        launch_cfg((int64_t)n_outer * h->W * h->N, 128, grid);
-        ea::k_pack<<<grid, 128, 0, h->stream>>>(h->P, h->R, n_outer, mode, tmp, dst);
+        launch_cfg((int64_t)nw, 128, grid);
+        ea::k_pack<<<grid, 128, 0, h->stream>>>(h->P, h->R, n_outer, mode, (const int8_t *)tmp,
+                                                (uint32_t *)(tmp + off_w), (int *)(tmp + off_f));
         h->launches++;
         e = cudaGetLastError();
     }
+    if (e == cudaSuccess) e = cudaMemcpyAsync(&bad, tmp + off_f, 4, cudaMemcpyDeviceToHost, h->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+    if (e == cudaSuccess && !bad) {
+        e = cudaMemcpyAsync(dst, tmp + off_w, 4 * nw, cudaMemcpyDeviceToDevice, h->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+    }
     cudaFree(tmp);
     if (e != cudaSuccess) return fail(h, EA_ERR_CUDA, std::string("pack: ") + cudaGetErrorString(e));
+    if (bad) return fail(h, EA_ERR_INVALID_ARG, "values must be +1 or -1");
     return recompute_energy(h);
 }
 
