@@ -8,6 +8,7 @@ from __future__ import annotations
 import ctypes as C
 import os
 import subprocess
+from fractions import Fraction
 from pathlib import Path
 
 import numpy as np
@@ -183,3 +184,82 @@ class Oracle:
         self.lib.eao_get_counters(self.h, C.byref(g), C.byref(n), st)
         return {"sweeps": g.value, "swap_rounds": n.value, "attempts": st[0], "accepted": st[1],
                 "swap_attempts": st[2], "swap_accepted": st[3]}
+
+
+    # ------------------------------------------------------------------ measurement
+    def pair_couplings(self):
+        """Two-copy set-up: realizations R/2.. get the couplings of 0..R/2-1 (the spins and
+        the random draws of the two halves stay different because they sit in different
+        words, R11).  The overlap between the copies r and r + R/2 is the
+        spin-glass order parameter q whose Binder ratio the paper plots (Fig. 20)."""
+        half = self.R // 2
+        assert self.R % 64 == 0, "R/2 must be a multiple of 32 (copies in different words)"
+        J = self.couplings()
+        J[half:] = J[:half]
+        return self.set_couplings(J)
+
+    def realization_pairs(self, word_pairs):
+        """Word pair (wa, wb) -> the 32 realization pairs (32 wa + b, 32 wb + b); wb = -1 is the
+        all-up reference.  Entries that touch a padding bit (index >= R) are None."""
+        out = []
+        for wa, wb in np.asarray(word_pairs, dtype=np.int64).reshape(-1, 2):
+            row = []
+            for b in range(32):
+                ra, rb = 32 * int(wa) + b, (32 * int(wb) + b if wb >= 0 else -1)
+                row.append((ra, rb) if ra < self.R and rb < self.R else None)
+            out.append(row)
+        return out
+
+    def measure(self, n_meas, sweeps_between, swap_interval, word_pairs, acc=None):
+        """n_meas times: sweep(sweeps_between, swap_interval), then one measurement of the
+        overlaps q of `word_pairs` and of the energies E, by temperature index.  Accumulates
+        exact integer sums (Python ints): n, sum q, sum q^2, sum q^4 as [pair][bit][t] and
+        sum E, sum E^2 as [r][t].  Returns (and, if given, continues) the accumulator dict."""
+        rp = self.realization_pairs(word_pairs)
+        P = len(rp)
+        if acc is None:
+            z = lambda *shape: np.zeros(shape, dtype=object) + 0
+            acc = {"n": 0, "q1": z(P, 32, self.nT), "q2": z(P, 32, self.nT), "q4": z(P, 32, self.nT),
+                   "e1": z(self.R, self.nT), "e2": z(self.R, self.nT)}
+        flat = [(p, b, pr) for p in range(P) for b, pr in enumerate(rp[p]) if pr is not None]
+        pairs = np.array([pr for _, _, pr in flat], dtype=np.int32).reshape(-1, 2)
+        for _ in range(int(n_meas)):
+            self.sweep(sweeps_between, swap_interval)
+            Q = self.overlap(pairs) if len(flat) else np.zeros((0, self.nT), dtype=np.int32)
+            E = self.energy()
+            for (p, b, _), qrow in zip(flat, Q):
+                for t in range(self.nT):
+                    q = int(qrow[t])
+                    acc["q1"][p, b, t] += q
+                    acc["q2"][p, b, t] += q * q
+                    acc["q4"][p, b, t] += q * q * q * q
+            for r in range(self.R):
+                for t in range(self.nT):
+                    e = int(E[r, t])
+                    acc["e1"][r, t] += e
+                    acc["e2"][r, t] += e * e
+            acc["n"] += 1
+        acc["valid"] = np.array([[pr is not None for pr in row] for row in rp], dtype=bool).reshape(P, 32)
+        return acc
+
+
+def binder_ratio(acc):
+    """Binder ratio of the overlap by temperature index, g = (3 - [<q^4>] / [<q^2>]^2) / 2:
+    <.> = time average of one realization pair, [.] = average over the valid pairs (disorder
+    average).  The paper plots it (Fig. 20) without printing the formula; this is
+    the standard definition of its reference [63] (R20).  Exact rational arithmetic,
+    rounded to double once at the end.  NaN where [<q^2>] = 0."""
+    n = acc["n"]
+    valid = acc["valid"]
+    M = int(valid.sum())
+    nT = acc["q2"].shape[2]
+    g = np.full(nT, np.nan)
+    for t in range(nT):
+        s2 = sum(int(v) for v in acc["q2"][valid, t])
+        s4 = sum(int(v) for v in acc["q4"][valid, t])
+        if n == 0 or M == 0 or s2 == 0:
+            continue
+        q2 = Fraction(s2, n * M)
+        q4 = Fraction(s4, n * M)
+        g[t] = float((3 - q4 / (q2 * q2)) / 2)
+    return g

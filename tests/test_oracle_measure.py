@@ -1,0 +1,143 @@
+"""Pins for the oracle's measurement layer (Fig. 20):
+two-copy coupling set-up, exact integer moments of the overlap and of the energy, Binder ratio.
+
+Expected values come from numpy over exported +-1 arrays (never from the oracle's own
+overlap / energy routines), from closed forms, or from exact enumeration.
+"""
+from fractions import Fraction
+
+import numpy as np
+
+from ea_inputs import random_pm1
+from oracle import Oracle, binder_ratio
+from test_oracle_chain import H_numpy
+
+
+def _q_numpy(s, ra, rb):
+    """overlap by temperature index from s[r][t][site] (+-1): plain dot products."""
+    a = s[ra].astype(np.int64)
+    b = s[rb].astype(np.int64) if rb >= 0 else np.ones_like(a)
+    return (a * b).sum(axis=1)
+
+
+def test_pair_couplings_copies_first_half_and_recomputes_energies():
+    L, nT, R = 4, 3, 64
+    o = Oracle(L, nT, R, np.array([1.2, 0.9, 0.5]), 17)
+    J0 = o.couplings()
+    assert (J0[:32] != J0[32:]).any()
+    assert o.pair_couplings() == 0
+    J = o.couplings()
+    assert (J[:32] == J0[:32]).all() and (J[32:] == J0[:32]).all()
+    s = o.spins_by_slot()
+    assert (s[:32] != s[32:]).any()          # the copies start from different spins
+    E = o.energy_by_slot()
+    for r in (0, 31, 32, 63):
+        for k in range(nT):
+            assert E[r, k] == H_numpy(s[r, k], J[r], L)
+
+
+def test_moments_equal_numpy_recomputation_from_exported_spins():
+    L, nT, R = 4, 4, 70                      # ragged: word 2 holds 6 realizations
+    betas = 1.0 / np.array([0.8, 1.1, 1.5, 2.0])
+    o = Oracle(L, nT, R, betas, 23)
+    wp = [[0, 1], [1, 2], [2, -1], [0, 0]]
+    rp = o.realization_pairs(wp)
+    assert rp[1][5] == (37, 69) and rp[1][6] is None and rp[2][5] == (69, -1) and rp[2][6] is None
+    acc = None
+    exp = {k: np.zeros((len(wp), 32, nT), dtype=object) + 0 for k in ("q1", "q2", "q4")}
+    e1 = np.zeros((R, nT), dtype=object) + 0
+    e2 = np.zeros((R, nT), dtype=object) + 0
+    n_meas = 6
+    for m in range(n_meas):
+        acc = o.measure(1, 3, 2, wp, acc)
+        s = o.spins()                        # [r][t][site] by temperature index
+        J = o.couplings()
+        for p, row in enumerate(rp):
+            for b, pr in enumerate(row):
+                if pr is None:
+                    continue
+                q = _q_numpy(s, *pr)
+                for t in range(nT):
+                    v = int(q[t])
+                    exp["q1"][p, b, t] += v
+                    exp["q2"][p, b, t] += v ** 2
+                    exp["q4"][p, b, t] += v ** 4
+        for r in range(0, R, 7):
+            for t in range(nT):
+                e = H_numpy(s[r, t], J[r], L)
+                e1[r, t] += e
+                e2[r, t] += e * e
+    assert acc["n"] == n_meas and o.counters()["sweeps"] == 3 * n_meas
+    for k in ("q1", "q2", "q4"):
+        assert (acc[k] == exp[k]).all(), k
+    rows = np.arange(0, R, 7)
+    assert (acc["e1"][rows] == e1[rows]).all() and (acc["e2"][rows] == e2[rows]).all()
+    assert (acc["q1"][3, :, :] == n_meas * L ** 3).all()          # a realization with itself: q = N
+    assert (acc["q1"][1, 6:, :] == 0).all() and not acc["valid"][1, 6:].any()
+    # measure(2, ...) then measure(4, ...) == six single measurements (continuation)
+    o2 = Oracle(L, nT, R, betas, 23)
+    a2 = o2.measure(4, 3, 2, wp, o2.measure(2, 3, 2, wp))
+    for k in ("q1", "q2", "q4", "e1", "e2"):
+        assert (a2[k] == acc[k]).all(), k
+
+
+def test_beta_zero_overlap_is_constant():
+    """beta = 0: every sweep complements every configuration, so q(a, b) never changes and
+    the magnetization alternates in sign: sum q^k = n q0^k, sum m = 0 for even n."""
+    L, nT, R = 4, 2, 64
+    o = Oracle(L, nT, R, np.zeros(nT), 5)
+    s0 = o.spins()
+    acc = o.measure(4, 1, 0, [[0, 1], [1, -1]])
+    for b in (0, 13, 31):
+        q0 = _q_numpy(s0, b, 32 + b)
+        m0 = _q_numpy(s0, 32 + b, -1)
+        for t in range(nT):
+            assert acc["q1"][0, b, t] == 4 * int(q0[t])
+            assert acc["q2"][0, b, t] == 4 * int(q0[t]) ** 2
+            assert acc["q4"][0, b, t] == 4 * int(q0[t]) ** 4
+            assert acc["q1"][1, b, t] == 0
+            assert acc["q2"][1, b, t] == 4 * int(m0[t]) ** 2
+
+
+def test_binder_of_all_256_states_of_the_2cube_is_one_over_N():
+    """Exact enumeration: the 256 configurations of the 2^3 lattice against the all-up
+    reference have the binomial moments [q^2] = N, [q^4] = 3N^2 - 2N, so g = 1/N = 0.125."""
+    L, R = 2, 256
+    o = Oracle(L, 1, R, np.array([1.0]), 3)
+    s = np.array([[[1 if (r >> i) & 1 else -1 for i in range(8)]] for r in range(R)], dtype=np.int8)
+    assert o.set_spins(s) == 0
+    acc = o.measure(1, 0, 0, [[w, -1] for w in range(8)])
+    assert acc["valid"].all() and acc["n"] == 1
+    assert sum(int(v) for v in acc["q2"].ravel()) == 256 * 8
+    assert sum(int(v) for v in acc["q4"].ravel()) == 256 * (3 * 64 - 16)
+    assert sum(int(v) for v in acc["q1"].ravel()) == 0
+    g = binder_ratio(acc)
+    assert g.shape == (1,) and g[0] == 0.125
+
+
+def test_binder_formula_on_synthetic_sums():
+    rng = np.random.default_rng(0)
+    P, nT, n = 3, 4, 50
+    q = rng.integers(-64, 65, size=(n, P, 32, nT))
+    valid = np.ones((P, 32), dtype=bool)
+    valid[2, 20:] = False
+    acc = {"n": n, "valid": valid,
+           "q2": (q.astype(object) ** 2).sum(axis=0), "q4": (q.astype(object) ** 4).sum(axis=0)}
+    g = binder_ratio(acc)
+    qf = q.astype(np.float64)
+    for t in range(nT):
+        m2 = (qf[:, valid, t] ** 2).mean(axis=0).mean()
+        m4 = (qf[:, valid, t] ** 4).mean(axis=0).mean()
+        assert abs(g[t] - 0.5 * (3.0 - m4 / m2 ** 2)) < 1e-12
+    # frozen copies: q = +-N every time -> g = 1 exactly; q = 0 -> undefined (NaN)
+    one = {"n": 7, "valid": np.ones((1, 32), dtype=bool),
+           "q2": np.full((1, 32, 2), 7 * 64 ** 2, dtype=object), "q4": np.full((1, 32, 2), 7 * 64 ** 4, dtype=object)}
+    assert (binder_ratio(one) == 1.0).all()
+    one["q2"][:, :, 1] = 0
+    one["q4"][:, :, 1] = 0
+    g = binder_ratio(one)
+    assert g[0] == 1.0 and np.isnan(g[1])
+    # a two-valued distribution, by hand: q in {1, 3} equally often: <q^2> = 5, <q^4> = 41
+    two = {"n": 2, "valid": np.ones((1, 1), dtype=bool),
+           "q2": np.array([[[10]]], dtype=object), "q4": np.array([[[82]]], dtype=object)}
+    assert binder_ratio(two)[0] == float((3 - Fraction(41, 25)) / 2)
