@@ -126,6 +126,49 @@ int ea_get_state(ea_handle *h, uint32_t *spin_words /* [n_temps][W][2][N/2] */,
                  uint8_t *temp_of_slot /* [R][n_temps] */, int32_t *energy_by_slot /* [R][n_temps] */,
                  uint64_t *sweeps_done, uint64_t *swap_rounds_done);
 
+/*
+ * ---- Measurement series (the observables of PAPER.md:317-339) ----
+ * The paper's spin-glass order parameter is the overlap q between two copies of one disorder
+ * realization (Binder ratio of the EA model, Fig. 20); it never prints the
+ * definitions, R16/R20 fix them.  All sums are exact integers accumulated on the
+ * device; no host round trip between measurements.
+ */
+
+/* J[r][d][site] = +-1, the inverse of ea_set_couplings. */
+int ea_get_couplings(ea_handle *h, int8_t *J /* [R][3][N] */);
+
+/* Two-copy set-up: realizations R/2 .. R-1 get the couplings of 0 .. R/2-1.  n_realizations must
+ * be a multiple of 64 so that the two copies of a realization sit in different words and hence
+ * see different random draws (R11); else EA_ERR_INVALID_ARG.  Spins are untouched
+ * (the halves were seeded differently); energies are recomputed. */
+int ea_pair_couplings(ea_handle *h);
+
+/* Start (or restart) a series: zero accumulators for n_word_pairs pairs of realization words.
+ * Pair p = (wa, wb) stands for the 32 realization pairs (32 wa + b, 32 wb + b), b = 0..31;
+ * wb = -1: all-up reference (q = magnetization).  Word index outside [0, W): EA_ERR_INVALID_ARG.
+ * Allocates device memory of its own (one more copy of the spin store), freed by ea_destroy
+ * or the next ea_measure_begin. */
+int ea_measure_begin(ea_handle *h, const int32_t *word_pairs /* [n_word_pairs][2] */, int n_word_pairs);
+
+/* n_meas times: ea_sweep(sweeps_between, swap_interval), then one measurement at equal
+ * temperature index t: q = sum_i s_i(ra, t) s_i(rb, t) for every realization pair of the series
+ * and E = ea_energy's value for every (r, t); adds 1, q, q^2, q^4, E, E^2 to the accumulators.
+ * Pairs that touch a padding bit (realization index >= R) accumulate nothing.  Asynchronous.
+ * EA_ERR_RANGE if the sweep counter would pass 2^32-1 or the number of measurements would pass
+ * 2^64 / (9 N^2) (64-bit sums of q^2 and E^2; the q^4 sums are 128-bit). */
+int ea_measure(ea_handle *h, int64_t n_meas, int64_t sweeps_between, int swap_interval);
+
+/* Copy the accumulators out (any pointer may be NULL).  q4[..][0] = low, [1] = high 64 bits. */
+int ea_get_moments(ea_handle *h, uint64_t *n_meas, int64_t *q1 /* [P][32][n_temps] */,
+                   uint64_t *q2 /* [P][32][n_temps] */, uint64_t *q4 /* [P][32][n_temps][2] */,
+                   int64_t *e1 /* [R][n_temps] */, uint64_t *e2 /* [R][n_temps] */);
+
+/* Binder ratio by temperature index, g[t] = (3 - [<q^4>] / [<q^2>]^2) / 2: <.> = average over the
+ * measurements of one realization pair, [.] = average over the series' valid realization pairs
+ * (disorder average).  Computed on the host from the integer sums in long double; agrees with
+ * the exact rational value to ~1e-18 relative.  NaN where no measurement was taken or [<q^2>] = 0. */
+int ea_get_binder(ea_handle *h, double *g /* [n_temps] */);
+
 /* Select the sweep implementation (EA_KERNEL_*); EA_ERR_UNSUPPORTED if it cannot run this shape. */
 int ea_set_kernel(ea_handle *h, int kernel);
 /* The implementation ea_sweep would use now (EA_KERNEL_GENERIC/RESIDENT/TILED/STREAM). */

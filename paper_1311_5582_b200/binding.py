@@ -17,6 +17,8 @@ _SYMBOLS = [
     "ea_set_spins", "ea_set_tables", "ea_get_tables", "ea_sweep", "ea_synchronize", "ea_energy",
     "ea_overlap", "ea_get_spins", "ea_get_state", "ea_set_kernel", "ea_get_kernel",
     "ea_launch_count", "ea_last_error", "ea_measure_int_peak",
+    "ea_get_couplings", "ea_pair_couplings", "ea_measure_begin", "ea_measure", "ea_get_moments",
+    "ea_get_binder",
 ]
 
 
@@ -57,7 +59,10 @@ def lib():
                        ("ea_sweep", [vp, i64, i32]), ("ea_synchronize", [vp]),
                        ("ea_energy", [vp, vp]), ("ea_overlap", [vp, vp, i32, vp]),
                        ("ea_get_spins", [vp, vp]), ("ea_get_state", [vp, vp, vp, vp, vp, vp]),
-                       ("ea_set_kernel", [vp, i32]), ("ea_get_kernel", [vp])):
+                       ("ea_set_kernel", [vp, i32]), ("ea_get_kernel", [vp]),
+                       ("ea_get_couplings", [vp, vp]), ("ea_pair_couplings", [vp]),
+                       ("ea_measure_begin", [vp, vp, i32]), ("ea_measure", [vp, i64, i64, i32]),
+                       ("ea_get_moments", [vp, vp, vp, vp, vp, vp, vp]), ("ea_get_binder", [vp, vp])):
         f = getattr(l, name)
         f.restype = i32
         f.argtypes = args
@@ -174,6 +179,39 @@ class EA:
         self._chk(self._l.ea_get_state(self.h, _p(words), _p(tau), _p(E), C.byref(g), C.byref(n)))
         return {"spin_words": words, "temp_of_slot": tau, "energy_by_slot": E,
                 "sweeps": g.value, "swap_rounds": n.value}
+
+    def get_couplings(self):
+        J = np.zeros((self.R, 3, self.N), dtype=np.int8)
+        self._chk(self._l.ea_get_couplings(self.h, _p(J)))
+        return J
+
+    def pair_couplings(self):
+        self._chk(self._l.ea_pair_couplings(self.h))
+
+    def measure_begin(self, word_pairs):
+        wp = np.ascontiguousarray(word_pairs, dtype=np.int32).reshape(-1, 2)
+        self._n_wp = len(wp)
+        self._chk(self._l.ea_measure_begin(self.h, _p(wp), len(wp)))
+
+    def measure(self, n_meas, sweeps_between, swap_interval):
+        self._chk(self._l.ea_measure(self.h, int(n_meas), int(sweeps_between), int(swap_interval)))
+
+    def get_moments(self):
+        """The integer accumulators as they are stored: q4 is [P][32][n_temps][2] = (low, high)."""
+        P = self._n_wp
+        n = C.c_uint64()
+        q1 = np.zeros((P, 32, self.nT), dtype=np.int64)
+        q2 = np.zeros((P, 32, self.nT), dtype=np.uint64)
+        q4 = np.zeros((P, 32, self.nT, 2), dtype=np.uint64)
+        e1 = np.zeros((self.R, self.nT), dtype=np.int64)
+        e2 = np.zeros((self.R, self.nT), dtype=np.uint64)
+        self._chk(self._l.ea_get_moments(self.h, C.byref(n), _p(q1), _p(q2), _p(q4), _p(e1), _p(e2)))
+        return {"n": n.value, "q1": q1, "q2": q2, "q4": q4, "e1": e1, "e2": e2}
+
+    def get_binder(self):
+        g = np.zeros(self.nT, dtype=np.float64)
+        self._chk(self._l.ea_get_binder(self.h, _p(g)))
+        return g
 
     def set_kernel(self, kernel):
         self._chk(self._l.ea_set_kernel(self.h, int(kernel)))

@@ -16,6 +16,7 @@
 #include "ea_tiled.cuh"
 #include "ea_stream.cuh"
 #include "ea_peak.cuh"
+#include "ea_measure.cuh"
 
 using ea::Params;
 
@@ -45,6 +46,13 @@ struct ea_handle {
     int kernel_sel = EA_KERNEL_AUTO;
     int64_t launches = 0;
     int sm_count = 0;
+    // measurement series (ea_measure_begin): own allocation, freed by ea_destroy / the next begin
+    char *d_meas = nullptr;
+    uint32_t *d_T = nullptr;           // spins gathered by temperature index, [t][w][i]
+    ea::Moments M{};
+    size_t meas_bytes = 0, meas_acc_off = 0;
+    uint64_t meas_n = 0;
+    bool meas_on = false;
     mutable std::string err;
 };
 
@@ -409,6 +417,7 @@ extern "C" void ea_destroy(ea_handle *h)
     if (!h) return;
     if (h->ws) cudaStreamSynchronize(h->stream);
     if (h->own_ws && h->ws) cudaFree(h->ws);
+    if (h->d_meas) cudaFree(h->d_meas);
     delete h;
 }
 
@@ -916,6 +925,167 @@ extern "C" int ea_get_state(ea_handle *h, uint32_t *spin_words, uint8_t *temp_of
     CUDA_TRY(h, cudaStreamSynchronize(h->stream));
     if (sweeps_done) *sweeps_done = h->g;
     if (swap_rounds_done) *swap_rounds_done = h->nswap;
+    return EA_OK;
+}
+
+// ---------------------------------------------------------------- measurement series
+extern "C" int ea_get_couplings(ea_handle *h, int8_t *J)
+{
+    if (!h || !J) return fail(h, EA_ERR_INVALID_ARG, "ea_get_couplings: null argument");
+    const size_t n = (size_t)h->R * 3 * h->N;
+    int8_t *d = nullptr;
+    CUDA_TRY(h, cudaMalloc((void **)&d, n));
+    int grid;
+    launch_cfg((int64_t)n, 256, grid);
+    ea::k_unpack_couplings<<<grid, 256, 0, h->stream>>>(h->P, h->R, d);
+    h->launches++;
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess) e = cudaMemcpyAsync(J, d, n, cudaMemcpyDeviceToHost, h->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+    cudaFree(d);
+    if (e != cudaSuccess) return fail(h, EA_ERR_CUDA, std::string("ea_get_couplings: ") + cudaGetErrorString(e));
+    return EA_OK;
+}
+
+extern "C" int ea_pair_couplings(ea_handle *h)
+{
+    if (!h) return EA_ERR_INVALID_ARG;
+    if (h->R % 64) return fail(h, EA_ERR_INVALID_ARG, "ea_pair_couplings: n_realizations must be a multiple of 64");
+    const size_t half = (size_t)(h->W / 2) * 3 * h->N;   // coup is [w][d][p][j]: each half is contiguous
+    CUDA_TRY(h, cudaMemcpyAsync(h->P.coup + half, h->P.coup, 4 * half, cudaMemcpyDeviceToDevice, h->stream));
+    return recompute_energy(h);
+}
+
+extern "C" int ea_measure_begin(ea_handle *h, const int32_t *word_pairs, int n_word_pairs)
+{
+    if (!h || n_word_pairs < 0 || (n_word_pairs && !word_pairs))
+        return fail(h, EA_ERR_INVALID_ARG, "ea_measure_begin: bad argument");
+    for (int p = 0; p < n_word_pairs; ++p)
+        if (word_pairs[2 * p] < 0 || word_pairs[2 * p] >= h->W || word_pairs[2 * p + 1] < -1 ||
+            word_pairs[2 * p + 1] >= h->W)
+            return fail(h, EA_ERR_INVALID_ARG, "ea_measure_begin: word index out of range");
+    const size_t nq = (size_t)n_word_pairs * 32 * h->nT, ne = (size_t)h->R * h->nT;
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t a = off; off = align256(off + bytes); return a; };
+    const size_t o_T = take(4 * (size_t)h->nT * h->W * h->N);
+    const size_t o_pairs = take(8 * (size_t)(n_word_pairs ? n_word_pairs : 1));
+    const size_t o_q1 = take(8 * nq), o_q2 = take(8 * nq), o_q4 = take(16 * nq);
+    const size_t o_e1 = take(8 * ne), o_e2 = take(8 * ne);
+    char *d = nullptr;
+    if (cudaMalloc((void **)&d, off) != cudaSuccess) {
+        cudaGetLastError();
+        return fail(h, EA_ERR_ALLOC, "ea_measure_begin: cudaMalloc failed");
+    }
+    cudaError_t e = cudaMemsetAsync(d + o_q1, 0, off - o_q1, h->stream);
+    if (e == cudaSuccess && n_word_pairs)
+        e = cudaMemcpyAsync(d + o_pairs, word_pairs, 8 * (size_t)n_word_pairs, cudaMemcpyHostToDevice, h->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);   // word_pairs is the caller's: copy done before returning
+    if (e != cudaSuccess) {
+        cudaFree(d);
+        return fail(h, EA_ERR_CUDA, std::string("ea_measure_begin: ") + cudaGetErrorString(e));
+    }
+    if (h->d_meas) cudaFree(h->d_meas);
+    h->d_meas = d;
+    h->meas_bytes = off;
+    h->meas_acc_off = o_q1;
+    h->d_T = (uint32_t *)(d + o_T);
+    h->M.wpairs = (const int32_t *)(d + o_pairs);
+    h->M.P = n_word_pairs;
+    h->M.R = h->R;
+    h->M.q1 = (int64_t *)(d + o_q1);
+    h->M.q2 = (uint64_t *)(d + o_q2);
+    h->M.q4 = (uint64_t *)(d + o_q4);
+    h->M.e1 = (int64_t *)(d + o_e1);
+    h->M.e2 = (uint64_t *)(d + o_e2);
+    h->meas_n = 0;
+    h->meas_on = true;
+    return EA_OK;
+}
+
+// one measurement of the current state, enqueued on the handle's stream
+static int measure_once(ea_handle *h)
+{
+    if (!h->energy_valid) { int rc = recompute_energy(h); if (rc != EA_OK) return rc; }
+    if (h->M.P > 0) {
+        const int nchunk = (h->N / 4 + ea::kGatherThreads - 1) / ea::kGatherThreads;
+        ea::k_gather_by_temp<<<h->W * nchunk, ea::kGatherThreads, 4 * (size_t)h->nT * h->nT, h->stream>>>(h->P, h->d_T);
+        ea::k_overlap_words<<<h->M.P * h->nT, 128, 0, h->stream>>>(h->P, h->d_T, h->M, nullptr);
+        h->launches += 2;
+    }
+    int grid;
+    launch_cfg((int64_t)h->R * h->nT, 128, grid);
+    ea::k_accum_energy<<<grid, 128, 0, h->stream>>>(h->P, h->M);
+    h->launches++;
+    CUDA_TRY(h, cudaGetLastError());
+    h->meas_n++;
+    return EA_OK;
+}
+
+extern "C" int ea_measure(ea_handle *h, int64_t n_meas, int64_t sweeps_between, int swap_interval)
+{
+    if (!h || n_meas < 0 || sweeps_between < 0 || swap_interval < 0)
+        return fail(h, EA_ERR_INVALID_ARG, "ea_measure: bad argument");
+    if (!h->meas_on) return fail(h, EA_ERR_INVALID_ARG, "ea_measure: call ea_measure_begin first");
+    const long double total = (long double)n_meas * (long double)sweeps_between;
+    if ((long double)h->g + total > 4294967295.0L)
+        return fail(h, EA_ERR_RANGE, "ea_measure: sweep counter would pass 2^32-1");
+    // sum E^2 <= n 9 N^2 and sum q^2 <= n N^2 must fit 64 bits
+    const long double cap = 18446744073709551615.0L / (9.0L * (long double)h->N * (long double)h->N);
+    if ((long double)h->meas_n + (long double)n_meas > cap)
+        return fail(h, EA_ERR_RANGE, "ea_measure: too many measurements for the 64-bit accumulators");
+    for (int64_t m = 0; m < n_meas; ++m) {
+        if (sweeps_between > 0) { int rc = ea_sweep(h, sweeps_between, swap_interval); if (rc != EA_OK) return rc; }
+        int rc = measure_once(h);
+        if (rc != EA_OK) return rc;
+    }
+    return EA_OK;
+}
+
+extern "C" int ea_get_moments(ea_handle *h, uint64_t *n_meas, int64_t *q1, uint64_t *q2, uint64_t *q4,
+                              int64_t *e1, uint64_t *e2)
+{
+    if (!h) return EA_ERR_INVALID_ARG;
+    if (!h->meas_on) return fail(h, EA_ERR_INVALID_ARG, "ea_get_moments: call ea_measure_begin first");
+    const size_t nq = (size_t)h->M.P * 32 * h->nT, ne = (size_t)h->R * h->nT;
+    if (q1 && nq) CUDA_TRY(h, cudaMemcpyAsync(q1, h->M.q1, 8 * nq, cudaMemcpyDeviceToHost, h->stream));
+    if (q2 && nq) CUDA_TRY(h, cudaMemcpyAsync(q2, h->M.q2, 8 * nq, cudaMemcpyDeviceToHost, h->stream));
+    if (q4 && nq) CUDA_TRY(h, cudaMemcpyAsync(q4, h->M.q4, 16 * nq, cudaMemcpyDeviceToHost, h->stream));
+    if (e1) CUDA_TRY(h, cudaMemcpyAsync(e1, h->M.e1, 8 * ne, cudaMemcpyDeviceToHost, h->stream));
+    if (e2) CUDA_TRY(h, cudaMemcpyAsync(e2, h->M.e2, 8 * ne, cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    if (n_meas) *n_meas = h->meas_n;
+    return EA_OK;
+}
+
+extern "C" int ea_get_binder(ea_handle *h, double *g)
+{
+    if (!h || !g) return fail(h, EA_ERR_INVALID_ARG, "ea_get_binder: null argument");
+    if (!h->meas_on) return fail(h, EA_ERR_INVALID_ARG, "ea_get_binder: call ea_measure_begin first");
+    const size_t nq = (size_t)h->M.P * 32 * h->nT;
+    std::vector<uint64_t> q2(nq), q4(2 * nq);
+    std::vector<int32_t> wp(2 * (size_t)h->M.P);
+    if (nq) {
+        CUDA_TRY(h, cudaMemcpyAsync(q2.data(), h->M.q2, 8 * nq, cudaMemcpyDeviceToHost, h->stream));
+        CUDA_TRY(h, cudaMemcpyAsync(q4.data(), h->M.q4, 16 * nq, cudaMemcpyDeviceToHost, h->stream));
+        CUDA_TRY(h, cudaMemcpyAsync(wp.data(), h->M.wpairs, 8 * (size_t)h->M.P, cudaMemcpyDeviceToHost, h->stream));
+    }
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    // g = (3 - [<q^4>] / [<q^2>]^2) / 2 = (3 - S4 n M / S2^2) / 2 with S = sums over measurements and
+    // valid pairs, n measurements, M valid pairs; 64-bit-mantissa long double throughout.
+    long double M = 0.0L;
+    for (int p = 0; p < h->M.P; ++p)
+        for (int b = 0; b < 32; ++b)
+            if (32 * wp[2 * p] + b < h->R && (wp[2 * p + 1] < 0 || 32 * wp[2 * p + 1] + b < h->R)) M += 1.0L;
+    for (int t = 0; t < h->nT; ++t) {
+        long double s2 = 0.0L, s4 = 0.0L;
+        for (size_t pb = 0; pb < (size_t)h->M.P * 32; ++pb) {   // invalid entries hold zeros
+            const size_t o = pb * h->nT + t;
+            s2 += (long double)q2[o];
+            s4 += (long double)q4[2 * o] + 18446744073709551616.0L * (long double)q4[2 * o + 1];
+        }
+        g[t] = (h->meas_n == 0 || s2 == 0.0L) ? std::nan("")
+                                              : (double)(0.5L * (3.0L - s4 * (long double)h->meas_n * M / (s2 * s2)));
+    }
     return EA_OK;
 }
 

@@ -1,0 +1,153 @@
+// ea_measure.cuh -- on-device measurements: overlaps of whole
+// realization words at equal temperature index, exact integer moments of the overlap and of
+// the energy (the inputs of the Binder ratio, Fig. 20), coupling export.
+// Product code: shares nothing with oracle/.
+#pragma once
+#include "ea_device.cuh"
+
+namespace ea {
+
+// Accumulators of one measurement series.  Pair p = (wa, wb) of realization words stands for
+// the 32 realization pairs (32 wa + b, 32 wb + b); wb = -1: all-up reference.
+struct Moments {
+    const int32_t *wpairs;   // [P][2]
+    int P, R;
+    int64_t *q1;             // [P][32][nT]  sum q
+    uint64_t *q2;            // [P][32][nT]  sum q^2
+    uint64_t *q4;            // [P][32][nT][2]  sum q^4, 128 bit: (low, high)
+    int64_t *e1;             // [R][nT]  sum E by temperature index
+    uint64_t *e2;            // [R][nT]  sum E^2
+};
+
+// ------------------------------------------------------------------ gather by temperature
+// T[t][w][i] = word whose bit b is the spin of realization 32w+b at the slot that currently
+// holds temperature index t (i = storage index p Nh + j, the same for every slot):
+//   T[t] = OR_k (spin[k] & M[k][t]),  M[k][t] = bits b with tau[32w+b][k] = t.
+// After this pass the 32 overlaps of a word pair are one XNOR + positional popcount per site,
+// although every bit of a word sits at its own temperature (R14).
+// Block = (word w, 1024 consecutive storage words); a thread owns one 128-bit vector and
+// produces the temperatures eight at a time (32 accumulator registers).
+constexpr int kGatherThreads = 256;
+
+__global__ void __launch_bounds__(kGatherThreads) k_gather_by_temp(Params P, uint32_t *T)
+{
+    extern __shared__ uint32_t sm_M[];   // [k][t]
+    const int nchunk = (P.N / 4 + kGatherThreads - 1) / kGatherThreads;
+    const int w = blockIdx.x / nchunk, chunk = blockIdx.x % nchunk;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int k = warp; k < P.nT; k += kGatherThreads / 32) {
+        const int t_mine = P.tau[(size_t)(32 * w + lane) * P.nT + k];
+        for (int t = 0; t < P.nT; ++t) {
+            const uint32_t m = __ballot_sync(0xFFFFFFFFu, t_mine == t);
+            if (lane == (t & 31)) sm_M[k * P.nT + t] = m;
+        }
+    }
+    __syncthreads();
+    const int v = chunk * kGatherThreads + threadIdx.x;   // vector index inside the lattice
+    if (v >= P.N / 4) return;
+    const uint4 *src = reinterpret_cast<const uint4 *>(P.spin) + (size_t)w * (P.N / 4) + v;
+    uint4 *dst = reinterpret_cast<uint4 *>(T) + (size_t)w * (P.N / 4) + v;
+    const size_t slot_stride = (size_t)P.W * (P.N / 4);
+    for (int t0 = 0; t0 < P.nT; t0 += 8) {
+        uint4 acc[8];
+#pragma unroll
+        for (int a = 0; a < 8; ++a) acc[a] = make_uint4(0u, 0u, 0u, 0u);
+        for (int k = 0; k < P.nT; ++k) {
+            const uint4 s = src[(size_t)k * slot_stride];
+#pragma unroll
+            for (int a = 0; a < 8; ++a) {
+                if (t0 + a >= P.nT) break;
+                const uint32_t m = sm_M[k * P.nT + t0 + a];
+                acc[a].x |= s.x & m; acc[a].y |= s.y & m; acc[a].z |= s.z & m; acc[a].w |= s.w & m;
+            }
+        }
+#pragma unroll
+        for (int a = 0; a < 8; ++a)
+            if (t0 + a < P.nT) dst[(size_t)(t0 + a) * slot_stride] = acc[a];
+    }
+}
+
+// ------------------------------------------------------------------ word overlaps + moments
+// Block = (pair p, temperature index t).  agree = ~(Ta ^ Tb) per site (Tb = all ones for the
+// reference), counted per bit lane in vertical (bit-sliced) counters, transposed to 32 integers
+// like k_energy; q = 2 agree - N.  Lane b then adds q, q^2, q^4 to the accumulators of
+// realization pair (32 wa + b, 32 wb + b): this block is their only writer, so no atomics and a
+// fixed summation order.  Padding bits (index >= R) accumulate nothing.  Q (optional): the
+// overlaps of this measurement, [P][32][nT].
+constexpr int kOverlapPlanes = 15;   // per-thread count <= ceil(N / 128) <= 2^14 for L <= 128
+
+__global__ void __launch_bounds__(128) k_overlap_words(Params P, const uint32_t *T, Moments M, int32_t *Q)
+{
+    __shared__ int sm_cnt[32];
+    const int p = blockIdx.x / P.nT, t = blockIdx.x % P.nT;
+    const int wa = M.wpairs[2 * p], wb = M.wpairs[2 * p + 1];
+    const uint32_t *Ta = T + ((size_t)t * P.W + wa) * P.N;
+    const uint32_t *Tb = wb >= 0 ? T + ((size_t)t * P.W + wb) * P.N : nullptr;
+    if (threadIdx.x < 32) sm_cnt[threadIdx.x] = 0;
+    __syncthreads();
+    uint32_t c[kOverlapPlanes];
+#pragma unroll
+    for (int i = 0; i < kOverlapPlanes; ++i) c[i] = 0;
+    for (int i = threadIdx.x; i < P.N; i += blockDim.x) {
+        uint32_t x = Tb ? ~(Ta[i] ^ Tb[i]) : Ta[i];
+#pragma unroll
+        for (int l = 0; l < kOverlapPlanes; ++l) {
+            const uint32_t carry = c[l] & x;
+            c[l] ^= x;
+            x = carry;
+        }
+    }
+    const int lane = threadIdx.x & 31;
+    int mine = 0;
+    for (int b = 0; b < 32; ++b) {
+        int v = 0;
+#pragma unroll
+        for (int l = 0; l < kOverlapPlanes; ++l) v += (int)((c[l] >> b) & 1u) << l;
+        v = __reduce_add_sync(0xFFFFFFFFu, v);
+        if (lane == b) mine = v;
+    }
+    atomicAdd(&sm_cnt[lane], mine);
+    __syncthreads();
+    if (threadIdx.x >= 32) return;
+    const int ra = 32 * wa + lane, rb = wb >= 0 ? 32 * wb + lane : -1;
+    const bool valid = ra < M.R && rb < M.R;
+    const int64_t q = valid ? 2 * (int64_t)sm_cnt[lane] - P.N : 0;
+    const size_t o = ((size_t)p * 32 + lane) * P.nT + t;
+    if (Q) Q[o] = (int32_t)q;
+    if (!valid) return;
+    const uint64_t s = (uint64_t)(q * q);
+    const uint64_t lo = s * s, hi = __umul64hi(s, s);
+    M.q1[o] += q;
+    M.q2[o] += s;
+    const uint64_t old = M.q4[2 * o];
+    M.q4[2 * o] = old + lo;
+    M.q4[2 * o + 1] += hi + (old + lo < old ? 1u : 0u);
+}
+
+// sum E and sum E^2 by temperature index; one thread per (r, t).
+__global__ void k_accum_energy(Params P, Moments M)
+{
+    const int tid = blockIdx.x * blockDim.x + threadIdx.x;
+    if (tid >= M.R * P.nT) return;
+    const int r = tid / P.nT, t = tid % P.nT;
+    const int64_t e = P.E[(size_t)r * P.nT + P.sigma[(size_t)r * P.nT + t]];
+    M.e1[tid] += e;
+    M.e2[tid] += (uint64_t)(e * e);
+}
+
+// ------------------------------------------------------------------ coupling export
+// out[r][d][i] = +-1, canonical site order (the inverse of k_pack mode 1).
+__global__ void k_unpack_couplings(Params P, int R, int8_t *out)
+{
+    const int64_t tid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (tid >= (int64_t)R * 3 * P.N) return;
+    const int i = (int)(tid % P.N);
+    const int d = (int)((tid / P.N) % 3);
+    const int r = (int)(tid / ((int64_t)P.N * 3));
+    const int x = i % P.L, y = (i / P.L) % P.L, z = i / (P.L * P.L);
+    const int p = (x + y + z) & 1, j = (x >> 1) + P.Lh * (y + P.L * z);
+    const uint32_t wv = P.coup[((size_t)(r >> 5) * 3 + d) * P.N + p * P.Nh + j];
+    out[tid] = ((wv >> (r & 31)) & 1u) ? 1 : -1;
+}
+
+}  // namespace ea

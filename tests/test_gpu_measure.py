@@ -1,0 +1,123 @@
+"""GPU parity of the measurement series: coupling export, two-copy
+set-up, integer moments of overlap and energy, Binder ratio -- CUDA path through the C ABI
+against the CPU oracle on the same seeded inputs.  Integers bit-exact; the Binder ratio (the
+one double-valued observable) within 1e-12 relative (north_star)."""
+import numpy as np
+import pytest
+
+from ea_inputs import random_couplings, temperature_ladder
+
+pytestmark = pytest.mark.gpu
+
+
+def _mods():
+    import __graft_entry__ as ge
+    ge.build()
+    import paper_1311_5582_b200 as pkg
+    from oracle import Oracle, binder_ratio
+    return pkg, Oracle, binder_ratio
+
+
+def _moments_as_ints(m):
+    """binding layout -> Python-int arrays like the oracle's."""
+    q4 = m["q4"][..., 0].astype(object) + m["q4"][..., 1].astype(object) * (1 << 64)
+    return {"n": m["n"], "q1": m["q1"].astype(object), "q2": m["q2"].astype(object), "q4": q4,
+            "e1": m["e1"].astype(object), "e2": m["e2"].astype(object)}
+
+
+def _compare(g, acc, binder_ratio):
+    m = _moments_as_ints(g.get_moments())
+    assert m["n"] == acc["n"]
+    for k in ("q1", "q2", "q4", "e1", "e2"):
+        assert (m[k] == acc[k]).all(), k
+    gb, ob = g.get_binder(), binder_ratio(acc)
+    assert (np.isnan(gb) == np.isnan(ob)).all()
+    ok = ~np.isnan(ob)
+    assert (np.abs(gb[ok] - ob[ok]) <= 1e-12 * np.abs(ob[ok])).all(), (gb, ob)
+
+
+@pytest.mark.parametrize("L,nT,R,kernel,wp,n_meas,between,swap", [
+    (4, 5, 70, 1, [[0, 1], [1, 2], [2, -1], [0, 0]], 5, 3, 2),      # generic, ragged R, odd n_T
+    (8, 8, 128, 2, [[0, 2], [1, 3], [3, -1]], 6, 4, 1),              # resident
+    (16, 6, 64, 2, [[0, 1]], 3, 2, 1),                               # resident, L = 16
+    (16, 4, 64, 3, [[0, 1], [1, -1]], 2, 2, 1),                      # tiled
+    (32, 4, 64, 4, [[0, 1]], 2, 1, 1),                               # stream
+    (6, 3, 40, 0, [[0, 1], [1, 0]], 4, 1, 0),                        # no PT, L = 6
+])
+def test_moments_and_binder_match_oracle(L, nT, R, kernel, wp, n_meas, between, swap):
+    pkg, Oracle, binder_ratio = _mods()
+    betas = 1.0 / temperature_ladder(nT, 0.8, 2.0)
+    g = pkg.EA(L, nT, R, betas, 31, kernel=kernel)
+    o = Oracle(L, nT, R, betas, 31)
+    if R % 64 == 0:
+        g.pair_couplings()
+        o.pair_couplings()
+        assert (g.get_couplings() == o.couplings()).all()
+        assert (g.energy() == o.energy()).all()
+    g.measure_begin(wp)
+    g.measure(n_meas, between, swap)
+    acc = o.measure(n_meas, between, swap, wp)
+    _compare(g, acc, binder_ratio)
+    # continue the same series, with a different cadence
+    g.measure(2, 1, swap)
+    acc = o.measure(2, 1, swap, wp, acc)
+    _compare(g, acc, binder_ratio)
+    # state after a measurement series is the plain trajectory
+    assert (g.energy() == o.energy()).all()
+    assert (g.get_state()["temp_of_slot"] == o.perm()[0]).all()
+    # a new series starts from zero
+    g.measure_begin(wp[:1])
+    m = g.get_moments()
+    assert m["n"] == 0 and not m["q2"].any() and not m["e2"].any()
+    assert np.isnan(g.get_binder()).all()
+    g.destroy()
+
+
+def test_get_couplings_round_trip_and_seeded_values():
+    pkg, Oracle, _ = _mods()
+    L, nT, R = 6, 2, 45
+    betas = np.array([1.0, 0.5])
+    g = pkg.EA(L, nT, R, betas, 9)
+    o = Oracle(L, nT, R, betas, 9)
+    assert (g.get_couplings() == o.couplings()).all()        # seeded couplings
+    J = random_couplings(R, L ** 3, seed=77)
+    g.set_couplings(J)
+    assert (g.get_couplings() == J).all()
+    g.destroy()
+
+
+def test_measure_zero_sweeps_between_repeats_the_same_sample():
+    pkg, Oracle, binder_ratio = _mods()
+    L, nT, R = 4, 3, 64
+    betas = np.array([1.5, 1.0, 0.5])
+    g = pkg.EA(L, nT, R, betas, 2)
+    o = Oracle(L, nT, R, betas, 2)
+    g.measure_begin([[0, 1]])
+    g.measure(3, 0, 1)
+    acc = o.measure(3, 0, 1, [[0, 1]])
+    _compare(g, acc, binder_ratio)
+    Q = g.overlap([[b, 32 + b] for b in range(32)])          # per-pair kernel against the word kernel
+    m = g.get_moments()
+    assert (m["q1"][0] == 3 * Q.astype(np.int64)).all()
+    g.destroy()
+
+
+def test_measure_errors_leave_state_unchanged():
+    pkg, _, _ = _mods()
+    g = pkg.EA(4, 2, 32, np.array([1.0, 0.5]), 1)
+    with pytest.raises(pkg.EAError) as e:
+        g.measure(1, 1, 1)                                   # no series yet
+    assert e.value.code == -1
+    with pytest.raises(pkg.EAError):
+        g.measure_begin([[0, 1]])                            # W = 1: word 1 does not exist
+    with pytest.raises(pkg.EAError):
+        g.measure_begin([[-1, 0]])
+    with pytest.raises(pkg.EAError):
+        g.pair_couplings()                                   # R = 32 is not a multiple of 64
+    g.measure_begin([[0, -1]])
+    with pytest.raises(pkg.EAError) as e:
+        g.measure(2, 2 ** 31, 1)                             # sweep counter would overflow
+    assert e.value.code == -4
+    st = g.get_state()
+    assert st["sweeps"] == 0 and g.get_moments()["n"] == 0
+    g.destroy()
