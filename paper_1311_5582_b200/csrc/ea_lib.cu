@@ -723,11 +723,11 @@ StreamPlan plan_stream_t(const ea_handle *h)
     const long long per_w = (long long)Sg::NSLAB * h->nT;
     pl.MW = (int)((pl.MS + per_w - 2) / per_w) + 1;
     const size_t nT = (size_t)h->nT, LTS = nT + 1, MTS = 3 * nT + 2;
-    size_t base = 64 + 16 * (size_t)h->n_bucket + (size_t)Sg::NS * Sg::NB * Sg::BUF_BYTES + 16 * (size_t)pl.MS * MTS +
-                  4 * ((size_t)pl.MS * LTS + 3 * LTS + MTS + 2 * Sg::NB * 32) + 2 * (size_t)pl.MW * 32 * nT;
+    size_t base = Sg::MBAR_BYTES + 16 * (size_t)h->n_bucket + (size_t)Sg::NST * Sg::BUF_BYTES + 16 * (size_t)pl.MS * MTS +
+                  4 * ((size_t)pl.MS * LTS + 3 * LTS + MTS + (size_t)pl.MS * 32) + 2 * (size_t)pl.MW * 32 * nT;
     pl.esm_off = (base + 15) & ~(size_t)15;
     pl.batch_off = pl.esm_off + 4 * (size_t)pl.MW * 32 * nT;
-    base = pl.batch_off + 16 * (size_t)pl.MS + 8 * nT;
+    base = pl.batch_off + 16 * (size_t)pl.MS + 12 * nT;
     const size_t cap = 227 * 1024;
     if (base > cap) return pl;
     pl.swap_win = (int)std::min<size_t>(128, (cap - base) / (4 * nT));

@@ -67,8 +67,10 @@ struct StreamGeom {
     static constexpr int OWN_BYTES = NTHR * 16;
     static constexpr int OTH_BYTES = (ZS + 2) * QPP * 16;
     static constexpr int BUF_BYTES = OWN_BYTES + OTH_BYTES;
-    static constexpr int NB = BUF_BYTES <= 20480 ? 4 : 2;  // slots per batch
-    static constexpr int NS = 2;                           // ring stages
+    static constexpr int NB = BUF_BYTES <= 20480 ? 4 : 2;  // slots per batch (same word and slab)
+    static constexpr int NST = 2 * NB;                     // ring stages of ONE slot each
+    static constexpr int MBAR_BYTES = 192;                 // full[NST], empty[NST], batch count
+    static_assert(NST <= 10 && 16 * NST + 8 <= MBAR_BYTES, "stage bookkeeping");
 };
 
 // ------------------------------------------------------------------ mbarrier / TMA bulk copy
@@ -80,6 +82,10 @@ __device__ __forceinline__ void mbar_init(uint64_t *bar, int count)
 __device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
 {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
 __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
 {
@@ -115,100 +121,100 @@ struct StreamCtx {
     int nT, LTS, MTS;
     int tid, lane, qx, y, zl;
     uint32_t ov, oyp, oym, ozp, ozm;   // byte offsets inside the other-parity buffer
-    uint64_t *full;              // [NS]: tiles landed
+    uint64_t *full;              // [NST]: the stage's tile has landed (TMA transaction count)
+    uint64_t *empty;             // [NST]: all warps have finished reading the stage
     const StreamBatch *batch;
     unsigned char *bufs;
     uint4 *mt;
     uint32_t *lt;
-    int32_t *Eacc;               // [2][NB][32]
+    int32_t *Eacc;               // [items][32] satisfied-bond counts of the running half-sweep
     RankCtx R;
 };
 
-// TMA bulk loads of batch b into ring stage st, issued by the lanes of one warp in
-// parallel (lane = 3 * slot + piece): per slot the slab's own-parity words (contiguous) and the
-// other parity's planes z0-1 .. z0+ZS (periodic wrap = 2 pieces).
+// The ring: NST stages of one slot each.  The block's items of a half-sweep are numbered
+// li = 0 .. i1-i0-1 in processing order; item li uses stage li % NST.  full[st] counts the TMA
+// bytes of a fill, empty[st] the 16 warps that have finished reading it: the only block-wide
+// barriers left are those of the grid barrier between half-sweeps, and a warp may run up to
+// NST - 1 slots ahead of the slowest one.
+//
+// TMA bulk loads of item li into stage st, issued by three lanes of one warp (lane = piece):
+// the slab's own-parity words (contiguous) and the other parity's planes z0-1 .. z0+ZS
+// (periodic wrap = 2 pieces).  `sub` = lane index inside the slot's group of three.
 template <int L>
-__device__ __forceinline__ void stream_issue(const StreamArgs &A, const StreamCtx<L> &C, int p, int b, int st)
+__device__ __forceinline__ void stream_issue_item(const StreamArgs &A, const StreamCtx<L> &C, int p, int li, int piece)
 {
     using Gm = ResGeom<L>;
     using Sg = StreamGeom<L>;
-    constexpr int N = Gm::N, Nh = Gm::Nh, QPP = Sg::QPP, ZS = Sg::ZS, NT = Sg::NTHR, NB = Sg::NB;
+    constexpr int N = Gm::N, Nh = Gm::Nh, QPP = Sg::QPP, ZS = Sg::ZS, NT = Sg::NTHR, NSLAB = Sg::NSLAB;
     constexpr uint32_t PLB = QPP * 16;       // bytes per plane and parity
     const Params &P = A.P;
-    const StreamBatch B = C.batch[b];
-    const int k0 = B.pos % C.nT, z0 = B.slab * ZS;
-    if (C.lane == 0) mbar_expect_tx(&C.full[st], (uint32_t)(B.cnt * Sg::BUF_BYTES));
-    __syncwarp();
-    const int i = C.lane / 3, piece = C.lane % 3;
-    if (i < B.cnt) {
-        const uint32_t *base = P.spin + ((size_t)(k0 + i) * P.W + B.w) * N;
-        unsigned char *dst = C.bufs + (size_t)(st * NB + i) * Sg::BUF_BYTES;
-        const uint32_t *ob = base + (1 - p) * Nh;
-        unsigned char *od = dst + Sg::OWN_BYTES;
-        const void *src;
-        uint32_t bytes;
-        if (piece == 0) {
-            src = base + p * Nh + (size_t)B.slab * NT * 4; bytes = Sg::OWN_BYTES;
-        } else if (z0 == 0) {
-            if (piece == 1) { dst = od; src = ob + (size_t)(L - 1) * QPP * 4; bytes = PLB; }
-            else { dst = od + PLB; src = ob; bytes = (ZS + 1) * PLB; }
-        } else if (z0 + ZS == L) {
-            if (piece == 1) { dst = od; src = ob + (size_t)(z0 - 1) * QPP * 4; bytes = (ZS + 1) * PLB; }
-            else { dst = od + (ZS + 1) * PLB; src = ob; bytes = PLB; }
-        } else {
-            dst = od; src = ob + (size_t)(z0 - 1) * QPP * 4; bytes = piece == 1 ? (ZS + 2) * PLB : 0u;
-        }
-        if (bytes) bulk_g2s(dst, src, bytes, &C.full[st]);
+    const int item = C.i0 + li, k = item % C.nT, grp = item / C.nT, w = grp / NSLAB, slab = grp % NSLAB;
+    const int st = li % Sg::NST, z0 = slab * ZS;
+    if (piece == 0) mbar_expect_tx(&C.full[st], (uint32_t)Sg::BUF_BYTES);
+    const uint32_t *base = P.spin + ((size_t)k * P.W + w) * N;
+    unsigned char *dst = C.bufs + (size_t)st * Sg::BUF_BYTES;
+    const uint32_t *ob = base + (1 - p) * Nh;
+    unsigned char *od = dst + Sg::OWN_BYTES;
+    const void *src;
+    uint32_t bytes;
+    if (piece == 0) {
+        src = base + p * Nh + (size_t)slab * NT * 4; bytes = Sg::OWN_BYTES;
+    } else if (z0 == 0) {
+        if (piece == 1) { dst = od; src = ob + (size_t)(L - 1) * QPP * 4; bytes = PLB; }
+        else { dst = od + PLB; src = ob; bytes = (ZS + 1) * PLB; }
+    } else if (z0 + ZS == L) {
+        if (piece == 1) { dst = od; src = ob + (size_t)(z0 - 1) * QPP * 4; bytes = (ZS + 1) * PLB; }
+        else { dst = od + (ZS + 1) * PLB; src = ob; bytes = PLB; }
+    } else {
+        dst = od; src = ob + (size_t)(z0 - 1) * QPP * 4; bytes = piece == 1 ? (ZS + 2) * PLB : 0u;
     }
+    if (bytes) bulk_g2s(dst, src, bytes, &C.full[st]);
 }
 
-// Start of a half-sweep: the first NS batches, one per warp.  The proxy fence orders the previous
-// phase's global stores (made visible by the grid barrier) before the asynchronous-proxy reads.
+// Start of a half-sweep (every stage is free: the grid barrier has just been passed): the first
+// NST items, issued by the lanes of the block's HIGHEST warp in parallel (lane = 3 * item + piece).
+// The proxy fence orders the previous phase's global stores (made visible by the grid barrier)
+// before the asynchronous-proxy reads.  efill: bit st = parity of the number of fills of stage st.
 template <int L>
-__device__ __forceinline__ void stream_prime(const StreamArgs &A, const StreamCtx<L> &C, int p)
-{
-    const int b = StreamGeom<L>::NTHR / 32 - 1 - (C.tid >> 5);   // the highest warps issue (scheduler priority)
-    if (b >= StreamGeom<L>::NS || b >= C.nb) return;
-    fence_proxy_async();
-    stream_issue<L>(A, C, p, b, b);
-}
-
-// End of a batch: block barrier (the stage is free, the batch's shared counters are complete),
-// then the HIGHEST warp refills the stage with batch b + NS and the next-highest one flushes the
-// satisfied-bond counters (ENERGY) to the global counters.  The warp scheduler serves high warp
-// ids first, so these two catch up with the others at once; a low warp in that role would run
-// alone afterwards and stretch every batch.
-template <int L, bool ENERGY>
-__device__ __forceinline__ void stream_batch_done(const StreamArgs &A, const StreamCtx<L> &C, int p, int b, int ebuf)
+__device__ __forceinline__ void stream_prime(const StreamArgs &A, const StreamCtx<L> &C, int p, uint32_t &efill)
 {
     using Sg = StreamGeom<L>;
-    constexpr int NB = Sg::NB, NS = Sg::NS, NW = Sg::NTHR / 32;
-    const Params &P = A.P;
-    const int warp = C.tid >> 5;
-    __syncthreads();
-    if (warp == NW - 1 && b + NS < C.nb) stream_issue<L>(A, C, p, b + NS, b % NS);
-    if (ENERGY && warp == NW - 2) {
-        const StreamBatch B = C.batch[b];
-        const int k0 = B.pos % C.nT;
-        int32_t *acc = C.Eacc + (b & 1) * NB * 32;
-        for (int a = C.lane; a < B.cnt * 32; a += 32) {
-            const int v = acc[a];
-            acc[a] = 0;
-            atomicAdd(A.Ecnt + (size_t)ebuf * P.Rp * C.nT + (size_t)(32 * B.w + (a & 31)) * C.nT + k0 + (a >> 5), v);
-        }
-    }
+    if ((C.tid >> 5) != Sg::NTHR / 32 - 1) return;
+    const int n = min(Sg::NST, C.i1 - C.i0);
+    fence_proxy_async();
+    if (C.lane < 3 * n) stream_issue_item<L>(A, C, p, C.lane / 3, C.lane % 3);
+    efill ^= (1u << n) - 1u;
 }
 
-// One half-sweep (parity p) over the block's batches; the first NS are in flight (stream_prime).
-// ENERGY: also count the satisfied bonds of the updated (parity-1) sites.
+// A warp has finished reading item li: release its stage; the block's highest warp (first in the
+// scheduler's order, so it runs ahead) then refills the stage of item li - 1, which the slowest
+// warp has normally left by now, with item li - 1 + NST.
+template <int L>
+__device__ __forceinline__ void stream_release(const StreamArgs &A, const StreamCtx<L> &C, int p, int li, uint32_t &efill)
+{
+    using Sg = StreamGeom<L>;
+    __syncwarp();
+    if (C.lane == 0) mbar_arrive(&C.empty[li % Sg::NST]);
+    if ((C.tid >> 5) != Sg::NTHR / 32 - 1) return;
+    const int lj = li - 1;
+    if (lj < 0 || lj + Sg::NST >= C.i1 - C.i0) return;
+    const int st = lj % Sg::NST;
+    mbar_wait(&C.empty[st], ((efill >> st) & 1u) ^ 1u);     // fill n is consumed in phase n - 1
+    if (C.lane < 3) stream_issue_item<L>(A, C, p, lj + Sg::NST, C.lane);
+    efill ^= 1u << st;
+    __syncwarp();
+}
+
+// One half-sweep (parity p) over the block's batches; the first NST items are in flight
+// (stream_prime).  ENERGY: also count the satisfied bonds of the updated (parity-1) sites.
 template <int L, bool FAST, bool ENERGY>
 __device__ __forceinline__ void stream_consume(const StreamArgs &A, const StreamCtx<L> &C, int p, uint32_t g,
-                                               uint32_t &phase, int ebuf)
+                                               uint32_t &phase, uint32_t &efill)
 {
     using Gm = ResGeom<L>;
     using Sg = StreamGeom<L>;
     constexpr int N = Gm::N, Nh = Gm::Nh, QR = Gm::QR, ZS = Sg::ZS, NT = Sg::NTHR;
-    constexpr int NB = Sg::NB, NS = Sg::NS, NSLAB = Sg::NSLAB;
+    constexpr int NST = Sg::NST, NSLAB = Sg::NSLAB;
     const Params &P = A.P;
     const int nT = C.nT, tid = C.tid;
     int cur_grp = -1, s = 0, q = 0;
@@ -217,7 +223,7 @@ __device__ __forceinline__ void stream_consume(const StreamArgs &A, const Stream
     for (int b = 0; b < C.nb; ++b) {
         __syncwarp();
         const StreamBatch B = C.batch[b];
-        const int cnt = B.cnt, st = b % NS, pos = B.pos, w = B.w;
+        const int cnt = B.cnt, pos = B.pos, w = B.w;
         const int k0 = pos % nT, grp = w * NSLAB + B.slab;
         if (grp != cur_grp) {        // couplings of my quad for this (word, slab) and parity
             cur_grp = grp;
@@ -230,18 +236,18 @@ __device__ __forceinline__ void stream_consume(const StreamArgs &A, const Stream
         }
         const uint32_t gw = P.w0 + (uint32_t)w;
         const uint32_t c3 = (uint32_t)p << 16;
-        mbar_wait(&C.full[st], (phase >> st) & 1u);
-        phase ^= 1u << st;
-        const unsigned char *stage = C.bufs + (size_t)(st * NB) * Sg::BUF_BYTES;
         if (!ENERGY) {
             for (int i = 0; i < cnt; ++i) {
-                const int li = pos + i - C.i0;
-                const char *buf = reinterpret_cast<const char *>(stage + (size_t)i * Sg::BUF_BYTES);
+                const int li = pos + i - C.i0, st = li % NST;
                 const uint4 rnd = philox_rk(g, (uint32_t)q, gw, c3 | (uint32_t)(k0 + i), A.rk);
+                mbar_wait(&C.full[st], (phase >> st) & 1u);
+                phase ^= 1u << st;
+                const char *buf = reinterpret_cast<const char *>(C.bufs + (size_t)st * Sg::BUF_BYTES);
                 const uint4 res = update_quad_mem<L, FAST, false, false, false>(
                     buf + 16 * tid, buf + Sg::OWN_BYTES, C.ov, C.oyp, C.oym, C.ozp, C.ozm, C.qx, C.lt + li * C.LTS,
                     C.mt + (size_t)li * C.MTS, C.R, J, s, rnd, fin);
                 reinterpret_cast<uint4 *>(P.spin + ((size_t)(k0 + i) * P.W + w) * N + p * Nh)[q] = res;
+                stream_release<L>(A, C, p, li, efill);
             }
         } else {
             for (int i0 = 0; i0 < cnt; i0 += 2) {      // pairs of slots: few live registers
@@ -250,13 +256,16 @@ __device__ __forceinline__ void stream_consume(const StreamArgs &A, const Stream
                 for (int h = 0; h < 2; ++h) {
                     const int i = i0 + h;
                     if (i < cnt) {
-                        const int li = pos + i - C.i0;
-                        const char *buf = reinterpret_cast<const char *>(stage + (size_t)i * Sg::BUF_BYTES);
+                        const int li = pos + i - C.i0, st = li % NST;
                         const uint4 rnd = philox_rk(g, (uint32_t)q, gw, c3 | (uint32_t)(k0 + i), A.rk);
+                        mbar_wait(&C.full[st], (phase >> st) & 1u);
+                        phase ^= 1u << st;
+                        const char *buf = reinterpret_cast<const char *>(C.bufs + (size_t)st * Sg::BUF_BYTES);
                         const uint4 res = update_quad_mem<L, FAST, true, false, false>(
                             buf + 16 * tid, buf + Sg::OWN_BYTES, C.ov, C.oyp, C.oym, C.ozp, C.ozm, C.qx,
                             C.lt + li * C.LTS, C.mt + (size_t)li * C.MTS, C.R, J, s, rnd, fin);
                         reinterpret_cast<uint4 *>(P.spin + ((size_t)(k0 + i) * P.W + w) * N + p * Nh)[q] = res;
+                        stream_release<L>(A, C, p, li, efill);
                         quad_sum(fin, en[h]);
                     } else {
 #pragma unroll
@@ -266,10 +275,26 @@ __device__ __forceinline__ void stream_consume(const StreamArgs &A, const Stream
                 uint32_t tot[kResPlanes];
                 warp_sum2(en, C.lane, tot);
                 const int i_mine = i0 + (C.lane >> 4);
-                if (i_mine < cnt && !(C.lane & 8)) add_counts(tot, C.lane & 7, C.Eacc + ((b & 1) * NB + i_mine) * 32);
+                if (i_mine < cnt && !(C.lane & 8)) add_counts(tot, C.lane & 7, C.Eacc + (pos + i_mine - C.i0) * 32);
             }
         }
-        stream_batch_done<L, ENERGY>(A, C, p, b, ebuf);
+    }
+}
+
+// End of the parity-1 half-sweep: the block's per-item shared counters go to the global
+// satisfied-bond counters [ebuf][r][k] (before the grid barrier, so that every block sees them
+// after it) and are cleared for the next energy sweep.
+template <int L>
+__device__ __forceinline__ void stream_flush_counts(const StreamArgs &A, const StreamCtx<L> &C, int ebuf)
+{
+    using Sg = StreamGeom<L>;
+    const Params &P = A.P;
+    __syncthreads();
+    for (int a = C.tid; a < (C.i1 - C.i0) * 32; a += Sg::NTHR) {
+        const int v = C.Eacc[a];
+        C.Eacc[a] = 0;
+        const int item = C.i0 + (a >> 5), k = item % C.nT, w = item / (Sg::NSLAB * C.nT);
+        atomicAdd(A.Ecnt + (size_t)ebuf * P.Rp * C.nT + (size_t)(32 * w + (a & 31)) * C.nT + k, v);
     }
 }
 
@@ -302,7 +327,7 @@ __global__ void __launch_bounds__(StreamGeom<L>::NTHR, 1) k_stream(const StreamA
 {
     using Gm = ResGeom<L>;
     using Sg = StreamGeom<L>;
-    constexpr int N = Gm::N, QR = Gm::QR, QPP = Sg::QPP, NT = Sg::NTHR, NB = Sg::NB, NS = Sg::NS;
+    constexpr int N = Gm::N, QR = Gm::QR, QPP = Sg::QPP, NT = Sg::NTHR, NB = Sg::NB, NST = Sg::NST;
     constexpr int NSLAB = Sg::NSLAB;
     extern __shared__ __align__(128) unsigned char smraw[];
     const Params &P = A.P;
@@ -318,15 +343,15 @@ __global__ void __launch_bounds__(StreamGeom<L>::NTHR, 1) k_stream(const StreamA
     const int w_first = C.i0 / per_w, nwt = (C.i1 - 1) / per_w - w_first + 1;   // words I meet (<= MW)
 
     // shared memory
-    uint64_t *mbar = reinterpret_cast<uint64_t *>(smraw);                        // full[NS], number of batches: 64 B reserved
-    uint4 *bucket = reinterpret_cast<uint4 *>(smraw + 64);                       // [n_bucket]
-    unsigned char *bufs = reinterpret_cast<unsigned char *>(bucket + A.n_bucket);   // [NS][NB][BUF_BYTES]
-    uint4 *mt = reinterpret_cast<uint4 *>(bufs + (size_t)NS * NB * Sg::BUF_BYTES);  // [MS][MTS]
+    uint64_t *mbar = reinterpret_cast<uint64_t *>(smraw);                        // full[NST], empty[NST], number of batches
+    uint4 *bucket = reinterpret_cast<uint4 *>(smraw + Sg::MBAR_BYTES);           // [n_bucket]
+    unsigned char *bufs = reinterpret_cast<unsigned char *>(bucket + A.n_bucket);   // [NST][BUF_BYTES]
+    uint4 *mt = reinterpret_cast<uint4 *>(bufs + (size_t)NST * Sg::BUF_BYTES);      // [MS][MTS]
     uint32_t *lt = reinterpret_cast<uint32_t *>(mt + (size_t)MS * MTS);          // [MS][LTS]
     uint32_t *thr = lt + MS * LTS;                                               // [3][LTS]
     uchar4 *trip = reinterpret_cast<uchar4 *>(thr + 3 * LTS);                    // [MTS]
-    int32_t *Eacc = reinterpret_cast<int32_t *>(trip + MTS);                     // [2][NB][32]
-    uint8_t *tau8 = reinterpret_cast<uint8_t *>(Eacc + 2 * NB * 32);             // [MW][32][nT]
+    int32_t *Eacc = reinterpret_cast<int32_t *>(trip + MTS);                     // [MS][32]
+    uint8_t *tau8 = reinterpret_cast<uint8_t *>(Eacc + MS * 32);                 // [MW][32][nT]
     uint8_t *sig8 = tau8 + (size_t)MW * 32 * nT;                                 // [MW][32][nT]
     const int SW = A.swap_win;
     int32_t *Esm = reinterpret_cast<int32_t *>(smraw + A.esm_off);               // [MW][32][nT] bond counts
@@ -334,6 +359,7 @@ __global__ void __launch_bounds__(StreamGeom<L>::NTHR, 1) k_stream(const StreamA
     uint32_t *swwin = reinterpret_cast<uint32_t *>(batch + MS);                  // [nT][SW] thresholds - 1
     int *swlo = reinterpret_cast<int *>(swwin + (size_t)nT * SW);                // [nT] first m of the stored range
     int *swhi = swlo + nT;                                                       // [nT] one past its last m
+    int *swk = swhi + nT;                                                        // [nT] decisions left | right << 1 of the range
 
     for (int a = tid; a < A.n_bucket; a += NTA) bucket[a] = A.bucket[a];
     for (int a = tid; a < 3 * LTS; a += NTA) thr[a] = P.thr32[a];
@@ -343,14 +369,17 @@ __global__ void __launch_bounds__(StreamGeom<L>::NTHR, 1) k_stream(const StreamA
         const int lo = P.swp_lo[t], cn = P.swp_cnt[t];
         swwin[a] = (m >= lo && m < lo + cn) ? P.swp_val[P.swp_off[t] + (m - lo)] : 0u;
     }
-    for (int t = tid; t + 1 < nT; t += NTA) { swlo[t] = P.swp_lo[t]; swhi[t] = P.swp_lo[t] + P.swp_cnt[t]; }
-    for (int a = tid; a < 2 * NB * 32; a += NTA) Eacc[a] = 0;
+    for (int t = tid; t + 1 < nT; t += NTA) {
+        swlo[t] = P.swp_lo[t]; swhi[t] = P.swp_lo[t] + P.swp_cnt[t];
+        swk[t] = (int)P.swp_kind[2 * t] | ((int)P.swp_kind[2 * t + 1] << 1);
+    }
+    for (int a = tid; a < MS * 32; a += NTA) Eacc[a] = 0;
     for (int a = tid; a < nwt * 32 * nT; a += NTA) {
         tau8[a] = P.tau[(size_t)32 * w_first * nT + a];
         sig8[a] = P.sigma[(size_t)32 * w_first * nT + a];
     }
     if (tid == 0) {
-        for (int i = 0; i < NS; ++i) mbar_init(&mbar[i], 1);
+        for (int i = 0; i < NST; ++i) { mbar_init(&mbar[i], 1); mbar_init(&mbar[NST + i], NT / 32); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         // my batch list: up to NB consecutive slots of one (word, slab) group each
         int nb = 0;
@@ -359,7 +388,7 @@ __global__ void __launch_bounds__(StreamGeom<L>::NTHR, 1) k_stream(const StreamA
             batch[nb] = StreamBatch{pos, cnt, grp / NSLAB, grp % NSLAB};
             pos += cnt;
         }
-        *reinterpret_cast<int *>(smraw + 48) = nb;
+        *reinterpret_cast<int *>(smraw + 16 * NST) = nb;
     }
     __syncthreads();
 
@@ -390,36 +419,40 @@ __global__ void __launch_bounds__(StreamGeom<L>::NTHR, 1) k_stream(const StreamA
         C.ozp = 16u * (uint32_t)((C.zl + 2) * QPP + row);
         C.ozm = 16u * (uint32_t)(C.zl * QPP + row);
     }
-    C.full = mbar; C.batch = batch; C.bufs = bufs; C.mt = mt; C.lt = lt; C.Eacc = Eacc;
-    C.nb = *reinterpret_cast<const int *>(smraw + 48);
+    C.full = mbar; C.empty = mbar + NST; C.batch = batch; C.bufs = bufs; C.mt = mt; C.lt = lt; C.Eacc = Eacc;
+    C.nb = *reinterpret_cast<const int *>(smraw + 16 * NST);
     C.R.thr = thr; C.R.bucket = bucket; C.R.LTS = LTS; C.R.nT = nT;
     C.R.key_lo = A.key_lo; C.R.key_top = A.n_bucket - 1; C.R.key_shift = A.key_shift;
     C.R.z0 = P.z[0]; C.R.z1 = P.z[1]; C.R.z2 = P.z[2];
     C.R.ones = A.ones; C.R.c48 = A.c48; C.R.cm16 = A.cm16; C.R.c16 = A.c16;
     __syncthreads();
 
-    uint32_t nswap = A.nswap0, phase = 0;
+    uint32_t nswap = A.nswap0, phase = 0, efill = 0;
     int ebuf = 0;
-    stream_prime<L>(A, C, 0);
+    stream_prime<L>(A, C, 0, efill);
     auto bar_compute = [&]() { __syncthreads(); };
     for (int it = 0; it < A.n_sweeps; ++it) {
         const uint32_t g = A.g0 + (uint32_t)it;
         const bool swap_now = A.swap_interval > 0 && ((uint64_t)g + 1) % (uint64_t)A.swap_interval == 0;
         const bool need_E = swap_now || it == A.n_sweeps - 1;
         trace_stamp(A, it, 0);
-        stream_consume<L, FAST, false>(A, C, 0, g, phase, ebuf);
+        stream_consume<L, FAST, false>(A, C, 0, g, phase, efill);
         trace_stamp(A, it, 1);
         stream_grid_sync(A.gbar);
         __syncwarp();   // thread 0 spins inside grid.sync: make its warp converge again before the hot loop
-        stream_prime<L>(A, C, 1);
+        stream_prime<L>(A, C, 1, efill);
         trace_stamp(A, it, 2);
-        if (need_E) stream_consume<L, FAST, true>(A, C, 1, g, phase, ebuf);
-        else stream_consume<L, FAST, false>(A, C, 1, g, phase, ebuf);
+        if (need_E) {
+            stream_consume<L, FAST, true>(A, C, 1, g, phase, efill);
+            stream_flush_counts<L>(A, C, ebuf);
+        } else {
+            stream_consume<L, FAST, false>(A, C, 1, g, phase, efill);
+        }
         trace_stamp(A, it, 3);
         stream_grid_sync(A.gbar);
         __syncwarp();   // thread 0 spins inside grid.sync: make its warp converge again before the hot loop
         // the next sweep's first tiles fly while the swap decisions are taken
-        if (it + 1 < A.n_sweeps) stream_prime<L>(A, C, 0);
+        if (it + 1 < A.n_sweeps) stream_prime<L>(A, C, 0, efill);
         trace_stamp(A, it, 4);
         if (!need_E) continue;
         const int32_t *cnt = A.Ecnt + (size_t)ebuf * P.Rp * nT;     // satisfied bonds by [r][k]
@@ -436,9 +469,11 @@ __global__ void __launch_bounds__(StreamGeom<L>::NTHR, 1) k_stream(const StreamA
                     const int sa = sg_[t], sb = sg_[t + 1];
                     const int m = (er[sb] - er[sa]) / 2;
                     const uint4 v = philox_rk(g, (uint32_t)t, P.r0 + (uint32_t)r, 2u << 16, A.rk);
-                    const bool acc = (m >= -SW && m < 0 && m >= swlo[t] && m < swhi[t])
-                                         ? v.x <= swwin[t * SW + m + SW]
-                                         : swap_accept(P, t, m, v.x);
+                    bool acc;           // everything but the far tail of the stored range is in shared memory
+                    if (m < swlo[t]) acc = swk[t] & 1;
+                    else if (m >= swhi[t]) acc = (swk[t] >> 1) & 1;
+                    else if (m >= -SW && m < 0) acc = v.x <= swwin[t * SW + m + SW];
+                    else acc = v.x <= P.swp_val[P.swp_off[t] + (m - swlo[t])];
                     if (acc) {
                         sg_[t] = (uint8_t)sb; sg_[t + 1] = (uint8_t)sa;
                         ta_[sa] = (uint8_t)(t + 1); ta_[sb] = (uint8_t)t;
