@@ -25,6 +25,9 @@
  *   ferromagnet : Binder-cumulant crossing near T = 4.51
  *   PT          : sigma/tau inverse permutations, energy multiset conserved,
  *                 <E>(T) with PT == without PT
+ *   field h     : flip-and-recompute dE, incremental == recomputed, exact
+ *                 (s -> -s, h -> -h) symmetry, Boltzmann stationarity on the
+ *                 2^3 lattice, saturation at large |h| (tests/test_oracle_field.py)
  * No function here is "parity unpinned".
  */
 #include <math.h>
@@ -65,6 +68,9 @@ typedef struct eao {
     double *beta;        /* [nT] */
     uint64_t *acc;       /* [nT][7]        acceptance thresholds              */
     uint64_t *swp;       /* [nT-1][3N+1]   swap thresholds, column m + 3N/2   */
+    int h;               /* external field of Eq. 1 (integer, R21); 0 unless eao_set_field */
+    uint64_t *accf;      /* h != 0: [nT][7][2] acceptance thresholds, last index (s+1)/2          */
+    uint64_t *swpf;      /* h != 0: [nT-1][2 Mf + 1], Mf = (3+|h|) N, column (E_a-E_b)/2 + Mf     */
     int8_t *s;           /* [slot k][site i][r]  +-1                          */
     int8_t *J;           /* [d][site i][r]       +-1, bond i -> i + d^        */
     int32_t *E;          /* [r][slot k]  incremental energy                   */
@@ -133,8 +139,9 @@ static int n_sat(const eao *o, int k, int r, int i)
 }
 int eao_n_sat(const eao *o, int k, int r, int site) { return n_sat(o, k, r, site); }
 
-/* H = - sum_<ij> J_ij s_i s_j (Eq. 1 at h = 0), from scratch:
- * every site contributes its three forward bonds. */
+/* H = - sum_<ij> J_ij s_i s_j + h sum_i s_i (Eq. 1, sign of the
+ * field term as printed; R21), from scratch: every site contributes
+ * its three forward bonds and its field term. */
 int32_t eao_energy_from_scratch(const eao *o, int r, int k)
 {
     int32_t H = 0;
@@ -147,6 +154,7 @@ int32_t eao_energy_from_scratch(const eao *o, int r, int k)
                 H -= J_(o, 0, i, r) * si * S_(o, k, site_of(o, x + 1, y, z), r);
                 H -= J_(o, 1, i, r) * si * S_(o, k, site_of(o, x, y + 1, z), r);
                 H -= J_(o, 2, i, r) * si * S_(o, k, site_of(o, x, y, z + 1), r);
+                H += o->h * si;
             }
     return H;
 }
@@ -183,7 +191,7 @@ static void init_from_seed(eao *o)
 void eao_destroy(eao *o)
 {
     if (!o) return;
-    free(o->beta); free(o->acc); free(o->swp); free(o->s); free(o->J);
+    free(o->beta); free(o->acc); free(o->swp); free(o->accf); free(o->swpf); free(o->s); free(o->J);
     free(o->E); free(o->tau); free(o->sigma); free(o->nbr); free(o);
 }
 
@@ -226,6 +234,53 @@ eao *eao_create(int L, int nT, int R, const double *betas, uint64_t seed, int r0
         for (int k = 0; k < nT; ++k) { o->tau[r * nT + k] = k; o->sigma[r * nT + k] = k; }
     recompute_all_energies(o);
     return o;
+}
+
+/* Constant external field h of Eq. 1 ("a constant external
+ * field, h, is included in our implementation").  Flipping s_i
+ * changes H by dE = (4 n_sat - 12) - 2 h s_i, so the look-up table gets the
+ * paper's 14 columns "7 possible local energies E, 2 spins S":
+ *   accf[t][c][(s+1)/2] = threshold(-beta_t dE).
+ * h is an integer so that H stays an exact integer (R21); E_a - E_b
+ * is then even, and the swap table is indexed by (E_a - E_b)/2:
+ *   swpf[t][d2 + Mf] = threshold((beta_t - beta_{t+1}) 2 d2),  |d2| <= Mf = (3+|h|) N.
+ * h = 0 restores the zero-field tables.  Energies are recomputed. */
+int eao_set_field(eao *o, int h)
+{
+    if (h < -64 || h > 64) return -1;
+    free(o->accf); free(o->swpf);
+    o->accf = NULL; o->swpf = NULL;
+    o->h = h;
+    if (h != 0) {
+        int64_t Mf = (int64_t)(3 + abs(h)) * o->N;
+        o->accf = (uint64_t *)malloc(sizeof(uint64_t) * o->nT * 14);
+        o->swpf = (uint64_t *)malloc(sizeof(uint64_t) * (size_t)(o->nT > 1 ? o->nT - 1 : 1) * (size_t)(2 * Mf + 1));
+        if (!o->accf || !o->swpf) return -2;
+        for (int t = 0; t < o->nT; ++t)
+            for (int c = 0; c < 7; ++c)
+                for (int sp = 0; sp < 2; ++sp) {
+                    int s = 2 * sp - 1;
+                    double dE = (double)(4 * c - 12 - 2 * h * s);
+                    o->accf[(t * 7 + c) * 2 + sp] = threshold_of(-(o->beta[t] * dE));
+                }
+        for (int t = 0; t + 1 < o->nT; ++t) {
+            double db = o->beta[t] - o->beta[t + 1];
+            for (int64_t d2 = -Mf; d2 <= Mf; ++d2)
+                o->swpf[(size_t)t * (size_t)(2 * Mf + 1) + (size_t)(d2 + Mf)] = threshold_of(db * (double)(2 * d2));
+        }
+    }
+    recompute_all_energies(o);
+    return 0;
+}
+int eao_get_field(const eao *o) { return o->h; }
+/* accf [nT][7][2], swpf [nT-1][2 (3+|h|) N + 1]; only for h != 0. */
+int eao_get_field_tables(const eao *o, uint64_t *accf, uint64_t *swpf)
+{
+    if (o->h == 0) return -1;
+    int64_t Mf = (int64_t)(3 + abs(o->h)) * o->N;
+    memcpy(accf, o->accf, sizeof(uint64_t) * o->nT * 14);
+    if (o->nT > 1) memcpy(swpf, o->swpf, sizeof(uint64_t) * (size_t)(o->nT - 1) * (size_t)(2 * Mf + 1));
+    return 0;
 }
 
 void eao_set_check(eao *o, int on) { o->check = on; }
@@ -278,7 +333,8 @@ void eao_get_tables(const eao *o, uint64_t *acc, uint64_t *swp)
  * shared by the 32 realizations of the word (R11), taken from
  *   PX(g, q, w, (p<<16)|k)[l],  j = (x>>1) + (L/2)(y + L z), q = j>>2, l = j&3
  * (DESIGN.md "RNG convention").  Flip iff draw < acc[tau][n_sat]
- * (Eq. 5 with the sign fixed by R1). */
+ * (Eq. 5 with the sign fixed by R1); with a field
+ * the column is (n_sat, s_i) and dE = 4 n_sat - 12 - 2 h s_i (eao_set_field). */
 static void half_sweep(eao *o, int p)
 {
     int L = o->L, nT = o->nT;
@@ -301,9 +357,12 @@ static void half_sweep(eao *o, int p)
                             int c = n_sat(o, k, r, i);
                             int t = o->tau[r * nT + k];
                             o->n_attempt++;
-                            if (u < o->acc[t * 7 + c]) {
-                                S_(o, k, i, r) = (int8_t)(-S_(o, k, i, r));
-                                o->E[r * nT + k] += 4 * c - 12;
+                            int si = S_(o, k, i, r);
+                            uint64_t thr = o->h == 0 ? o->acc[t * 7 + c]
+                                                     : o->accf[(t * 7 + c) * 2 + (si + 1) / 2];
+                            if (u < thr) {
+                                S_(o, k, i, r) = (int8_t)(-si);
+                                o->E[r * nT + k] += 4 * c - 12 - 2 * o->h * si;
                                 o->n_accept++;
                             }
                         }
@@ -325,12 +384,19 @@ static void swap_round(eao *o, uint64_t g_done)
         for (int t = (int)(o->nswap & 1); t + 1 < nT; t += 2) {
             int a = sg[t], b = sg[t + 1];
             int dE = E[a] - E[b];
-            int m = dE / 4;              /* exact: dE is a multiple of 4 */
+            int m = dE / 4;              /* exact at h = 0: dE is a multiple of 4 */
             eao_philox4x32_10((uint32_t)g_done, (uint32_t)t, (uint32_t)(o->r0 + r), 2u << 16,
                               o->k0, o->k1, out);
             uint64_t v = out[0];
             o->n_swap_attempt++;
-            if (v < o->swp[(size_t)t * (2 * M + 1) + (m + M)]) {
+            uint64_t thr;
+            if (o->h == 0) {
+                thr = o->swp[(size_t)t * (2 * M + 1) + (m + M)];
+            } else {                     /* dE is even: column dE/2 of the field table */
+                int64_t Mf = (int64_t)(3 + abs(o->h)) * o->N;
+                thr = o->swpf[(size_t)t * (size_t)(2 * Mf + 1) + (size_t)(dE / 2 + Mf)];
+            }
+            if (v < thr) {
                 sg[t] = b; sg[t + 1] = a;
                 ta[a] = t + 1; ta[b] = t;
                 o->n_swap_accept++;

@@ -65,6 +65,12 @@ def _load():
     lib.eao_n_sat.restype = i32
     lib.eao_n_sat.argtypes = [vp, i32, i32, i32]
     lib.eao_philox4x32_10.argtypes = [C.c_uint32] * 6 + [vp]
+    lib.eao_set_field.restype = i32
+    lib.eao_set_field.argtypes = [vp, i32]
+    lib.eao_get_field.restype = i32
+    lib.eao_get_field.argtypes = [vp]
+    lib.eao_get_field_tables.restype = i32
+    lib.eao_get_field_tables.argtypes = [vp, vp, vp]
     _lib = lib
     return lib
 
@@ -127,6 +133,24 @@ class Oracle:
         swp = np.ascontiguousarray(swp, dtype=np.uint64)
         assert acc.shape == (self.nT, 7) and swp.shape == (self.nT - 1, 3 * self.N + 1)
         self.lib.eao_set_tables(self.h, _ptr(acc), _ptr(swp))
+
+    def set_field(self, h):
+        """Constant external field h of Eq. 1 (integer); energies are recomputed."""
+        rc = self.lib.eao_set_field(self.h, int(h))
+        if rc != 0:
+            raise ValueError(f"eao_set_field -> {rc}")
+
+    def field(self) -> int:
+        return int(self.lib.eao_get_field(self.h))
+
+    def field_tables(self):
+        """(accf [nT][7][2], swpf [nT-1][2 (3+|h|) N + 1]) for h != 0."""
+        Mf = (3 + abs(self.field())) * self.N
+        accf = np.zeros((self.nT, 7, 2), dtype=np.uint64)
+        swpf = np.zeros((max(self.nT - 1, 1), 2 * Mf + 1), dtype=np.uint64)
+        if self.lib.eao_get_field_tables(self.h, _ptr(accf), _ptr(swpf)) != 0:
+            raise ValueError("no field tables at h = 0")
+        return accf, swpf[: self.nT - 1]
 
     def sweep(self, n_sweeps, swap_interval):
         rc = self.lib.eao_sweep(self.h, int(n_sweeps), int(swap_interval))
