@@ -169,6 +169,26 @@ int ea_get_moments(ea_handle *h, uint64_t *n_meas, int64_t *q1 /* [P][32][n_temp
  * the exact rational value to ~1e-18 relative.  NaN where no measurement was taken or [<q^2>] = 0. */
 int ea_get_binder(ea_handle *h, double *g /* [n_temps] */);
 
+/*
+ * ---- External field ----
+ * Constant field h of Eq. 1 ("a constant external field, h, is included in our
+ * implementation"), sign as printed: H = -sum J s s + h sum_i s_i.  Flipping s_i costs
+ * dE = 4 n_sat - 12 - 2 h s_i, so the acceptance table has the paper's 14 columns (7 local energies
+ * x 2 spins).  h is an integer, |h| <= 64 (R21: H stays an exact
+ * integer; the swap table is then indexed by (E_a - E_b)/2).  Tables are rebuilt on the host in
+ * double from betas, energies are recomputed, the sweep counter is kept.  With h != 0 only
+ * EA_KERNEL_GENERIC runs (ea_set_kernel(other) -> EA_ERR_UNSUPPORTED, ea_set_tables ->
+ * EA_ERR_UNSUPPORTED, ea_get_tables keeps returning the zero-field tables); h = 0 restores the
+ * zero-field path.
+ */
+int ea_set_field(ea_handle *h, int field);
+int ea_get_field(ea_handle *h);
+/* accf[t][c][(s+1)/2] = floor(2^32 min(1, exp(-beta_t (4c - 12 - 2 h s)))), c = n_sat, s = +-1;
+ * swpf[t][d2 + Mf] = floor(2^32 min(1, exp((beta_t - beta_{t+1}) 2 d2))), |d2| <= Mf = (3+|h|) N.
+ * EA_ERR_INVALID_ARG when no field is set. */
+int ea_get_field_tables(ea_handle *h, uint64_t *accf /* [n_temps][7][2] */,
+                        uint64_t *swpf /* [n_temps-1][2 (3+|h|) N + 1] */);
+
 /* Select the sweep implementation (EA_KERNEL_*); EA_ERR_UNSUPPORTED if it cannot run this shape. */
 int ea_set_kernel(ea_handle *h, int kernel);
 /* The implementation ea_sweep would use now (EA_KERNEL_GENERIC/RESIDENT/TILED/STREAM). */

@@ -18,7 +18,7 @@ _SYMBOLS = [
     "ea_overlap", "ea_get_spins", "ea_get_state", "ea_set_kernel", "ea_get_kernel",
     "ea_launch_count", "ea_last_error", "ea_measure_int_peak",
     "ea_get_couplings", "ea_pair_couplings", "ea_measure_begin", "ea_measure", "ea_get_moments",
-    "ea_get_binder",
+    "ea_get_binder", "ea_set_field", "ea_get_field", "ea_get_field_tables",
 ]
 
 
@@ -62,7 +62,9 @@ def lib():
                        ("ea_set_kernel", [vp, i32]), ("ea_get_kernel", [vp]),
                        ("ea_get_couplings", [vp, vp]), ("ea_pair_couplings", [vp]),
                        ("ea_measure_begin", [vp, vp, i32]), ("ea_measure", [vp, i64, i64, i32]),
-                       ("ea_get_moments", [vp, vp, vp, vp, vp, vp, vp]), ("ea_get_binder", [vp, vp])):
+                       ("ea_get_moments", [vp, vp, vp, vp, vp, vp, vp]), ("ea_get_binder", [vp, vp]),
+                       ("ea_set_field", [vp, i32]), ("ea_get_field", [vp]),
+                       ("ea_get_field_tables", [vp, vp, vp])):
         f = getattr(l, name)
         f.restype = i32
         f.argtypes = args
@@ -212,6 +214,19 @@ class EA:
         g = np.zeros(self.nT, dtype=np.float64)
         self._chk(self._l.ea_get_binder(self.h, _p(g)))
         return g
+
+    def set_field(self, field):
+        self._chk(self._l.ea_set_field(self.h, int(field)))
+
+    def get_field(self):
+        return int(self._l.ea_get_field(self.h))
+
+    def get_field_tables(self):
+        Mf = (3 + abs(self.get_field())) * self.N
+        accf = np.zeros((self.nT, 7, 2), dtype=np.uint64)
+        swpf = np.zeros((max(self.nT - 1, 0), 2 * Mf + 1), dtype=np.uint64)
+        self._chk(self._l.ea_get_field_tables(self.h, _p(accf), _p(swpf)))
+        return accf, swpf
 
     def set_kernel(self, kernel):
         self._chk(self._l.ea_set_kernel(self.h, int(kernel)))

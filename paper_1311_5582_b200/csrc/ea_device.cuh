@@ -28,6 +28,12 @@ struct Params {
     const int32_t *swp_off;  // [nT-1] offset into swp_val
     const uint8_t *swp_kind; // [nT-1][2] decision left / right of the stored range (0 never, 1 always)
     const uint32_t *swp_val; // (threshold - 1) for thresholds in (0, 2^32)
+    // external field (ea_set_field; generic kernels only).  Appended last: the offsets of the
+    // members above, which the fast kernels read from the constant bank, do not move.
+    int h;                   // field of Eq. 1 (integer); 0: zero-field path
+    int ediv;                // swap tables are indexed by (E_a - E_b) / ediv: 4 at h = 0, else 2
+    const uint32_t *thrF;    // [14][nT+1]: class 2 n_sat + (s+1)/2, (threshold - 1) in pos order, sentinel
+    int zF[14];              // per class: number of zero thresholds, or -1: dE <= 0, always flips
 };
 
 // ---------------------------------------------------------------------------------

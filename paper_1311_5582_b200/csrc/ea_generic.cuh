@@ -90,6 +90,85 @@ __global__ void __launch_bounds__(128) k_half_sweep_generic(Params P, int p, uin
     }
 }
 
+// ------------------------------------------------------------------ f2: half-sweep with a field
+// H = -sum J s s + h sum s (Eq. 1; R21): dE = 4 n_sat - 12 - 2 h s_i, so the
+// acceptance class of a bit is (n_sat, s_i): the paper's 14 table columns.  Per
+// class one rank search and one rank mask; classes with dE <= 0 always flip.  Same thread
+// mapping and draws as k_half_sweep_generic.
+__global__ void __launch_bounds__(128) k_half_sweep_field(Params P, int p, uint32_t g)
+{
+    extern __shared__ uint32_t sm_thr[];   // [14][nT+1]
+    for (int a = threadIdx.x; a < 14 * P.LTS; a += blockDim.x) sm_thr[a] = P.thrF[a];
+    __syncthreads();
+    const int nq = P.Nh >> 2;
+    const int64_t tid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (tid >= (int64_t)P.nT * P.W * nq) return;
+    const int q = (int)(tid % nq);
+    const int w = (int)((tid / nq) % P.W);
+    const int k = (int)(tid / ((int64_t)nq * P.W));
+    uint32_t *sp = P.spin + ((size_t)k * P.W + w) * P.N;
+    const uint32_t *cp = P.coup + (size_t)w * 3 * P.N;
+    const uint32_t *lt = P.lt + ((size_t)w * P.nT + k) * P.LTS;
+    const uint4 rnd = philox4x32_10(g, (uint32_t)q, P.w0 + (uint32_t)w, ((uint32_t)p << 16) | (uint32_t)k,
+                                    P.k0, P.k1);
+#pragma unroll
+    for (int l = 0; l < 4; ++l) {
+        const int j = 4 * q + l;
+        uint32_t s;
+        const Planes pl = site_planes(sp, cp, p, j, P.L, P.Lh, P.Nh, P.N, &s);
+        const uint32_t u = pick(rnd, l);
+        uint32_t acc = 0;
+        for (int c = 0; c < 7; ++c) {
+            const uint32_t ind = ((c & 1) ? pl.b0 : ~pl.b0) & ((c & 2) ? pl.b1 : ~pl.b1) & ((c & 4) ? pl.b2 : ~pl.b2);
+            for (int up = 0; up < 2; ++up) {
+                const int cls = 2 * c + up, z = P.zF[cls];
+                const uint32_t mine = ind & (up ? s : ~s);
+                if (mine == 0u) continue;
+                acc |= z < 0 ? mine : mine & lt[rank_of(u, sm_thr + cls * P.LTS, z, P.nT)];
+            }
+        }
+        sp[p * P.Nh + j] = s ^ acc;
+    }
+}
+
+// Field term of the energy: E[r][k] += h * (2 * (number of up spins) - N).  One block per (w, k),
+// vertical counters like k_energy; runs after it.
+constexpr int kFieldPlanes = 15;   // per-thread count <= ceil(N / 128) <= 2^14
+
+__global__ void __launch_bounds__(128) k_field_energy(Params P)
+{
+    __shared__ int sm_cnt[32];
+    const int w = blockIdx.x / P.nT, k = blockIdx.x % P.nT;
+    const uint32_t *sp = P.spin + ((size_t)k * P.W + w) * P.N;
+    if (threadIdx.x < 32) sm_cnt[threadIdx.x] = 0;
+    __syncthreads();
+    uint32_t c[kFieldPlanes];
+#pragma unroll
+    for (int i = 0; i < kFieldPlanes; ++i) c[i] = 0;
+    for (int i = threadIdx.x; i < P.N; i += blockDim.x) {
+        uint32_t x = sp[i];
+#pragma unroll
+        for (int l = 0; l < kFieldPlanes; ++l) {
+            const uint32_t carry = c[l] & x;
+            c[l] ^= x;
+            x = carry;
+        }
+    }
+    const int lane = threadIdx.x & 31;
+    int mine = 0;
+    for (int b = 0; b < 32; ++b) {
+        int v = 0;
+#pragma unroll
+        for (int l = 0; l < kFieldPlanes; ++l) v += (int)((c[l] >> b) & 1u) << l;
+        v = __reduce_add_sync(0xFFFFFFFFu, v);
+        if (lane == b) mine = v;
+    }
+    atomicAdd(&sm_cnt[lane], mine);
+    __syncthreads();
+    if (threadIdx.x < 32)
+        P.E[(size_t)(32 * w + threadIdx.x) * P.nT + k] += P.h * (2 * sm_cnt[threadIdx.x] - P.N);
+}
+
 // ------------------------------------------------------------------ a8: energy from scratch
 // E[r][k] = 3N - 2 * (number of satisfied bonds); every bond has exactly one parity-1 end, so
 // the satisfied bonds are sum over parity-1 sites of n_sat.  One block per (w, k); per-thread
@@ -162,7 +241,7 @@ __global__ void __launch_bounds__(256) k_pt_swap(Params P, uint32_t g_done, uint
     const int32_t *E = P.E + (size_t)r * P.nT;
     for (int t = (int)(round & 1u) + 2 * warp; t + 1 < P.nT; t += 2 * nwarp) {
         const int a = sg[t], b = sg[t + 1];
-        const int m = (E[a] - E[b]) / 4;
+        const int m = (E[a] - E[b]) / P.ediv;
         const uint4 v = philox4x32_10(g_done, (uint32_t)t, P.r0 + (uint32_t)r, 2u << 16, P.k0, P.k1);
         if (swap_accept(P, t, m, v.x)) {
             sg[t] = (uint8_t)b; sg[t + 1] = (uint8_t)a;

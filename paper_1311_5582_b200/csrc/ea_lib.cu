@@ -53,6 +53,11 @@ struct ea_handle {
     size_t meas_bytes = 0, meas_acc_off = 0;
     uint64_t meas_n = 0;
     bool meas_on = false;
+    // external field (ea_set_field): own allocation for the 14-class thresholds and the trimmed
+    // field swap table; freed by ea_destroy / the next ea_set_field
+    int field = 0;
+    char *d_field = nullptr;
+    std::vector<uint64_t> accf, swpf;  // host copies: [nT][7][2], [nT-1][2 (3+|h|) N + 1]
     mutable std::string err;
 };
 
@@ -209,9 +214,60 @@ static bool build_bucket_table(const std::vector<uint32_t> &thr32, const int z[3
 // acc: per class c = 4,5,6 a column sorted coldest-first ("pos" order), stored as thr-1 with
 // the leading zero thresholds counted in z[c] (R8).  swp: each row trimmed to the
 // entries strictly between 0 and 2^32.
+// Trimmed form of a swap table with rows [nT-1][2 M + 1], column = index + M: per row the first
+// stored index, the number of stored entries, their offset in `val`, the decisions left and right
+// of the stored range (0 never, 1 always) and (threshold - 1) for thresholds in (0, 2^32).  Lossless.
+struct SwapTrim {
+    std::vector<int32_t> lo, cnt, off;
+    std::vector<uint8_t> kind;
+    std::vector<uint32_t> val;
+};
+static const uint64_t kTwo32 = (uint64_t)1 << 32;
+static int trim_swap_table(ea_handle *h, const uint64_t *swp, int nT, int64_t M, SwapTrim &o)
+{
+    const int64_t cols = 2 * M + 1;
+    o.lo.assign(nT, 0); o.cnt.assign(nT, 0); o.off.assign(nT, 0);
+    o.kind.assign((size_t)2 * nT, 0);
+    o.val.clear();
+    for (int t = 0; t + 1 < nT; ++t) {
+        const uint64_t *row = swp + (size_t)t * cols;
+        bool inc = true, dec = true;
+        for (int64_t a = 0; a < cols; ++a) {
+            if (row[a] > kTwo32) return fail(h, EA_ERR_INVALID_ARG, "swp threshold above 2^32");
+            if (a && row[a] < row[a - 1]) inc = false;
+            if (a && row[a] > row[a - 1]) dec = false;
+        }
+        if (!inc && !dec) return fail(h, EA_ERR_INVALID_ARG, "swp row not monotone in m");
+        int64_t a = 0;
+        while (a < cols && (row[a] == 0 || row[a] == kTwo32) && row[a] == row[0]) ++a;
+        int64_t b = a;
+        while (b < cols && row[b] != 0 && row[b] != kTwo32) ++b;
+        for (int64_t c2 = b; c2 < cols; ++c2)
+            if (row[c2] != row[cols - 1]) return fail(h, EA_ERR_INVALID_ARG, "swp row not monotone in m");
+        o.lo[t] = (int32_t)(a - M); o.cnt[t] = (int32_t)(b - a); o.off[t] = (int32_t)o.val.size();
+        o.kind[2 * t] = row[0] == kTwo32;
+        o.kind[2 * t + 1] = row[cols - 1] == kTwo32;
+        for (int64_t c2 = a; c2 < b; ++c2) o.val.push_back((uint32_t)(row[c2] - 1));
+    }
+    return EA_OK;
+}
+static int upload_swap_trim(ea_handle *h, const SwapTrim &o, uint32_t *d_val)
+{
+    const int nT = h->nT;
+    cudaStream_t s = h->stream;
+    CUDA_TRY(h, cudaMemcpyAsync(h->d_swp_lo, o.lo.data(), 4 * nT, cudaMemcpyHostToDevice, s));
+    CUDA_TRY(h, cudaMemcpyAsync(h->d_swp_cnt, o.cnt.data(), 4 * nT, cudaMemcpyHostToDevice, s));
+    CUDA_TRY(h, cudaMemcpyAsync(h->d_swp_off, o.off.data(), 4 * nT, cudaMemcpyHostToDevice, s));
+    CUDA_TRY(h, cudaMemcpyAsync(h->d_swp_kind, o.kind.data(), 2 * nT, cudaMemcpyHostToDevice, s));
+    if (!o.val.empty())
+        CUDA_TRY(h, cudaMemcpyAsync(d_val, o.val.data(), 4 * o.val.size(), cudaMemcpyHostToDevice, s));
+    CUDA_TRY(h, cudaStreamSynchronize(s));
+    return EA_OK;
+}
+
 static int upload_tables(ea_handle *h, const std::vector<uint64_t> &acc, const std::vector<uint64_t> &swp)
 {
-    const int nT = h->nT, M = 3 * h->N / 2, cols = 2 * M + 1;
+    const int nT = h->nT, M = 3 * h->N / 2;
     for (int t = 0; t < nT; ++t)
         for (int c = 0; c < 7; ++c) {
             const uint64_t v = acc[(size_t)t * 7 + c];
@@ -238,40 +294,13 @@ static int upload_tables(ea_handle *h, const std::vector<uint64_t> &acc, const s
         col[nT] = 0xFFFFFFFFu;
         z[c - 4] = zc;
     }
-    std::vector<int32_t> lo(nT, 0), cnt(nT, 0), off(nT, 0);
-    std::vector<uint8_t> kind((size_t)2 * nT, 0);
-    std::vector<uint32_t> val;
-    for (int t = 0; t + 1 < nT; ++t) {
-        const uint64_t *row = swp.data() + (size_t)t * cols;
-        bool inc = true, dec = true;
-        for (int a = 0; a < cols; ++a) {
-            if (row[a] > TWO32) return fail(h, EA_ERR_INVALID_ARG, "swp threshold above 2^32");
-            if (a && row[a] < row[a - 1]) inc = false;
-            if (a && row[a] > row[a - 1]) dec = false;
-        }
-        if (!inc && !dec) return fail(h, EA_ERR_INVALID_ARG, "swp row not monotone in m");
-        int a = 0;
-        while (a < cols && (row[a] == 0 || row[a] == TWO32) && row[a] == row[0]) ++a;
-        int b = a;
-        while (b < cols && row[b] != 0 && row[b] != TWO32) ++b;
-        for (int c2 = b; c2 < cols; ++c2)
-            if (row[c2] != row[cols - 1]) return fail(h, EA_ERR_INVALID_ARG, "swp row not monotone in m");
-        lo[t] = a - M; cnt[t] = b - a; off[t] = (int32_t)val.size();
-        kind[2 * t] = row[0] == TWO32;
-        kind[2 * t + 1] = row[cols - 1] == TWO32;
-        for (int c2 = a; c2 < b; ++c2) val.push_back((uint32_t)(row[c2] - 1));
-    }
-    if (val.size() > h->swp_val_cap) return fail(h, EA_ERR_ALLOC, "swap table overflow");
+    SwapTrim tr;
+    { int rc = trim_swap_table(h, swp.data(), nT, M, tr); if (rc != EA_OK) return rc; }
+    if (tr.val.size() > h->swp_val_cap) return fail(h, EA_ERR_ALLOC, "swap table overflow");
     cudaStream_t s = h->stream;
     CUDA_TRY(h, cudaStreamSynchronize(s));
     CUDA_TRY(h, cudaMemcpyAsync(h->d_thr32, thr32.data(), 4 * thr32.size(), cudaMemcpyHostToDevice, s));
-    CUDA_TRY(h, cudaMemcpyAsync(h->d_swp_lo, lo.data(), 4 * nT, cudaMemcpyHostToDevice, s));
-    CUDA_TRY(h, cudaMemcpyAsync(h->d_swp_cnt, cnt.data(), 4 * nT, cudaMemcpyHostToDevice, s));
-    CUDA_TRY(h, cudaMemcpyAsync(h->d_swp_off, off.data(), 4 * nT, cudaMemcpyHostToDevice, s));
-    CUDA_TRY(h, cudaMemcpyAsync(h->d_swp_kind, kind.data(), 2 * nT, cudaMemcpyHostToDevice, s));
-    if (!val.empty())
-        CUDA_TRY(h, cudaMemcpyAsync(h->d_swp_val, val.data(), 4 * val.size(), cudaMemcpyHostToDevice, s));
-    CUDA_TRY(h, cudaStreamSynchronize(s));
+    { int rc = upload_swap_trim(h, tr, h->d_swp_val); if (rc != EA_OK) return rc; }
     {
         std::vector<uint4> tab;
         std::vector<uchar4> trip;
@@ -293,6 +322,10 @@ static int recompute_energy(ea_handle *h)
 {
     ea::k_energy<<<h->W * h->nT, 128, 0, h->stream>>>(h->P);
     h->launches++;
+    if (h->field != 0) {
+        ea::k_field_energy<<<h->W * h->nT, 128, 0, h->stream>>>(h->P);
+        h->launches++;
+    }
     CUDA_TRY(h, cudaGetLastError());
     h->energy_valid = true;
     return EA_OK;
@@ -366,6 +399,8 @@ extern "C" ea_handle *ea_create_ex(int L, int n_temps, int n_realizations, const
     P.k0 = (uint32_t)seed; P.k1 = (uint32_t)(seed >> 32);
     P.r0 = (uint32_t)first_realization; P.w0 = (uint32_t)(first_realization >> 5);
     P.desc = desc ? 1 : 0;
+    P.h = 0; P.ediv = 4; P.thrF = nullptr;
+    for (int c = 0; c < 14; ++c) P.zF[c] = -1;
     P.spin = (uint32_t *)(h->ws + lay.spin);
     P.coup = (uint32_t *)(h->ws + lay.coup);
     P.lt = (uint32_t *)(h->ws + lay.lt);
@@ -418,6 +453,7 @@ extern "C" void ea_destroy(ea_handle *h)
     if (h->ws) cudaStreamSynchronize(h->stream);
     if (h->own_ws && h->ws) cudaFree(h->ws);
     if (h->d_meas) cudaFree(h->d_meas);
+    if (h->d_field) cudaFree(h->d_field);
     delete h;
 }
 
@@ -481,6 +517,7 @@ extern "C" int ea_set_spins(ea_handle *h, const int8_t *s)
 extern "C" int ea_set_tables(ea_handle *h, const uint64_t *acc, const uint64_t *swp)
 {
     if (!h || !acc || (h->nT > 1 && !swp)) return fail(h, EA_ERR_INVALID_ARG, "ea_set_tables: null argument");
+    if (h->field != 0) return fail(h, EA_ERR_UNSUPPORTED, "ea_set_tables: zero-field tables only (field is set)");
     const size_t cols = 3 * (size_t)h->N + 1;
     std::vector<uint64_t> a(acc, acc + (size_t)h->nT * 7);
     std::vector<uint64_t> s;
@@ -496,16 +533,103 @@ extern "C" int ea_get_tables(ea_handle *h, uint64_t *acc, uint64_t *swp)
     return EA_OK;
 }
 
+// ---------------------------------------------------------------- external field
+extern "C" int ea_set_field(ea_handle *h, int field)
+{
+    if (!h) return EA_ERR_INVALID_ARG;
+    if (field < -64 || field > 64) return fail(h, EA_ERR_INVALID_ARG, "ea_set_field: |h| <= 64");
+    const int nT = h->nT, LTS = nT + 1;
+    if (field == 0) {
+        if (h->field == 0) return EA_OK;
+        CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+        h->field = 0;
+        h->P.h = 0; h->P.ediv = 4; h->P.thrF = nullptr; h->P.swp_val = h->d_swp_val;
+        for (int c = 0; c < 14; ++c) h->P.zF[c] = -1;
+        const std::vector<uint64_t> acc = h->acc, swp = h->swp;
+        int rc = upload_tables(h, acc, swp);                  // the zero-field swap table again
+        if (rc != EA_OK) return rc;
+        if (h->d_field) { cudaFree(h->d_field); h->d_field = nullptr; }
+        h->accf.clear(); h->swpf.clear();
+        return recompute_energy(h);
+    }
+    // tables in double on the host, same formulas as at h = 0 (R21)
+    const int64_t Mf = (int64_t)(3 + std::abs(field)) * h->N, cols = 2 * Mf + 1;
+    std::vector<uint64_t> accf((size_t)nT * 14), swpf((size_t)(nT > 1 ? nT - 1 : 0) * (size_t)cols);
+    for (int t = 0; t < nT; ++t)
+        for (int c = 0; c < 7; ++c)
+            for (int up = 0; up < 2; ++up) {
+                const double dE = (double)(4 * c - 12 - 2 * field * (2 * up - 1));
+                accf[((size_t)t * 7 + c) * 2 + up] = threshold_of(-(h->betas[t] * dE));
+            }
+    for (int t = 0; t + 1 < nT; ++t) {
+        const double db = h->betas[t] - h->betas[t + 1];
+        for (int64_t d2 = -Mf; d2 <= Mf; ++d2)
+            swpf[(size_t)t * (size_t)cols + (size_t)(d2 + Mf)] = threshold_of(db * (double)(2 * d2));
+    }
+    // class thresholds in pos order (coldest first), as (threshold - 1); classes with dE <= 0 flip always
+    std::vector<uint32_t> thrF((size_t)14 * LTS, 0xFFFFFFFFu);
+    int zF[14];
+    for (int c = 0; c < 7; ++c)
+        for (int up = 0; up < 2; ++up) {
+            const int cls = 2 * c + up, dE = 4 * c - 12 - 2 * field * (2 * up - 1);
+            if (dE <= 0) { zF[cls] = -1; continue; }
+            int zc = 0;
+            for (int pos = 0; pos < nT; ++pos) {
+                const int t = h->desc ? pos : nT - 1 - pos;
+                const uint64_t v = accf[((size_t)t * 7 + c) * 2 + up];
+                if (v == 0) { zc = pos + 1; thrF[(size_t)cls * LTS + pos] = 0; }
+                else thrF[(size_t)cls * LTS + pos] = (uint32_t)(v - 1);
+            }
+            zF[cls] = zc;
+        }
+    SwapTrim tr;
+    { int rc = trim_swap_table(h, swpf.data(), nT, Mf, tr); if (rc != EA_OK) return rc; }
+    const size_t o_val = align256(4 * thrF.size());
+    char *d = nullptr;
+    if (cudaMalloc((void **)&d, o_val + 4 * (tr.val.size() + 1)) != cudaSuccess) {
+        cudaGetLastError();
+        return fail(h, EA_ERR_ALLOC, "ea_set_field: cudaMalloc failed");
+    }
+    cudaError_t e = cudaStreamSynchronize(h->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d, thrF.data(), 4 * thrF.size(), cudaMemcpyHostToDevice, h->stream);
+    if (e != cudaSuccess) { cudaFree(d); return fail(h, EA_ERR_CUDA, std::string("ea_set_field: ") + cudaGetErrorString(e)); }
+    { int rc = upload_swap_trim(h, tr, (uint32_t *)(d + o_val)); if (rc != EA_OK) { cudaFree(d); return rc; } }
+    if (h->d_field) cudaFree(h->d_field);
+    h->d_field = d;
+    h->field = field;
+    h->P.h = field; h->P.ediv = 2; h->P.thrF = (const uint32_t *)d; h->P.swp_val = (const uint32_t *)(d + o_val);
+    for (int c = 0; c < 14; ++c) h->P.zF[c] = zF[c];
+    h->accf.swap(accf);
+    h->swpf.swap(swpf);
+    return recompute_energy(h);
+}
+
+extern "C" int ea_get_field(ea_handle *h) { return h ? h->field : 0; }
+
+extern "C" int ea_get_field_tables(ea_handle *h, uint64_t *accf, uint64_t *swpf)
+{
+    if (!h) return EA_ERR_INVALID_ARG;
+    if (h->field == 0) return fail(h, EA_ERR_INVALID_ARG, "ea_get_field_tables: no field is set");
+    if (accf) std::memcpy(accf, h->accf.data(), 8 * h->accf.size());
+    if (swpf && !h->swpf.empty()) std::memcpy(swpf, h->swpf.data(), 8 * h->swpf.size());
+    return EA_OK;
+}
+
 // ---------------------------------------------------------------- sweep
 static int sweep_generic(ea_handle *h, int64_t n_sweeps, int swap_interval)
 {
     const int64_t nthreads = (int64_t)h->nT * h->W * (h->N / 8);
     int grid;
     launch_cfg(nthreads, 128, grid);
-    const size_t smem = 4 * 3 * (size_t)(h->nT + 1);
+    const size_t smem = 4 * (h->field ? 14 : 3) * (size_t)(h->nT + 1);
     for (int64_t it = 0; it < n_sweeps; ++it) {
-        ea::k_half_sweep_generic<<<grid, 128, smem, h->stream>>>(h->P, 0, (uint32_t)h->g);
-        ea::k_half_sweep_generic<<<grid, 128, smem, h->stream>>>(h->P, 1, (uint32_t)h->g);
+        if (h->field) {
+            ea::k_half_sweep_field<<<grid, 128, smem, h->stream>>>(h->P, 0, (uint32_t)h->g);
+            ea::k_half_sweep_field<<<grid, 128, smem, h->stream>>>(h->P, 1, (uint32_t)h->g);
+        } else {
+            ea::k_half_sweep_generic<<<grid, 128, smem, h->stream>>>(h->P, 0, (uint32_t)h->g);
+            ea::k_half_sweep_generic<<<grid, 128, smem, h->stream>>>(h->P, 1, (uint32_t)h->g);
+        }
         h->launches += 2;
         h->energy_valid = false;
         h->g++;
@@ -825,6 +949,7 @@ static int sweep_stream(ea_handle *h, int64_t n_sweeps, int swap_interval)
 
 static int pick_kernel(const ea_handle *h)
 {
+    if (h->field != 0) return EA_KERNEL_GENERIC;     // the fast kernels are zero-field only
     if (h->kernel_sel != EA_KERNEL_AUTO) return h->kernel_sel;
     if (plan_resident(h).ok) return EA_KERNEL_RESIDENT;
     if (plan_stream(h).ok) return EA_KERNEL_STREAM;
@@ -836,6 +961,7 @@ extern "C" int ea_set_kernel(ea_handle *h, int kernel)
 {
     if (!h) return EA_ERR_INVALID_ARG;
     if (kernel == EA_KERNEL_AUTO || kernel == EA_KERNEL_GENERIC) { h->kernel_sel = kernel; return EA_OK; }
+    if (h->field != 0) return fail(h, EA_ERR_UNSUPPORTED, "ea_set_kernel: only the generic kernel runs with a field");
     if (kernel == EA_KERNEL_RESIDENT && plan_resident(h).ok) { h->kernel_sel = kernel; return EA_OK; }
     if (kernel == EA_KERNEL_TILED && plan_tiled(h).ok) { h->kernel_sel = kernel; return EA_OK; }
     if (kernel == EA_KERNEL_STREAM && plan_stream(h).ok) { h->kernel_sel = kernel; return EA_OK; }
