@@ -5,6 +5,8 @@ through the C ABI of libea_b200.so.
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--sweeps-per-step 5000]
   python bench.py --impl reference ...      # the CPU oracle, as it stands, on the host cores
+  python bench.py --field 1                 # the same workload with h = 1 (generic kernel)
+  python bench.py --measure-every 10        # two-copy overlap/energy moments every 10 sweeps
 
 A *step* = `sweeps_per_step` full checkerboard sweeps, each followed by a PT round (config's
 swap_interval), of the whole workload: every row of SURVEY.md section 8(a) on the hot path.
@@ -77,15 +79,17 @@ def _clock_summary(samples):
 
 # ------------------------------------------------------------------ CPU oracle legs
 def _oracle_worker(args):
-    L, nT, betas, seed, r0, sweeps, swap = args
+    L, nT, betas, seed, r0, sweeps, swap, field = args
     from oracle import Oracle
     o = Oracle(L, nT, 32, betas, seed, r0=r0)
+    if field:
+        o.set_field(field)
     t = time.perf_counter()
     o.sweep(sweeps, swap)
     return time.perf_counter() - t
 
 
-def oracle_sample(cfg, words, sweeps, procs):
+def oracle_sample(cfg, words, sweeps, procs, field=0):
     """Time the oracle, as it stands, on `words` realization words of cfg (one word = 32
     realizations, all temperatures) for `sweeps` sweeps, `procs` processes (one word each at a
     time).  Returns (ps per attempt over the wall time, wall seconds)."""
@@ -93,7 +97,7 @@ def oracle_sample(cfg, words, sweeps, procs):
     from oracle import build_oracle
     build_oracle()
     betas = betas_for(cfg)
-    jobs = [(cfg.L, cfg.n_temps, betas, cfg.seed, 32 * w, sweeps, cfg.swap_interval) for w in range(words)]
+    jobs = [(cfg.L, cfg.n_temps, betas, cfg.seed, 32 * w, sweeps, cfg.swap_interval, field) for w in range(words)]
     t = time.perf_counter()
     if procs == 1:
         for j in jobs:
@@ -114,10 +118,10 @@ def run_reference(a, cfg):
     words = min(cores, cfg.W)
     sweeps = max(1, int(1.5e8 / (32 * cfg.n_temps * cfg.N)))      # ~4 s of one core per word
     for _ in range(max(a.warmup, 1)):           # at least once: builds the oracle, starts the pool
-        oracle_sample(cfg, words, 1, words)
+        oracle_sample(cfg, words, 1, words, a.field)
     vals, walls = [], []
     for _ in range(a.steps):
-        v, wsec = oracle_sample(cfg, words, sweeps, words)
+        v, wsec = oracle_sample(cfg, words, sweeps, words, a.field)
         vals.append(v); walls.append(wsec)
     value = float(np.mean(vals))
     sample = f"{words} of {cfg.W} words (32 realizations x {cfg.n_temps} temperatures each) x {sweeps} sweeps per step"
@@ -177,6 +181,22 @@ def run_cuda(a, cfg):
     sps = a.sweeps_per_step
     # weak scaling: every rank owns cfg.R realizations; rank r simulates global words r*W..
     sim = EA(cfg.L, cfg.n_temps, cfg.R, betas, cfg.seed, first_realization=shard_first_realization(rank, cfg.R))
+    if a.field:
+        sim.set_field(a.field)
+    me = a.measure_every
+    if me:
+        # two copies of every disorder realization (words w and w + W/2), overlap and energy
+        # moments accumulated on the device every `me` sweeps (ea_measure)
+        assert cfg.R % 64 == 0 and sps % me == 0, "--measure-every needs R % 64 == 0 and sweeps-per-step % M == 0"
+        sim.pair_couplings()
+        sim.measure_begin([[w, w + cfg.W // 2] for w in range(cfg.W // 2)])
+
+    def step():
+        if me:
+            sim.measure(sps // me, me, cfg.swap_interval)
+        else:
+            sim.sweep(sps, cfg.swap_interval)
+
     kernel = sim.get_kernel()
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
 
@@ -185,7 +205,7 @@ def run_cuda(a, cfg):
 
     # ---- kernel-resident timing: state in HBM/SMEM, no host buffers
     for _ in range(a.warmup):
-        sim.sweep(sps, cfg.swap_interval)
+        step()
     barrier()
     samples, stop = [], threading.Event()
     th = threading.Thread(target=_clock_sampler, args=(stop, samples), daemon=True)
@@ -196,7 +216,7 @@ def run_cuda(a, cfg):
     for e0, e1 in ev:
         flush_l2()
         e0.record()
-        sim.sweep(sps, cfg.swap_interval)
+        step()
         e1.record()
     barrier()
     stop.set(); th.join()
@@ -213,12 +233,14 @@ def run_cuda(a, cfg):
     Jpin.numpy()[...] = random_couplings(cfg.R, cfg.N, 1000 + rank)
     Jnp = Jpin.numpy()
     e2e_steps = max(2, min(a.steps, 3))
-    sim.set_couplings(Jnp); sim.sweep(sps, cfg.swap_interval); sim.energy()
+    sim.set_couplings(Jnp); step(); sim.energy()
     barrier()
     t0 = time.perf_counter()
     for _ in range(e2e_steps):
         sim.set_couplings(Jnp)
-        sim.sweep(sps, cfg.swap_interval)
+        if me:
+            sim.pair_couplings()
+        step()
         E = sim.energy()
     barrier()
     e2e_ms = max_over_ranks((time.perf_counter() - t0) * 1e3, world)
@@ -262,7 +284,7 @@ def run_cuda(a, cfg):
     cores = len(os.sched_getaffinity(0))
     words = min(cores, cfg.W)
     o_sweeps = max(1, int(4.0e8 / (32 * cfg.n_temps * cfg.N)))     # ~10 s per core
-    cpu_ps, cpu_wall = oracle_sample(cfg, words, o_sweeps, words)
+    cpu_ps, cpu_wall = oracle_sample(cfg, words, o_sweeps, words, a.field)
     sample = f"{words} of {cfg.W} words (32 realizations x {cfg.n_temps} temperatures each) x {o_sweeps} sweeps, {cpu_wall:.1f} s wall"
 
     out = {
@@ -271,6 +293,7 @@ def run_cuda(a, cfg):
         "dtype": "u32 bit-sliced words (32 realizations each), u32 Philox draws", "data": "synthetic",
         "config": {"workload": cfg.name, "L": cfg.L, "n_temps": cfg.n_temps, "realizations_per_gpu": cfg.R,
                    "swap_interval": cfg.swap_interval, "sweeps_per_step": sps, "seed": cfg.seed,
+                   "field": a.field, "measure_every": me,
                    "kernel": {1: "generic", 2: "resident", 3: "tiled", 4: "stream"}.get(kernel, str(kernel)),
                    "l2": "flushed between timed steps (256 MiB write); state is re-read from HBM each step",
                    "parallelism": f"shard by realization word x{world}, no collective"},
@@ -296,6 +319,9 @@ def main():
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--config", type=int, default=4)
     ap.add_argument("--sweeps-per-step", type=int, default=5000)
+    ap.add_argument("--field", type=int, default=0, help="external field h (SURVEY 8(f2)); default 0 = headline workload")
+    ap.add_argument("--measure-every", type=int, default=0,
+                    help="accumulate two-copy overlap / energy moments every M sweeps (SURVEY 8(f1)); default off")
     a = ap.parse_args()
     a.warmup = max(a.warmup, 3) if a.impl == "cuda" else a.warmup
     cfg = CONFIGS[a.config]

@@ -1133,9 +1133,13 @@ static int measure_once(ea_handle *h)
 {
     if (!h->energy_valid) { int rc = recompute_energy(h); if (rc != EA_OK) return rc; }
     if (h->M.P > 0) {
-        const int nchunk = (h->N / 4 + ea::kGatherThreads - 1) / ea::kGatherThreads;
-        ea::k_gather_by_temp<<<h->W * nchunk, ea::kGatherThreads, 4 * (size_t)h->nT * h->nT, h->stream>>>(h->P, h->d_T);
-        ea::k_overlap_words<<<h->M.P * h->nT, 128, 0, h->stream>>>(h->P, h->d_T, h->M, nullptr);
+        const int nchunk = (h->N / 4 + ea::kGatherThreads - 1) / ea::kGatherThreads, ngrp = (h->nT + 7) / 8;
+        ea::k_gather_by_temp<<<h->W * nchunk * ngrp, ea::kGatherThreads, 4 * 8 * (size_t)h->nT, h->stream>>>(h->P, h->d_T);
+        const int per_thread = 4 * ((h->N + 511) / 512), grid = h->M.P * h->nT;      // counts per thread < 2^PL
+        if (per_thread < (1 << 6)) ea::k_overlap_words<6><<<grid, 128, 0, h->stream>>>(h->P, h->d_T, h->M, nullptr);
+        else if (per_thread < (1 << 9)) ea::k_overlap_words<9><<<grid, 128, 0, h->stream>>>(h->P, h->d_T, h->M, nullptr);
+        else if (per_thread < (1 << 12)) ea::k_overlap_words<12><<<grid, 128, 0, h->stream>>>(h->P, h->d_T, h->M, nullptr);
+        else ea::k_overlap_words<15><<<grid, 128, 0, h->stream>>>(h->P, h->d_T, h->M, nullptr);
         h->launches += 2;
     }
     int grid;

@@ -25,21 +25,23 @@ struct Moments {
 //   T[t] = OR_k (spin[k] & M[k][t]),  M[k][t] = bits b with tau[32w+b][k] = t.
 // After this pass the 32 overlaps of a word pair are one XNOR + positional popcount per site,
 // although every bit of a word sits at its own temperature (R14).
-// Block = (word w, 1024 consecutive storage words); a thread owns one 128-bit vector and
-// produces the temperatures eight at a time (32 accumulator registers).
+// Block = (word w, 1024 consecutive storage words, group of eight temperature indices); a thread
+// owns one 128-bit vector: it reads the n_T slots' vectors once and produces eight outputs
+// (32 accumulator registers).
 constexpr int kGatherThreads = 256;
 
 __global__ void __launch_bounds__(kGatherThreads) k_gather_by_temp(Params P, uint32_t *T)
 {
-    extern __shared__ uint32_t sm_M[];   // [k][t]
-    const int nchunk = (P.N / 4 + kGatherThreads - 1) / kGatherThreads;
-    const int w = blockIdx.x / nchunk, chunk = blockIdx.x % nchunk;
+    extern __shared__ uint32_t sm_M[];   // [k][8]: bits of slot k at temperature index t0 + a
+    const int nchunk = (P.N / 4 + kGatherThreads - 1) / kGatherThreads, ngrp = (P.nT + 7) / 8;
+    const int w = blockIdx.x / (nchunk * ngrp), chunk = (blockIdx.x / ngrp) % nchunk, t0 = 8 * (blockIdx.x % ngrp);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     for (int k = warp; k < P.nT; k += kGatherThreads / 32) {
         const int t_mine = P.tau[(size_t)(32 * w + lane) * P.nT + k];
-        for (int t = 0; t < P.nT; ++t) {
-            const uint32_t m = __ballot_sync(0xFFFFFFFFu, t_mine == t);
-            if (lane == (t & 31)) sm_M[k * P.nT + t] = m;
+#pragma unroll
+        for (int a = 0; a < 8; ++a) {
+            const uint32_t m = __ballot_sync(0xFFFFFFFFu, t_mine == t0 + a);
+            if (lane == a) sm_M[k * 8 + a] = m;
         }
     }
     __syncthreads();
@@ -48,23 +50,21 @@ __global__ void __launch_bounds__(kGatherThreads) k_gather_by_temp(Params P, uin
     const uint4 *src = reinterpret_cast<const uint4 *>(P.spin) + (size_t)w * (P.N / 4) + v;
     uint4 *dst = reinterpret_cast<uint4 *>(T) + (size_t)w * (P.N / 4) + v;
     const size_t slot_stride = (size_t)P.W * (P.N / 4);
-    for (int t0 = 0; t0 < P.nT; t0 += 8) {
-        uint4 acc[8];
+    uint4 acc[8];
 #pragma unroll
-        for (int a = 0; a < 8; ++a) acc[a] = make_uint4(0u, 0u, 0u, 0u);
-        for (int k = 0; k < P.nT; ++k) {
-            const uint4 s = src[(size_t)k * slot_stride];
+    for (int a = 0; a < 8; ++a) acc[a] = make_uint4(0u, 0u, 0u, 0u);
+#pragma unroll 4
+    for (int k = 0; k < P.nT; ++k) {
+        const uint4 s = src[(size_t)k * slot_stride];
 #pragma unroll
-            for (int a = 0; a < 8; ++a) {
-                if (t0 + a >= P.nT) break;
-                const uint32_t m = sm_M[k * P.nT + t0 + a];
-                acc[a].x |= s.x & m; acc[a].y |= s.y & m; acc[a].z |= s.z & m; acc[a].w |= s.w & m;
-            }
+        for (int a = 0; a < 8; ++a) {
+            const uint32_t m = sm_M[k * 8 + a];      // zero for t0 + a >= nT
+            acc[a].x |= s.x & m; acc[a].y |= s.y & m; acc[a].z |= s.z & m; acc[a].w |= s.w & m;
         }
-#pragma unroll
-        for (int a = 0; a < 8; ++a)
-            if (t0 + a < P.nT) dst[(size_t)(t0 + a) * slot_stride] = acc[a];
     }
+#pragma unroll
+    for (int a = 0; a < 8; ++a)
+        if (t0 + a < P.nT) dst[(size_t)(t0 + a) * slot_stride] = acc[a];
 }
 
 // ------------------------------------------------------------------ word overlaps + moments
@@ -74,10 +74,11 @@ __global__ void __launch_bounds__(kGatherThreads) k_gather_by_temp(Params P, uin
 // realization pair (32 wa + b, 32 wb + b): this block is their only writer, so no atomics and a
 // fixed summation order.  Padding bits (index >= R) accumulate nothing.  Q (optional): the
 // overlaps of this measurement, [P][32][nT].
-constexpr int kOverlapPlanes = 15;   // per-thread count <= ceil(N / 128) <= 2^14 for L <= 128
-
+// PL = planes of the per-thread counters: per-thread count <= 4 ceil(N / 512) < 2^PL.
+template <int PL>
 __global__ void __launch_bounds__(128) k_overlap_words(Params P, const uint32_t *T, Moments M, int32_t *Q)
 {
+    constexpr int kOverlapPlanes = PL;
     __shared__ int sm_cnt[32];
     const int p = blockIdx.x / P.nT, t = blockIdx.x % P.nT;
     const int wa = M.wpairs[2 * p], wb = M.wpairs[2 * p + 1];
@@ -88,13 +89,31 @@ __global__ void __launch_bounds__(128) k_overlap_words(Params P, const uint32_t 
     uint32_t c[kOverlapPlanes];
 #pragma unroll
     for (int i = 0; i < kOverlapPlanes; ++i) c[i] = 0;
-    for (int i = threadIdx.x; i < P.N; i += blockDim.x) {
-        uint32_t x = Tb ? ~(Ta[i] ^ Tb[i]) : Ta[i];
+    // 128-bit loads, four vectors of each word in flight per thread before the first add
+    const uint4 *Va = reinterpret_cast<const uint4 *>(Ta), *Vb = reinterpret_cast<const uint4 *>(Tb);
+    const int nv = P.N / 4;
+    for (int i0 = threadIdx.x; i0 < nv; i0 += 4 * blockDim.x) {
+        uint4 xa[4], xb[4];
 #pragma unroll
-        for (int l = 0; l < kOverlapPlanes; ++l) {
-            const uint32_t carry = c[l] & x;
-            c[l] ^= x;
-            x = carry;
+        for (int u = 0; u < 4; ++u) {
+            const int i = i0 + u * blockDim.x;
+            xa[u] = i < nv ? Va[i] : make_uint4(0u, 0u, 0u, 0u);
+            xb[u] = (i < nv && Vb) ? Vb[i] : make_uint4(~0u, ~0u, ~0u, ~0u);   // all-up reference
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            // agree = ~(a ^ b); out-of-range vectors are (0, ~0): agree = 0, counts nothing
+            const uint32_t xs[4] = {~(xa[u].x ^ xb[u].x), ~(xa[u].y ^ xb[u].y), ~(xa[u].z ^ xb[u].z), ~(xa[u].w ^ xb[u].w)};
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                uint32_t x = xs[e];
+#pragma unroll
+                for (int l = 0; l < kOverlapPlanes; ++l) {
+                    const uint32_t carry = c[l] & x;
+                    c[l] ^= x;
+                    x = carry;
+                }
+            }
         }
     }
     const int lane = threadIdx.x & 31;

@@ -541,12 +541,27 @@ __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs
     uint8_t *sig8 = tau8 + 32 * nT;                                  // [32][nT]
 
     // ---- load state: lattices of my slots, tables, permutation of my 32 realizations
-    for (int k = 0; k < nk; ++k) {
-        const uint4 *src = reinterpret_cast<const uint4 *>(P.spin + ((size_t)(k0 + k) * P.W + w) * N);
-        uint4 *dst = reinterpret_cast<uint4 *>(sp + (size_t)k * N);
-        for (int a = tid; a < N / 4; a += NT) dst[a] = src[a];
-        for (int a = tid; a < LTS; a += NT) lt[k * LTS + a] = P.lt[((size_t)w * nT + k0 + k) * LTS + a];
+    {   // lattices: eight independent 128-bit loads in flight per thread before the first store
+        // (one load per round trip cost ~25 us per launch when the state comes from HBM)
+        constexpr int VL = N / 4;
+        const int total = nk * VL;
+        for (int base = 0; base < total; base += 8 * NT) {
+            uint4 v[8];
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                const int e = base + u * NT + tid;
+                if (e < total)
+                    v[u] = reinterpret_cast<const uint4 *>(P.spin + ((size_t)(k0 + e / VL) * P.W + w) * N)[e % VL];
+            }
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                const int e = base + u * NT + tid;
+                if (e < total) reinterpret_cast<uint4 *>(sp)[e] = v[u];
+            }
+        }
     }
+    for (int k = 0; k < nk; ++k)
+        for (int a = tid; a < LTS; a += NT) lt[k * LTS + a] = P.lt[((size_t)w * nT + k0 + k) * LTS + a];
     for (int a = tid; a < 3 * LTS; a += NT) thr[a] = P.thr32[a];
     for (int a = tid; a < A.n_bucket; a += NT) bucket[a] = A.bucket[a];
     for (int a = tid; a < 32 * nT; a += NT) {
