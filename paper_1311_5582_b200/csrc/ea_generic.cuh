@@ -61,14 +61,10 @@ __global__ void k_build_lt(Params P)
 // ------------------------------------------------------------------ a2-a7: generic half-sweep
 // One thread per (slot k, word w, quad q): four sites, one Philox call
 // PX(g, q, w, (p<<16)|k) (R17).  Global memory only; any even L.
-__global__ void __launch_bounds__(128) k_half_sweep_generic(Params P, int p, uint32_t g)
+// work item `tid` in [0, nT W Nh/4) of the zero-field half-sweep; sm_thr = smem copy of thr32
+__device__ __forceinline__ void half_sweep_item(const Params &P, int p, uint32_t g, int64_t tid, const uint32_t *sm_thr)
 {
-    extern __shared__ uint32_t sm_thr[];   // [3][nT+1]
-    for (int a = threadIdx.x; a < 3 * P.LTS; a += blockDim.x) sm_thr[a] = P.thr32[a];
-    __syncthreads();
     const int nq = P.Nh >> 2;
-    const int64_t tid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (tid >= (int64_t)P.nT * P.W * nq) return;
     const int q = (int)(tid % nq);
     const int w = (int)((tid / nq) % P.W);
     const int k = (int)(tid / ((int64_t)nq * P.W));
@@ -90,19 +86,25 @@ __global__ void __launch_bounds__(128) k_half_sweep_generic(Params P, int p, uin
     }
 }
 
+__global__ void __launch_bounds__(128) k_half_sweep_generic(Params P, int p, uint32_t g)
+{
+    extern __shared__ uint32_t sm_thr[];   // [3][nT+1]
+    for (int a = threadIdx.x; a < 3 * P.LTS; a += blockDim.x) sm_thr[a] = P.thr32[a];
+    __syncthreads();
+    const int64_t tid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (tid >= (int64_t)P.nT * P.W * (P.Nh >> 2)) return;
+    half_sweep_item(P, p, g, tid, sm_thr);
+}
+
 // ------------------------------------------------------------------ f2: half-sweep with a field
 // H = -sum J s s + h sum s (Eq. 1; R21): dE = 4 n_sat - 12 - 2 h s_i, so the
 // acceptance class of a bit is (n_sat, s_i): the paper's 14 table columns.  Per
 // class one rank search and one rank mask; classes with dE <= 0 always flip.  Same thread
 // mapping and draws as k_half_sweep_generic.
-__global__ void __launch_bounds__(128) k_half_sweep_field(Params P, int p, uint32_t g)
+__device__ __forceinline__ void half_sweep_field_item(const Params &P, int p, uint32_t g, int64_t tid,
+                                                      const uint32_t *sm_thr)
 {
-    extern __shared__ uint32_t sm_thr[];   // [14][nT+1]
-    for (int a = threadIdx.x; a < 14 * P.LTS; a += blockDim.x) sm_thr[a] = P.thrF[a];
-    __syncthreads();
     const int nq = P.Nh >> 2;
-    const int64_t tid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (tid >= (int64_t)P.nT * P.W * nq) return;
     const int q = (int)(tid % nq);
     const int w = (int)((tid / nq) % P.W);
     const int k = (int)(tid / ((int64_t)nq * P.W));
@@ -131,14 +133,24 @@ __global__ void __launch_bounds__(128) k_half_sweep_field(Params P, int p, uint3
     }
 }
 
+__global__ void __launch_bounds__(128) k_half_sweep_field(Params P, int p, uint32_t g)
+{
+    extern __shared__ uint32_t sm_thr[];   // [14][nT+1]
+    for (int a = threadIdx.x; a < 14 * P.LTS; a += blockDim.x) sm_thr[a] = P.thrF[a];
+    __syncthreads();
+    const int64_t tid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (tid >= (int64_t)P.nT * P.W * (P.Nh >> 2)) return;
+    half_sweep_field_item(P, p, g, tid, sm_thr);
+}
+
 // Field term of the energy: E[r][k] += h * (2 * (number of up spins) - N).  One block per (w, k),
 // vertical counters like k_energy; runs after it.
 constexpr int kFieldPlanes = 15;   // per-thread count <= ceil(N / 128) <= 2^14
 
-__global__ void __launch_bounds__(128) k_field_energy(Params P)
+// item = (w, k) handled by the whole block; sm_cnt = 32 ints of shared memory
+__device__ __forceinline__ void field_energy_item(const Params &P, int item, int *sm_cnt)
 {
-    __shared__ int sm_cnt[32];
-    const int w = blockIdx.x / P.nT, k = blockIdx.x % P.nT;
+    const int w = item / P.nT, k = item % P.nT;
     const uint32_t *sp = P.spin + ((size_t)k * P.W + w) * P.N;
     if (threadIdx.x < 32) sm_cnt[threadIdx.x] = 0;
     __syncthreads();
@@ -167,6 +179,13 @@ __global__ void __launch_bounds__(128) k_field_energy(Params P)
     __syncthreads();
     if (threadIdx.x < 32)
         P.E[(size_t)(32 * w + threadIdx.x) * P.nT + k] += P.h * (2 * sm_cnt[threadIdx.x] - P.N);
+    __syncthreads();
+}
+
+__global__ void __launch_bounds__(128) k_field_energy(Params P)
+{
+    __shared__ int sm_cnt[32];
+    field_energy_item(P, blockIdx.x, sm_cnt);
 }
 
 // ------------------------------------------------------------------ a8: energy from scratch
@@ -186,10 +205,9 @@ __device__ __forceinline__ void vadd(uint32_t (&c)[kEnergyPlanes], uint32_t x, i
     }
 }
 
-__global__ void __launch_bounds__(128) k_energy(Params P)
+__device__ __forceinline__ void energy_item(const Params &P, int item, int *sm_cnt)
 {
-    __shared__ int sm_cnt[32];
-    const int w = blockIdx.x / P.nT, k = blockIdx.x % P.nT;
+    const int w = item / P.nT, k = item % P.nT;
     const uint32_t *sp = P.spin + ((size_t)k * P.W + w) * P.N;
     const uint32_t *cp = P.coup + (size_t)w * 3 * P.N;
     if (threadIdx.x < 32) sm_cnt[threadIdx.x] = 0;
@@ -217,6 +235,13 @@ __global__ void __launch_bounds__(128) k_energy(Params P)
     __syncthreads();
     if (threadIdx.x < 32)
         P.E[(size_t)(32 * w + threadIdx.x) * P.nT + k] = 3 * P.N - 2 * sm_cnt[threadIdx.x];
+    __syncthreads();
+}
+
+__global__ void __launch_bounds__(128) k_energy(Params P)
+{
+    __shared__ int sm_cnt[32];
+    energy_item(P, blockIdx.x, sm_cnt);
 }
 
 // ------------------------------------------------------------------ a9: PT swap round
@@ -233,9 +258,9 @@ __device__ __forceinline__ bool swap_accept(const Params &P, int t, int m, uint3
 
 // One block per word: lane = realization bit, warps stride over the disjoint pairs of this
 // round (R4); then the rank masks of the word are rebuilt.  No lattice word moves.
-__global__ void __launch_bounds__(256) k_pt_swap(Params P, uint32_t g_done, uint32_t round)
+__device__ __forceinline__ void pt_swap_word(const Params &P, int w, uint32_t g_done, uint32_t round)
 {
-    const int w = blockIdx.x, lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
     const int r = 32 * w + lane;
     uint8_t *sg = P.sigma + (size_t)r * P.nT, *ta = P.tau + (size_t)r * P.nT;
     const int32_t *E = P.E + (size_t)r * P.nT;
@@ -250,6 +275,74 @@ __global__ void __launch_bounds__(256) k_pt_swap(Params P, uint32_t g_done, uint
     }
     __syncthreads();
     for (int k = warp; k < P.nT; k += nwarp) build_lt_row(P, w, k, lane);
+}
+
+__global__ void __launch_bounds__(256) k_pt_swap(Params P, uint32_t g_done, uint32_t round)
+{
+    pt_swap_word(P, blockIdx.x, g_done, round);
+}
+
+// ------------------------------------------------------------------ persistent generic path
+// All sweeps of a call in ONE cooperative launch for lattices that have no shared-memory path
+// (L = 2, 4, 6, 12, ... and every L with a field): the same work items as the kernels above,
+// dealt out grid-stride, with a grid-wide barrier where the one-launch-per-step path has a
+// kernel boundary.  For the small configs (1 and 3) the step time was launch latency (3-4
+// launches of ~7 us per sweep); the barrier costs about 1 us.
+struct PersistArgs {
+    Params P;
+    uint32_t g0;          // global index of the first sweep of this call
+    int n_sweeps;
+    int swap_interval;
+    uint32_t nswap0;      // swap rounds done before this call
+    unsigned int *gbar;   // grid barrier word, zero before the launch
+};
+
+__device__ __forceinline__ void persist_grid_sync(unsigned int *bar)
+{
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const unsigned int add = blockIdx.x == 0 ? 0x80000000u - (gridDim.x - 1) : 1u;
+        __threadfence();
+        const unsigned int old = atomicAdd(bar, add);
+        while ((((old ^ *reinterpret_cast<volatile unsigned int *>(bar)) & 0x80000000u) == 0u)) { }
+        __threadfence();
+    }
+    __syncthreads();
+}
+
+template <bool FIELD>
+__global__ void __launch_bounds__(256) k_generic_persistent(const PersistArgs A)
+{
+    extern __shared__ uint32_t sm_thr[];   // [3 or 14][nT+1]
+    __shared__ int sm_cnt[32];
+    const Params &P = A.P;
+    const int ncls = FIELD ? 14 : 3;
+    for (int a = threadIdx.x; a < ncls * P.LTS; a += blockDim.x) sm_thr[a] = FIELD ? P.thrF[a] : P.thr32[a];
+    __syncthreads();
+    const int64_t n_items = (int64_t)P.nT * P.W * (P.Nh >> 2);
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    uint32_t nswap = A.nswap0;
+    for (int it = 0; it < A.n_sweeps; ++it) {
+        const uint32_t g = A.g0 + (uint32_t)it;
+        for (int p = 0; p < 2; ++p) {
+            for (int64_t tid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; tid < n_items; tid += stride) {
+                if (FIELD) half_sweep_field_item(P, p, g, tid, sm_thr);
+                else half_sweep_item(P, p, g, tid, sm_thr);
+            }
+            persist_grid_sync(A.gbar);
+        }
+        const bool swap_now = A.swap_interval > 0 && ((uint64_t)g + 1) % (uint64_t)A.swap_interval == 0;
+        if (!swap_now && it != A.n_sweeps - 1) continue;
+        for (int item = blockIdx.x; item < P.W * P.nT; item += gridDim.x) {   // energies of the finished sweep
+            energy_item(P, item, sm_cnt);
+            if (FIELD) field_energy_item(P, item, sm_cnt);
+        }
+        if (!swap_now) continue;
+        persist_grid_sync(A.gbar);
+        for (int w = blockIdx.x; w < P.W; w += gridDim.x) pt_swap_word(P, w, g, nswap & 1u);
+        ++nswap;
+        persist_grid_sync(A.gbar);
+    }
 }
 
 // ------------------------------------------------------------------ a10: overlap

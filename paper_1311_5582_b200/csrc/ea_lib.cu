@@ -616,8 +616,54 @@ extern "C" int ea_get_field_tables(ea_handle *h, uint64_t *accf, uint64_t *swpf)
 }
 
 // ---------------------------------------------------------------- sweep
+// One cooperative launch for all sweeps of the call (k_generic_persistent).  Returns
+// cudaErrorCooperativeLaunchTooLarge / NotSupported style errors to the caller, which then falls
+// back to one launch per step.
+static cudaError_t launch_generic_persistent(ea_handle *h, int n_sweeps, int swap_interval)
+{
+    int coop = 0, dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
+    if (!coop) return cudaErrorNotSupported;
+    const void *kern = h->field ? (const void *)ea::k_generic_persistent<true> : (const void *)ea::k_generic_persistent<false>;
+    const size_t smem = 4 * (h->field ? 14 : 3) * (size_t)(h->nT + 1);
+    int per_sm = 0;
+    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, 256, smem);
+    if (e != cudaSuccess) return e;
+    if (per_sm < 1) return cudaErrorCooperativeLaunchTooLarge;
+    // Only problems whose work items all get a thread of their own (one wave): these are the
+    // launch-latency-bound ones.  Larger problems are throughput-bound and run faster with one
+    // launch per step (measured on config 4 with a field: 1.46 against 1.85 ps per attempt).
+    const int64_t n_items = (int64_t)h->nT * h->W * (h->N / 8);
+    if ((n_items + 255) / 256 > (int64_t)per_sm * h->sm_count) return cudaErrorCooperativeLaunchTooLarge;
+    const int64_t want = std::max<int64_t>((n_items + 255) / 256, std::min<int64_t>((int64_t)h->W * h->nT, h->sm_count));
+    const int grid = (int)std::min<int64_t>(want, (int64_t)per_sm * h->sm_count);
+    ea::PersistArgs A{};
+    A.P = h->P; A.g0 = (uint32_t)h->g; A.n_sweeps = n_sweeps; A.swap_interval = swap_interval;
+    A.nswap0 = (uint32_t)h->nswap;
+    A.gbar = (unsigned int *)(h->d_Ecnt + 2 * (size_t)h->Rp * h->nT);
+    e = cudaMemsetAsync(A.gbar, 0, 4, h->stream);
+    if (e != cudaSuccess) return e;
+    void *args[] = {(void *)&A};
+    return cudaLaunchCooperativeKernel(kern, dim3((unsigned)grid), dim3(256), args, smem, h->stream);
+}
+
 static int sweep_generic(ea_handle *h, int64_t n_sweeps, int swap_interval)
 {
+    // persistent path first (EA_GENERIC_STEPWISE=1 forces the one-launch-per-step path: tests)
+    const char *stepwise = std::getenv("EA_GENERIC_STEPWISE");
+    while (n_sweeps > 0 && !(stepwise && stepwise[0] == '1')) {
+        const int chunk = (int)std::min<int64_t>(n_sweeps, 1 << 30);
+        const cudaError_t e = launch_generic_persistent(h, chunk, swap_interval);
+        if (e == cudaErrorCooperativeLaunchTooLarge || e == cudaErrorNotSupported) { cudaGetLastError(); break; }
+        if (e != cudaSuccess) return fail(h, EA_ERR_CUDA, std::string("generic persistent launch: ") + cudaGetErrorString(e));
+        h->launches++;
+        if (swap_interval > 0) h->nswap += (h->g + (uint64_t)chunk) / (uint64_t)swap_interval - h->g / (uint64_t)swap_interval;
+        h->g += (uint64_t)chunk;
+        h->energy_valid = true;       // the last sweep of a launch always ends with the energies
+        n_sweeps -= chunk;
+    }
+    if (n_sweeps == 0) return EA_OK;
     const int64_t nthreads = (int64_t)h->nT * h->W * (h->N / 8);
     int grid;
     launch_cfg(nthreads, 128, grid);

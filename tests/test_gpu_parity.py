@@ -194,3 +194,35 @@ def test_auto_picks_resident_for_L16():
     g = EA(32, 4, 32, np.array([1.0, 0.9, 0.8, 0.7]), 1)
     assert g.get_kernel() == 4
     g.destroy()
+
+
+@pytest.mark.parametrize("L,nT,R,swap,ns,h", [
+    (4, 16, 1, 1, 60, 0),          # config 1 shape
+    (12, 20, 64, 2, 7, 0),         # config 3 shape; the call ends between two swap rounds
+    (6, 5, 33, 3, 10, 0),
+    (16, 6, 64, 1, 4, 0),          # 6144 work items: still one wave
+    (16, 24, 640, 1, 5, 0),        # more work items than one wave: stepwise launches either way
+    (4, 6, 40, 1, 9, 2),           # with a field
+])
+def test_generic_stepwise_launches_equal_the_persistent_kernel(monkeypatch, L, nT, R, swap, ns, h):
+    """EA_KERNEL_GENERIC runs as one cooperative launch per call (k_generic_persistent); if that
+    launch is impossible it falls back to one launch per half-sweep / energy / swap round.
+    EA_GENERIC_STEPWISE=1 forces the fall-back: both must follow the oracle."""
+    betas = 1.0 / temperature_ladder(nT, 0.6, 2.2)
+    for stepwise in ("0", "1"):
+        monkeypatch.setenv("EA_GENERIC_STEPWISE", stepwise)
+        g, o = _pair(L, nT, R, betas, 77, 1)
+        if h:
+            g.set_field(h); o.set_field(h)
+        n0 = g.launch_count()
+        done = 0
+        for chunk in (1, ns - 3, 2):
+            g.sweep(chunk, swap); o.sweep(chunk, swap); done += chunk
+            _assert_same(g, o, f"stepwise={stepwise} after {done} sweeps")
+        launches = g.launch_count() - n0
+        if stepwise == "0":
+            if nT * ((R + 31) // 32) * (L ** 3 // 8) <= 148 * 256:    # one wave: persistent launch
+                assert launches <= 3 + 3 * 2      # one sweep launch per call (+ lazily recomputed energies)
+        else:
+            assert launches >= 2 * ns
+        g.destroy()
