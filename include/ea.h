@@ -163,6 +163,13 @@ int ea_get_moments(ea_handle *h, uint64_t *n_meas, int64_t *q1 /* [P][32][n_temp
                    uint64_t *q2 /* [P][32][n_temps] */, uint64_t *q4 /* [P][32][n_temps][2] */,
                    int64_t *e1 /* [R][n_temps] */, uint64_t *e2 /* [R][n_temps] */);
 
+/* Round trips in temperature space, the parallel-tempering diagnostic behind "the choice of
+ * temperatures is crucial", observed at the measurements of the series: a replica
+ * that is at temperature index 0 after having been at index n_temps-1 completes one round trip
+ * (R22).  trips[r] = round trips completed by the n_temps replicas of realization r
+ * since ea_measure_begin. */
+int ea_get_round_trips(ea_handle *h, uint64_t *trips /* [R] */);
+
 /* Binder ratio by temperature index, g[t] = (3 - [<q^4>] / [<q^2>]^2) / 2: <.> = average over the
  * measurements of one realization pair, [.] = average over the series' valid realization pairs
  * (disorder average).  Computed on the host from the integer sums in long double; agrees with

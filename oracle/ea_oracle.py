@@ -263,8 +263,28 @@ class Oracle:
                     acc["e1"][r, t] += e
                     acc["e2"][r, t] += e * e
             acc["n"] += 1
+            round_trip_update(acc.setdefault("label", np.zeros((self.R, self.nT), dtype=np.int8)),
+                              acc.setdefault("trips", np.zeros(self.R, dtype=np.int64)), self.perm()[0])
         acc["valid"] = np.array([[pr is not None for pr in row] for row in rp], dtype=bool).reshape(P, 32)
         return acc
+
+
+def round_trip_update(label, trips, tau):
+    """Round trips of the replicas in temperature space (the diagnostic behind "the choice of
+    temperatures is crucial"), observed at measurement times.  tau[r][k] = temperature
+    index of the replica in slot k.  label[r][k]: 0 = has not touched an end yet, 1 = was last at
+    temperature index 0, 2 = was last at index nT-1.  A replica that comes back to index 0 after
+    having been at nT-1 completes one round trip of its realization (R22)."""
+    R, nT = tau.shape
+    for r in range(R):
+        for k in range(nT):
+            t = int(tau[r, k])
+            if t == 0:
+                if label[r, k] == 2:
+                    trips[r] += 1
+                label[r, k] = 1
+            elif t == nT - 1:
+                label[r, k] = 2
 
 
 def binder_ratio(acc):

@@ -1143,6 +1143,7 @@ extern "C" int ea_measure_begin(ea_handle *h, const int32_t *word_pairs, int n_w
     const size_t o_pairs = take(8 * (size_t)(n_word_pairs ? n_word_pairs : 1));
     const size_t o_q1 = take(8 * nq), o_q2 = take(8 * nq), o_q4 = take(16 * nq);
     const size_t o_e1 = take(8 * ne), o_e2 = take(8 * ne);
+    const size_t o_label = take(ne), o_trips = take(8 * (size_t)h->R);
     char *d = nullptr;
     if (cudaMalloc((void **)&d, off) != cudaSuccess) {
         cudaGetLastError();
@@ -1169,6 +1170,8 @@ extern "C" int ea_measure_begin(ea_handle *h, const int32_t *word_pairs, int n_w
     h->M.q4 = (uint64_t *)(d + o_q4);
     h->M.e1 = (int64_t *)(d + o_e1);
     h->M.e2 = (uint64_t *)(d + o_e2);
+    h->M.label = (uint8_t *)(d + o_label);
+    h->M.trips = (unsigned long long *)(d + o_trips);
     h->meas_n = 0;
     h->meas_on = true;
     return EA_OK;
@@ -1230,6 +1233,15 @@ extern "C" int ea_get_moments(ea_handle *h, uint64_t *n_meas, int64_t *q1, uint6
     if (e2) CUDA_TRY(h, cudaMemcpyAsync(e2, h->M.e2, 8 * ne, cudaMemcpyDeviceToHost, h->stream));
     CUDA_TRY(h, cudaStreamSynchronize(h->stream));
     if (n_meas) *n_meas = h->meas_n;
+    return EA_OK;
+}
+
+extern "C" int ea_get_round_trips(ea_handle *h, uint64_t *trips)
+{
+    if (!h || !trips) return fail(h, EA_ERR_INVALID_ARG, "ea_get_round_trips: null argument");
+    if (!h->meas_on) return fail(h, EA_ERR_INVALID_ARG, "ea_get_round_trips: call ea_measure_begin first");
+    CUDA_TRY(h, cudaMemcpyAsync(trips, h->M.trips, 8 * (size_t)h->R, cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
     return EA_OK;
 }
 

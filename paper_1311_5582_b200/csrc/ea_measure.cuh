@@ -17,6 +17,8 @@ struct Moments {
     uint64_t *q4;            // [P][32][nT][2]  sum q^4, 128 bit: (low, high)
     int64_t *e1;             // [R][nT]  sum E by temperature index
     uint64_t *e2;            // [R][nT]  sum E^2
+    uint8_t *label;          // [R][nT]  by slot: 0 no end touched yet, 1 last at index 0, 2 last at nT-1
+    unsigned long long *trips;   // [R]  completed round trips 0 -> nT-1 -> 0 of the realization's replicas
 };
 
 // ------------------------------------------------------------------ gather by temperature
@@ -143,7 +145,9 @@ __global__ void __launch_bounds__(128) k_overlap_words(Params P, const uint32_t 
     M.q4[2 * o + 1] += hi + (old + lo < old ? 1u : 0u);
 }
 
-// sum E and sum E^2 by temperature index; one thread per (r, t).
+// sum E and sum E^2 by temperature index, and the round-trip bookkeeping of the replica in
+// slot k = t (R22: a replica that is back at temperature index 0 after having been at
+// nT-1 completes a round trip; observed at measurement times).  One thread per (r, t).
 __global__ void k_accum_energy(Params P, Moments M)
 {
     const int tid = blockIdx.x * blockDim.x + threadIdx.x;
@@ -152,6 +156,13 @@ __global__ void k_accum_energy(Params P, Moments M)
     const int64_t e = P.E[(size_t)r * P.nT + P.sigma[(size_t)r * P.nT + t]];
     M.e1[tid] += e;
     M.e2[tid] += (uint64_t)(e * e);
+    const int at = P.tau[tid];            // temperature index of the replica in slot t
+    if (at == 0) {
+        if (M.label[tid] == 2) atomicAdd(&M.trips[r], 1ull);
+        M.label[tid] = 1;
+    } else if (at == P.nT - 1) {
+        M.label[tid] = 2;
+    }
 }
 
 // ------------------------------------------------------------------ coupling export

@@ -30,6 +30,8 @@ def _compare(g, acc, binder_ratio):
     assert m["n"] == acc["n"]
     for k in ("q1", "q2", "q4", "e1", "e2"):
         assert (m[k] == acc[k]).all(), k
+    if "trips" in acc:
+        assert (g.get_round_trips().astype(np.int64) == acc["trips"]).all(), "round trips"
     gb, ob = g.get_binder(), binder_ratio(acc)
     assert (np.isnan(gb) == np.isnan(ob)).all()
     ok = ~np.isnan(ob)
@@ -120,4 +122,27 @@ def test_measure_errors_leave_state_unchanged():
     assert e.value.code == -4
     st = g.get_state()
     assert st["sweeps"] == 0 and g.get_moments()["n"] == 0
+    g.destroy()
+
+
+def test_round_trips_match_oracle_and_the_transposition_network():
+    pkg, Oracle, binder_ratio = _mods()
+    # a ladder narrow enough for replicas to travel, measured after every sweep
+    L, nT, R = 4, 6, 70
+    betas = 1.0 / temperature_ladder(nT, 1.6, 2.4)
+    g = pkg.EA(L, nT, R, betas, 12)
+    o = Oracle(L, nT, R, betas, 12)
+    g.measure_begin([])
+    g.measure(300, 1, 1)
+    acc = o.measure(300, 1, 1, [])
+    trips = g.get_round_trips().astype(np.int64)
+    assert (trips == acc["trips"]).all() and trips.sum() > 0
+    assert np.isnan(g.get_binder()).all()                    # a series without pairs
+    g.destroy()
+    # equal betas: every swap accepted, 61 rounds of the odd-even transposition network
+    g = pkg.EA(2, 6, 3, np.full(6, 0.7), 9, kernel=1)
+    o = Oracle(2, 6, 3, np.full(6, 0.7), 9)
+    g.measure_begin([])
+    g.measure(61, 1, 1)
+    assert (g.get_round_trips().astype(np.int64) == o.measure(61, 1, 1, [])["trips"]).all()
     g.destroy()

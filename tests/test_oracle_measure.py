@@ -141,3 +141,50 @@ def test_binder_formula_on_synthetic_sums():
     two = {"n": 2, "valid": np.ones((1, 1), dtype=bool),
            "q2": np.array([[[10]]], dtype=object), "q4": np.array([[[82]]], dtype=object)}
     assert binder_ratio(two)[0] == float((3 - Fraction(41, 25)) / 2)
+
+
+def test_round_trip_update_by_hand():
+    """One replica (slot 0 of realization 0) walking 0 1 2 1 0 1 2 2 1 0 over three temperature
+    indices completes two round trips; the other slots are parked in the middle."""
+    from oracle import round_trip_update
+    walk = [0, 1, 2, 1, 0, 1, 2, 2, 1, 0]
+    label = np.zeros((1, 3), dtype=np.int8)
+    trips = np.zeros(1, dtype=np.int64)
+    seen = []
+    for t in walk:
+        round_trip_update(label, trips, np.array([[t, 1, 1]]))
+        seen.append(int(trips[0]))
+    assert seen == [0, 0, 0, 0, 1, 1, 1, 1, 1, 2]
+    assert label[0, 1] == 0 and label[0, 2] == 0             # never touched an end
+    # starting at the far end counts as well; starting at index 0 needs a visit to the far end first
+    label[:] = 0; trips[:] = 0
+    for t in (2, 1, 0, 0, 1, 2, 0):
+        round_trip_update(label, trips, np.array([[t, 1, 1]]))
+    assert trips[0] == 2
+
+
+def test_round_trips_of_the_odd_even_transposition_network():
+    """Equal betas: every swap is accepted (threshold 2^32), so parallel tempering is the
+    odd-even transposition network: every replica moves one index per round and turns at the
+    ends.  An independent simulation of that network gives the expected round-trip counts."""
+    L, nT, R, rounds = 2, 6, 3, 61
+    o = Oracle(L, nT, R, np.full(nT, 0.7), 9)
+    acc = o.measure(rounds, 1, 1, [])
+    assert o.counters()["swap_accepted"] == o.counters()["swap_attempts"] > 0
+    pos = list(range(nT))                                    # pos[k] = temperature index of slot k
+    label, trips = [0] * nT, 0
+    for n in range(rounds):
+        at = {t: k for k, t in enumerate(pos)}
+        for t in range(n & 1, nT - 1, 2):                    # round n pairs (t, t+1), t = n & 1, ...
+            a, b = at[t], at[t + 1]
+            pos[a], pos[b] = t + 1, t
+        for k in range(nT):
+            if pos[k] == 0:
+                trips += label[k] == 2
+                label[k] = 1
+            elif pos[k] == nT - 1:
+                label[k] = 2
+    assert trips > 0 and (acc["trips"] == trips).all()
+    # without parallel tempering nobody moves
+    o = Oracle(L, nT, R, 1.0 / np.linspace(0.5, 2.0, nT), 9)
+    assert (o.measure(20, 1, 0, [])["trips"] == 0).all()
