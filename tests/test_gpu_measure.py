@@ -146,3 +146,15 @@ def test_round_trips_match_oracle_and_the_transposition_network():
     g.measure(61, 1, 1)
     assert (g.get_round_trips().astype(np.int64) == o.measure(61, 1, 1, [])["trips"]).all()
     g.destroy()
+
+
+def test_binder_convergence_example_runs_and_orders_temperatures():
+    """The Fig. 21 example in a short version: with PT the cold Binder ratio of the
+    late window is large, the hot one small, and g falls with temperature."""
+    _mods()
+    from paper_1311_5582_b200.examples.binder_convergence import run
+    windows, g = run(L=4, pairs=256, n_temps=8, max_log2=11, min_log2=8, swap_interval=1)
+    assert windows == [(256, 512), (512, 1024), (1024, 2048)] and g.shape == (3, 8)
+    assert np.isfinite(g).all() and (g <= 1.0).all()
+    assert g[-1, 0] > 0.8 and g[-1, -1] < 0.5
+    assert (np.diff(g[-1]) < 0.02).all()
