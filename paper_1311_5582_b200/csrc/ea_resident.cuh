@@ -576,10 +576,14 @@ __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs
         swm[4 * t] = P.swp_lo[t]; swm[4 * t + 1] = P.swp_cnt[t]; swm[4 * t + 2] = P.swp_off[t];
         swm[4 * t + 3] = (int)P.swp_kind[2 * t] | ((int)P.swp_kind[2 * t + 1] << 1);
     }
-    for (int a = tid; a < (nT - 1) * SW; a += NT) {         // window m = -SW + i of row t
+    __syncthreads();                                        // swm is complete
+    // window m = -SW + i of row t: range constants from shared memory, so that the global loads
+    // of the iterations are independent (they were three dependent round trips each: ~12 us)
+#pragma unroll 4
+    for (int a = tid; a < (nT - 1) * SW; a += NT) {
         const int t = a / SW, m = -SW + a % SW;
-        const int lo = P.swp_lo[t], cnt = P.swp_cnt[t];
-        swwin[a] = (m >= lo && m < lo + cnt) ? P.swp_val[P.swp_off[t] + (m - lo)] : 0u;
+        const int lo = swm[4 * t], cnt = swm[4 * t + 1];
+        swwin[a] = (m >= lo && m < lo + cnt) ? P.swp_val[swm[4 * t + 2] + (m - lo)] : 0u;
     }
 
     // ---- per-thread geometry and couplings (registers, both parities)

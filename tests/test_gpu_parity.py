@@ -61,6 +61,10 @@ def _skip_unsupported(kernel, L):
     (64, 3, 33, 1, 2),         # L = 64: one-plane slabs in the streaming kernel, odd n_temps
     (32, 64, 32, 1, 2),        # the most temperatures the library takes
     (16, 64, 5, 2, 3),         # 64 temperatures in the resident kernel (cluster of 8)
+    (8, 1, 33, 1, 5),          # a single temperature: swap rounds have no pair
+    (16, 2, 32, 1, 4),         # two temperatures: only even rounds have a pair
+    (32, 1, 32, 1, 2),
+    (4, 1, 1, 1, 7),           # the smallest problem the library takes besides L = 2
 ])
 def test_trajectory_matches_oracle(kernel, L, nT, R, swap, ns):
     _skip_unsupported(kernel, L)
