@@ -244,13 +244,21 @@ class Oracle:
         if acc is None:
             z = lambda *shape: np.zeros(shape, dtype=object) + 0
             acc = {"n": 0, "q1": z(P, 32, self.nT), "q2": z(P, 32, self.nT), "q4": z(P, 32, self.nT),
-                   "e1": z(self.R, self.nT), "e2": z(self.R, self.nT)}
+                   "e1": z(self.R, self.nT), "e2": z(self.R, self.nT), "corr": z(P, 32, self.nT, self.L)}
         flat = [(p, b, pr) for p in range(P) for b, pr in enumerate(rp[p]) if pr is not None]
         pairs = np.array([pr for _, _, pr in flat], dtype=np.int32).reshape(-1, 2)
         for _ in range(int(n_meas)):
             self.sweep(sweeps_between, swap_interval)
             Q = self.overlap(pairs) if len(flat) else np.zeros((0, self.nT), dtype=np.int32)
             E = self.energy()
+            if len(flat):
+                s = self.spins()                     # [r][t][site], by temperature index
+                for p, b, (ra, rb) in flat:
+                    for t in range(self.nT):
+                        qf = s[ra, t].astype(np.int64) * (s[rb, t].astype(np.int64) if rb >= 0 else 1)
+                        c = plane_correlation(qf, self.L)
+                        for d in range(self.L):
+                            acc["corr"][p, b, t, d] += int(c[d])
             for (p, b, _), qrow in zip(flat, Q):
                 for t in range(self.nT):
                     q = int(qrow[t])
@@ -267,6 +275,42 @@ class Oracle:
                               acc.setdefault("trips", np.zeros(self.R, dtype=np.int64)), self.perm()[0])
         acc["valid"] = np.array([[pr is not None for pr in row] for row in rp], dtype=bool).reshape(P, 32)
         return acc
+
+
+def plane_correlation(q_field, L):
+    """C(d) = sum over the three axes mu and the planes p of S_mu(p) S_mu((p + d) mod L), where
+    S_mu(p) = sum of the local overlaps q_i = s_i^a s_i^b over the plane (coordinate mu of i) = p.
+    q_field[site], site = x + L (y + L z).  These plane sums are all the wave-vector dependent
+    susceptibility along the axes needs (R23); sum_d C(d) = 3 q^2."""
+    f = np.asarray(q_field, dtype=np.int64).reshape(L, L, L)         # [z][y][x]
+    C = np.zeros(L, dtype=np.int64)
+    for axes in ((0, 1), (0, 2), (1, 2)):                             # planes of fixed x, y, z
+        S = f.sum(axis=axes)
+        for d in range(L):
+            C[d] += int((S * np.roll(S, -d)).sum())                   # roll(S, -d)[p] = S[(p + d) mod L]
+    return C
+
+
+def correlation_length(acc, L):
+    """Second-moment correlation length by temperature index (the quantity of the paper's
+    Fig. 19, which prints no formula; R23):
+      chi(k) = [<|q~(k)|^2>] / N averaged over the three axes = sum_d cos(k d) [<C(d)>] / (3 N),
+      xi = sqrt(chi(0) / chi(k_min) - 1) / (2 sin(k_min / 2)),  k_min = 2 pi / L.
+    Exact integer sums, the cosines in double; NaN where chi(k_min) <= 1e-12 chi(0), where
+    chi(0) < chi(k_min), or where nothing was measured."""
+    import math
+    valid = acc["valid"]
+    nT = acc["corr"].shape[2]
+    xi = np.full(nT, np.nan)
+    if acc["n"] == 0 or not valid.any():
+        return xi
+    for t in range(nT):
+        Cd = [sum(int(v) for v in acc["corr"][valid, t, d]) for d in range(L)]
+        chi0 = float(sum(Cd))
+        chik = sum(math.cos(2.0 * math.pi * d / L) * float(Cd[d]) for d in range(L))
+        if chik > 1e-12 * chi0 and chi0 >= chik:     # chi(k_min) = 0 up to rounding: undefined
+            xi[t] = math.sqrt(chi0 / chik - 1.0) / (2.0 * math.sin(math.pi / L))
+    return xi
 
 
 def round_trip_update(label, trips, tau):

@@ -188,3 +188,61 @@ def test_round_trips_of_the_odd_even_transposition_network():
     # without parallel tempering nobody moves
     o = Oracle(L, nT, R, 1.0 / np.linspace(0.5, 2.0, nT), 9)
     assert (o.measure(20, 1, 0, [])["trips"] == 0).all()
+
+
+def test_plane_correlation_against_fourier_transform_and_closed_forms():
+    """C(d) must reproduce |q~(k)|^2 summed over the three axes for every k = 2 pi m / L (a direct
+    complex Fourier sum over sites, written here), sum to 3 q^2, and equal the closed forms of a
+    uniform and of a striped configuration."""
+    from oracle import plane_correlation
+    rng = np.random.default_rng(4)
+    for L in (2, 4, 6):
+        N = L ** 3
+        q = (2 * rng.integers(0, 2, N) - 1).astype(np.int64)
+        C = plane_correlation(q, L)
+        assert C.sum() == 3 * int(q.sum()) ** 2
+        i = np.arange(N)
+        coords = (i % L, (i // L) % L, i // (L * L))
+        for m in range(L):
+            k = 2 * np.pi * m / L
+            direct = sum(abs((q * np.exp(1j * k * c)).sum()) ** 2 for c in coords)
+            from_C = sum(np.cos(k * d) * C[d] for d in range(L))
+            assert abs(direct - from_C) < 1e-6 * max(1.0, direct)
+    L = 4
+    N = L ** 3
+    assert (plane_correlation(np.ones(N, dtype=np.int64), L) == 3 * L * L ** 4).all()
+    x = np.arange(N) % L
+    stripes = np.where(x < L // 2, 1, -1)                   # +1 for x < L/2: only the x planes are non-zero
+    want = [L ** 4 * (L - 4 * min(d, L - d)) for d in range(L)]
+    assert plane_correlation(stripes, L).tolist() == want
+
+
+def test_measure_accumulates_plane_correlations_and_xi_formula():
+    from oracle import correlation_length, plane_correlation
+    L, nT, R = 4, 3, 64
+    o = Oracle(L, nT, R, 1.0 / np.array([1.0, 2.0, 4.0]), 6)
+    wp = [[0, 1], [1, -1]]
+    acc = None
+    exp = np.zeros((2, 32, nT, L), dtype=object) + 0
+    for _ in range(3):
+        acc = o.measure(1, 2, 1, wp, acc)
+        s = o.spins().astype(np.int64)
+        for b in (0, 7, 31):
+            for t in range(nT):
+                exp[0, b, t] += plane_correlation(s[b, t] * s[32 + b, t], L)
+                exp[1, b, t] += plane_correlation(s[32 + b, t], L)
+    for b in (0, 7, 31):
+        assert (acc["corr"][:, b] == exp[:, b]).all()
+    assert (acc["corr"].sum(axis=3) == 3 * acc["q2"]).all()              # sum_d C(d) = 3 q^2
+    # xi from synthetic sums: C(d) = A + B cos(2 pi d / L) gives chi(0) = L A, chi(k_min) = L B / 2
+    L2, A, B = 8, 1000, 600
+    C = np.array([round(A + B * np.cos(2 * np.pi * d / L2)) for d in range(L2)], dtype=object)
+    syn = {"n": 1, "valid": np.ones((1, 1), dtype=bool), "corr": C.reshape(1, 1, 1, L2)}
+    chi0 = float(sum(C))
+    chik = sum(np.cos(2 * np.pi * d / L2) * float(C[d]) for d in range(L2))
+    want = np.sqrt(chi0 / chik - 1.0) / (2 * np.sin(np.pi / L2))
+    assert abs(correlation_length(syn, L2)[0] - want) < 1e-12 * want
+    assert abs(want - np.sqrt(L2 * A / (L2 * B / 2) - 1) / (2 * np.sin(np.pi / L2))) < 0.02 * want
+    # a uniform overlap has no weight at k_min: xi undefined (NaN)
+    uni = {"n": 1, "valid": np.ones((1, 1), dtype=bool), "corr": np.full((1, 1, 1, L2), 5, dtype=object)}
+    assert np.isnan(correlation_length(uni, L2)[0])
