@@ -163,6 +163,19 @@ int ea_get_moments(ea_handle *h, uint64_t *n_meas, int64_t *q1 /* [P][32][n_temp
                    uint64_t *q2 /* [P][32][n_temps] */, uint64_t *q4 /* [P][32][n_temps][2] */,
                    int64_t *e1 /* [R][n_temps] */, uint64_t *e2 /* [R][n_temps] */);
 
+/* Plane-sum correlations of the local overlap q_i = s_i(ra, t) s_i(rb, t), accumulated by every
+ * measurement: C[p][b][t][d] = sum over measurements, over the three axes mu and over the planes c
+ * of S_mu(c) S_mu((c + d) mod L), S_mu(c) = sum of q_i over the plane (coordinate mu of i) = c
+ * (R23).  sum_d C = 3 * (sum of q^2).  Not accumulated for L > 85. */
+int ea_get_correlation(ea_handle *h, int64_t *C /* [P][32][n_temps][L] */);
+
+/* Second-moment correlation length by temperature index (the quantity of the paper's Fig. 19,
+ * PAPER.md:329): chi(k) = sum_d cos(k d) [<C(d)>] / (3 N), xi = sqrt(chi(0)/chi(k_min) - 1) /
+ * (2 sin(k_min/2)), k_min = 2 pi / L, [.] = average over the series' valid realization pairs.
+ * Host arithmetic in long double from the integer sums.  NaN where nothing was measured,
+ * chi(k_min) <= 1e-12 chi(0) or chi(0) < chi(k_min). */
+int ea_get_correlation_length(ea_handle *h, double *xi /* [n_temps] */);
+
 /* Round trips in temperature space, the parallel-tempering diagnostic behind "the choice of
  * temperatures is crucial", observed at the measurements of the series: a replica
  * that is at temperature index 0 after having been at index n_temps-1 completes one round trip

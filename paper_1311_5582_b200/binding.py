@@ -19,7 +19,7 @@ _SYMBOLS = [
     "ea_launch_count", "ea_last_error", "ea_measure_int_peak",
     "ea_get_couplings", "ea_pair_couplings", "ea_measure_begin", "ea_measure", "ea_get_moments",
     "ea_get_binder", "ea_set_field", "ea_get_field", "ea_get_field_tables",
-    "ea_get_round_trips",
+    "ea_get_round_trips", "ea_get_correlation", "ea_get_correlation_length",
 ]
 
 
@@ -65,7 +65,8 @@ def lib():
                        ("ea_measure_begin", [vp, vp, i32]), ("ea_measure", [vp, i64, i64, i32]),
                        ("ea_get_moments", [vp, vp, vp, vp, vp, vp, vp]), ("ea_get_binder", [vp, vp]),
                        ("ea_set_field", [vp, i32]), ("ea_get_field", [vp]),
-                       ("ea_get_field_tables", [vp, vp, vp]), ("ea_get_round_trips", [vp, vp])):
+                       ("ea_get_field_tables", [vp, vp, vp]), ("ea_get_round_trips", [vp, vp]),
+                       ("ea_get_correlation", [vp, vp]), ("ea_get_correlation_length", [vp, vp])):
         f = getattr(l, name)
         f.restype = i32
         f.argtypes = args
@@ -210,6 +211,16 @@ class EA:
         e2 = np.zeros((self.R, self.nT), dtype=np.uint64)
         self._chk(self._l.ea_get_moments(self.h, C.byref(n), _p(q1), _p(q2), _p(q4), _p(e1), _p(e2)))
         return {"n": n.value, "q1": q1, "q2": q2, "q4": q4, "e1": e1, "e2": e2}
+
+    def get_correlation(self):
+        C_ = np.zeros((self._n_wp, 32, self.nT, self.L), dtype=np.int64)
+        self._chk(self._l.ea_get_correlation(self.h, _p(C_)))
+        return C_
+
+    def get_correlation_length(self):
+        xi = np.zeros(self.nT, dtype=np.float64)
+        self._chk(self._l.ea_get_correlation_length(self.h, _p(xi)))
+        return xi
 
     def get_round_trips(self):
         trips = np.zeros(self.R, dtype=np.uint64)

@@ -1143,6 +1143,7 @@ extern "C" int ea_measure_begin(ea_handle *h, const int32_t *word_pairs, int n_w
     const size_t o_pairs = take(8 * (size_t)(n_word_pairs ? n_word_pairs : 1));
     const size_t o_q1 = take(8 * nq), o_q2 = take(8 * nq), o_q4 = take(16 * nq);
     const size_t o_e1 = take(8 * ne), o_e2 = take(8 * ne);
+    const size_t o_corr = take(8 * nq * (size_t)h->L);
     const size_t o_label = take(ne), o_trips = take(8 * (size_t)h->R);
     char *d = nullptr;
     if (cudaMalloc((void **)&d, off) != cudaSuccess) {
@@ -1170,6 +1171,7 @@ extern "C" int ea_measure_begin(ea_handle *h, const int32_t *word_pairs, int n_w
     h->M.q4 = (uint64_t *)(d + o_q4);
     h->M.e1 = (int64_t *)(d + o_e1);
     h->M.e2 = (uint64_t *)(d + o_e2);
+    h->M.corr = (long long *)(d + o_corr);
     h->M.label = (uint8_t *)(d + o_label);
     h->M.trips = (unsigned long long *)(d + o_trips);
     h->meas_n = 0;
@@ -1189,6 +1191,20 @@ static int measure_once(ea_handle *h)
         else if (per_thread < (1 << 9)) ea::k_overlap_words<9><<<grid, 128, 0, h->stream>>>(h->P, h->d_T, h->M, nullptr);
         else if (per_thread < (1 << 12)) ea::k_overlap_words<12><<<grid, 128, 0, h->stream>>>(h->P, h->d_T, h->M, nullptr);
         else ea::k_overlap_words<15><<<grid, 128, 0, h->stream>>>(h->P, h->d_T, h->M, nullptr);
+        if (h->L <= 85) {       // plane-sum correlations: 3 axes x L planes x >= 1 thread in a block of 256
+            const int nsub = std::max(1, ea::kCorrThreads / (3 * h->L));
+            const int per_thread = (h->L * h->L + nsub - 1) / nsub;            // sites per thread < 2^PL
+            const bool stage = 4 * (size_t)h->N <= 128 * 1024;
+            const size_t sm = 4 * (size_t)((32 * (3 * h->L + 1) + 3) & ~3) + (stage ? 4 * (size_t)h->N : 0);
+            void (*kern)(Params, const uint32_t *, ea::Moments);
+            if (per_thread < (1 << 6)) kern = stage ? ea::k_plane_corr<6, true> : ea::k_plane_corr<6, false>;
+            else if (per_thread < (1 << 9)) kern = stage ? ea::k_plane_corr<9, true> : ea::k_plane_corr<9, false>;
+            else if (per_thread < (1 << 12)) kern = stage ? ea::k_plane_corr<12, true> : ea::k_plane_corr<12, false>;
+            else kern = stage ? ea::k_plane_corr<15, true> : ea::k_plane_corr<15, false>;
+            CUDA_TRY(h, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
+            kern<<<grid, ea::kCorrThreads, sm, h->stream>>>(h->P, h->d_T, h->M);
+            h->launches++;
+        }
         h->launches += 2;
     }
     int grid;
@@ -1233,6 +1249,43 @@ extern "C" int ea_get_moments(ea_handle *h, uint64_t *n_meas, int64_t *q1, uint6
     if (e2) CUDA_TRY(h, cudaMemcpyAsync(e2, h->M.e2, 8 * ne, cudaMemcpyDeviceToHost, h->stream));
     CUDA_TRY(h, cudaStreamSynchronize(h->stream));
     if (n_meas) *n_meas = h->meas_n;
+    return EA_OK;
+}
+
+extern "C" int ea_get_correlation(ea_handle *h, int64_t *C)
+{
+    if (!h || !C) return fail(h, EA_ERR_INVALID_ARG, "ea_get_correlation: null argument");
+    if (!h->meas_on) return fail(h, EA_ERR_INVALID_ARG, "ea_get_correlation: call ea_measure_begin first");
+    const size_t n = (size_t)h->M.P * 32 * h->nT * h->L;
+    if (n) CUDA_TRY(h, cudaMemcpyAsync(C, h->M.corr, 8 * n, cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    return EA_OK;
+}
+
+extern "C" int ea_get_correlation_length(ea_handle *h, double *xi)
+{
+    if (!h || !xi) return fail(h, EA_ERR_INVALID_ARG, "ea_get_correlation_length: null argument");
+    if (!h->meas_on) return fail(h, EA_ERR_INVALID_ARG, "ea_get_correlation_length: call ea_measure_begin first");
+    const int L = h->L, nT = h->nT;
+    const size_t n = (size_t)h->M.P * 32 * nT * L;
+    std::vector<int64_t> C(n);
+    if (n) CUDA_TRY(h, cudaMemcpyAsync(C.data(), h->M.corr, 8 * n, cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    // chi(k) ~ sum_d cos(k d) [<C(d)>]; the common factor 1 / (3 N n M) cancels in chi(0) / chi(k_min).
+    // Invalid (padding) pairs hold zeros.  xi = sqrt(chi(0) / chi(k_min) - 1) / (2 sin(pi / L)).
+    const long double pi = 3.14159265358979323846264338327950288L;
+    for (int t = 0; t < nT; ++t) {
+        long double chi0 = 0.0L, chik = 0.0L;
+        for (int d = 0; d < L; ++d) {
+            long double cd = 0.0L;
+            for (size_t pb = 0; pb < (size_t)h->M.P * 32; ++pb) cd += (long double)C[(pb * nT + t) * L + d];
+            chi0 += cd;
+            chik += std::cos(2.0L * pi * (long double)d / (long double)L) * cd;
+        }
+        xi[t] = (h->meas_n > 0 && chik > 1e-12L * chi0 && chi0 >= chik)
+                    ? (double)(std::sqrt(chi0 / chik - 1.0L) / (2.0L * std::sin(pi / (long double)L)))
+                    : std::nan("");
+    }
     return EA_OK;
 }
 

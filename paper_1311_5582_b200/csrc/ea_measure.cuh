@@ -17,6 +17,7 @@ struct Moments {
     uint64_t *q4;            // [P][32][nT][2]  sum q^4, 128 bit: (low, high)
     int64_t *e1;             // [R][nT]  sum E by temperature index
     uint64_t *e2;            // [R][nT]  sum E^2
+    long long *corr;         // [P][32][nT][L]  sum of C(d) = sum_mu sum_p S_mu(p) S_mu(p + d)  (R23)
     uint8_t *label;          // [R][nT]  by slot: 0 no end touched yet, 1 last at index 0, 2 last at nT-1
     unsigned long long *trips;   // [R]  completed round trips 0 -> nT-1 -> 0 of the realization's replicas
 };
@@ -143,6 +144,91 @@ __global__ void __launch_bounds__(128) k_overlap_words(Params P, const uint32_t 
     const uint64_t old = M.q4[2 * o];
     M.q4[2 * o] = old + lo;
     M.q4[2 * o + 1] += hi + (old + lo < old ? 1u : 0u);
+}
+
+// ------------------------------------------------------------------ plane-sum correlations
+// Block = (pair p, temperature index t).  S_mu(c)[b] = sum of the local overlaps q_i = +-1 of
+// realization pair b over the plane (coordinate mu of i) = c; then
+//   C(d)[b] += sum_mu sum_c S_mu(c)[b] S_mu((c + d) mod L)[b]
+// (R23: all that the wave-vector dependent susceptibility along the axes needs; the
+// Fourier sum over the L values is done on the host).  The agreement words ~(Ta ^ Tb) of the
+// lattice are staged in shared memory with coalesced 128-bit loads (STAGE; lattices of up to
+// 128 KiB, L <= 32), then thread = (axis mu, plane c, sub) walks its share of the plane's L^2
+// sites (scattered: the store is checkerboard-ordered), counts agreeing bits in vertical
+// counters, and the counts of a plane's threads meet in shared memory.  One block per (p, t)
+// is the only writer of its accumulators: no global atomics, fixed order.
+constexpr int kCorrThreads = 256;
+
+template <int PL, bool STAGE>
+__global__ void __launch_bounds__(kCorrThreads) k_plane_corr(Params P, const uint32_t *T, Moments M)
+{
+    extern __shared__ __align__(16) int sm_corr[];
+    const int L = P.L;
+    // sm_S[b][mu L + c], row stride 3L + 1 (odd): conflict-free both when the lanes of a warp walk
+    // the planes (counting) and when they walk the bits (correlation sums)
+    const int RS = 3 * L + 1;
+    int *sm_S = sm_corr;                                         // [32][RS], padded to a multiple of 4 ints
+    uint32_t *sm_A = reinterpret_cast<uint32_t *>(sm_corr + ((32 * RS + 3) & ~3));   // [N] (STAGE)
+    const int p = blockIdx.x / P.nT, t = blockIdx.x % P.nT;
+    const int wa = M.wpairs[2 * p], wb = M.wpairs[2 * p + 1];
+    const uint32_t *Ta = T + ((size_t)t * P.W + wa) * P.N;
+    const uint32_t *Tb = wb >= 0 ? T + ((size_t)t * P.W + wb) * P.N : nullptr;
+    for (int a = threadIdx.x; a < 32 * RS; a += blockDim.x) sm_S[a] = 0;
+    if (STAGE) {
+        const uint4 *Va = reinterpret_cast<const uint4 *>(Ta), *Vb = reinterpret_cast<const uint4 *>(Tb);
+        for (int i = threadIdx.x; i < P.N / 4; i += blockDim.x) {
+            const uint4 a = Va[i];
+            const uint4 b = Vb ? Vb[i] : make_uint4(~0u, ~0u, ~0u, ~0u);
+            reinterpret_cast<uint4 *>(sm_A)[i] = make_uint4(~(a.x ^ b.x), ~(a.y ^ b.y), ~(a.z ^ b.z), ~(a.w ^ b.w));
+        }
+    }
+    __syncthreads();
+    const int nsub = max(1, (int)blockDim.x / (3 * L));          // threads per plane
+    const int mu = threadIdx.x / (L * nsub), rem = threadIdx.x % (L * nsub);
+    const int c = rem / nsub, sub = rem % nsub;                  // the lanes of a warp share a plane: their
+                                                                 // sites are neighbours in x (or y for mu = 0)
+    if (mu < 3) {
+        uint32_t cnt[PL];
+#pragma unroll
+        for (int l = 0; l < PL; ++l) cnt[l] = 0;
+        // (u, v) = the two coordinates inside the plane, stepped without divisions
+        int u = sub % L, v = sub / L;
+        const int du = nsub % L, dv = nsub / L;
+        for (int m = sub; m < L * L; m += nsub) {
+            const int x = mu == 0 ? c : u, y = mu == 1 ? c : (mu == 0 ? u : v), z = mu == 2 ? c : v;
+            const int i = ((x + y + z) & 1) * P.Nh + (x >> 1) + P.Lh * (y + L * z);
+            uint32_t w = STAGE ? sm_A[i] : (Tb ? ~(Ta[i] ^ Tb[i]) : Ta[i]);
+            u += du; v += dv;
+            if (u >= L) { u -= L; ++v; }
+#pragma unroll
+            for (int l = 0; l < PL; ++l) {
+                const uint32_t carry = cnt[l] & w;
+                cnt[l] ^= w;
+                w = carry;
+            }
+        }
+        for (int b = 0; b < 32; ++b) {
+            int v = 0;
+#pragma unroll
+            for (int l = 0; l < PL; ++l) v += (int)((cnt[l] >> b) & 1u) << l;
+            if (v) atomicAdd(&sm_S[b * RS + mu * L + c], v);
+        }
+    }
+    __syncthreads();
+    for (int a = threadIdx.x; a < 32 * RS; a += blockDim.x) sm_S[a] = 2 * sm_S[a] - L * L;   // agree - disagree
+    __syncthreads();
+    const int b = threadIdx.x & 31;
+    const int ra = 32 * wa + b, rb = wb >= 0 ? 32 * wb + b : -1;
+    if (ra >= M.R || rb >= M.R) return;
+    for (int d = threadIdx.x >> 5; d < L; d += blockDim.x >> 5) {
+        long long s = 0;
+        for (int a = 0; a < 3; ++a)
+            for (int q = 0; q < L; ++q) {
+                const int q2 = q + d >= L ? q + d - L : q + d;
+                s += (long long)sm_S[b * RS + a * L + q] * (long long)sm_S[b * RS + a * L + q2];
+            }
+        M.corr[(((size_t)p * 32 + b) * P.nT + t) * L + d] += s;
+    }
 }
 
 // sum E and sum E^2 by temperature index, and the round-trip bookkeeping of the replica in

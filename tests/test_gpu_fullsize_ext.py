@@ -35,6 +35,8 @@ def test_cfg4_two_copy_measurement_series_on_sampled_word_pairs():
     g.measure_begin(wp)
     g.measure(n_meas, between, cfg.swap_interval)
     m = g.get_moments()
+    corr = g.get_correlation()
+    from oracle import plane_correlation
     st = g.get_state()
     for w in (0, 13, 31):
         a = Oracle(cfg.L, cfg.n_temps, 32, betas, cfg.seed, r0=32 * w)
@@ -45,15 +47,23 @@ def test_cfg4_two_copy_measurement_series_on_sampled_word_pairs():
         q4 = np.zeros((32, cfg.n_temps), dtype=object) + 0
         e1 = np.zeros((64, cfg.n_temps), dtype=np.int64)
         e2 = np.zeros_like(e1)
+        cd = np.zeros((32, cfg.n_temps, cfg.L), dtype=np.int64)
         for _ in range(n_meas):
             a.sweep(between, cfg.swap_interval)
             b.sweep(between, cfg.swap_interval)
             q = (a.spins().astype(np.int64) * b.spins().astype(np.int64)).sum(axis=2)   # [32][t]
             q1 += q; q2 += q * q; q4 += q.astype(object) ** 4
+            sa, sb = a.spins().astype(np.int64), b.spins().astype(np.int64)
+            for bit in (0, 17, 31):
+                for t in (0, 11, cfg.n_temps - 1):
+                    cd[bit, t] += plane_correlation(sa[bit, t] * sb[bit, t], cfg.L)
             E = np.concatenate([a.energy(), b.energy()]).astype(np.int64)
             e1 += E; e2 += E * E
         assert (m["q1"][w] == q1).all() and (m["q2"][w].astype(np.int64) == q2).all()
         assert (m["q4"][w][..., 0].astype(object) + m["q4"][w][..., 1].astype(object) * (1 << 64) == q4).all()
+        for bit in (0, 17, 31):
+            for t in (0, 11, cfg.n_temps - 1):
+                assert (corr[w, bit, t] == cd[bit, t]).all()
         rows = np.r_[32 * w:32 * w + 32, 32 * (w + half):32 * (w + half) + 32]
         assert (m["e1"][rows] == e1).all() and (m["e2"][rows].astype(np.int64) == e2).all()
         assert (_word_spins(st, w, cfg.L) == a.spins_by_slot()).all()

@@ -30,6 +30,12 @@ def _compare(g, acc, binder_ratio):
     assert m["n"] == acc["n"]
     for k in ("q1", "q2", "q4", "e1", "e2"):
         assert (m[k] == acc[k]).all(), k
+    assert (g.get_correlation().astype(object) == acc["corr"]).all(), "plane correlations"
+    from oracle import correlation_length
+    gx, ox = g.get_correlation_length(), correlation_length(acc, g.L)
+    assert (np.isnan(gx) == np.isnan(ox)).all(), (gx, ox)
+    okx = ~np.isnan(ox)
+    assert (np.abs(gx[okx] - ox[okx]) <= 1e-12 * np.abs(ox[okx])).all(), (gx, ox)
     if "trips" in acc:
         assert (g.get_round_trips().astype(np.int64) == acc["trips"]).all(), "round trips"
     gb, ob = g.get_binder(), binder_ratio(acc)
