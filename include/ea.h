@@ -42,7 +42,8 @@ enum {
  * that supports the lattice; all produce identical results. */
 enum {
     EA_KERNEL_AUTO = 0,
-    EA_KERNEL_GENERIC = 1,   /* any even L: one launch per half-sweep, global memory        */
+    EA_KERNEL_GENERIC = 1,   /* any even L, global memory: one cooperative launch per call when
+                                the work fits one wave, else one launch per half-sweep       */
     EA_KERNEL_RESIDENT = 2,  /* L in {8,16}: lattices resident in shared memory, one launch
                                 for all sweeps of the call, PT inside a thread-block cluster */
     EA_KERNEL_TILED = 3,     /* L = 16, 32, 64: z-slab tiles, one launch per half-sweep, lattice
@@ -152,7 +153,8 @@ int ea_measure_begin(ea_handle *h, const int32_t *word_pairs /* [n_word_pairs][2
 
 /* n_meas times: ea_sweep(sweeps_between, swap_interval), then one measurement at equal
  * temperature index t: q = sum_i s_i(ra, t) s_i(rb, t) for every realization pair of the series
- * and E = ea_energy's value for every (r, t); adds 1, q, q^2, q^4, E, E^2 to the accumulators.
+ * and E = ea_energy's value for every (r, t); adds 1, q, q^2, q^4, E, E^2 to the accumulators,
+ * and updates the plane-sum correlations and the round-trip counters (below).
  * Pairs that touch a padding bit (realization index >= R) accumulate nothing.  Asynchronous.
  * EA_ERR_RANGE if the sweep counter would pass 2^32-1 or the number of measurements would pass
  * 2^64 / (9 N^2) (64-bit sums of q^2 and E^2; the q^4 sums are 128-bit). */
