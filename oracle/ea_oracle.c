@@ -493,6 +493,35 @@ void eao_get_energy_by_slot(const eao *o, int32_t *E)
 {
     memcpy(E, o->E, sizeof(int32_t) * o->R * o->nT);
 }
+/* Resume from a checkpoint ("spin configurations are dumped to the GPU global memory
+ * periodically"): spins by slot, the temperature permutation and the two
+ * counters that address the random draws.  tau must be a permutation of
+ * 0..nT-1 for every realization; energies are recomputed. */
+int eao_set_state(eao *o, const int8_t *s, const int32_t *tau, uint64_t g, uint64_t nswap)
+{
+    int nT = o->nT;
+    if (g > 0xFFFFFFFFull) return -4;
+    for (int r = 0; r < o->R; ++r) {
+        uint64_t seen = 0, seen_hi = 0;
+        for (int k = 0; k < nT; ++k) {
+            int t = tau[r * nT + k];
+            if (t < 0 || t >= nT) return -1;
+            if (t < 64) { if ((seen >> t) & 1u) return -1; seen |= (uint64_t)1 << t; }
+            else { if ((seen_hi >> (t - 64)) & 1u) return -1; seen_hi |= (uint64_t)1 << (t - 64); }
+        }
+    }
+    if (eao_set_spins(o, s) != 0) return -1;
+    for (int r = 0; r < o->R; ++r)
+        for (int k = 0; k < nT; ++k) {
+            int t = tau[r * nT + k];
+            o->tau[r * nT + k] = t;
+            o->sigma[r * nT + t] = k;
+        }
+    o->g = g;
+    o->nswap = nswap;
+    return 0;
+}
+
 void eao_get_counters(const eao *o, uint64_t *g, uint64_t *nswap, int64_t *stats)
 {
     *g = o->g; *nswap = o->nswap;

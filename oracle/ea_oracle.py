@@ -65,6 +65,8 @@ def _load():
     lib.eao_n_sat.restype = i32
     lib.eao_n_sat.argtypes = [vp, i32, i32, i32]
     lib.eao_philox4x32_10.argtypes = [C.c_uint32] * 6 + [vp]
+    lib.eao_set_state.restype = i32
+    lib.eao_set_state.argtypes = [vp, vp, vp, u64, u64]
     lib.eao_set_field.restype = i32
     lib.eao_set_field.argtypes = [vp, i32]
     lib.eao_get_field.restype = i32
@@ -133,6 +135,15 @@ class Oracle:
         swp = np.ascontiguousarray(swp, dtype=np.uint64)
         assert acc.shape == (self.nT, 7) and swp.shape == (self.nT - 1, 3 * self.N + 1)
         self.lib.eao_set_tables(self.h, _ptr(acc), _ptr(swp))
+
+    def set_state(self, spins_by_slot, tau, sweeps, swap_rounds):
+        """Resume from a checkpoint: s[r][slot][site], tau[r][slot], the two counters."""
+        s = np.ascontiguousarray(spins_by_slot, dtype=np.int8)
+        t = np.ascontiguousarray(tau, dtype=np.int32)
+        assert s.shape == (self.R, self.nT, self.N) and t.shape == (self.R, self.nT)
+        rc = self.lib.eao_set_state(self.h, _ptr(s), _ptr(t), int(sweeps), int(swap_rounds))
+        if rc != 0:
+            raise ValueError(f"eao_set_state -> {rc}")
 
     def set_field(self, h):
         """Constant external field h of Eq. 1 (integer); energies are recomputed."""

@@ -334,3 +334,30 @@ def test_ferromagnet_binder_crossing_near_4p51():
     i = int(np.nonzero(d > 0)[0].max())
     Tx = Ts[i] + (Ts[i + 1] - Ts[i]) * d[i] / (d[i] - d[i + 1])
     assert 4.25 <= Tx <= 4.8, (Tx, U)
+
+
+def test_checkpoint_resume_continues_the_same_trajectory():
+    """A run interrupted at sweep a and resumed from (spins by slot, tau, counters) in a fresh
+    object equals the uninterrupted run: the state is exactly that tuple."""
+    L, nT, R = 4, 5, 37
+    betas = 1.0 / np.geomspace(0.7, 2.5, nT)
+    a = Oracle(L, nT, R, betas, 15)
+    a.sweep(7, 2)                                 # ends between two swap rounds (round parity matters)
+    c = a.counters()
+    b = Oracle(L, nT, R, betas, 99)               # another seed: nothing may leak from create
+    b.set_couplings(a.couplings())
+    with pytest.raises(ValueError):
+        bad = a.perm()[0].copy(); bad[3, 0] = bad[3, 1]
+        b.set_state(a.spins_by_slot(), bad, c["sweeps"], c["swap_rounds"])
+    # the draws are keyed by the seed: resume needs the same seed
+    b = Oracle(L, nT, R, betas, 15)
+    b.set_couplings(a.couplings())
+    b.set_state(a.spins_by_slot(), a.perm()[0], c["sweeps"], c["swap_rounds"])
+    assert (b.energy() == a.energy()).all() and (b.perm()[1] == a.perm()[1]).all()
+    a.sweep(9, 2); b.sweep(9, 2)
+    assert (a.spins_by_slot() == b.spins_by_slot()).all()
+    assert (a.perm()[0] == b.perm()[0]).all() and (a.energy() == b.energy()).all()
+    ref = Oracle(L, nT, R, betas, 15)
+    ref.sweep(16, 2)
+    assert (ref.spins_by_slot() == b.spins_by_slot()).all() and (ref.perm()[0] == b.perm()[0]).all()
+    assert b.counters()["sweeps"] == 16 and b.counters()["swap_rounds"] == 8
