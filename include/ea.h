@@ -127,6 +127,17 @@ int ea_get_state(ea_handle *h, uint32_t *spin_words /* [n_temps][W][2][N/2] */,
                  uint8_t *temp_of_slot /* [R][n_temps] */, int32_t *energy_by_slot /* [R][n_temps] */,
                  uint64_t *sweeps_done, uint64_t *swap_rounds_done);
 
+/* Resume from a checkpoint taken with ea_get_state ("spin configurations are dumped ...
+ * periodically"): packed spins by slot, the temperature permutation and the two
+ * counters that address the random draws.  The handle must have been created with the same
+ * shape, betas and seed (and given the same couplings / field) as the one that was saved.
+ * temp_of_slot[r] must be a permutation of 0..n_temps-1 (EA_ERR_INVALID_ARG), sweeps_done
+ * <= 2^32-1 (EA_ERR_RANGE).  Padding bits of the last word are taken as given.  Rank masks and
+ * energies are recomputed. */
+int ea_set_state(ea_handle *h, const uint32_t *spin_words /* [n_temps][W][2][N/2] */,
+                 const uint8_t *temp_of_slot /* [R][n_temps] */, uint64_t sweeps_done,
+                 uint64_t swap_rounds_done);
+
 /*
  * ---- Measurement series (the observables of PAPER.md:317-339) ----
  * The paper's spin-glass order parameter is the overlap q between two copies of one disorder

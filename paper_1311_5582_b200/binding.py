@@ -19,7 +19,7 @@ _SYMBOLS = [
     "ea_launch_count", "ea_last_error", "ea_measure_int_peak",
     "ea_get_couplings", "ea_pair_couplings", "ea_measure_begin", "ea_measure", "ea_get_moments",
     "ea_get_binder", "ea_set_field", "ea_get_field", "ea_get_field_tables",
-    "ea_get_round_trips", "ea_get_correlation", "ea_get_correlation_length",
+    "ea_get_round_trips", "ea_get_correlation", "ea_get_correlation_length", "ea_set_state",
 ]
 
 
@@ -70,6 +70,8 @@ def lib():
         f = getattr(l, name)
         f.restype = i32
         f.argtypes = args
+    l.ea_set_state.restype = i32
+    l.ea_set_state.argtypes = [vp, vp, vp, u64, u64]
     l.ea_launch_count.restype = i64
     l.ea_launch_count.argtypes = [vp]
     l.ea_last_error.restype = C.c_char_p
@@ -244,6 +246,13 @@ class EA:
         swpf = np.zeros((max(self.nT - 1, 0), 2 * Mf + 1), dtype=np.uint64)
         self._chk(self._l.ea_get_field_tables(self.h, _p(accf), _p(swpf)))
         return accf, swpf
+
+    def set_state(self, state):
+        """Resume from the dict get_state() returned (on a handle with the same shape, betas, seed)."""
+        words = np.ascontiguousarray(state["spin_words"], dtype=np.uint32)
+        tau = np.ascontiguousarray(state["temp_of_slot"], dtype=np.uint8)
+        assert words.shape == (self.nT, self.W, 2, self.N // 2) and tau.shape == (self.R, self.nT)
+        self._chk(self._l.ea_set_state(self.h, _p(words), _p(tau), int(state["sweeps"]), int(state["swap_rounds"])))
 
     def set_kernel(self, kernel):
         self._chk(self._l.ea_set_kernel(self.h, int(kernel)))

@@ -36,6 +36,15 @@ __global__ void k_identity_perm(Params P)
     P.sigma[tid] = k;
 }
 
+// sigma = inverse of tau, per realization (after tau was replaced: ea_set_state)
+__global__ void k_invert_perm(Params P)
+{
+    const int tid = blockIdx.x * blockDim.x + threadIdx.x;
+    if (tid >= P.Rp * P.nT) return;
+    const int r = tid / P.nT, k = tid % P.nT;
+    P.sigma[(size_t)r * P.nT + P.tau[tid]] = (uint8_t)k;
+}
+
 // ------------------------------------------------------------------ rank masks
 // lt[w][k][n] = bits b whose temperature rank pos(tau[32w+b][k]) >= n, n = 0..nT
 // (the paper's "swap the rows of the table, not the lattices", in bit-sliced

@@ -1330,6 +1330,39 @@ extern "C" int ea_get_binder(ea_handle *h, double *g)
     return EA_OK;
 }
 
+// ---------------------------------------------------------------- checkpoint / resume
+extern "C" int ea_set_state(ea_handle *h, const uint32_t *spin_words, const uint8_t *temp_of_slot,
+                            uint64_t sweeps_done, uint64_t swap_rounds_done)
+{
+    if (!h || !spin_words || !temp_of_slot) return fail(h, EA_ERR_INVALID_ARG, "ea_set_state: null argument");
+    if (sweeps_done > 0xFFFFFFFFull) return fail(h, EA_ERR_RANGE, "ea_set_state: sweep counter above 2^32-1");
+    const int nT = h->nT;
+    std::vector<uint8_t> tau((size_t)h->Rp * nT);
+    for (int r = 0; r < h->Rp; ++r) {
+        uint64_t seen = 0;                                   // n_temps <= 64
+        for (int k = 0; k < nT; ++k) {
+            const int t = r < h->R ? temp_of_slot[(size_t)r * nT + k] : k;   // padding realizations: identity
+            if (t >= nT || ((seen >> t) & 1u))
+                return fail(h, EA_ERR_INVALID_ARG, "ea_set_state: temp_of_slot is not a permutation");
+            seen |= (uint64_t)1 << t;
+            tau[(size_t)r * nT + k] = (uint8_t)t;
+        }
+    }
+    CUDA_TRY(h, cudaMemcpyAsync(h->P.spin, spin_words, 4 * (size_t)nT * h->W * h->N, cudaMemcpyHostToDevice, h->stream));
+    CUDA_TRY(h, cudaMemcpyAsync(h->P.tau, tau.data(), tau.size(), cudaMemcpyHostToDevice, h->stream));
+    int grid;
+    launch_cfg((int64_t)h->Rp * nT, 128, grid);
+    ea::k_invert_perm<<<grid, 128, 0, h->stream>>>(h->P);
+    h->launches++;
+    CUDA_TRY(h, cudaGetLastError());
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));           // tau lives on this stack frame
+    h->g = sweeps_done;
+    h->nswap = swap_rounds_done;
+    int rc = rebuild_lt(h);
+    if (rc != EA_OK) return rc;
+    return recompute_energy(h);
+}
+
 // ---------------------------------------------------------------- measurement helper
 extern "C" int ea_measure_int_peak(void *cuda_stream, double *out)
 {

@@ -230,3 +230,28 @@ def test_generic_stepwise_launches_equal_the_persistent_kernel(monkeypatch, L, n
         else:
             assert launches >= 2 * ns
         g.destroy()
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_checkpoint_resume(kernel):
+    """ea_get_state -> ea_set_state on a fresh handle continues the trajectory bit for bit
+    (PAPER.md:120), and the resumed run still follows the oracle; bad input changes nothing."""
+    L, nT, R = {1: 6, 2: 8, 3: 16, 4: 32}[kernel], 5, 37
+    betas = 1.0 / temperature_ladder(nT, 0.7, 2.5)
+    g, o = _pair(L, nT, R, betas, 15, kernel)
+    g.sweep(7, 2); o.sweep(7, 2)                  # stops between two swap rounds
+    ck = g.get_state()
+    assert ck["sweeps"] == 7 and ck["swap_rounds"] == 3
+    from paper_1311_5582_b200 import EA, EAError
+    g2 = EA(L, nT, R, betas, 15, kernel=kernel)
+    g2.sweep(3, 1)                                # some other history to overwrite
+    bad = dict(ck); bad["temp_of_slot"] = ck["temp_of_slot"].copy(); bad["temp_of_slot"][2, 0] = bad["temp_of_slot"][2, 1]
+    with pytest.raises(EAError):
+        g2.set_state(bad)
+    assert g2.get_state()["sweeps"] == 3          # rejected input left the handle alone
+    g2.set_state(ck)
+    _assert_same(g2, o, "right after resume")
+    g.sweep(9, 2); g2.sweep(9, 2); o.sweep(9, 2)
+    _assert_same(g2, o, "resumed run")
+    _assert_same(g, o, "uninterrupted run")
+    g.destroy(); g2.destroy()
