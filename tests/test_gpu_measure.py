@@ -164,3 +164,36 @@ def test_binder_convergence_example_runs_and_orders_temperatures():
     assert np.isfinite(g).all() and (g <= 1.0).all()
     assert g[-1, 0] > 0.8 and g[-1, -1] < 0.5
     assert (np.diff(g[-1]) < 0.02).all()
+
+
+def test_shard_measurements_and_field_equal_the_full_run():
+    """A handle that simulates words 1..2 of a larger problem (first_realization = 32) gives those
+    words' moments, correlations, round trips and field trajectory of the full run."""
+    pkg, Oracle, _ = _mods()
+    L, nT, R = 8, 6, 128
+    betas = 1.0 / temperature_ladder(nT, 1.2, 2.4)
+    full = pkg.EA(L, nT, R, betas, 9)
+    part = pkg.EA(L, nT, 64, betas, 9, first_realization=32)
+    for x in (full, part):
+        x.set_field(1)
+        x.sweep(3, 1)
+        x.set_field(0)
+    full.measure_begin([[1, 2], [2, -1]])
+    part.measure_begin([[0, 1], [1, -1]])
+    full.measure(40, 1, 1)
+    part.measure(40, 1, 1)
+    mf, mp = full.get_moments(), part.get_moments()
+    for k in ("q1", "q2", "q4"):
+        assert (mf[k] == mp[k]).all(), k
+    assert (mf["e1"][32:96] == mp["e1"]).all() and (mf["e2"][32:96] == mp["e2"]).all()
+    assert (full.get_correlation() == part.get_correlation()).all()
+    assert (full.get_round_trips()[32:96] == part.get_round_trips()).all()
+    assert full.get_round_trips()[32:96].sum() > 0
+    ck = part.get_state()
+    again = pkg.EA(L, nT, 64, betas, 9, first_realization=32)
+    again.set_state(ck)
+    again.sweep(5, 1); part.sweep(5, 1); full.sweep(5, 1)
+    assert (again.get_state()["spin_words"] == part.get_state()["spin_words"]).all()
+    assert (full.get_state()["spin_words"][:, 1:3] == part.get_state()["spin_words"]).all()
+    for x in (full, part, again):
+        x.destroy()
