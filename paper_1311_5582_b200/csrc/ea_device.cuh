@@ -32,8 +32,9 @@ struct Params {
     // members above, which the fast kernels read from the constant bank, do not move.
     int h;                   // field of Eq. 1 (integer); 0: zero-field path
     int ediv;                // swap tables are indexed by (E_a - E_b) / ediv: 4 at h = 0, else 2
-    const uint32_t *thrF;    // [14][nT+1]: class 2 n_sat + (s+1)/2, (threshold - 1) in pos order, sentinel
-    int zF[14];              // per class: number of zero thresholds, or -1: dE <= 0, always flips
+    const uint32_t *thrF;    // [18][nT+1]: rows 0..13 = class 2 n_sat + (s+1)/2, rows 14..17 = the four
+                             // columns of accept_mask_field (|h| <= 2); (threshold - 1) in pos order, sentinel
+    int zF[18];              // per row: number of zero thresholds, or -1: dE <= 0, always flips
 };
 
 // ---------------------------------------------------------------------------------
@@ -104,6 +105,31 @@ __device__ __forceinline__ uint32_t accept_mask(const Planes &p, uint32_t m4, ui
     const uint32_t t1 = m5 | (~p.b0 & m4);
     const uint32_t t2 = m6 | (~p.b1 & t1);
     return ~p.b2 | t2;
+}
+
+// Field with |h| <= 2.  dE = 4 n_sat - 12 - 2 h s depends on (n_sat, s) only
+// through a shifted index:
+//   h = +-1:  c'  = n_sat + x,    dE = 4 (c' - 3) - 2;   h = +-2:  c'' = n_sat + 2 x,  dE = 4 (c'' - 4),
+// x = [s = -1] for h > 0, [s = +1] for h < 0 (a one-bit bit-sliced add).  Column j = 0..3 stands for
+// dE_j = 4 j + 2 (odd h) or 4 j + 4 (even h); smaller dE always flip.  m_j = bits whose temperature
+// accepts a flip of column j for this draw.
+__device__ __forceinline__ uint32_t accept_mask_field(const Planes &p, uint32_t s, int h, uint32_t m0,
+                                                      uint32_t m1, uint32_t m2, uint32_t m3)
+{
+    const uint32_t x = h > 0 ? ~s : s;
+    if (h & 1) {
+        const uint32_t p0 = p.b0 ^ x, c0 = p.b0 & x;
+        const uint32_t p1 = p.b1 ^ c0, c1 = p.b1 & c0;
+        const uint32_t p2 = p.b2 ^ c1;                       // c' = (p2 p1 p0) in 0..7; columns <-> c' = 4..7
+        const uint32_t lo = (m0 & ~p0) | (m1 & p0), hi = (m2 & ~p0) | (m3 & p0);
+        return ~p2 | (lo & ~p1) | (hi & p1);
+    }
+    const uint32_t p0 = p.b0;
+    const uint32_t p1 = p.b1 ^ x, c1 = p.b1 & x;
+    const uint32_t p2 = p.b2 ^ c1, p3 = p.b2 & c1;           // c'' = (p3 p2 p1 p0) in 0..8; columns <-> 5..8
+    const uint32_t in567 = p2 & (p1 | p0);
+    const uint32_t sel = (m0 & ~p1) | (p1 & ((m1 & ~p0) | (m2 & p0)));   // c'' = 5: p1 = 0 (and p0 = 1)
+    return (p3 & m3) | (~p3 & (~in567 | sel));
 }
 
 // n_c(u) = number of pos with threshold <= u = z + #{n in [z, nT): thr32[n] < u};

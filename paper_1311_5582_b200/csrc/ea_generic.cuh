@@ -128,6 +128,14 @@ __device__ __forceinline__ void half_sweep_field_item(const Params &P, int p, ui
         uint32_t s;
         const Planes pl = site_planes(sp, cp, p, j, P.L, P.Lh, P.Nh, P.N, &s);
         const uint32_t u = pick(rnd, l);
+        if (P.h >= -2 && P.h <= 2) {          // four threshold columns instead of fourteen classes
+            uint32_t m[4];
+#pragma unroll
+            for (int jc = 0; jc < 4; ++jc)
+                m[jc] = lt[rank_of(u, sm_thr + (14 + jc) * P.LTS, P.zF[14 + jc], P.nT)];
+            sp[p * P.Nh + j] = s ^ accept_mask_field(pl, s, P.h, m[0], m[1], m[2], m[3]);
+            continue;
+        }
         uint32_t acc = 0;
         for (int c = 0; c < 7; ++c) {
             const uint32_t ind = ((c & 1) ? pl.b0 : ~pl.b0) & ((c & 2) ? pl.b1 : ~pl.b1) & ((c & 4) ? pl.b2 : ~pl.b2);
@@ -144,8 +152,8 @@ __device__ __forceinline__ void half_sweep_field_item(const Params &P, int p, ui
 
 __global__ void __launch_bounds__(128) k_half_sweep_field(Params P, int p, uint32_t g)
 {
-    extern __shared__ uint32_t sm_thr[];   // [14][nT+1]
-    for (int a = threadIdx.x; a < 14 * P.LTS; a += blockDim.x) sm_thr[a] = P.thrF[a];
+    extern __shared__ uint32_t sm_thr[];   // [18][nT+1]
+    for (int a = threadIdx.x; a < 18 * P.LTS; a += blockDim.x) sm_thr[a] = P.thrF[a];
     __syncthreads();
     const int64_t tid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (tid >= (int64_t)P.nT * P.W * (P.Nh >> 2)) return;
@@ -322,10 +330,10 @@ __device__ __forceinline__ void persist_grid_sync(unsigned int *bar)
 template <bool FIELD>
 __global__ void __launch_bounds__(256) k_generic_persistent(const PersistArgs A)
 {
-    extern __shared__ uint32_t sm_thr[];   // [3 or 14][nT+1]
+    extern __shared__ uint32_t sm_thr[];   // [3 or 18][nT+1]
     __shared__ int sm_cnt[32];
     const Params &P = A.P;
-    const int ncls = FIELD ? 14 : 3;
+    const int ncls = FIELD ? 18 : 3;
     for (int a = threadIdx.x; a < ncls * P.LTS; a += blockDim.x) sm_thr[a] = FIELD ? P.thrF[a] : P.thr32[a];
     __syncthreads();
     const int64_t n_items = (int64_t)P.nT * P.W * (P.Nh >> 2);

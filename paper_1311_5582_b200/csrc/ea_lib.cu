@@ -400,7 +400,7 @@ extern "C" ea_handle *ea_create_ex(int L, int n_temps, int n_realizations, const
     P.r0 = (uint32_t)first_realization; P.w0 = (uint32_t)(first_realization >> 5);
     P.desc = desc ? 1 : 0;
     P.h = 0; P.ediv = 4; P.thrF = nullptr;
-    for (int c = 0; c < 14; ++c) P.zF[c] = -1;
+    for (int c = 0; c < 18; ++c) P.zF[c] = -1;
     P.spin = (uint32_t *)(h->ws + lay.spin);
     P.coup = (uint32_t *)(h->ws + lay.coup);
     P.lt = (uint32_t *)(h->ws + lay.lt);
@@ -544,7 +544,7 @@ extern "C" int ea_set_field(ea_handle *h, int field)
         CUDA_TRY(h, cudaStreamSynchronize(h->stream));
         h->field = 0;
         h->P.h = 0; h->P.ediv = 4; h->P.thrF = nullptr; h->P.swp_val = h->d_swp_val;
-        for (int c = 0; c < 14; ++c) h->P.zF[c] = -1;
+        for (int c = 0; c < 18; ++c) h->P.zF[c] = -1;
         const std::vector<uint64_t> acc = h->acc, swp = h->swp;
         int rc = upload_tables(h, acc, swp);                  // the zero-field swap table again
         if (rc != EA_OK) return rc;
@@ -567,8 +567,19 @@ extern "C" int ea_set_field(ea_handle *h, int field)
             swpf[(size_t)t * (size_t)cols + (size_t)(d2 + Mf)] = threshold_of(db * (double)(2 * d2));
     }
     // class thresholds in pos order (coldest first), as (threshold - 1); classes with dE <= 0 flip always
-    std::vector<uint32_t> thrF((size_t)14 * LTS, 0xFFFFFFFFu);
-    int zF[14];
+    std::vector<uint32_t> thrF((size_t)18 * LTS, 0xFFFFFFFFu);
+    int zF[18];
+    for (int j = 0; j < 4; ++j) {       // |h| <= 2: rows 14..17 = columns dE_j = 4 j + 2 (odd h) / 4 j + 4 (even h)
+        const double dE = (double)((field & 1) ? 4 * j + 2 : 4 * j + 4);
+        int zc = 0;
+        for (int pos = 0; pos < nT; ++pos) {
+            const int t = h->desc ? pos : nT - 1 - pos;
+            const uint64_t v = threshold_of(-(h->betas[t] * dE));
+            if (v == 0) { zc = pos + 1; thrF[(size_t)(14 + j) * LTS + pos] = 0; }
+            else thrF[(size_t)(14 + j) * LTS + pos] = (uint32_t)(v - 1);
+        }
+        zF[14 + j] = zc;
+    }
     for (int c = 0; c < 7; ++c)
         for (int up = 0; up < 2; ++up) {
             const int cls = 2 * c + up, dE = 4 * c - 12 - 2 * field * (2 * up - 1);
@@ -598,7 +609,7 @@ extern "C" int ea_set_field(ea_handle *h, int field)
     h->d_field = d;
     h->field = field;
     h->P.h = field; h->P.ediv = 2; h->P.thrF = (const uint32_t *)d; h->P.swp_val = (const uint32_t *)(d + o_val);
-    for (int c = 0; c < 14; ++c) h->P.zF[c] = zF[c];
+    for (int c = 0; c < 18; ++c) h->P.zF[c] = zF[c];
     h->accf.swap(accf);
     h->swpf.swap(swpf);
     return recompute_energy(h);
@@ -626,7 +637,7 @@ static cudaError_t launch_generic_persistent(ea_handle *h, int n_sweeps, int swa
     cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
     if (!coop) return cudaErrorNotSupported;
     const void *kern = h->field ? (const void *)ea::k_generic_persistent<true> : (const void *)ea::k_generic_persistent<false>;
-    const size_t smem = 4 * (h->field ? 14 : 3) * (size_t)(h->nT + 1);
+    const size_t smem = 4 * (h->field ? 18 : 3) * (size_t)(h->nT + 1);
     int per_sm = 0;
     cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, 256, smem);
     if (e != cudaSuccess) return e;
@@ -667,7 +678,7 @@ static int sweep_generic(ea_handle *h, int64_t n_sweeps, int swap_interval)
     const int64_t nthreads = (int64_t)h->nT * h->W * (h->N / 8);
     int grid;
     launch_cfg(nthreads, 128, grid);
-    const size_t smem = 4 * (h->field ? 14 : 3) * (size_t)(h->nT + 1);
+    const size_t smem = 4 * (h->field ? 18 : 3) * (size_t)(h->nT + 1);
     for (int64_t it = 0; it < n_sweeps; ++it) {
         if (h->field) {
             ea::k_half_sweep_field<<<grid, 128, smem, h->stream>>>(h->P, 0, (uint32_t)h->g);
