@@ -144,6 +144,30 @@ __device__ __forceinline__ int rank_of(uint32_t u, const uint32_t *thr32, int z,
     return lo;
 }
 
+// Positional popcount across a warp.  c[0..PL) are bit-sliced per-thread counters (plane i has
+// weight 2^i, bit b of every plane belongs to realization b); the sum over the 32 lanes must stay
+// below 2^PL.  Five butterfly levels of bit-sliced ripple adds (2 LOP3 + 1 SHFL per plane and
+// level) leave the warp total in every lane; lane b then returns the integer of bit position b.
+template <int PL>
+__device__ __forceinline__ int warp_positional_sum(uint32_t (&c)[PL], int lane)
+{
+#pragma unroll
+    for (int off = 16; off >= 1; off >>= 1) {
+        uint32_t carry = 0;
+#pragma unroll
+        for (int i = 0; i < PL; ++i) {
+            const uint32_t g = __shfl_xor_sync(0xFFFFFFFFu, c[i], off);
+            const uint32_t s = xor3(c[i], g, carry);
+            carry = maj3(c[i], g, carry);
+            c[i] = s;
+        }
+    }
+    int v = 0;
+#pragma unroll
+    for (int i = 0; i < PL; ++i) v += (int)((c[i] >> lane) & 1u) << i;
+    return v;
+}
+
 // Coordinates of checkerboard index j of parity p:  j = xh + Lh (y + L z), x = 2 xh + ((y+z+p)&1).
 struct Site { int xh, y, z, s; };
 __device__ __forceinline__ Site site_of(int j, int p, int L, int Lh)

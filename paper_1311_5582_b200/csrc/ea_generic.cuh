@@ -162,11 +162,13 @@ __global__ void __launch_bounds__(128) k_half_sweep_field(Params P, int p, uint3
 
 // Field term of the energy: E[r][k] += h * (2 * (number of up spins) - N).  One block per (w, k),
 // vertical counters like k_energy; runs after it.
-constexpr int kFieldPlanes = 15;   // per-thread count <= ceil(N / 128) <= 2^14
-
+// PL planes in all: the per-thread count (<= ceil(N / blockDim)) must stay below 2^(PL-5), the
+// warp total below 2^PL.
 // item = (w, k) handled by the whole block; sm_cnt = 32 ints of shared memory
+template <int PL>
 __device__ __forceinline__ void field_energy_item(const Params &P, int item, int *sm_cnt)
 {
+    constexpr int kFieldPlanes = PL;
     const int w = item / P.nT, k = item % P.nT;
     const uint32_t *sp = P.spin + ((size_t)k * P.W + w) * P.N;
     if (threadIdx.x < 32) sm_cnt[threadIdx.x] = 0;
@@ -174,47 +176,42 @@ __device__ __forceinline__ void field_energy_item(const Params &P, int item, int
     uint32_t c[kFieldPlanes];
 #pragma unroll
     for (int i = 0; i < kFieldPlanes; ++i) c[i] = 0;
+#pragma unroll 4
     for (int i = threadIdx.x; i < P.N; i += blockDim.x) {
         uint32_t x = sp[i];
 #pragma unroll
-        for (int l = 0; l < kFieldPlanes; ++l) {
+        for (int l = 0; l < kFieldPlanes - 5; ++l) {
             const uint32_t carry = c[l] & x;
             c[l] ^= x;
             x = carry;
         }
     }
     const int lane = threadIdx.x & 31;
-    int mine = 0;
-    for (int b = 0; b < 32; ++b) {
-        int v = 0;
-#pragma unroll
-        for (int l = 0; l < kFieldPlanes; ++l) v += (int)((c[l] >> b) & 1u) << l;
-        v = __reduce_add_sync(0xFFFFFFFFu, v);
-        if (lane == b) mine = v;
-    }
-    atomicAdd(&sm_cnt[lane], mine);
+    atomicAdd(&sm_cnt[lane], warp_positional_sum<PL>(c, lane));
     __syncthreads();
     if (threadIdx.x < 32)
         P.E[(size_t)(32 * w + threadIdx.x) * P.nT + k] += P.h * (2 * sm_cnt[threadIdx.x] - P.N);
     __syncthreads();
 }
 
+template <int PL>
 __global__ void __launch_bounds__(128) k_field_energy(Params P)
 {
     __shared__ int sm_cnt[32];
-    field_energy_item(P, blockIdx.x, sm_cnt);
+    field_energy_item<PL>(P, blockIdx.x, sm_cnt);
 }
 
 // ------------------------------------------------------------------ a8: energy from scratch
 // E[r][k] = 3N - 2 * (number of satisfied bonds); every bond has exactly one parity-1 end, so
 // the satisfied bonds are sum over parity-1 sites of n_sat.  One block per (w, k); per-thread
 // bit-sliced (vertical) counters, then a transposition to 32 integers with warp reductions.
-constexpr int kEnergyPlanes = 14;   // per-thread count <= 6 * ceil(Nh / 128)
-
-__device__ __forceinline__ void vadd(uint32_t (&c)[kEnergyPlanes], uint32_t x, int from)
+// PL planes in all: the per-thread count (<= 6 ceil(Nh / blockDim)) must stay below 2^(PL-5), the
+// warp total below 2^PL.
+template <int PL>
+__device__ __forceinline__ void vadd(uint32_t (&c)[PL], uint32_t x, int from)
 {
 #pragma unroll
-    for (int i = 0; i < kEnergyPlanes; ++i) {
+    for (int i = 0; i < PL - 5; ++i) {
         if (i < from) continue;
         const uint32_t t = c[i] & x;
         c[i] ^= x;
@@ -222,8 +219,10 @@ __device__ __forceinline__ void vadd(uint32_t (&c)[kEnergyPlanes], uint32_t x, i
     }
 }
 
+template <int PL>
 __device__ __forceinline__ void energy_item(const Params &P, int item, int *sm_cnt)
 {
+    constexpr int kEnergyPlanes = PL;
     const int w = item / P.nT, k = item % P.nT;
     const uint32_t *sp = P.spin + ((size_t)k * P.W + w) * P.N;
     const uint32_t *cp = P.coup + (size_t)w * 3 * P.N;
@@ -232,33 +231,36 @@ __device__ __forceinline__ void energy_item(const Params &P, int item, int *sm_c
     uint32_t c[kEnergyPlanes];
 #pragma unroll
     for (int i = 0; i < kEnergyPlanes; ++i) c[i] = 0;
-    for (int j = threadIdx.x; j < P.Nh; j += blockDim.x) {
-        uint32_t s;
-        const Planes pl = site_planes(sp, cp, 1, j, P.L, P.Lh, P.Nh, P.N, &s);
-        vadd(c, pl.b0, 0);
-        vadd(c, pl.b1, 1);
-        vadd(c, pl.b2, 2);
+    // four sites' loads in flight before the first add
+    for (int j0 = threadIdx.x; j0 < P.Nh; j0 += 4 * blockDim.x) {
+        Planes pl[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int j = j0 + u * blockDim.x;
+            uint32_t s;
+            if (j < P.Nh) pl[u] = site_planes(sp, cp, 1, j, P.L, P.Lh, P.Nh, P.N, &s);
+            else pl[u].b0 = pl[u].b1 = pl[u].b2 = 0u;
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            vadd<PL>(c, pl[u].b0, 0);
+            vadd<PL>(c, pl[u].b1, 1);
+            vadd<PL>(c, pl[u].b2, 2);
+        }
     }
     const int lane = threadIdx.x & 31;
-    int mine = 0;
-    for (int b = 0; b < 32; ++b) {
-        int v = 0;
-#pragma unroll
-        for (int i = 0; i < kEnergyPlanes; ++i) v += (int)((c[i] >> b) & 1u) << i;
-        v = __reduce_add_sync(0xFFFFFFFFu, v);
-        if (lane == b) mine = v;
-    }
-    atomicAdd(&sm_cnt[lane], mine);
+    atomicAdd(&sm_cnt[lane], warp_positional_sum<PL>(c, lane));
     __syncthreads();
     if (threadIdx.x < 32)
         P.E[(size_t)(32 * w + threadIdx.x) * P.nT + k] = 3 * P.N - 2 * sm_cnt[threadIdx.x];
     __syncthreads();
 }
 
+template <int PL>
 __global__ void __launch_bounds__(128) k_energy(Params P)
 {
     __shared__ int sm_cnt[32];
-    energy_item(P, blockIdx.x, sm_cnt);
+    energy_item<PL>(P, blockIdx.x, sm_cnt);
 }
 
 // ------------------------------------------------------------------ a9: PT swap round
@@ -351,8 +353,8 @@ __global__ void __launch_bounds__(256) k_generic_persistent(const PersistArgs A)
         const bool swap_now = A.swap_interval > 0 && ((uint64_t)g + 1) % (uint64_t)A.swap_interval == 0;
         if (!swap_now && it != A.n_sweeps - 1) continue;
         for (int item = blockIdx.x; item < P.W * P.nT; item += gridDim.x) {   // energies of the finished sweep
-            energy_item(P, item, sm_cnt);
-            if (FIELD) field_energy_item(P, item, sm_cnt);
+            energy_item<22>(P, item, sm_cnt);                 // 22 planes: any lattice the library takes
+            if (FIELD) field_energy_item<22>(P, item, sm_cnt);
         }
         if (!swap_now) continue;
         persist_grid_sync(A.gbar);

@@ -320,10 +320,17 @@ static int upload_tables(ea_handle *h, const std::vector<uint64_t> &acc, const s
 // ---------------------------------------------------------------- small helpers
 static int recompute_energy(ea_handle *h)
 {
-    ea::k_energy<<<h->W * h->nT, 128, 0, h->stream>>>(h->P);
+    // counter planes: per-thread count (6 Nh / 128 bonds, N / 128 up spins) < 2^(PL - 5)
+    const int grid = h->W * h->nT;
+    const long long per_thread = 6ll * ((h->N / 2 + 127) / 128);
+    if (per_thread < (1 << 8)) ea::k_energy<13><<<grid, 128, 0, h->stream>>>(h->P);
+    else if (per_thread < (1 << 12)) ea::k_energy<17><<<grid, 128, 0, h->stream>>>(h->P);
+    else ea::k_energy<22><<<grid, 128, 0, h->stream>>>(h->P);
     h->launches++;
     if (h->field != 0) {
-        ea::k_field_energy<<<h->W * h->nT, 128, 0, h->stream>>>(h->P);
+        if (per_thread < (1 << 8)) ea::k_field_energy<13><<<grid, 128, 0, h->stream>>>(h->P);
+        else if (per_thread < (1 << 12)) ea::k_field_energy<17><<<grid, 128, 0, h->stream>>>(h->P);
+        else ea::k_field_energy<22><<<grid, 128, 0, h->stream>>>(h->P);
         h->launches++;
     }
     CUDA_TRY(h, cudaGetLastError());

@@ -89,9 +89,9 @@ __global__ void __launch_bounds__(128) k_overlap_words(Params P, const uint32_t 
     const uint32_t *Tb = wb >= 0 ? T + ((size_t)t * P.W + wb) * P.N : nullptr;
     if (threadIdx.x < 32) sm_cnt[threadIdx.x] = 0;
     __syncthreads();
-    uint32_t c[kOverlapPlanes];
+    uint32_t c[kOverlapPlanes + 5];          // five more planes for the sum over the warp's lanes
 #pragma unroll
-    for (int i = 0; i < kOverlapPlanes; ++i) c[i] = 0;
+    for (int i = 0; i < kOverlapPlanes + 5; ++i) c[i] = 0;
     // 128-bit loads, four vectors of each word in flight per thread before the first add
     const uint4 *Va = reinterpret_cast<const uint4 *>(Ta), *Vb = reinterpret_cast<const uint4 *>(Tb);
     const int nv = P.N / 4;
@@ -120,15 +120,7 @@ __global__ void __launch_bounds__(128) k_overlap_words(Params P, const uint32_t 
         }
     }
     const int lane = threadIdx.x & 31;
-    int mine = 0;
-    for (int b = 0; b < 32; ++b) {
-        int v = 0;
-#pragma unroll
-        for (int l = 0; l < kOverlapPlanes; ++l) v += (int)((c[l] >> b) & 1u) << l;
-        v = __reduce_add_sync(0xFFFFFFFFu, v);
-        if (lane == b) mine = v;
-    }
-    atomicAdd(&sm_cnt[lane], mine);
+    atomicAdd(&sm_cnt[lane], warp_positional_sum<PL + 5>(c, lane));
     __syncthreads();
     if (threadIdx.x >= 32) return;
     const int ra = 32 * wa + lane, rb = wb >= 0 ? 32 * wb + lane : -1;
