@@ -179,7 +179,7 @@ int ea_get_moments(ea_handle *h, uint64_t *n_meas, int64_t *q1 /* [P][32][n_temp
 /* Plane-sum correlations of the local overlap q_i = s_i(ra, t) s_i(rb, t), accumulated by every
  * measurement: C[p][b][t][d] = sum over measurements, over the three axes mu and over the planes c
  * of S_mu(c) S_mu((c + d) mod L), S_mu(c) = sum of q_i over the plane (coordinate mu of i) = c
- * (R23).  sum_d C = 3 * (sum of q^2).  Not accumulated for L > 85. */
+ * (R23).  sum_d C = 3 * (sum of q^2). */
 int ea_get_correlation(ea_handle *h, int64_t *C /* [P][32][n_temps][L] */);
 
 /* Second-moment correlation length by temperature index (the quantity of the paper's Fig. 19,

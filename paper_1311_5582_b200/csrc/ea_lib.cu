@@ -1209,8 +1209,9 @@ static int measure_once(ea_handle *h)
         else if (per_thread < (1 << 9)) ea::k_overlap_words<9><<<grid, 128, 0, h->stream>>>(h->P, h->d_T, h->M, nullptr);
         else if (per_thread < (1 << 12)) ea::k_overlap_words<12><<<grid, 128, 0, h->stream>>>(h->P, h->d_T, h->M, nullptr);
         else ea::k_overlap_words<15><<<grid, 128, 0, h->stream>>>(h->P, h->d_T, h->M, nullptr);
-        if (h->L <= 85) {       // plane-sum correlations: 3 axes x L planes x >= 1 thread in a block of 256
-            const int nsub = std::max(1, ea::kCorrThreads / (3 * h->L));
+        if (3 * h->L <= ea::kCorrThreads) {     // plane-sum correlations: 3 axes x L planes x nsub threads per block
+            int nsub = 1;
+            while (2 * nsub <= 32 && 2 * nsub * 3 * h->L <= ea::kCorrThreads) nsub *= 2;
             const int per_thread = (h->L * h->L + nsub - 1) / nsub;            // sites per thread < 2^PL
             const bool stage = 4 * (size_t)h->N <= 128 * 1024;
             const size_t sm = 4 * (size_t)((32 * (3 * h->L + 1) + 3) & ~3) + (stage ? 4 * (size_t)h->N : 0);

@@ -146,10 +146,12 @@ __global__ void __launch_bounds__(128) k_overlap_words(Params P, const uint32_t 
 // Fourier sum over the L values is done on the host).  The agreement words ~(Ta ^ Tb) of the
 // lattice are staged in shared memory with coalesced 128-bit loads (STAGE; lattices of up to
 // 128 KiB, L <= 32), then thread = (axis mu, plane c, sub) walks its share of the plane's L^2
-// sites (scattered: the store is checkerboard-ordered), counts agreeing bits in vertical
-// counters, and the counts of a plane's threads meet in shared memory.  One block per (p, t)
-// is the only writer of its accumulators: no global atomics, fixed order.
-constexpr int kCorrThreads = 256;
+// sites (scattered: the store is checkerboard-ordered) and counts agreeing bits in vertical
+// counters.  The nsub threads of a plane (a power of two, adjacent lanes of one warp) add their
+// counters with a bit-sliced butterfly and share out the 32 bit positions, so every plane sum has
+// one writer.  One block per (p, t) is the only writer of its accumulators: no atomics at all,
+// fixed order.
+constexpr int kCorrThreads = 512;
 
 template <int PL, bool STAGE>
 __global__ void __launch_bounds__(kCorrThreads) k_plane_corr(Params P, const uint32_t *T, Moments M)
@@ -175,14 +177,16 @@ __global__ void __launch_bounds__(kCorrThreads) k_plane_corr(Params P, const uin
         }
     }
     __syncthreads();
-    const int nsub = max(1, (int)blockDim.x / (3 * L));          // threads per plane
+    int nsub = 1;                                                // threads per plane: power of two <= 32
+    while (2 * nsub <= 32 && 2 * nsub * 3 * L <= (int)blockDim.x) nsub *= 2;
     const int mu = threadIdx.x / (L * nsub), rem = threadIdx.x % (L * nsub);
     const int c = rem / nsub, sub = rem % nsub;                  // the lanes of a warp share a plane: their
                                                                  // sites are neighbours in x (or y for mu = 0)
-    if (mu < 3) {
-        uint32_t cnt[PL];
+    {
+        uint32_t cnt[PL + 5];                                    // five planes of headroom for the butterfly
 #pragma unroll
-        for (int l = 0; l < PL; ++l) cnt[l] = 0;
+        for (int l = 0; l < PL + 5; ++l) cnt[l] = 0;
+        if (mu < 3) {
         // (u, v) = the two coordinates inside the plane, stepped without divisions
         int u = sub % L, v = sub / L;
         const int du = nsub % L, dv = nsub / L;
@@ -199,12 +203,24 @@ __global__ void __launch_bounds__(kCorrThreads) k_plane_corr(Params P, const uin
                 w = carry;
             }
         }
-        for (int b = 0; b < 32; ++b) {
-            int v = 0;
-#pragma unroll
-            for (int l = 0; l < PL; ++l) v += (int)((cnt[l] >> b) & 1u) << l;
-            if (v) atomicAdd(&sm_S[b * RS + mu * L + c], v);
         }
+        for (int off = 1; off < nsub; off <<= 1) {               // sum over the plane's threads (all lanes shuffle)
+            uint32_t carry = 0;
+#pragma unroll
+            for (int l = 0; l < PL + 5; ++l) {
+                const uint32_t g = __shfl_xor_sync(0xFFFFFFFFu, cnt[l], off);
+                const uint32_t sum = xor3(cnt[l], g, carry);
+                carry = maj3(cnt[l], g, carry);
+                cnt[l] = sum;
+            }
+        }
+        if (mu < 3)
+            for (int b = sub; b < 32; b += nsub) {               // my share of the bit positions
+                int v = 0;
+#pragma unroll
+                for (int l = 0; l < PL + 5; ++l) v += (int)((cnt[l] >> b) & 1u) << l;
+                sm_S[b * RS + mu * L + c] = v;
+            }
     }
     __syncthreads();
     for (int a = threadIdx.x; a < 32 * RS; a += blockDim.x) sm_S[a] = 2 * sm_S[a] - L * L;   // agree - disagree
