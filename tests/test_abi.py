@@ -56,3 +56,18 @@ def test_product_does_not_touch_oracle():
             assert "import oracle" not in text and "from oracle" not in text and "ea_oracle" not in text
     for path in (ROOT / "oracle").rglob("*.py"):
         assert "paper_1311_5582_b200" not in path.read_text().replace("(paper_1311_5582_b200)", "")
+
+
+def test_header_is_plain_c_and_the_c_example_links(built, tmp_path):
+    """include/ea.h must compile as C (the boundary is a C ABI), and the C example must build and
+    link against libea_b200.so with nothing but the header (it is run on the GPU box only)."""
+    import subprocess
+    inc = ROOT / "include"
+    subprocess.check_call(["gcc", "-std=c99", "-Wall", "-Werror", "-pedantic", "-fsyntax-only", "-x", "c",
+                           str(inc / "ea.h")])
+    src = ROOT / "paper_1311_5582_b200" / "examples" / "ea_demo.c"
+    exe = tmp_path / "ea_demo"
+    subprocess.check_call(["gcc", "-std=c99", "-Wall", "-Werror", str(src), "-I", str(inc),
+                           "-L", str(built.library_path().parent), "-lea_b200", "-lm",
+                           f"-Wl,-rpath,{built.library_path().parent}", "-o", str(exe)])
+    assert exe.exists()

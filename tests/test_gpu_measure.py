@@ -197,3 +197,22 @@ def test_shard_measurements_and_field_equal_the_full_run():
     assert (full.get_state()["spin_words"][:, 1:3] == part.get_state()["spin_words"]).all()
     for x in (full, part, again):
         x.destroy()
+
+
+def test_c_example_runs_from_plain_c(tmp_path):
+    """The C ABI from a C program (no Python in the process): builds, runs, prints a physical table:
+    E/N near the +-J ground-state energy (about -1.79) at T = 0.5 and a Binder ratio that falls with T."""
+    import subprocess
+    from pathlib import Path
+    pkg, _, _ = _mods()
+    root = Path(__file__).resolve().parents[1]
+    exe = tmp_path / "ea_demo"
+    lib_dir = pkg.library_path().parent
+    subprocess.check_call(["gcc", "-std=c99", str(root / "paper_1311_5582_b200" / "examples" / "ea_demo.c"),
+                           "-I", str(root / "include"), "-L", str(lib_dir), "-lea_b200", "-lm",
+                           f"-Wl,-rpath,{lib_dir}", "-o", str(exe)])
+    out = subprocess.run([str(exe)], capture_output=True, text=True, timeout=120)
+    assert out.returncode == 0, out.stderr
+    rows = [[float(x) for x in line.split()] for line in out.stdout.splitlines()[1:]]
+    assert len(rows) == 16 and abs(rows[0][0] - 0.5) < 1e-3 and abs(rows[-1][0] - 2.0) < 1e-3
+    assert -1.80 < rows[0][1] < -1.74 and rows[0][2] > 0.85 and rows[-1][2] < 0.3
