@@ -51,6 +51,9 @@ def _compare(g, acc, binder_ratio):
     (16, 4, 64, 3, [[0, 1], [1, -1]], 2, 2, 1),                      # tiled
     (32, 4, 64, 4, [[0, 1]], 2, 1, 1),                               # stream
     (6, 3, 40, 0, [[0, 1], [1, 0]], 4, 1, 0),                        # no PT, L = 6
+    (12, 3, 64, 0, [[0, 1], [1, -1]], 2, 2, 1),                      # L = 12: 8 threads per plane, 36 planes
+    (64, 2, 64, 0, [[0, 1]], 1, 1, 1),                               # L = 64: correlations without staging
+    (4, 64, 64, 0, [[1, 0]], 2, 1, 1),                               # 64 temperatures: eight gather groups
 ])
 def test_moments_and_binder_match_oracle(L, nT, R, kernel, wp, n_meas, between, swap):
     pkg, Oracle, binder_ratio = _mods()
