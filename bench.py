@@ -258,14 +258,18 @@ def run_cuda(a, cfg):
     peak = measure_int_peak(torch.cuda.current_stream().cuda_stream)
     # resident kernel: one launch per step, so the step time IS the kernel's launch duration;
     # generic path: the step is sweep + energy + swap launches and the figure is for the step.
-    alu_ops_per_step = ALU_OPS_PER_WORD_UPDATE * cfg.n_temps * cfg.W * cfg.N * sps
+    # 30 on every update + 7.75 for the energy pass, which only runs on sweeps followed by a swap
+    # round (and the last sweep of a call): 38 for the configs' PT every sweep
+    e_frac = (1.0 / cfg.swap_interval) if cfg.swap_interval > 0 else 1.0 / sps
+    ops_per_update = 30.0 + (ALU_OPS_PER_WORD_UPDATE - 30.0) * e_frac
+    alu_ops_per_step = ops_per_update * cfg.n_temps * cfg.W * cfg.N * sps
     achieved = alu_ops_per_step / (float(np.mean(step_ms)) * 1e-3)
     roofline = {"bound": "alu", "achieved": achieved / 1e12, "peak": peak["lop3"] / 1e12, "unit": "Tlaneop/s",
                 "frac": achieved / peak["lop3"], "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(a.config),
-                "note": "ALU-pipe lane-ops: %.0f per word update (DESIGN.md s8) / measured LOP3 issue peak "
+                "note": "ALU-pipe lane-ops: %.1f per word update (DESIGN.md s8) / measured LOP3 issue peak "
                         "(ea_measure_int_peak, same process); IMAD peak %.2f, LOP3+IMAD mix %.2f Tlaneop/s; "
                         "ncu: ALU pipe %s busy on the occupied SMs (profiles/)"
-                        % (ALU_OPS_PER_WORD_UPDATE, peak["imad"] / 1e12, peak["mix"] / 1e12,
+                        % (ops_per_update, peak["imad"] / 1e12, peak["mix"] / 1e12,
                            NCU_ALU_PIPE_BUSY.get(a.config, "n/a"))}
     if kernel == 4:
         # streaming kernel: algorithmic bytes = per half-sweep and item, tile read (own parity 8 KiB +
@@ -319,12 +323,17 @@ def main():
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--config", type=int, default=4)
     ap.add_argument("--sweeps-per-step", type=int, default=5000)
+    ap.add_argument("--swap-interval", type=int, default=None,
+                    help="override the config's PT cadence (the paper's own benchmark swaps every 10 sweeps, PAPER.md:307)")
     ap.add_argument("--field", type=int, default=0, help="external field h (SURVEY 8(f2)); default 0 = headline workload")
     ap.add_argument("--measure-every", type=int, default=0,
                     help="accumulate two-copy overlap / energy moments every M sweeps (SURVEY 8(f1)); default off")
     a = ap.parse_args()
     a.warmup = max(a.warmup, 3) if a.impl == "cuda" else a.warmup
     cfg = CONFIGS[a.config]
+    if a.swap_interval is not None:
+        import dataclasses
+        cfg = dataclasses.replace(cfg, swap_interval=a.swap_interval)
     if a.impl == "reference":
         run_reference(a, cfg)
     else:
