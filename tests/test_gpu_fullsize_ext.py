@@ -93,3 +93,29 @@ def test_cfg4_with_field_on_sampled_words():
         assert (st["temp_of_slot"][32 * w:32 * w + 32] == o.perm()[0]).all()
         assert (E[32 * w:32 * w + 32] == o.energy()).all()
     g.destroy()
+
+
+@pytest.mark.parametrize("L,nT,R,sweeps,words", [
+    (16, 24, 8192, 12, (0, 100, 255)),      # four times config 4: 512 resident blocks on 148 SMs (several waves)
+    (32, 32, 2048, 3, (0, 37, 63)),         # eight times config 5: more work items than the streaming plan takes
+])
+def test_problems_larger_than_the_gpu_on_sampled_words(L, nT, R, sweeps, words):
+    """More realization words than the device can hold at once: the launch runs in waves (resident)
+    or falls back to a path without co-residency requirements; sampled words must still follow
+    the oracle bit for bit."""
+    pkg, Oracle = _mods()
+    from ea_inputs import temperature_ladder
+    betas = 1.0 / temperature_ladder(nT, 0.8, 2.0)
+    g = pkg.EA(L, nT, R, betas, 44)
+    kernel = g.get_kernel()
+    g.sweep(sweeps, 1)
+    st = g.get_state()
+    E = g.energy()
+    for w in words:
+        o = Oracle(L, nT, 32, betas, 44, r0=32 * w)
+        o.sweep(sweeps, 1)
+        assert (_word_spins(st, w, L) == o.spins_by_slot()).all(), (kernel, w)
+        assert (st["temp_of_slot"][32 * w:32 * w + 32] == o.perm()[0]).all()
+        assert (E[32 * w:32 * w + 32] == o.energy()).all()
+    print("kernel used:", kernel)
+    g.destroy()
