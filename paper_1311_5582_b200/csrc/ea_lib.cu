@@ -897,14 +897,15 @@ static int sweep_tiled(ea_handle *h, int64_t n_sweeps, int swap_interval)
 
 // ---------------------------------------------------------------- streaming path (L = 32, 64)
 namespace {
-struct StreamPlan { bool ok; int grid, MS, MW, swap_win; size_t smem, esm_off, batch_off; };
+struct StreamPlan { bool ok; int grid, MS, MW, swap_win; size_t smem, esm_off, batch_off; int Wn; };
 
+// plan for one launch over Wn realization words
 template <int L>
-StreamPlan plan_stream_t(const ea_handle *h)
+StreamPlan plan_stream_words(const ea_handle *h, int Wn)
 {
     using Sg = ea::StreamGeom<L>;
-    StreamPlan pl{false, 0, 0, 0, 0, 0, 0, 0};
-    const long long T = (long long)h->W * Sg::NSLAB * h->nT;
+    StreamPlan pl{false, 0, 0, 0, 0, 0, 0, 0, Wn};
+    const long long T = (long long)Wn * Sg::NSLAB * h->nT;
     if (T >= (1ll << 31)) return pl;
     pl.grid = (int)std::min<long long>(h->sm_count, T);
     pl.MS = (int)((T + pl.grid - 1) / pl.grid);
@@ -924,15 +925,30 @@ StreamPlan plan_stream_t(const ea_handle *h)
     return pl;
 }
 
+// Words never interact, so a problem whose per-block tables do not fit shared memory is run as
+// several launches over balanced groups of words, each for all sweeps of the call: the fewest
+// groups whose plan fits.
+template <int L>
+StreamPlan plan_stream_t(const ea_handle *h)
+{
+    for (int groups = 1; groups <= h->W; ++groups) {
+        const int Wn = (h->W + groups - 1) / groups;
+        const StreamPlan pl = plan_stream_words<L>(h, Wn);
+        if (pl.ok) return pl;
+        if (Wn == 1) break;
+    }
+    return StreamPlan{false, 0, 0, 0, 0, 0, 0, 0, 0};
+}
+
 StreamPlan plan_stream(const ea_handle *h)
 {
     int coop = 0, dev = 0;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
-    if (!coop) return StreamPlan{false, 0, 0, 0, 0, 0, 0, 0};
+    if (!coop) return StreamPlan{false, 0, 0, 0, 0, 0, 0, 0, 0};
     if (h->L == 32) return plan_stream_t<32>(h);
     if (h->L == 64) return plan_stream_t<64>(h);
-    return StreamPlan{false, 0, 0, 0, 0, 0, 0, 0};
+    return StreamPlan{false, 0, 0, 0, 0, 0, 0, 0, 0};
 }
 
 template <int L>
@@ -958,18 +974,34 @@ static int sweep_stream(ea_handle *h, int64_t n_sweeps, int swap_interval)
     int64_t left = n_sweeps;
     while (left > 0) {
         const int chunk = (int)std::min<int64_t>(left, 1 << 30);
+      for (int w_off = 0; w_off < h->W; w_off += pl.Wn) {      // groups of words, each for all sweeps of the chunk
+        const int Wg = std::min(pl.Wn, h->W - w_off);
+        const StreamPlan pg = Wg == pl.Wn ? pl : (h->L == 32 ? plan_stream_words<32>(h, Wg) : plan_stream_words<64>(h, Wg));
+        if (!pg.ok) return fail(h, EA_ERR_UNSUPPORTED, "stream kernel: word group does not fit");
         ea::StreamArgs A{};
         A.P = h->P;
+        A.Wn = Wg;
+        {   // this group's view of the state: pointers, w0 and r0 move to its first word
+            Params &Q = A.P;
+            Q.spin += (size_t)w_off * h->N;
+            Q.coup += (size_t)w_off * 3 * h->N;
+            Q.lt += (size_t)w_off * h->nT * (h->nT + 1);
+            Q.tau += (size_t)32 * w_off * h->nT;
+            Q.sigma += (size_t)32 * w_off * h->nT;
+            Q.E += (size_t)32 * w_off * h->nT;
+            Q.w0 += (uint32_t)w_off;
+            Q.r0 += 32u * (uint32_t)w_off;
+        }
         A.g0 = (uint32_t)h->g;
         A.n_sweeps = chunk;
         A.swap_interval = swap_interval;
         A.nswap0 = (uint32_t)h->nswap;
-        A.Ecnt = h->d_Ecnt;
+        A.Ecnt = h->d_Ecnt + (size_t)32 * w_off * h->nT;
         A.gbar = (unsigned int *)(h->d_Ecnt + 2 * (size_t)h->Rp * h->nT);
         A.bucket = h->d_bucket; A.n_bucket = h->n_bucket; A.trip = h->d_trip;
         A.key_lo = h->key_lo; A.key_shift = h->key_shift;
         A.ones = 0xFFFFFFFFu; A.c48 = 48u; A.cm16 = (uint32_t)-16; A.c16 = 16u;
-        A.MS = pl.MS; A.MW = pl.MW; A.swap_win = pl.swap_win; A.esm_off = (int)pl.esm_off; A.batch_off = (int)pl.batch_off;
+        A.MS = pg.MS; A.MW = pg.MW; A.swap_win = pg.swap_win; A.esm_off = (int)pg.esm_off; A.batch_off = (int)pg.batch_off;
         for (int r = 0; r < 10; ++r) {
             A.rk[2 * r] = h->P.k0 + (uint32_t)r * 0x9E3779B9u;
             A.rk[2 * r + 1] = h->P.k1 + (uint32_t)r * 0xBB67AE85u;
@@ -977,15 +1009,15 @@ static int sweep_stream(ea_handle *h, int64_t n_sweeps, int swap_interval)
         // debug aid: EA_STREAM_TRACE=<file> dumps per-block phase time stamps of the first 8 sweeps
         const char *trace_path = std::getenv("EA_STREAM_TRACE");
         unsigned long long *d_trace = nullptr;
-        const size_t trace_n = (size_t)pl.grid * 64;
+        const size_t trace_n = (size_t)pg.grid * 64;
         if (trace_path && cudaMalloc((void **)&d_trace, 8 * trace_n) == cudaSuccess) {
             cudaMemsetAsync(d_trace, 0, 8 * trace_n, h->stream);
             A.trace = d_trace;
         }
         // counters and the grid-barrier word start from zero in every launch
         CUDA_TRY(h, cudaMemsetAsync(h->d_Ecnt, 0, 2 * 4 * (size_t)h->Rp * h->nT + 256, h->stream));
-        const cudaError_t e = h->L == 32 ? launch_stream_t<32>(h, A, pl, h->fast_rank)
-                                         : launch_stream_t<64>(h, A, pl, h->fast_rank);
+        const cudaError_t e = h->L == 32 ? launch_stream_t<32>(h, A, pg, h->fast_rank)
+                                         : launch_stream_t<64>(h, A, pg, h->fast_rank);
         if (d_trace) {
             std::vector<unsigned long long> tr(trace_n);
             cudaMemcpyAsync(tr.data(), d_trace, 8 * trace_n, cudaMemcpyDeviceToHost, h->stream);
@@ -993,7 +1025,7 @@ static int sweep_stream(ea_handle *h, int64_t n_sweeps, int swap_interval)
             if (FILE *f = std::fopen(trace_path, "wb")) { std::fwrite(tr.data(), 8, trace_n, f); std::fclose(f); }
             cudaFree(d_trace);
         }
-        if (e == cudaErrorCooperativeLaunchTooLarge && h->kernel_sel == EA_KERNEL_AUTO) {
+        if (e == cudaErrorCooperativeLaunchTooLarge && h->kernel_sel == EA_KERNEL_AUTO && w_off == 0) {
             // the SMs are not all free (another context holds some): same result, one launch per
             // half-sweep instead of one cooperative launch
             cudaGetLastError();
@@ -1001,6 +1033,7 @@ static int sweep_stream(ea_handle *h, int64_t n_sweeps, int swap_interval)
         }
         if (e != cudaSuccess) return fail(h, EA_ERR_CUDA, std::string("stream launch: ") + cudaGetErrorString(e));
         h->launches++;
+      }
         if (swap_interval > 0) h->nswap += (h->g + (uint64_t)chunk) / (uint64_t)swap_interval - h->g / (uint64_t)swap_interval;
         h->g += (uint64_t)chunk;
         left -= chunk;

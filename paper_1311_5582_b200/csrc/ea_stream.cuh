@@ -32,6 +32,8 @@ struct StreamArgs {
     int n_sweeps;
     int swap_interval;
     uint32_t nswap0;         // swap rounds done before this call
+    int Wn;                  // realization words of THIS launch (P's pointers, w0 and r0 are offset to
+                             // its first word; P.W and P.Rp stay the strides of the whole problem)
     int32_t *Ecnt;           // [2][Rp][nT] satisfied-bond counters (zero on entry)
     const uint4 *bucket;
     const uchar4 *trip;
@@ -336,7 +338,7 @@ __global__ void __launch_bounds__(StreamGeom<L>::NTHR, 1) k_stream(const StreamA
     constexpr int NTA = NT;
 
     StreamCtx<L> C;
-    const long long T = (long long)P.W * NSLAB * nT;
+    const long long T = (long long)A.Wn * NSLAB * nT;
     C.i0 = (int)(T * blockIdx.x / gridDim.x);
     C.i1 = (int)(T * (blockIdx.x + 1) / gridDim.x);
     const int per_w = NSLAB * nT;

@@ -97,12 +97,13 @@ def test_cfg4_with_field_on_sampled_words():
 
 @pytest.mark.parametrize("L,nT,R,sweeps,words", [
     (16, 24, 8192, 12, (0, 100, 255)),      # four times config 4: 512 resident blocks on 148 SMs (several waves)
-    (32, 32, 2048, 3, (0, 37, 63)),         # eight times config 5: more work items than the streaming plan takes
+    (32, 32, 2048, 3, (0, 37, 63)),         # eight times config 5: the streaming kernel runs word group by word group
+    (32, 32, 608, 2, (0, 9, 10, 18)),       # 19 words: two groups of 10 and 9 (first and last word of each)
 ])
 def test_problems_larger_than_the_gpu_on_sampled_words(L, nT, R, sweeps, words):
     """More realization words than the device can hold at once: the launch runs in waves (resident)
-    or falls back to a path without co-residency requirements; sampled words must still follow
-    the oracle bit for bit."""
+    or word group by word group (streaming: words never interact, so each group runs all sweeps
+    of the call on its own); sampled words must still follow the oracle bit for bit."""
     pkg, Oracle = _mods()
     from ea_inputs import temperature_ladder
     betas = 1.0 / temperature_ladder(nT, 0.8, 2.0)
@@ -118,4 +119,5 @@ def test_problems_larger_than_the_gpu_on_sampled_words(L, nT, R, sweeps, words):
         assert (st["temp_of_slot"][32 * w:32 * w + 32] == o.perm()[0]).all()
         assert (E[32 * w:32 * w + 32] == o.energy()).all()
     print("kernel used:", kernel)
+    assert kernel == (2 if L == 16 else 4)
     g.destroy()
