@@ -325,15 +325,19 @@ def main():
     ap.add_argument("--sweeps-per-step", type=int, default=5000)
     ap.add_argument("--swap-interval", type=int, default=None,
                     help="override the config's PT cadence (the paper's own benchmark swaps every 10 sweeps, PAPER.md:307)")
+    ap.add_argument("--realizations", type=int, default=None,
+                    help="override the config's number of disorder realizations per GPU (scaling studies)")
     ap.add_argument("--field", type=int, default=0, help="external field h (SURVEY 8(f2)); default 0 = headline workload")
     ap.add_argument("--measure-every", type=int, default=0,
                     help="accumulate two-copy overlap / energy moments every M sweeps (SURVEY 8(f1)); default off")
     a = ap.parse_args()
     a.warmup = max(a.warmup, 3) if a.impl == "cuda" else a.warmup
     cfg = CONFIGS[a.config]
+    import dataclasses
     if a.swap_interval is not None:
-        import dataclasses
         cfg = dataclasses.replace(cfg, swap_interval=a.swap_interval)
+    if a.realizations is not None:
+        cfg = dataclasses.replace(cfg, R=a.realizations, name=f"{cfg.name}_R{a.realizations}")
     if a.impl == "reference":
         run_reference(a, cfg)
     else:
