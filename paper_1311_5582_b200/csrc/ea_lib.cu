@@ -38,7 +38,8 @@ struct ea_handle {
     size_t swp_val_cap = 0;
     int32_t *d_Ecnt = nullptr;         // satisfied-bond counters of the tiled path
     uint4 *d_bucket = nullptr;         // fast rank table (ea_resident.cuh), 16 B entries
-    int n_bucket = 0, key_lo = 0, key_shift = 0;
+    int n_bucket = 0;
+    ea::RankKey K{};                   // bucket key parameters of the fast rank table
     uchar4 *d_trip = nullptr;          // [3 nT + 1] combined rank -> (n4, n5, n6)
     bool fast_rank = false;
     uint64_t g = 0, nswap = 0;
@@ -127,18 +128,38 @@ void launch_cfg(int64_t n, int block, int &grid) { grid = (int)((n + block - 1) 
 
 
 // ---------------------------------------------------------------- fast rank table
-// Buckets of the draw u by its leading bits: key(u) = bits of (float)u (truncating conversion)
-// >> (23 - MB) = exponent and MB mantissa bits; table index = max(key - key_lo, 0), covering
-// every u up to 2^32 - 1.  Entry = { 16 * (n4 + n5 + n6 at the bucket's lower edge), thr4, thr5,
-// thr6 }: n_c = number of class-c thresholds <= the lower edge, thr_c = the class-c
-// (threshold - 1) inside the bucket or 0xFFFFFFFF.  Buckets holding several thresholds of one
-// class, and all u < 2^8 (index 0), point at row 3 nT + 1 of the mask tables = "use the exact
-// search".  MB is the smallest of 3..6 that leaves < 1e-5 of the draws on the slow path.  (Measured
-// on config 4: a finer table removes the slow quads, worth 5 %, but spreads the look-ups over more
-// shared-memory banks, which costs 6 %.)
+// Buckets of the draw u by a monotone key with logarithmic steps that the kernels evaluate on the
+// FMA pipe (ea_resident.cuh, RankCtx):
+//   key(u) = bits(g) >> (23 - MB),   g = sat(float_rz(u) * 2^-E + 2^(8-E)),
+// E = number of bits of the largest threshold (every larger u takes the same decisions and
+// saturates onto the last bucket), the added constant merging all u << 2^8 into the first.  The
+// host evaluates the same function exactly (the sum is exact in double, the cast rounds once as
+// the device's fused multiply-add does) and finds every bucket's range of u by bisection.
+// Entry = { ~thr4, n4 + n5 + n6 at the bucket's lower edge, ~thr5, ~thr6 }: n_c = number of class-c
+// thresholds <= the lower edge, thr_c = the class-c (threshold - 1) inside the bucket or
+// 0xFFFFFFFF.  Buckets holding several thresholds of one class point at row 3 nT + 1 of the mask
+// tables = "use the exact search".  MB is the smallest of 3..6 that leaves < 1e-5 of the draws on
+// the slow path.
 // trip[n] = the triple (n4, n5, n6) whose sum is n (unique: each n_c is monotone in u).
+namespace {
+struct KeyFn {
+    int E, MB;
+    int operator()(uint32_t u) const
+    {
+        double f = (double)u;                                  // cvt.rz.f32.u32: keep the leading 24 bits
+        if (u >> 24) { const int sh = 8 - __builtin_clz(u); f = (double)((u >> sh) << sh); }
+        const double x = std::ldexp(f, -E) + std::ldexp(1.0, 8 - E);   // exact in double
+        float g = (float)x;                                    // one rounding to nearest even, as fma.rn
+        if (g > 1.0f) g = 1.0f;                                // .sat
+        uint32_t b;
+        std::memcpy(&b, &g, 4);
+        return (int)(b >> (23 - MB));
+    }
+};
+}  // namespace
+
 static bool build_bucket_table(const std::vector<uint32_t> &thr32, const int z[3], int nT,
-                               std::vector<uint4> &tab, std::vector<uchar4> &trip, int &key_lo, int &key_shift)
+                               std::vector<uint4> &tab, std::vector<uchar4> &trip, ea::RankKey &K)
 {
     auto rank_c = [&](int c, uint64_t u) {   // n_c(u) = z_c + #{i >= z_c : thr32[c][i] < u}
         int n = z[c];
@@ -151,30 +172,39 @@ static bool build_bucket_table(const std::vector<uint32_t> &thr32, const int z[3
         trip[(size_t)(a + b + c)] = make_uchar4((unsigned char)a, (unsigned char)b, (unsigned char)c, 0);
     };
     note(0);
+    uint32_t tmax = 0;
     for (int c = 0; c < 3; ++c)
-        for (int i = z[c]; i < nT; ++i) note((uint64_t)thr32[(size_t)c * (nT + 1) + i] + 1);
-    const int LOWEXP = 8;
-    const uint32_t slow_row = 16u * (uint32_t)(3 * nT + 1);
+        for (int i = z[c]; i < nT; ++i) {
+            const uint32_t v = thr32[(size_t)c * (nT + 1) + i];
+            note((uint64_t)v + 1);
+            if (v != 0xFFFFFFFFu) tmax = std::max(tmax, v);
+        }
+    int E = 9;
+    while (E < 32 && (tmax >> E)) ++E;                     // 2^E > every threshold - 1
+    const uint32_t slow_row = (uint32_t)(3 * nT + 1);
     for (int MB = 3; MB <= 6; ++MB) {
-        auto key_of = [&](uint32_t u) -> int {
-            if (u == 0) return 0;
-            int e = 31;
-            while (!((u >> e) & 1u)) --e;
-            const uint32_t mant = e >= MB ? (u >> (e - MB)) & ((1u << MB) - 1) : (u << (MB - e)) & ((1u << MB) - 1);
-            return ((e + 127) << MB) | (int)mant;
-        };
-        const int klo = key_of(1u << LOWEXP) - 1;
-        const int khi = key_of(0xFFFFFFFFu);
+        const KeyFn key{E, MB};
+        const int klo = key(0), khi = key(0xFFFFFFFFu);
         const int n = khi - klo + 1;
         if (n > kMaxBucket) continue;
+        // first u of every bucket (2^32 for an empty bucket at the top)
+        std::vector<uint64_t> first((size_t)n + 1);
+        first[0] = 0;
+        first[(size_t)n] = (uint64_t)1 << 32;
+        for (int b = 1; b < n; ++b) {
+            uint64_t lo = first[(size_t)b - 1], hi = (uint64_t)1 << 32;   // smallest u with key(u) - klo >= b
+            while (lo < hi) {
+                const uint64_t mid = (lo + hi) >> 1;
+                if (key((uint32_t)mid) - klo >= b) hi = mid; else lo = mid + 1;
+            }
+            first[(size_t)b] = lo;
+        }
         std::vector<uint4> t((size_t)n);
-        t[0] = make_uint4(slow_row, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu);
-        double slow_mass = std::ldexp(1.0, LOWEXP - 32);
-        for (int K = klo + 1; K <= khi; ++K) {
-            const int e = (K >> MB) - 127;
-            const uint64_t m = (uint64_t)(K & ((1 << MB) - 1));
-            const uint64_t lo_u = (((uint64_t)1 << MB) | m) << (e - MB);
-            const uint64_t hi_u = lo_u + ((uint64_t)1 << (e - MB)) - 1;
+        double slow_mass = 0.0;
+        for (int b = 0; b < n; ++b) {
+            const uint64_t lo_u = first[(size_t)b], end_u = first[(size_t)b + 1];
+            if (end_u <= lo_u) { t[(size_t)b] = make_uint4(0u, slow_row, 0u, 0u); continue; }   // empty: never read
+            const uint64_t hi_u = end_u - 1;
             uint32_t nsum = 0, inb[3] = {0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu};
             bool slow = false;
             for (int c = 0; c < 3; ++c) {
@@ -189,21 +219,17 @@ static bool build_bucket_table(const std::vector<uint32_t> &thr32, const int z[3
             }
             if (slow) {
                 slow_mass += (double)(hi_u - lo_u + 1) / 4294967296.0;
-                t[(size_t)(K - klo)] = make_uint4(slow_row, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu);
+                t[(size_t)b] = make_uint4(0u, slow_row, 0u, 0u);
             } else {
-                t[(size_t)(K - klo)] = make_uint4(16u * nsum, inb[0], inb[1], inb[2]);
+                t[(size_t)b] = make_uint4(~inb[0], nsum, ~inb[1], ~inb[2]);
             }
         }
         if (slow_mass < 1e-5 || MB == 6) {
             if (slow_mass > 1e-3) return false;
-            // entries above the largest threshold are identical: keep one (the kernels clamp)
-            size_t keep = t.size();
-            while (keep > 1 && t[keep - 2].x == t[keep - 1].x && t[keep - 2].y == 0xFFFFFFFFu &&
-                   t[keep - 2].z == 0xFFFFFFFFu && t[keep - 2].w == 0xFFFFFFFFu &&
-                   t[keep - 1].y == 0xFFFFFFFFu && t[keep - 1].z == 0xFFFFFFFFu && t[keep - 1].w == 0xFFFFFFFFu)
-                --keep;
-            t.resize(keep);
-            tab = t; key_lo = klo; key_shift = 23 - MB;
+            tab = t;
+            K.kscale = std::ldexp(1.0f, -E); K.kadd = std::ldexp(1.0f, 8 - E);
+            K.kmul = 1u << (9 + MB); K.c16 = 16u;
+            K.key_lo = klo; K.n_bucket = n;
             return true;
         }
     }
@@ -304,7 +330,8 @@ static int upload_tables(ea_handle *h, const std::vector<uint64_t> &acc, const s
     {
         std::vector<uint4> tab;
         std::vector<uchar4> trip;
-        h->fast_rank = build_bucket_table(thr32, z, nT, tab, trip, h->key_lo, h->key_shift);
+        h->fast_rank = build_bucket_table(thr32, z, nT, tab, trip, h->K);
+        if (!h->fast_rank) { h->K = ea::RankKey{}; h->K.c16 = 16u; }
         h->n_bucket = h->fast_rank ? (int)tab.size() : 0;
         CUDA_TRY(h, cudaMemcpyAsync(h->d_trip, trip.data(), 4 * trip.size(), cudaMemcpyHostToDevice, s));
         if (h->fast_rank)
@@ -785,9 +812,8 @@ static int sweep_resident(ea_handle *h, int64_t n_sweeps, int swap_interval)
         A.swap_interval = swap_interval;
         A.nswap0 = (uint32_t)h->nswap;
         A.C = pl.C; A.S = pl.S;
-        A.bucket = h->d_bucket; A.n_bucket = h->n_bucket; A.trip = h->d_trip;
-        A.key_lo = h->key_lo; A.key_shift = h->key_shift; A.swap_win = pl.swap_win;
-        A.ones = 0xFFFFFFFFu; A.c48 = 48u; A.cm16 = (uint32_t)-16; A.c16 = 16u;
+        A.bucket = h->d_bucket; A.K = h->K; A.trip = h->d_trip;
+        A.swap_win = pl.swap_win;
         for (int r = 0; r < 10; ++r) {
             A.rk[2 * r] = h->P.k0 + (uint32_t)r * 0x9E3779B9u;
             A.rk[2 * r + 1] = h->P.k1 + (uint32_t)r * 0xBB67AE85u;
@@ -858,9 +884,7 @@ static int sweep_tiled(ea_handle *h, int64_t n_sweeps, int swap_interval)
     if (!pl.ok) return fail(h, EA_ERR_UNSUPPORTED, "tiled kernel: shape not supported");
     ea::TiledArgs A{};
     A.P = h->P; A.SK = pl.SK; A.n_kgroups = pl.nkg; A.Ecnt = h->d_Ecnt;
-    A.bucket = h->d_bucket; A.n_bucket = h->n_bucket; A.trip = h->d_trip;
-    A.key_lo = h->key_lo; A.key_shift = h->key_shift;
-    A.ones = 0xFFFFFFFFu; A.c48 = 48u; A.cm16 = (uint32_t)-16; A.c16 = 16u;
+    A.bucket = h->d_bucket; A.K = h->K; A.trip = h->d_trip;
     for (int r = 0; r < 10; ++r) {
         A.rk[2 * r] = h->P.k0 + (uint32_t)r * 0x9E3779B9u;
         A.rk[2 * r + 1] = h->P.k1 + (uint32_t)r * 0xBB67AE85u;
@@ -998,9 +1022,7 @@ static int sweep_stream(ea_handle *h, int64_t n_sweeps, int swap_interval)
         A.nswap0 = (uint32_t)h->nswap;
         A.Ecnt = h->d_Ecnt + (size_t)32 * w_off * h->nT;
         A.gbar = (unsigned int *)(h->d_Ecnt + 2 * (size_t)h->Rp * h->nT);
-        A.bucket = h->d_bucket; A.n_bucket = h->n_bucket; A.trip = h->d_trip;
-        A.key_lo = h->key_lo; A.key_shift = h->key_shift;
-        A.ones = 0xFFFFFFFFu; A.c48 = 48u; A.cm16 = (uint32_t)-16; A.c16 = 16u;
+        A.bucket = h->d_bucket; A.K = h->K; A.trip = h->d_trip;
         A.MS = pg.MS; A.MW = pg.MW; A.swap_win = pg.swap_win; A.esm_off = (int)pg.esm_off; A.batch_off = (int)pg.batch_off;
         for (int r = 0; r < 10; ++r) {
             A.rk[2 * r] = h->P.k0 + (uint32_t)r * 0x9E3779B9u;

@@ -18,6 +18,15 @@
 namespace ea {
 namespace cg = cooperative_groups;
 
+// Bucket key of a draw, filled by the host (ea_lib.cu: build_bucket_table / fill_rank_key).
+// All of it is data (kernel parameters), opaque to ptxas: the multiplies stay on the FMA pipe.
+struct RankKey {
+    float kscale, kadd;       // g = sat(float_rz(u) * kscale + kadd): kscale = 2^-E, kadd = 2^(8 - E)
+    uint32_t kmul;            // key = hi32(bits(g) * kmul) = bits(g) >> (23 - MB), kmul = 2^(9 + MB)
+    uint32_t c16;             // 16
+    int key_lo, n_bucket;     // table index = key - key_lo in [0, n_bucket)
+};
+
 struct ResArgs {
     Params P;
     uint32_t g0;          // global index of the first sweep of this call
@@ -28,9 +37,8 @@ struct ResArgs {
     const uint4 *bucket;      // fast rank table (FAST variant), device memory, 16 B entries
     const uchar4 *trip;       // [3 nT + 1] (n4, n5, n6) of every combined rank
     uint32_t rk[20];          // Philox round keys (k0 + r*0x9E3779B9, k1 + r*0xBB67AE85), r = 0..9
-    int n_bucket, key_lo, key_shift;
+    RankKey K;                // bucket key of a draw (see RankCtx)
     int swap_win;             // swap thresholds for m in [-swap_win, -1] are staged in smem
-    uint32_t ones, c48, cm16, c16; // 0xFFFFFFFF, 48, (uint32_t)-16, 16: see RankCtx
 };
 
 // Mask table of one slot from its rank masks (one warp): row n = { lt[n4], lt[n5], lt[n6], 0 },
@@ -53,6 +61,50 @@ __device__ __forceinline__ uint4 philox_rk(uint32_t c0, uint32_t c1, uint32_t c2
 {
 #pragma unroll
     for (int r = 0; r < 10; ++r) {
+        const uint64_t p0 = (uint64_t)0xD2511F53u * c0;
+        const uint64_t p1 = (uint64_t)0xCD9E8D57u * c2;
+        const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ rk[2 * r];
+        const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ rk[2 * r + 1];
+        c1 = (uint32_t)p1;
+        c3 = (uint32_t)p0;
+        c0 = n0;
+        c2 = n2;
+    }
+    return make_uint4(c0, c1, c2, c3);
+}
+
+// The flip draws of a thread all have the counter (sweep g, quad q, word gw, parity | slot):
+// q and gw are fixed per thread, g and the last field are the same for the whole warp.  Round 0
+// and half of rounds 1 and 2 therefore depend on per-thread constants only (PhiloxQuad, computed
+// once per word) or on warp-uniform values (uniform datapath): per call a thread executes 15
+// IMAD.WIDE and 17 LOP3 instead of 20 and 20.  Same function as philox_rk(g, q, gw, c3, rk).
+struct PhiloxQuad { uint32_t ph, pl, c1w; };
+
+__device__ __forceinline__ PhiloxQuad philox_quad_init(uint32_t q, uint32_t gw, const uint32_t (&rk)[20])
+{
+    const uint64_t p1 = (uint64_t)0xCD9E8D57u * gw;
+    const uint32_t a0 = (uint32_t)(p1 >> 32) ^ q ^ rk[0];          // c0 after round 0
+    const uint64_t p0 = (uint64_t)0xD2511F53u * a0;                // round 1's first product
+    PhiloxQuad h;
+    h.ph = (uint32_t)(p0 >> 32); h.pl = (uint32_t)p0; h.c1w = (uint32_t)p1;
+    return h;
+}
+
+__device__ __forceinline__ uint4 philox_quad(const PhiloxQuad &h, uint32_t g, uint32_t ctr3, const uint32_t (&rk)[20])
+{
+    // round 0 (c0 = g, c1 = q, c2 = gw, c3 = ctr3): everything left is warp-uniform
+    const uint64_t pg = (uint64_t)0xD2511F53u * g;
+    uint32_t c2 = (uint32_t)(pg >> 32) ^ ctr3 ^ rk[1];
+    uint32_t c3 = (uint32_t)pg;
+    uint32_t c1 = h.c1w;
+    // round 1: p0 = M0 * c0 is the per-thread constant (ph : pl)
+    const uint64_t q1 = (uint64_t)0xCD9E8D57u * c2;
+    uint32_t c0 = (uint32_t)(q1 >> 32) ^ c1 ^ rk[2];               // uniform
+    c2 = h.ph ^ c3 ^ rk[3];
+    c1 = (uint32_t)q1;
+    c3 = h.pl;
+#pragma unroll
+    for (int r = 2; r < 10; ++r) {
         const uint64_t p0 = (uint64_t)0xD2511F53u * c0;
         const uint64_t p1 = (uint64_t)0xCD9E8D57u * c2;
         const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ rk[2 * r];
@@ -116,32 +168,52 @@ __device__ __forceinline__ Planes planes_after(const Planes &p, uint32_t acc)
 }
 
 // ------------------------------------------------------------------ rank of a draw
-// FAST: one 128-bit look-up keyed by the leading bits of the draw (float exponent + MB
-// mantissa bits, truncating conversion), then one 128-bit look-up of the three accept masks.
-//   bucket entry = { 16 * (n4 + n5 + n6 at the bucket's lower edge), thr4, thr5, thr6 }
+// FAST: one 128-bit look-up keyed by the leading bits of the draw, then one 128-bit look-up of the
+// three accept masks.
+//   key(u)  = bits(g) >> (23 - MB),  g = sat(float_rz(u) * 2^-E + 2^(8-E))   (I2FP, FFMA.SAT, IMAD.HI)
+// is a monotone function of u with logarithmic steps (MB mantissa bits per octave); the added
+// constant merges all u << 2^8 into the first bucket and the saturation all u >= 2^E (E = number
+// of bits of the largest threshold) into the last one, so neither end needs a clamp and most
+// draws (86 % for config 4) share ONE shared-memory address (broadcast, no bank conflicts).  The
+// host evaluates the same function in double (exactly) to find every bucket's range of u.
+//   bucket entry = { ~thr4, n4 + n5 + n6 at the bucket's lower edge, ~thr5, ~thr6 }
 // where n_c = number of class-c thresholds <= the lower edge and thr_c = the (threshold - 1)
 // of class c inside the bucket, or 0xFFFFFFFF if there is none (at most one per class).
 // The COMBINED rank n = n4 + n5 + n6 of the draw is the lower-edge value plus (thr_c < u) for
 // the three classes.  As u grows the triple (n4, n5, n6) only ever changes at a threshold, so
 // n determines the triple: the per-slot mask table `mt` (3 nT + 2 rows of 16 bytes, rebuilt
 // after every swap round) holds in row n the three rank masks { lt[n4], lt[n5], lt[n6], 0 }.
-// Buckets with several thresholds of one class, and draws < 2^8, point at the last row, whose
-// fourth word is 0x80000000: the caller then redoes the quad with the exact binary search.
-// The three compares run on the FMA pipe: hi32(u * (2^32-1) + thr) = u - (thr < u).
+// Buckets with several thresholds of one class, and the first bucket (u < 2^8), point at the last
+// row, whose fourth word is 0x80000000: the caller then redoes the quad with the exact binary search.
+// The three compares are carries: (thr < u) = carry of u + ~thr (IADD3 with carry-out), summed
+// into n by IADD3.X / IMAD.X.  (A 32 x 32 + 64 multiply-add would put them on the FMA pipe, but
+// ptxas lowers mad.wide with a register addend to IMAD.WIDE + IADD3 + IADD3.X.)
 struct RankCtx {
     const uint32_t *thr;     // smem [3][LTS]  (exact search only)
-    const uint4 *bucket;     // smem
-    int LTS, nT, key_lo, key_top, key_shift;   // table index = min(max(key - key_lo, 0), key_top)
+    const char *bucket0;     // smem: bucket table base - 16 * key_lo (byte address)
+    int LTS, nT;
     int z0, z1, z2;
-    uint32_t ones, c48, cm16, c16;   // 0xFFFFFFFF, 48, -16, 16 from kernel parameters (opaque to
-                                     // ptxas, so the multiply-adds stay IMADs on the FMA pipe)
+    float kscale, kadd;
+    uint32_t kmul, c16;
 };
 
-__device__ __forceinline__ uint32_t hi_mad(uint32_t u, uint32_t m, uint32_t t)
+__device__ __forceinline__ void rank_ctx_key(RankCtx &R, const RankKey &K, const uint4 *bucket)
 {
-    uint64_t x;
-    asm("mad.wide.u32 %0, %1, %2, %3;" : "=l"(x) : "r"(u), "r"(m), "l"((uint64_t)t));
-    return (uint32_t)(x >> 32);
+    R.bucket0 = reinterpret_cast<const char *>(bucket) - 16 * (ptrdiff_t)K.key_lo;
+    R.kscale = K.kscale; R.kadd = K.kadd; R.kmul = K.kmul; R.c16 = K.c16;
+}
+
+// n + (u + a overflows) + (u + b overflows) + (u + c overflows): three carries (IADD3 with a
+// predicate carry-out) and their sum with n (IADD3.X / IMAD.X)
+__device__ __forceinline__ uint32_t add3_carries(uint32_t u, uint32_t n, uint32_t a, uint32_t b, uint32_t c)
+{
+    uint32_t r;
+    asm("{\n\t.reg .b32 t, r1, r2;\n\t"
+        "add.cc.u32 t, %1, %3;\n\taddc.u32 r1, %2, 0;\n\t"
+        "add.cc.u32 t, %1, %4;\n\taddc.u32 r2, r1, 0;\n\t"
+        "add.cc.u32 t, %1, %5;\n\taddc.u32 %0, r2, 0;\n\t}"
+        : "=r"(r) : "r"(u), "r"(n), "r"(a), "r"(b), "r"(c));
+    return r;
 }
 __device__ __forceinline__ uint32_t mad_lo(uint32_t a, uint32_t b, uint32_t c)
 {
@@ -154,14 +226,12 @@ __device__ __forceinline__ uint32_t mad_lo(uint32_t a, uint32_t b, uint32_t c)
 __device__ __forceinline__ uint32_t accept_fast(const RankCtx &R, const uint4 *mt, uint32_t u,
                                                 const Planes &p, uint32_t *flag)
 {
-    const int key = (int)(__float_as_uint(__uint2float_rz(u)) >> R.key_shift);
-    // every bucket above the largest threshold holds the same entry: clamping keeps the 86 % of
-    // the draws that land there on ONE shared-memory address (broadcast, no bank conflicts)
-    const uint32_t boff = mad_lo((uint32_t)min(max(key - R.key_lo, 0), R.key_top), R.c16, 0u);
-    const uint4 e = *reinterpret_cast<const uint4 *>(reinterpret_cast<const char *>(R.bucket) + boff);
-    const uint32_t d = hi_mad(u, R.ones, e.y) + hi_mad(u, R.ones, e.z) + hi_mad(u, R.ones, e.w);
-    const uint32_t off = mad_lo(d, R.cm16, mad_lo(u, R.c48, e.x));   // e.x + 16 * (3u - d)
-    const uint4 row = *reinterpret_cast<const uint4 *>(reinterpret_cast<const char *>(mt) + off);
+    float g;
+    asm("fma.rn.sat.f32 %0, %1, %2, %3;" : "=f"(g) : "f"(__uint2float_rz(u)), "f"(R.kscale), "f"(R.kadd));
+    const uint32_t key = __umulhi(__float_as_uint(g), R.kmul);
+    const uint4 e = *reinterpret_cast<const uint4 *>(R.bucket0 + mad_lo(key, R.c16, 0u));
+    const uint32_t n = add3_carries(u, e.y, e.x, e.z, e.w);
+    const uint4 row = *reinterpret_cast<const uint4 *>(reinterpret_cast<const char *>(mt) + mad_lo(n, R.c16, 0u));
     *flag |= row.w;
     return accept_mask(p, row.x, row.y, row.z);
 }
@@ -323,16 +393,6 @@ __device__ __forceinline__ void update_quad_off(uint32_t *sp, const uint32_t *lt
     const uint4 res = update_quad_mem<L, FAST, ENERGY, UNIS, true>(self_q, oth_b, 16u * q, oyp, oym, ozp, ozm,
                                                              q & (Gm::QR - 1), lt, mt, R, J, s, rnd, fin);
     *reinterpret_cast<uint4 *>(self_q) = res;
-}
-
-// resident kernel: neighbour offsets packed two per register (16-bit halves, + in the low half)
-template <int L, bool FAST, bool ENERGY>
-__device__ __forceinline__ void update_quad(uint32_t *sp, const uint32_t *lt, const uint4 *mt, const RankCtx &R,
-                                            const QuadJ &J, int p, int s, int q, uint32_t offY, uint32_t offZ,
-                                            const uint4 rnd, Planes (&fin)[4])
-{
-    update_quad_off<L, FAST, ENERGY, true>(sp, lt, mt, R, J, p, s, q, offY & 0xFFFFu, offY >> 16, offZ & 0xFFFFu,
-                                     offZ >> 16, rnd, fin);
 }
 
 // tiled kernel: neighbour quad indices
@@ -528,7 +588,7 @@ __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs
     // shared memory: the rank table first (fixed offset 0), lattices next (16 B aligned)
     const int MTS = 3 * nT + 2, SW = A.swap_win;
     uint4 *bucket = reinterpret_cast<uint4 *>(smem);                 // [n_bucket] 16 B entries
-    uint32_t *sp = smem + 4 * (size_t)A.n_bucket;                    // [S][2][Nh]
+    uint32_t *sp = smem + 4 * (size_t)A.K.n_bucket;                    // [S][2][Nh]
     uint4 *mt = reinterpret_cast<uint4 *>(sp + (size_t)S * N);       // [S][MTS] mask tables
     uint32_t *lt = reinterpret_cast<uint32_t *>(mt + (size_t)S * MTS);   // [S][LTS]
     uint32_t *thr = lt + S * LTS;                                    // [3][LTS]
@@ -563,7 +623,7 @@ __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs
     for (int k = 0; k < nk; ++k)
         for (int a = tid; a < LTS; a += NT) lt[k * LTS + a] = P.lt[((size_t)w * nT + k0 + k) * LTS + a];
     for (int a = tid; a < 3 * LTS; a += NT) thr[a] = P.thr32[a];
-    for (int a = tid; a < A.n_bucket; a += NT) bucket[a] = A.bucket[a];
+    for (int a = tid; a < A.K.n_bucket; a += NT) bucket[a] = A.bucket[a];
     for (int a = tid; a < 32 * nT; a += NT) {
         tau8[a] = P.tau[(size_t)32 * w * nT + a];
         sig8[a] = P.sigma[(size_t)32 * w * nT + a];
@@ -593,16 +653,17 @@ __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs
     const uint32_t *cp = P.coup + (size_t)w * 3 * N;
     const QuadJ J0 = load_quad_j<L>(cp, 0, s0, q, qx, qym, qzm);
     const QuadJ J1 = load_quad_j<L>(cp, 1, 1 - s0, q, qx, qym, qzm);
-    uint32_t offY = (uint32_t)(16 * qyp) | ((uint32_t)(16 * qym) << 16);
-    uint32_t offZ = (uint32_t)(16 * qzp) | ((uint32_t)(16 * qzm) << 16);
-    asm volatile("" : "+r"(offY), "+r"(offZ));    // opaque: keep in registers, do not rematerialize
+    // neighbour byte offsets: per-thread constants kept in registers (opaque, so that ptxas does
+    // not rematerialize them); the loads are [register + uniform slot base + parity immediate]
+    uint32_t oyp = 16u * (uint32_t)qyp, oym = 16u * (uint32_t)qym, ozp = 16u * (uint32_t)qzp, ozm = 16u * (uint32_t)qzm;
+    asm volatile("" : "+r"(oyp), "+r"(oym), "+r"(ozp), "+r"(ozm));
 
     RankCtx R;
-    R.thr = thr; R.bucket = bucket; R.LTS = LTS; R.nT = nT;
-    R.key_lo = A.key_lo; R.key_top = A.n_bucket - 1; R.key_shift = A.key_shift;
+    R.thr = thr; R.LTS = LTS; R.nT = nT;
     R.z0 = P.z[0]; R.z1 = P.z[1]; R.z2 = P.z[2];
-    R.ones = A.ones; R.c48 = A.c48; R.cm16 = A.cm16; R.c16 = A.c16;
+    rank_ctx_key(R, A.K, bucket);
     const uint32_t gw = P.w0 + (uint32_t)w;
+    const PhiloxQuad PQ = philox_quad_init((uint32_t)q, gw, A.rk);
     cg::cluster_group cl = cg::this_cluster();
     __syncthreads();
     for (int kl = tid >> 5; kl < nk; kl += NT >> 5) build_mt(mt + (size_t)kl * MTS, lt + kl * LTS, trip, nT, lane);
@@ -616,16 +677,16 @@ __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs
         Planes fin[4];
         // ---------------- parity 0
         for (int kl = sg; kl < nk; kl += G) {
-            const uint4 rnd = philox_rk(g, (uint32_t)q, gw, (uint32_t)(k0 + kl), A.rk);
-            update_quad<L, FAST, false>(sp + (size_t)kl * N, lt + kl * LTS, mt + (size_t)kl * MTS, R, J0, 0, s0, q, offY, offZ, rnd, fin);
+            const uint4 rnd = philox_quad(PQ, g, (uint32_t)(k0 + kl), A.rk);
+            update_quad_off<L, FAST, false, true>(sp + (size_t)kl * N, lt + kl * LTS, mt + (size_t)kl * MTS, R, J0, 0, s0, q, oyp, oym, ozp, ozm, rnd, fin);
         }
         __syncthreads();
         // ---------------- parity 1 (+ satisfied-bond count of the finished sweep)
         if (!need_E) {
             for (int kl = sg; kl < nk; kl += G) {
-                const uint4 rnd = philox_rk(g, (uint32_t)q, gw, (1u << 16) | (uint32_t)(k0 + kl), A.rk);
-                update_quad<L, FAST, false>(sp + (size_t)kl * N, lt + kl * LTS, mt + (size_t)kl * MTS, R, J1, 1, 1 - s0, q, offY, offZ,
-                                            rnd, fin);
+                const uint4 rnd = philox_quad(PQ, g, (1u << 16) | (uint32_t)(k0 + kl), A.rk);
+                update_quad_off<L, FAST, false, true>(sp + (size_t)kl * N, lt + kl * LTS, mt + (size_t)kl * MTS, R, J1, 1, 1 - s0, q,
+                                                      oyp, oym, ozp, ozm, rnd, fin);
             }
             __syncthreads();
             continue;
@@ -636,9 +697,9 @@ __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs
             for (int i = 0; i < 4; ++i) {
                 const int kl = kb + i * G;
                 if (kl < nk) {
-                    const uint4 rnd = philox_rk(g, (uint32_t)q, gw, (1u << 16) | (uint32_t)(k0 + kl), A.rk);
-                    update_quad<L, FAST, true>(sp + (size_t)kl * N, lt + kl * LTS, mt + (size_t)kl * MTS, R, J1, 1, 1 - s0, q, offY,
-                                               offZ, rnd, fin);
+                    const uint4 rnd = philox_quad(PQ, g, (1u << 16) | (uint32_t)(k0 + kl), A.rk);
+                    update_quad_off<L, FAST, true, true>(sp + (size_t)kl * N, lt + kl * LTS, mt + (size_t)kl * MTS, R, J1, 1, 1 - s0, q,
+                                                         oyp, oym, ozp, ozm, rnd, fin);
                     quad_sum(fin, en[i]);
                 } else {
 #pragma unroll

@@ -37,8 +37,7 @@ struct StreamArgs {
     int32_t *Ecnt;           // [2][Rp][nT] satisfied-bond counters (zero on entry)
     const uint4 *bucket;
     const uchar4 *trip;
-    int n_bucket, key_lo, key_shift;
-    uint32_t ones, c48, cm16, c16;
+    RankKey K;
     uint32_t rk[20];
     int MS;                  // most items one block can get = ceil(items / grid)
     int MW;                  // most words one block can meet
@@ -221,6 +220,7 @@ __device__ __forceinline__ void stream_consume(const StreamArgs &A, const Stream
     const int nT = C.nT, tid = C.tid;
     int cur_grp = -1, s = 0, q = 0;
     QuadJ J;
+    PhiloxQuad PQ{};
     Planes fin[4];
     for (int b = 0; b < C.nb; ++b) {
         __syncwarp();
@@ -235,13 +235,13 @@ __device__ __forceinline__ void stream_consume(const StreamArgs &A, const Stream
             const int qym = C.qx + QR * (wrap_dec(C.y, L) + L * z);
             const int qzm = C.qx + QR * (C.y + L * wrap_dec(z, L));
             J = load_quad_j<L>(P.coup + (size_t)w * 3 * N, p, s, q, C.qx, qym, qzm);
+            PQ = philox_quad_init((uint32_t)q, P.w0 + (uint32_t)w, A.rk);
         }
-        const uint32_t gw = P.w0 + (uint32_t)w;
         const uint32_t c3 = (uint32_t)p << 16;
         if (!ENERGY) {
             for (int i = 0; i < cnt; ++i) {
                 const int li = pos + i - C.i0, st = li % NST;
-                const uint4 rnd = philox_rk(g, (uint32_t)q, gw, c3 | (uint32_t)(k0 + i), A.rk);
+                const uint4 rnd = philox_quad(PQ, g, c3 | (uint32_t)(k0 + i), A.rk);
                 mbar_wait(&C.full[st], (phase >> st) & 1u);
                 phase ^= 1u << st;
                 const char *buf = reinterpret_cast<const char *>(C.bufs + (size_t)st * Sg::BUF_BYTES);
@@ -259,7 +259,7 @@ __device__ __forceinline__ void stream_consume(const StreamArgs &A, const Stream
                     const int i = i0 + h;
                     if (i < cnt) {
                         const int li = pos + i - C.i0, st = li % NST;
-                        const uint4 rnd = philox_rk(g, (uint32_t)q, gw, c3 | (uint32_t)(k0 + i), A.rk);
+                        const uint4 rnd = philox_quad(PQ, g, c3 | (uint32_t)(k0 + i), A.rk);
                         mbar_wait(&C.full[st], (phase >> st) & 1u);
                         phase ^= 1u << st;
                         const char *buf = reinterpret_cast<const char *>(C.bufs + (size_t)st * Sg::BUF_BYTES);
@@ -347,7 +347,7 @@ __global__ void __launch_bounds__(StreamGeom<L>::NTHR, 1) k_stream(const StreamA
     // shared memory
     uint64_t *mbar = reinterpret_cast<uint64_t *>(smraw);                        // full[NST], empty[NST], number of batches
     uint4 *bucket = reinterpret_cast<uint4 *>(smraw + Sg::MBAR_BYTES);           // [n_bucket]
-    unsigned char *bufs = reinterpret_cast<unsigned char *>(bucket + A.n_bucket);   // [NST][BUF_BYTES]
+    unsigned char *bufs = reinterpret_cast<unsigned char *>(bucket + A.K.n_bucket);   // [NST][BUF_BYTES]
     uint4 *mt = reinterpret_cast<uint4 *>(bufs + (size_t)NST * Sg::BUF_BYTES);      // [MS][MTS]
     uint32_t *lt = reinterpret_cast<uint32_t *>(mt + (size_t)MS * MTS);          // [MS][LTS]
     uint32_t *thr = lt + MS * LTS;                                               // [3][LTS]
@@ -363,7 +363,7 @@ __global__ void __launch_bounds__(StreamGeom<L>::NTHR, 1) k_stream(const StreamA
     int *swhi = swlo + nT;                                                       // [nT] one past its last m
     int *swk = swhi + nT;                                                        // [nT] decisions left | right << 1 of the range
 
-    for (int a = tid; a < A.n_bucket; a += NTA) bucket[a] = A.bucket[a];
+    for (int a = tid; a < A.K.n_bucket; a += NTA) bucket[a] = A.bucket[a];
     for (int a = tid; a < 3 * LTS; a += NTA) thr[a] = P.thr32[a];
     for (int a = tid; a < MTS - 1; a += NTA) trip[a] = A.trip[a];
     for (int a = tid; a < (nT - 1) * SW; a += NTA) {         // window m = -SW + i of row t
@@ -423,10 +423,9 @@ __global__ void __launch_bounds__(StreamGeom<L>::NTHR, 1) k_stream(const StreamA
     }
     C.full = mbar; C.empty = mbar + NST; C.batch = batch; C.bufs = bufs; C.mt = mt; C.lt = lt; C.Eacc = Eacc;
     C.nb = *reinterpret_cast<const int *>(smraw + 16 * NST);
-    C.R.thr = thr; C.R.bucket = bucket; C.R.LTS = LTS; C.R.nT = nT;
-    C.R.key_lo = A.key_lo; C.R.key_top = A.n_bucket - 1; C.R.key_shift = A.key_shift;
+    C.R.thr = thr; C.R.LTS = LTS; C.R.nT = nT;
+    rank_ctx_key(C.R, A.K, bucket);
     C.R.z0 = P.z[0]; C.R.z1 = P.z[1]; C.R.z2 = P.z[2];
-    C.R.ones = A.ones; C.R.c48 = A.c48; C.R.cm16 = A.cm16; C.R.c16 = A.c16;
     __syncthreads();
 
     uint32_t nswap = A.nswap0, phase = 0, efill = 0;

@@ -23,8 +23,7 @@ struct TiledArgs {
     int32_t *Ecnt;           // [Rp][nT] satisfied-bond counters (ENERGY pass), zeroed by k_tiled_finish
     const uint4 *bucket;
     const uchar4 *trip;      // [3 nT + 1] (n4, n5, n6) of every combined rank
-    int n_bucket, key_lo, key_shift;
-    uint32_t ones, c48, cm16, c16;
+    RankKey K;
     uint32_t rk[20];
 };
 
@@ -58,13 +57,13 @@ __global__ void __launch_bounds__(TileGeom<L>::NTHR, 1) k_tiled_half(const Tiled
 
     const int MTS = 3 * nT + 2;
     uint4 *bucket = reinterpret_cast<uint4 *>(smem);               // [n_bucket]
-    uint4 *mt = bucket + A.n_bucket;                               // [SK][MTS] mask tables
+    uint4 *mt = bucket + A.K.n_bucket;                               // [SK][MTS] mask tables
     uint32_t *lt = reinterpret_cast<uint32_t *>(mt + (size_t)SK * MTS);   // [SK][LTS]
     uint32_t *thr = lt + SK * LTS;                                 // [3][LTS]
     uchar4 *trip = reinterpret_cast<uchar4 *>(thr + 3 * LTS);      // [MTS]
     int32_t *Eacc = (int32_t *)(trip + MTS);                       // [SK][32]
 
-    for (int a = tid; a < A.n_bucket; a += NT) bucket[a] = A.bucket[a];
+    for (int a = tid; a < A.K.n_bucket; a += NT) bucket[a] = A.bucket[a];
     for (int a = tid; a < nk * LTS; a += NT) lt[a] = P.lt[((size_t)w * nT + k0) * LTS + a];
     for (int a = tid; a < 3 * LTS; a += NT) thr[a] = P.thr32[a];
     for (int a = tid; a < MTS - 1; a += NT) trip[a] = A.trip[a];
@@ -77,10 +76,9 @@ __global__ void __launch_bounds__(TileGeom<L>::NTHR, 1) k_tiled_half(const Tiled
     const QuadJ J = load_quad_j<L>(P.coup + (size_t)w * 3 * N, p, s, q, qx, qym, qzm);
     // neighbour byte offsets do not fit 16 bits for L = 32, 64: pass quad indices * 16 directly
     RankCtx R;
-    R.thr = thr; R.bucket = bucket; R.LTS = LTS; R.nT = nT;
-    R.key_lo = A.key_lo; R.key_top = A.n_bucket - 1; R.key_shift = A.key_shift;
+    R.thr = thr; R.LTS = LTS; R.nT = nT;
+    rank_ctx_key(R, A.K, bucket);
     R.z0 = P.z[0]; R.z1 = P.z[1]; R.z2 = P.z[2];
-    R.ones = A.ones; R.c48 = A.c48; R.cm16 = A.cm16; R.c16 = A.c16;
     const uint32_t gw = P.w0 + (uint32_t)w;
     const uint32_t c3 = (uint32_t)p << 16;
     __syncthreads();
