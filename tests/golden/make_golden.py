@@ -5,8 +5,8 @@ BASELINE.json's configs.  Calls only oracle/ (plus numpy layout helpers); never 
 
   python tests/golden/make_golden.py <config 1..5> <word> <max_sweeps> [state_dir]
 
-With a state_dir the oracle's state (spins by slot, temperature permutation, counters) is
-saved there at every checkpoint and a later call resumes from it through eao_set_state
+With a state_dir the oracle's state (spins by slot as packed bits, temperature permutation,
+counters) is saved there at every checkpoint and a later call resumes from it through eao_set_state
 (whose interrupted-run == uninterrupted-run property tests/test_oracle_chain.py pins), so a
 100000-sweep word (about 1.7 h of one core) survives an interruption.
 
@@ -52,7 +52,8 @@ def main():
         spent = old.get("oracle_seconds", 0.0)
     if state_path and os.path.exists(state_path):
         st = np.load(state_path)
-        o.set_state(st["spins_by_slot"], st["tau"], int(st["sweeps"]), int(st["swap_rounds"]))
+        bits = np.unpackbits(st["spin_bits"])[: R * cfg.n_temps * cfg.N].reshape(R, cfg.n_temps, cfg.N)
+        o.set_state((2 * bits.astype(np.int8) - 1), st["tau"], int(st["sweeps"]), int(st["swap_rounds"]))
         done = int(st["sweeps"])
         print("resumed at sweep", done, flush=True)
     t0 = time.time() - (spent if done else 0.0)
@@ -62,15 +63,16 @@ def main():
         if state_path:
             os.makedirs(state_dir, exist_ok=True)
             c = o.counters()
-            np.savez(state_path + ".tmp.npz", spins_by_slot=o.spins_by_slot(), tau=o.perm()[0],
+            np.savez(state_path + ".tmp.npz", spin_bits=np.packbits(o.spins_by_slot() > 0), tau=o.perm()[0],
                      sweeps=c["sweeps"], swap_rounds=c["swap_rounds"])
             os.replace(state_path + ".tmp.npz", state_path)
         words = spins_to_words(o.spins_by_slot(), cfg.L)[:, 0]
         tau, _ = o.perm()
         taup = np.zeros((32, cfg.n_temps), dtype=np.uint8); taup[:R] = tau
         Ep = np.zeros((32, cfg.n_temps), dtype=np.int32); Ep[:R] = o.energy_by_slot()
-        out["checkpoints"][str(cp)] = {"digest": word_digest(words, taup[:R], Ep[:R]),
-                                        "E_sum": int(o.energy().astype(np.int64).sum())}
+        new = {"digest": word_digest(words, taup[:R], Ep[:R]), "E_sum": int(o.energy().astype(np.int64).sum())}
+        assert out["checkpoints"].get(str(cp), new) == new, f"checkpoint {cp}: recomputed digest differs from the stored one"
+        out["checkpoints"][str(cp)] = new
         out["oracle_seconds"] = round(time.time() - t0, 1)
         with open(path + ".tmp", "w") as f:
             json.dump(out, f, indent=1)
