@@ -27,6 +27,18 @@ def needs_build() -> bool:
 
 
 def build_library(force: bool = False, verbose: bool = False) -> Path:
+    """Build under an exclusive file lock: concurrent callers (one rank per GPU) wait for the one
+    that builds and then find the library up to date."""
+    import fcntl
+    with open(PKG / ".build.lock", "w") as lock:
+        fcntl.flock(lock, fcntl.LOCK_EX)
+        try:
+            return _build_locked(force, verbose)
+        finally:
+            fcntl.flock(lock, fcntl.LOCK_UN)
+
+
+def _build_locked(force: bool, verbose: bool) -> Path:
     if not force and not needs_build():
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
