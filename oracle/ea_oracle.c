@@ -25,6 +25,9 @@
  *   ferromagnet : Binder-cumulant crossing near T = 4.51
  *   PT          : sigma/tau inverse permutations, energy multiset conserved,
  *                 <E>(T) with PT == without PT
+ *   replica draws (eao_set_draw_mode 1, the paper's coding): beta = 0 complement, gauge
+ *                 covariance, incremental == recomputed, 2^3 enumeration with and without PT,
+ *                 composition, independence of realizations (tests/test_oracle_replica.py)
  *   field h     : flip-and-recompute dE, incremental == recomputed, exact
  *                 (s -> -s, h -> -h) symmetry, Boltzmann stationarity on the
  *                 2^3 lattice, saturation at large |h| (tests/test_oracle_field.py)
@@ -79,6 +82,9 @@ typedef struct eao {
     int32_t *nbr;        /* [site i][6]: +x,-x,+y,-y,+z,-z neighbour sites (periodic) */
     uint64_t g;          /* sweeps done  */
     uint64_t nswap;      /* swap rounds done */
+    int draw_mode;       /* 0: one draw per (site, word, slot) shared by the word's 32 realizations (R11);
+                            1: one draw per (site, realization, slot) -- the paper's own coding, in which the
+                            bits of a word are the temperature replicas of one realization (eao_set_draw_mode) */
     int check;           /* recompute-and-compare energies every sweep */
     int64_t check_failures;
     int64_t n_attempt, n_accept, n_swap_attempt, n_swap_accept;
@@ -370,6 +376,52 @@ static void half_sweep(eao *o, int p)
                 }
 }
 
+/* Second workload (R24): the paper packs the spins of the temperature
+ * replicas of ONE disorder realization at a site into a word ("spins from different
+ * temperature replicas at the same position are encoded into an integer", :186 AMSC, :281 CAMSC),
+ * and every replica is "an independent Monte Carlo process" (Figure 3) with its own
+ * random number.  Model, tables, sweep order and parallel tempering are unchanged; only the draw is
+ * now one uint32 per (site, REALIZATION, slot):
+ *   PX(g, q, r, ((6+p)<<16)|k)[l],  r = global realization index, q = j>>2, l = j&3.
+ * Flip iff draw < acc[tau][n_sat] exactly as in half_sweep. */
+static void half_sweep_replica_draws(eao *o, int p)
+{
+    int L = o->L, nT = o->nT;
+    uint32_t out[4];
+    for (int k = 0; k < nT; ++k)
+        for (int z = 0; z < L; ++z)
+            for (int y = 0; y < L; ++y)
+                for (int x = 0; x < L; ++x) {
+                    if (((x + y + z) & 1) != p) continue;
+                    int i = x + L * (y + L * z);
+                    uint32_t j = (uint32_t)((x >> 1) + (L / 2) * (y + L * z));
+                    for (int r = 0; r < o->R; ++r) {
+                        eao_philox4x32_10((uint32_t)o->g, j >> 2, (uint32_t)(o->r0 + r),
+                                          ((uint32_t)(6 + p) << 16) | (uint32_t)k, o->k0, o->k1, out);
+                        uint64_t u = out[j & 3];
+                        int c = n_sat(o, k, r, i);
+                        int t = o->tau[r * nT + k];
+                        o->n_attempt++;
+                        int si = S_(o, k, i, r);
+                        uint64_t thr = o->h == 0 ? o->acc[t * 7 + c]
+                                                 : o->accf[(t * 7 + c) * 2 + (si + 1) / 2];
+                        if (u < thr) {
+                            S_(o, k, i, r) = (int8_t)(-si);
+                            o->E[r * nT + k] += 4 * c - 12 - 2 * o->h * si;
+                            o->n_accept++;
+                        }
+                    }
+                }
+}
+
+int eao_set_draw_mode(eao *o, int mode)
+{
+    if (mode != 0 && mode != 1) return -1;
+    o->draw_mode = mode;
+    return 0;
+}
+int eao_get_draw_mode(const eao *o) { return o->draw_mode; }
+
 /* One parallel-tempering round (temperatures
  * (table rows) are exchanged, lattices stay where they are).  Round n pairs
  * temperature indices (t, t+1) for t = n&1, n&1 + 2, ... (R4);
@@ -414,8 +466,13 @@ int eao_sweep(eao *o, int64_t n_sweeps, int swap_interval)
     if (n_sweeps < 0 || swap_interval < 0) return -1;
     if (o->g + (uint64_t)n_sweeps > 0xFFFFFFFFull) return -4;
     for (int64_t it = 0; it < n_sweeps; ++it) {
-        half_sweep(o, 0);
-        half_sweep(o, 1);
+        if (o->draw_mode == 0) {
+            half_sweep(o, 0);
+            half_sweep(o, 1);
+        } else {
+            half_sweep_replica_draws(o, 0);
+            half_sweep_replica_draws(o, 1);
+        }
         if (o->check) {
             for (int r = 0; r < o->R; ++r)
                 for (int k = 0; k < o->nT; ++k)

@@ -69,6 +69,10 @@ def _load():
     lib.eao_set_state.argtypes = [vp, vp, vp, u64, u64]
     lib.eao_set_field.restype = i32
     lib.eao_set_field.argtypes = [vp, i32]
+    lib.eao_set_draw_mode.restype = i32
+    lib.eao_set_draw_mode.argtypes = [vp, i32]
+    lib.eao_get_draw_mode.restype = i32
+    lib.eao_get_draw_mode.argtypes = [vp]
     lib.eao_get_field.restype = i32
     lib.eao_get_field.argtypes = [vp]
     lib.eao_get_field_tables.restype = i32
@@ -144,6 +148,15 @@ class Oracle:
         rc = self.lib.eao_set_state(self.h, _ptr(s), _ptr(t), int(sweeps), int(swap_rounds))
         if rc != 0:
             raise ValueError(f"eao_set_state -> {rc}")
+
+    def set_draw_mode(self, mode):
+        """0: one draw per (site, word, slot) (default); 1: one per (site, realization, slot) --
+        the paper's own coding, bits of a word = temperature replicas (R24)."""
+        if self.lib.eao_set_draw_mode(self.h, int(mode)) != 0:
+            raise ValueError("draw mode must be 0 or 1")
+
+    def draw_mode(self) -> int:
+        return int(self.lib.eao_get_draw_mode(self.h))
 
     def set_field(self, h):
         """Constant external field h of Eq. 1 (integer); energies are recomputed."""
