@@ -8,6 +8,8 @@ through the C ABI of libea_b200.so.
   python bench.py --impl reference ...      # the CPU oracle, as it stands, on the host cores
   python bench.py --field 1                 # the same workload with h = 1 (generic kernel)
   python bench.py --measure-every 10        # two-copy overlap/energy moments every 10 sweeps
+  python bench.py --layout replica --sweeps-per-step 200   # the paper's own coding (bits = temperature
+                                            # replicas of one realization, one random number per replica)
 
 A *step* = `sweeps_per_step` full checkerboard sweeps, each followed by a PT round (config's
 swap_interval), of the whole workload: every row of SURVEY.md section 8(a) on the hot path.
@@ -308,13 +310,17 @@ def run_cuda(a, cfg):
     sps = a.sweeps_per_step
     me = a.measure_every
     # the golden digests describe the BASELINE config itself, as rank 0 simulates it
-    plain = not (a.field or me or a.realizations is not None or a.swap_interval is not None)
+    replica = a.layout == "replica"
+    plain = not (a.field or me or a.realizations is not None or a.swap_interval is not None or replica)
 
     def make():
         # weak scaling: every rank owns cfg.R realizations; rank r simulates global words r*W..
         sim = EA(cfg.L, cfg.n_temps, cfg.R, betas, cfg.seed, first_realization=shard_first_realization(rank, cfg.R))
         if a.field:
             sim.set_field(a.field)
+        if replica:
+            from paper_1311_5582_b200 import EA_LAYOUT_REPLICA_BITS
+            sim.set_layout(EA_LAYOUT_REPLICA_BITS)
         if me:
             # two copies of every disorder realization (words w and w + W/2), overlap and energy
             # moments accumulated on the device every `me` sweeps (ea_measure)
@@ -404,7 +410,10 @@ def run_cuda(a, cfg):
     peak = measure_int_peak(torch.cuda.current_stream().cuda_stream)
     # resident / streaming kernel: one launch per step, so the step time IS the kernel's launch
     # duration; generic path: the step is sweep + energy + swap launches and the figure is for the step.
-    ops_per_update = alu_ops_per_update(cfg, sps)
+    # second layout: per attempt 5 (Philox XOR3, one call per four sites of ONE replica) + 6 (class of
+    # the replica's bit from the three planes) + 2 (64-bit compare) + 2 (flip bit) + 14 / n_temps
+    # (bonds and adder, shared by the word's replicas) ALU-pipe lane-ops: x 32 per "word update"
+    ops_per_update = 32.0 * (15.0 + 14.0 / cfg.n_temps) if replica else alu_ops_per_update(cfg, sps)
     step_s = float(np.mean(step_ms)) * 1e-3
     achieved = ops_per_update * cfg.n_temps * cfg.W * cfg.N * sps / step_s
     prof = ncu_profile_numbers(a.config) if plain else None
@@ -420,7 +429,7 @@ def run_cuda(a, cfg):
         roofline["hbm_view"] = hbm_view(cfg, sps, step_s)
 
     per_config = None
-    if a.per_config and world == 1:
+    if a.per_config and world == 1 and not replica:
         per_config = per_config_block(torch, EA, flush_l2, peak["lop3"], a.config if plain and sps >= 1000 else None)
         if plain and sps >= 1000:
             ent = {"workload": cfg.name, "kernel": KERNEL_NAMES.get(kernel), "sweeps_per_step": sps,
@@ -444,7 +453,7 @@ def run_cuda(a, cfg):
         "dtype": "u32 bit-sliced words (32 realizations each), u32 Philox draws", "data": "synthetic",
         "config": {"workload": cfg.name, "L": cfg.L, "n_temps": cfg.n_temps, "realizations_per_gpu": cfg.R,
                    "swap_interval": cfg.swap_interval, "sweeps_per_step": sps, "seed": cfg.seed,
-                   "field": a.field, "measure_every": me,
+                   "field": a.field, "measure_every": me, "layout": a.layout,
                    "kernel": KERNEL_NAMES.get(kernel, str(kernel)),
                    "l2": "flushed between timed steps (256 MiB write); state is re-read from HBM each step",
                    "parallelism": f"shard by realization word x{world}, no collective"},
@@ -494,6 +503,9 @@ def main():
     ap.add_argument("--field", type=int, default=0, help="external field h (SURVEY 8(f2)); default 0 = headline workload")
     ap.add_argument("--measure-every", type=int, default=0,
                     help="accumulate two-copy overlap / energy moments every M sweeps (SURVEY 8(f1)); default off")
+    ap.add_argument("--layout", default="realization", choices=["realization", "replica"],
+                    help="multispin coding: bits = realizations (BASELINE configs) or the paper's own bits = temperature "
+                         "replicas with one random number per replica (SURVEY 8(f3), ea_set_layout)")
     ap.add_argument("--no-per-config", dest="per_config", action="store_false",
                     help="skip the per_config block (ps per attempt of the other BASELINE configs)")
     ap.add_argument("--ref-cores", type=int, default=0, help="--impl reference: processes to use (default: all cores)")

@@ -48,9 +48,24 @@ enum {
                                 for all sweeps of the call, PT inside a thread-block cluster */
     EA_KERNEL_TILED = 3,     /* L = 16, 32, 64: z-slab tiles, one launch per half-sweep, lattice
                                 read in place from global memory (L1/L2)                     */
-    EA_KERNEL_STREAM = 4     /* L = 32, 64: one persistent cooperative launch for all sweeps; z-slab
+    EA_KERNEL_STREAM = 4,    /* L = 32, 64: one persistent cooperative launch for all sweeps; z-slab
                                 tiles streamed through shared memory by TMA bulk copies, two
                                 grid-wide barriers per sweep, PT decided redundantly per block */
+    EA_KERNEL_REPLICA = 5    /* the one kernel of EA_LAYOUT_REPLICA_BITS (ea_set_layout): reported by
+                                ea_get_kernel, not selectable                                  */
+};
+
+/* Multispin coding (ea_set_layout).  Two workloads with the same model, tables, initial state and
+ * parallel tempering, different random-number conventions (DESIGN.md section 2 and R24):
+ *   REALIZATION_BITS  bit b of word w = disorder realization 32 w + b; one random number per
+ *                     (site, word, slot) shared by the word's 32 realizations (the default, and
+ *                     the layout of BASELINE.json's configs);
+ *   REPLICA_BITS      the paper's own coding: a word = the temperature
+ *                     replicas of ONE realization at one site, one random number per
+ *                     (site, realization, slot), one thread block per realization. */
+enum {
+    EA_LAYOUT_REALIZATION_BITS = 0,
+    EA_LAYOUT_REPLICA_BITS = 1
 };
 
 /*
@@ -221,6 +236,15 @@ int ea_get_field(ea_handle *h);
  * EA_ERR_INVALID_ARG when no field is set. */
 int ea_get_field_tables(ea_handle *h, uint64_t *accf /* [n_temps][7][2] */,
                         uint64_t *swpf /* [n_temps-1][2 (3+|h|) N + 1] */);
+
+/* Switch the multispin coding of the handle (EA_LAYOUT_*).  The physical state (spins, couplings,
+ * permutation, energies, counters) is kept: only the random numbers consumed by later sweeps
+ * follow the other convention, so ea_set_layout is normally called right after ea_create.
+ * Accessors keep their formats (ea_get_state returns words in the REALIZATION_BITS packing).
+ * REPLICA_BITS needs L <= 32 (a realization's replicas stay in shared memory), n_temps <= 64,
+ * h = 0: otherwise EA_ERR_UNSUPPORTED and nothing changes. */
+int ea_set_layout(ea_handle *h, int layout);
+int ea_get_layout(ea_handle *h);
 
 /* Select the sweep implementation (EA_KERNEL_*); EA_ERR_UNSUPPORTED if it cannot run this shape. */
 int ea_set_kernel(ea_handle *h, int kernel);

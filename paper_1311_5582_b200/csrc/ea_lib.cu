@@ -17,6 +17,7 @@
 #include "ea_stream.cuh"
 #include "ea_peak.cuh"
 #include "ea_measure.cuh"
+#include "ea_replica.cuh"
 
 using ea::Params;
 
@@ -56,6 +57,15 @@ struct ea_handle {
     bool meas_on = false;
     // external field (ea_set_field): own allocation for the 14-class thresholds and the trimmed
     // field swap table; freed by ea_destroy / the next ea_set_field
+    // second layout (ea_set_layout, ea_replica.cuh): own allocation for the T storage (spins by
+    // realization, packed coupling bits, the probability table); r_valid / t_valid say which of the
+    // two spin stores is current
+    int layout = EA_LAYOUT_REALIZATION_BITS;
+    char *d_rep = nullptr;
+    uint32_t *d_spinT = nullptr, *d_jbit = nullptr;
+    uint64_t *d_acc64 = nullptr;
+    int ncube = 0, NW = 0;
+    bool r_valid = true, t_valid = false;
     int field = 0;
     char *d_field = nullptr;
     std::vector<uint64_t> accf, swpf;  // host copies: [nT][7][2], [nT-1][2 (3+|h|) N + 1]
@@ -344,9 +354,41 @@ static int upload_tables(ea_handle *h, const std::vector<uint64_t> &acc, const s
     return EA_OK;
 }
 
+// ---------------------------------------------------------------- second layout: which store is current
+static ea::ReplicaArgs replica_args(const ea_handle *h)
+{
+    ea::ReplicaArgs A{};
+    A.P = h->P; A.spinT = h->d_spinT; A.jbit = h->d_jbit; A.acc64 = h->d_acc64; A.ncube = h->ncube; A.NW = h->NW;
+    return A;
+}
+// the first layout's spin words are what every accessor and measurement kernel reads
+static int ensure_r(ea_handle *h)
+{
+    if (h->layout != EA_LAYOUT_REPLICA_BITS || h->r_valid) return EA_OK;
+    int grid;
+    launch_cfg((int64_t)h->nT * h->W * h->N, 256, grid);
+    ea::k_t2r<<<grid, 256, 0, h->stream>>>(replica_args(h));
+    h->launches++;
+    CUDA_TRY(h, cudaGetLastError());
+    h->r_valid = true;
+    return EA_OK;
+}
+static int ensure_t(ea_handle *h)
+{
+    if (h->t_valid) return EA_OK;
+    int grid;
+    launch_cfg((int64_t)h->Rp * h->ncube * h->N + (int64_t)h->Rp * 6 * h->NW, 256, grid);
+    ea::k_r2t<<<grid, 256, 0, h->stream>>>(replica_args(h));
+    h->launches++;
+    CUDA_TRY(h, cudaGetLastError());
+    h->t_valid = true;
+    return EA_OK;
+}
+
 // ---------------------------------------------------------------- small helpers
 static int recompute_energy(ea_handle *h)
 {
+    { int rc = ensure_r(h); if (rc != EA_OK) return rc; }
     // counter planes: per-thread count (6 Nh / 128 bonds, N / 128 up spins) < 2^(PL - 5)
     const int grid = h->W * h->nT;
     const long long per_thread = 6ll * ((h->N / 2 + 127) / 128);
@@ -488,6 +530,7 @@ extern "C" void ea_destroy(ea_handle *h)
     if (h->own_ws && h->ws) cudaFree(h->ws);
     if (h->d_meas) cudaFree(h->d_meas);
     if (h->d_field) cudaFree(h->d_field);
+    if (h->d_rep) cudaFree(h->d_rep);
     delete h;
 }
 
@@ -539,12 +582,16 @@ static int pack_from_host(ea_handle *h, const int8_t *src, int n_outer, int mode
 extern "C" int ea_set_couplings(ea_handle *h, const int8_t *J)
 {
     if (!h || !J) return fail(h, EA_ERR_INVALID_ARG, "ea_set_couplings: null argument");
+    { int rc = ensure_r(h); if (rc != EA_OK) return rc; }
+    h->t_valid = false;
     return pack_from_host(h, J, 3, 1, h->P.coup);
 }
 
 extern "C" int ea_set_spins(ea_handle *h, const int8_t *s)
 {
     if (!h || !s) return fail(h, EA_ERR_INVALID_ARG, "ea_set_spins: null argument");
+    { int rc = ensure_r(h); if (rc != EA_OK) return rc; }     // a rejected input leaves the state as it was
+    h->t_valid = false;
     return pack_from_host(h, s, h->nT, 0, h->P.spin);
 }
 
@@ -572,6 +619,8 @@ extern "C" int ea_set_field(ea_handle *h, int field)
 {
     if (!h) return EA_ERR_INVALID_ARG;
     if (field < -64 || field > 64) return fail(h, EA_ERR_INVALID_ARG, "ea_set_field: |h| <= 64");
+    if (field != 0 && h->layout == EA_LAYOUT_REPLICA_BITS)
+        return fail(h, EA_ERR_UNSUPPORTED, "ea_set_field: the replica-bits layout runs at h = 0 only");
     const int nT = h->nT, LTS = nT + 1;
     if (field == 0) {
         if (h->field == 0) return EA_OK;
@@ -1066,8 +1115,73 @@ static int sweep_stream(ea_handle *h, int64_t n_sweeps, int swap_interval)
     return EA_OK;
 }
 
+
+// ---------------------------------------------------------------- second layout
+namespace {
+size_t replica_smem(const ea_handle *h, int ncube, int NW)
+{
+    return 4 * ((size_t)ncube * h->N + 6 * (size_t)NW) + 8 * 7 * (size_t)h->nT + 4 * 128 + 128 + 16;
+}
+}  // namespace
+
+extern "C" int ea_set_layout(ea_handle *h, int layout)
+{
+    if (!h || (layout != EA_LAYOUT_REALIZATION_BITS && layout != EA_LAYOUT_REPLICA_BITS))
+        return fail(h, EA_ERR_INVALID_ARG, "ea_set_layout: bad argument");
+    if (layout == h->layout) return EA_OK;
+    if (layout == EA_LAYOUT_REALIZATION_BITS) {
+        { int rc = ensure_r(h); if (rc != EA_OK) return rc; }
+        h->layout = layout;
+        h->t_valid = false;
+        return rebuild_lt(h);                     // the permutation has moved since the masks were built
+    }
+    if (h->field != 0) return fail(h, EA_ERR_UNSUPPORTED, "ea_set_layout: the replica-bits layout runs at h = 0 only");
+    const int ncube = (h->nT + 31) / 32, NW = (h->N / 2 + 31) / 32;
+    if (replica_smem(h, ncube, NW) > 227 * 1024)
+        return fail(h, EA_ERR_UNSUPPORTED, "ea_set_layout: a realization's replicas do not fit shared memory (L <= 32)");
+    if (!h->d_rep) {
+        const size_t b_spin = align256(4 * (size_t)h->Rp * ncube * h->N), b_j = align256(4 * (size_t)h->Rp * 6 * NW);
+        if (cudaMalloc((void **)&h->d_rep, b_spin + b_j + 8 * 7 * (size_t)h->nT) != cudaSuccess)
+            return fail(h, EA_ERR_ALLOC, "ea_set_layout: cudaMalloc failed");
+        h->d_spinT = (uint32_t *)h->d_rep;
+        h->d_jbit = (uint32_t *)(h->d_rep + b_spin);
+        h->d_acc64 = (uint64_t *)(h->d_rep + b_spin + b_j);
+    }
+    h->ncube = ncube; h->NW = NW;
+    h->layout = layout;
+    h->r_valid = true; h->t_valid = false;
+    return EA_OK;
+}
+extern "C" int ea_get_layout(ea_handle *h) { return h ? h->layout : EA_ERR_INVALID_ARG; }
+
+static int sweep_replica(ea_handle *h, int64_t n_sweeps, int swap_interval)
+{
+    if (!h->energy_valid) { int rc = recompute_energy(h); if (rc != EA_OK) return rc; }
+    { int rc = ensure_t(h); if (rc != EA_OK) return rc; }
+    // the probability table, row = temperature index; h->acc outlives the copy
+    CUDA_TRY(h, cudaMemcpyAsync(h->d_acc64, h->acc.data(), 8 * 7 * (size_t)h->nT, cudaMemcpyHostToDevice, h->stream));
+    const size_t smem = replica_smem(h, h->ncube, h->NW);
+    CUDA_TRY(h, cudaFuncSetAttribute(ea::k_replica_sweep, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int64_t left = n_sweeps;
+    while (left > 0) {
+        const int chunk = (int)std::min<int64_t>(left, 1 << 30);
+        ea::ReplicaArgs A = replica_args(h);
+        A.g0 = (uint32_t)h->g; A.n_sweeps = chunk; A.swap_interval = swap_interval; A.nswap0 = (uint32_t)h->nswap;
+        ea::k_replica_sweep<<<h->Rp, 256, smem, h->stream>>>(A);
+        CUDA_TRY(h, cudaGetLastError());
+        h->launches++;
+        h->r_valid = false;
+        if (swap_interval > 0) h->nswap += (h->g + (uint64_t)chunk) / (uint64_t)swap_interval - h->g / (uint64_t)swap_interval;
+        h->g += (uint64_t)chunk;
+        left -= chunk;
+    }
+    h->energy_valid = true;
+    return EA_OK;
+}
+
 static int pick_kernel(const ea_handle *h)
 {
+    if (h->layout == EA_LAYOUT_REPLICA_BITS) return EA_KERNEL_REPLICA;
     if (h->field != 0) return EA_KERNEL_GENERIC;     // the fast kernels are zero-field only
     if (h->kernel_sel != EA_KERNEL_AUTO) return h->kernel_sel;
     if (plan_resident(h).ok) return EA_KERNEL_RESIDENT;
@@ -1079,6 +1193,8 @@ static int pick_kernel(const ea_handle *h)
 extern "C" int ea_set_kernel(ea_handle *h, int kernel)
 {
     if (!h) return EA_ERR_INVALID_ARG;
+    if (h->layout == EA_LAYOUT_REPLICA_BITS)
+        return kernel == EA_KERNEL_AUTO ? EA_OK : fail(h, EA_ERR_UNSUPPORTED, "ea_set_kernel: the replica-bits layout has one kernel");
     if (kernel == EA_KERNEL_AUTO || kernel == EA_KERNEL_GENERIC) { h->kernel_sel = kernel; return EA_OK; }
     if (h->field != 0) return fail(h, EA_ERR_UNSUPPORTED, "ea_set_kernel: only the generic kernel runs with a field");
     if (kernel == EA_KERNEL_RESIDENT && plan_resident(h).ok) { h->kernel_sel = kernel; return EA_OK; }
@@ -1093,6 +1209,7 @@ extern "C" int ea_sweep(ea_handle *h, int64_t n_sweeps, int swap_interval)
     if (!h || n_sweeps < 0 || swap_interval < 0) return fail(h, EA_ERR_INVALID_ARG, "ea_sweep: bad argument");
     if (h->g + (uint64_t)n_sweeps > 0xFFFFFFFFull) return fail(h, EA_ERR_RANGE, "ea_sweep: sweep counter would pass 2^32-1");
     if (n_sweeps == 0) return EA_OK;
+    if (pick_kernel(h) == EA_KERNEL_REPLICA) return sweep_replica(h, n_sweeps, swap_interval);
     if (pick_kernel(h) == EA_KERNEL_RESIDENT) return sweep_resident(h, n_sweeps, swap_interval);
     if (pick_kernel(h) == EA_KERNEL_TILED) return sweep_tiled(h, n_sweeps, swap_interval);
     if (pick_kernel(h) == EA_KERNEL_STREAM) return sweep_stream(h, n_sweeps, swap_interval);
@@ -1123,6 +1240,7 @@ extern "C" int ea_overlap(ea_handle *h, const int32_t *pairs, int n_pairs, int32
         if (pairs[2 * p] < 0 || pairs[2 * p] >= h->R || pairs[2 * p + 1] < -1 || pairs[2 * p + 1] >= h->R)
             return fail(h, EA_ERR_INVALID_ARG, "ea_overlap: realization index out of range");
     if (n_pairs == 0) return EA_OK;
+    { int rc = ensure_r(h); if (rc != EA_OK) return rc; }
     int32_t *d = nullptr;
     const size_t nb_p = 8 * (size_t)n_pairs, nb_q = 4 * (size_t)n_pairs * h->nT;
     CUDA_TRY(h, cudaMalloc((void **)&d, nb_p + nb_q));
@@ -1142,6 +1260,7 @@ extern "C" int ea_overlap(ea_handle *h, const int32_t *pairs, int n_pairs, int32
 extern "C" int ea_get_spins(ea_handle *h, int8_t *s)
 {
     if (!h || !s) return fail(h, EA_ERR_INVALID_ARG, "ea_get_spins: null argument");
+    { int rc = ensure_r(h); if (rc != EA_OK) return rc; }
     const size_t n = (size_t)h->R * h->nT * h->N;
     int8_t *d = nullptr;
     CUDA_TRY(h, cudaMalloc((void **)&d, n));
@@ -1162,6 +1281,7 @@ extern "C" int ea_get_state(ea_handle *h, uint32_t *spin_words, uint8_t *temp_of
 {
     if (!h) return EA_ERR_INVALID_ARG;
     if (energy_by_slot && !h->energy_valid) { int rc = recompute_energy(h); if (rc != EA_OK) return rc; }
+    { int rc = ensure_r(h); if (rc != EA_OK) return rc; }
     const size_t n = (size_t)h->R * h->nT;
     if (spin_words)
         CUDA_TRY(h, cudaMemcpyAsync(spin_words, h->P.spin, 4 * (size_t)h->nT * h->W * h->N, cudaMemcpyDeviceToHost, h->stream));
@@ -1196,6 +1316,8 @@ extern "C" int ea_pair_couplings(ea_handle *h)
 {
     if (!h) return EA_ERR_INVALID_ARG;
     if (h->R % 64) return fail(h, EA_ERR_INVALID_ARG, "ea_pair_couplings: n_realizations must be a multiple of 64");
+    { int rc = ensure_r(h); if (rc != EA_OK) return rc; }
+    h->t_valid = false;
     const size_t half = (size_t)(h->W / 2) * 3 * h->N;   // coup is [w][d][p][j]: each half is contiguous
     CUDA_TRY(h, cudaMemcpyAsync(h->P.coup + half, h->P.coup, 4 * half, cudaMemcpyDeviceToDevice, h->stream));
     return recompute_energy(h);
@@ -1256,6 +1378,7 @@ extern "C" int ea_measure_begin(ea_handle *h, const int32_t *word_pairs, int n_w
 static int measure_once(ea_handle *h)
 {
     if (!h->energy_valid) { int rc = recompute_energy(h); if (rc != EA_OK) return rc; }
+    { int rc = ensure_r(h); if (rc != EA_OK) return rc; }
     if (h->M.P > 0) {
         const int nchunk = (h->N / 4 + ea::kGatherThreads - 1) / ea::kGatherThreads, ngrp = (h->nT + 7) / 8;
         ea::k_gather_by_temp<<<h->W * nchunk * ngrp, ea::kGatherThreads, 4 * 8 * (size_t)h->nT, h->stream>>>(h->P, h->d_T);
@@ -1422,6 +1545,7 @@ extern "C" int ea_set_state(ea_handle *h, const uint32_t *spin_words, const uint
             tau[(size_t)r * nT + k] = (uint8_t)t;
         }
     }
+    h->r_valid = true; h->t_valid = false;
     CUDA_TRY(h, cudaMemcpyAsync(h->P.spin, spin_words, 4 * (size_t)nT * h->W * h->N, cudaMemcpyHostToDevice, h->stream));
     CUDA_TRY(h, cudaMemcpyAsync(h->P.tau, tau.data(), tau.size(), cudaMemcpyHostToDevice, h->stream));
     int grid;
