@@ -13,6 +13,7 @@
 
 #include "ea_generic.cuh"
 #include "ea_resident.cuh"
+#include "ea_small.cuh"
 #include "ea_tiled.cuh"
 #include "ea_stream.cuh"
 #include "ea_peak.cuh"
@@ -788,7 +789,7 @@ static int sweep_generic(ea_handle *h, int64_t n_sweeps, int swap_interval)
 
 // ---------------------------------------------------------------- resident path (L = 8, 16)
 namespace {
-struct ResPlan { bool ok; int C, S, G, swap_win; size_t smem; };
+struct ResPlan { bool ok; int C, S, G, swap_win; size_t smem; bool any; int NQP; size_t any_off; };
 
 // shared memory of k_resident without the swap-threshold window (layout: ea_resident.cuh)
 size_t resident_smem(const ea_handle *h, int S)
@@ -801,13 +802,16 @@ size_t resident_smem(const ea_handle *h, int S)
 
 ResPlan plan_resident(const ea_handle *h)
 {
-    ResPlan pl{false, 1, 0, 1, 0, 0};
-    if (h->L != 8 && h->L != 16) return pl;
+    ResPlan pl{false, 1, 0, 1, 0, 0, false, 0, 0};
+    // run-time geometry: + the word's couplings (3 N words) and the neighbour table (3 words per site)
+    const size_t extra = (h->L != 8 && h->L != 16) ? 24 * (size_t)h->N + 16 : 0;
+    pl.any = h->L != 8 && h->L != 16;          // any other even L: run-time geometry (ea_small.cuh)
+    if (pl.any && h->N / 2 > 1024) return pl;  // one thread per site of a parity: L <= 12
     const size_t cap = 227 * 1024;
     int C = 0;
     for (int c = 1; c <= 8; c *= 2) {            // cluster sizes 1, 2, 4, 8 (others fail to launch)
         const int S = (h->nT + c - 1) / c;
-        if (resident_smem(h, S) <= cap) { C = c; break; }
+        if (resident_smem(h, S) + extra <= cap) { C = c; break; }
     }
     if (!C) return pl;
     // small problems: spread the slots over more SMs (cluster sizes 2, 4, 8)
@@ -817,10 +821,15 @@ ResPlan plan_resident(const ea_handle *h)
     pl.S = (h->nT + C - 1) / C;
     pl.G = 1;
     if (h->L == 8) { pl.G = 8; while (pl.G > 1 && pl.G > pl.S) pl.G >>= 1; }
+    if (pl.any) {
+        pl.NQP = (h->N / 2 + 31) / 32 * 32;                  // thread = site: sites of a parity, padded to warps
+        pl.G = std::max(1, std::min(pl.S, 1024 / pl.NQP));
+    }
     // the swap-threshold window takes what is left, up to 128 entries per temperature pair
     const size_t base = resident_smem(h, pl.S);
-    pl.swap_win = (int)std::min<size_t>(128, (cap - base) / (4 * (size_t)h->nT));
-    pl.smem = base + 4 * (size_t)h->nT * pl.swap_win;
+    pl.swap_win = (int)std::min<size_t>(128, (cap - base - extra) / (4 * (size_t)h->nT));
+    pl.any_off = (base + 4 * (size_t)h->nT * pl.swap_win + 15) & ~(size_t)15;
+    pl.smem = pl.any_off + extra;
     pl.ok = true;
     return pl;
 }
@@ -834,6 +843,25 @@ cudaError_t launch_resident_t(const ea_handle *h, const ea::ResArgs &A, const Re
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3((unsigned)(h->W * pl.C));
     cfg.blockDim = dim3((unsigned)(ea::ResGeom<L>::NQ * G));
+    cfg.dynamicSmemBytes = pl.smem;
+    cfg.stream = h->stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = (unsigned)pl.C;
+    at[0].val.clusterDim.y = 1;
+    at[0].val.clusterDim.z = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, A);
+}
+cudaError_t launch_resident_any(const ea_handle *h, const ea::ResArgs &A, const ResPlan &pl, bool fast)
+{
+    auto kern = fast ? ea::k_resident_any<true> : ea::k_resident_any<false>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem);
+    if (e != cudaSuccess) return e;
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3((unsigned)(h->W * pl.C));
+    cfg.blockDim = dim3((unsigned)(pl.NQP * pl.G));
     cfg.dynamicSmemBytes = pl.smem;
     cfg.stream = h->stream;
     cudaLaunchAttribute at[1];
@@ -869,7 +897,9 @@ static int sweep_resident(ea_handle *h, int64_t n_sweeps, int swap_interval)
         }
         cudaError_t e = cudaErrorInvalidValue;
         const bool fast = h->fast_rank;
-        if (h->L == 16) e = launch_resident_t<16, 1>(h, A, pl, fast);
+        A.NQP = pl.NQP; A.G = pl.G; A.any_off = (int)pl.any_off;
+        if (pl.any) e = launch_resident_any(h, A, pl, fast);
+        else if (h->L == 16) e = launch_resident_t<16, 1>(h, A, pl, fast);
         else if (pl.G == 8) e = launch_resident_t<8, 8>(h, A, pl, fast);
         else if (pl.G == 4) e = launch_resident_t<8, 4>(h, A, pl, fast);
         else if (pl.G == 2) e = launch_resident_t<8, 2>(h, A, pl, fast);

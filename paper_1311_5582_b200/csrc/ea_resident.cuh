@@ -39,6 +39,8 @@ struct ResArgs {
     uint32_t rk[20];          // Philox round keys (k0 + r*0x9E3779B9, k1 + r*0xBB67AE85), r = 0..9
     RankKey K;                // bucket key of a draw (see RankCtx)
     int swap_win;             // swap thresholds for m in [-swap_win, -1] are staged in smem
+    int NQP, G;               // k_resident_any (ea_small.cuh): quads per parity padded to whole warps, slot groups
+    int any_off;              // ... byte offset (16 B aligned) of its coupling copy and neighbour table in smem
 };
 
 // Mask table of one slot from its rank masks (one warp): row n = { lt[n4], lt[n5], lt[n6], 0 },

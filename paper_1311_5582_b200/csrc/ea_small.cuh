@@ -1,0 +1,337 @@
+// ea_small.cuh -- the shared-memory-resident sweep kernel for ANY even L whose lattices fit
+// shared memory (L = 2, 4, 6, 10, 12, 14, ...: the lattices of BASELINE.json's configs 1 and 3).
+//
+// Same organisation as k_resident (ea_resident.cuh): one thread-block cluster per realization
+// word, the slots shared out over its blocks, every slot's lattice in shared memory for all
+// sweeps of the call, parallel tempering inside the cluster over distributed
+// shared memory (table rows move, no lattice word does).  What differs is the
+// geometry: the lattice side is a run-time value and a row of L/2 same-parity sites is not a
+// whole number of quads (L = 12: 6 sites), so a thread finds the six neighbours of each of its
+// four sites in a table built once per launch (site_of / nbr_of, compare-select wrap) and reads them
+// as single words; the word's couplings sit in shared memory next to the lattices.  These
+// problems are far too small to fill a B200: what this kernel removes is the per-sweep launch /
+// grid-barrier latency of the global-memory path (config 3: 18 -> 4 us per sweep).
+#pragma once
+#include "ea_resident.cuh"
+
+namespace ea {
+
+// n_sat planes of site (p, j) from shared memory only: lattice `sp` ([2][Nh]), the word's couplings
+// `js` ([d][p][j], 3 N words) and the neighbour table `nb` ([3][p][j]: checkerboard indices in the
+// other parity's array, + in the low and - in the high 16 bits; built once per launch, so the hot
+// loop has no division by the run-time L).  Thread = site: a warp's accesses are stride-1.
+__device__ __forceinline__ Planes site_planes_tab(const uint32_t *sp, const uint32_t *js, const uint32_t *nb, int p, int j,
+                                                  int Nh, int N, uint32_t *self_out)
+{
+    const int me = p * Nh + j, ot = (1 - p) * Nh;
+    const uint32_t tx = nb[me], ty = nb[N + me], tz = nb[2 * N + me];
+    const int xp = (int)(tx & 0xFFFFu), xm = (int)(tx >> 16), yp = (int)(ty & 0xFFFFu), ym = (int)(ty >> 16);
+    const int zp = (int)(tz & 0xFFFFu), zm = (int)(tz >> 16);
+    const uint32_t *so = sp + ot;
+    const uint32_t s = sp[me];
+    const uint32_t e0 = xor3(s, js[me], so[xp]);
+    const uint32_t e1 = xor3(s, js[ot + xm], so[xm]);
+    const uint32_t e2 = xor3(s, js[N + me], so[yp]);
+    const uint32_t e3 = xor3(s, js[N + ot + ym], so[ym]);
+    const uint32_t e4 = xor3(s, js[2 * N + me], so[zp]);
+    const uint32_t e5 = xor3(s, js[2 * N + ot + zm], so[zm]);
+    *self_out = s;
+    return nsat_planes(e0, e1, e2, e3, e4, e5);
+}
+
+// New word of site (p, j) of lattice `sp` for the draw u.  FAST: ranks from the bucket table; the
+// rare flagged site is redone with the exact search.
+template <bool FAST, bool ENERGY>
+__device__ __forceinline__ void update_site_any(uint32_t *sp, const uint32_t *js, const uint32_t *nb, const uint32_t *lt,
+                                                const uint4 *mt, const RankCtx &R, int p, int j, int Nh, int N,
+                                                uint32_t u, Planes &fin)
+{
+    uint32_t s, flag = FAST ? 0u : 0x80000000u, acc = 0u;
+    const Planes pl = site_planes_tab(sp, js, nb, p, j, Nh, N, &s);
+    if (FAST) acc = accept_fast(R, mt, u, pl, &flag);
+    if ((int)flag < 0) acc = accept_exact(R, lt, u, pl);
+    sp[p * Nh + j] = s ^ acc;
+    if (ENERGY) fin = planes_after(pl, acc);
+}
+
+// warp_sum4 (ea_resident.cuh) for NP-plane counts: four slots in flight, two halving levels, three
+// plain ones; every lane of the 8-lane group 2 (lane>>4) + ((lane>>3)&1) ends with that slot's sum.
+template <int NP>
+__device__ __forceinline__ void warp_sum4_t(uint32_t (&en)[4][NP], int lane, uint32_t (&out)[NP + 5])
+{
+    const uint32_t hi16 = (lane & 16) ? 0xFFFFFFFFu : 0u, hi8 = (lane & 8) ? 0xFFFFFFFFu : 0u;
+    uint32_t a[2][NP + 1];
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+        uint32_t keep[NP], got[NP];
+#pragma unroll
+        for (int i = 0; i < NP; ++i) {
+            keep[i] = mux(en[h][i], en[2 + h][i], hi16);
+            got[i] = __shfl_xor_sync(0xFFFFFFFFu, mux(en[2 + h][i], en[h][i], hi16), 16);
+        }
+        vsum<NP>(keep, got, a[h]);
+    }
+    uint32_t b[NP + 2], c[NP + 3], d[NP + 4];
+    {
+        uint32_t keep[NP + 1], got[NP + 1];
+#pragma unroll
+        for (int i = 0; i < NP + 1; ++i) {
+            keep[i] = mux(a[0][i], a[1][i], hi8);
+            got[i] = __shfl_xor_sync(0xFFFFFFFFu, mux(a[1][i], a[0][i], hi8), 8);
+        }
+        vsum<NP + 1>(keep, got, b);
+    }
+    {
+        uint32_t got[NP + 2];
+#pragma unroll
+        for (int i = 0; i < NP + 2; ++i) got[i] = __shfl_xor_sync(0xFFFFFFFFu, b[i], 4);
+        vsum<NP + 2>(b, got, c);
+    }
+    {
+        uint32_t got[NP + 3];
+#pragma unroll
+        for (int i = 0; i < NP + 3; ++i) got[i] = __shfl_xor_sync(0xFFFFFFFFu, c[i], 2);
+        vsum<NP + 3>(c, got, d);
+    }
+    {
+        uint32_t got[NP + 4];
+#pragma unroll
+        for (int i = 0; i < NP + 4; ++i) got[i] = __shfl_xor_sync(0xFFFFFFFFu, d[i], 1);
+        vsum<NP + 4>(d, got, out);
+    }
+}
+
+// add_counts (ea_resident.cuh) for NPL planes
+template <int NPL>
+__device__ __forceinline__ void add_counts_t(const uint32_t (&tot)[NPL], int i, int *acc_row)
+{
+    uint32_t lo = 0, hi = 0;
+#pragma unroll
+    for (int j = 0; j < NPL; ++j) {
+        lo += ((tot[j] >> i) & 0x00010001u) * (1u << j);
+        hi += ((tot[j] >> (i + 8)) & 0x00010001u) * (1u << j);
+    }
+    atomicAdd(acc_row + i, (int)(lo & 0xFFFFu));
+    atomicAdd(acc_row + i + 16, (int)(lo >> 16));
+    atomicAdd(acc_row + i + 8, (int)(hi & 0xFFFFu));
+    atomicAdd(acc_row + i + 24, (int)(hi >> 16));
+}
+
+template <bool FAST>
+__global__ void __launch_bounds__(1024, 1) k_resident_any(const ResArgs A)
+{
+    const int L = A.P.L, Lh = A.P.Lh, N = A.P.N, Nh = A.P.Nh, NSP = A.NQP, G = A.G, NT = NSP * G;
+    extern __shared__ __align__(16) uint32_t smem[];
+    const Params &P = A.P;
+    const int nT = P.nT, LTS = P.LTS, S = A.S, C = A.C;
+    const int w = blockIdx.x / C, rank = blockIdx.x % C;
+    const int k0 = rank * S;
+    const int nk = max(0, min(S, nT - k0));      // slots owned by this block
+    const int tid = threadIdx.x, lane = tid & 31;
+    // thread = (slot group, site of one parity): a warp's shared-memory accesses are stride-1 and the
+    // four sites of a quad, which share a Philox call, sit in adjacent lanes (each computes it).
+    // Sites are padded to whole warps (a warp never straddles two slot groups: the energy butterfly
+    // sums the 32 lanes of one slot); the padding threads only take part in barriers and shuffles.
+    const int sg = tid / NSP, j = tid % NSP, q = j >> 2;
+    const bool live = j < Nh;
+
+    // shared memory: the rank table first (fixed offset 0), lattices next (16 B aligned)
+    const int MTS = 3 * nT + 2, SW = A.swap_win;
+    uint4 *bucket = reinterpret_cast<uint4 *>(smem);                 // [n_bucket] 16 B entries
+    uint32_t *sp = smem + 4 * (size_t)A.K.n_bucket;                    // [S][2][Nh]
+    uint4 *mt = reinterpret_cast<uint4 *>(sp + (size_t)S * N);       // [S][MTS] mask tables
+    uint32_t *lt = reinterpret_cast<uint32_t *>(mt + (size_t)S * MTS);   // [S][LTS]
+    uint32_t *thr = lt + S * LTS;                                    // [3][LTS]
+    uchar4 *trip = reinterpret_cast<uchar4 *>(thr + 3 * LTS);        // [MTS]
+    int32_t *Eacc = (int32_t *)(trip + MTS);                         // [S][32] satisfied-bond counts
+    int32_t *swm = Eacc + S * 32;                                    // [nT][4]: lo, cnt, off, kinds
+    uint32_t *swwin = (uint32_t *)(swm + 4 * nT);                    // [nT][SW] thresholds - 1
+    int16_t *Eall = (int16_t *)(swwin + nT * SW);                    // [2][nT][32], by swap-round parity
+    uint8_t *tau8 = (uint8_t *)(Eall + 2 * nT * 32);                 // [32][nT]
+    uint8_t *sig8 = tau8 + 32 * nT;                                  // [32][nT]
+    uint32_t *js = reinterpret_cast<uint32_t *>(smem) + A.any_off / 4;  // [3][2][Nh] the word's couplings
+    uint32_t *nb = js + 3 * N;                                       // [3][2][Nh] neighbour table
+
+    // ---- load state: lattices of my slots, tables, permutation of my 32 realizations
+    {   // lattices: eight independent 128-bit loads in flight per thread before the first store
+        // (one load per round trip cost ~25 us per launch when the state comes from HBM)
+        const int VL = N / 4;
+        const int total = nk * VL;
+        for (int base = 0; base < total; base += 8 * NT) {
+            uint4 v[8];
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                const int e = base + u * NT + tid;
+                if (e < total)
+                    v[u] = reinterpret_cast<const uint4 *>(P.spin + ((size_t)(k0 + e / VL) * P.W + w) * N)[e % VL];
+            }
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                const int e = base + u * NT + tid;
+                if (e < total) reinterpret_cast<uint4 *>(sp)[e] = v[u];
+            }
+        }
+    }
+    for (int k = 0; k < nk; ++k)
+        for (int a = tid; a < LTS; a += NT) lt[k * LTS + a] = P.lt[((size_t)w * nT + k0 + k) * LTS + a];
+    for (int a = tid; a < 3 * LTS; a += NT) thr[a] = P.thr32[a];
+    for (int a = tid; a < A.K.n_bucket; a += NT) bucket[a] = A.bucket[a];
+    for (int a = tid; a < 32 * nT; a += NT) {
+        tau8[a] = P.tau[(size_t)32 * w * nT + a];
+        sig8[a] = P.sigma[(size_t)32 * w * nT + a];
+    }
+    for (int a = tid; a < S * 32; a += NT) Eacc[a] = 0;
+    for (int a = tid; a < 2 * nT * 32; a += NT)
+        Eall[a] = (int16_t)P.E[(size_t)(32 * w + (a & 31)) * nT + ((a >> 5) % nT)];   // |E| <= 3N <= 12288
+    for (int a = tid; a < MTS - 1; a += NT) trip[a] = A.trip[a];
+    for (int t = tid; t + 1 < nT; t += NT) {
+        swm[4 * t] = P.swp_lo[t]; swm[4 * t + 1] = P.swp_cnt[t]; swm[4 * t + 2] = P.swp_off[t];
+        swm[4 * t + 3] = (int)P.swp_kind[2 * t] | ((int)P.swp_kind[2 * t + 1] << 1);
+    }
+    __syncthreads();                                        // swm is complete
+    // window m = -SW + i of row t: range constants from shared memory, so that the global loads
+    // of the iterations are independent (they were three dependent round trips each: ~12 us)
+#pragma unroll 4
+    for (int a = tid; a < (nT - 1) * SW; a += NT) {
+        const int t = a / SW, m = -SW + a % SW;
+        const int lo = swm[4 * t], cnt = swm[4 * t + 1];
+        swwin[a] = (m >= lo && m < lo + cnt) ? P.swp_val[swm[4 * t + 2] + (m - lo)] : 0u;
+    }
+
+    for (int a = tid; a < 3 * N; a += NT) js[a] = P.coup[(size_t)w * 3 * N + a];
+    for (int a = tid; a < N; a += NT) {
+        const int pp = a / Nh, ja = a - pp * Nh;
+        const Nbr n = nbr_of(site_of(ja, pp, L, Lh), L, Lh);
+        nb[a] = (uint32_t)n.xp | ((uint32_t)n.xm << 16);
+        nb[N + a] = (uint32_t)n.yp | ((uint32_t)n.ym << 16);
+        nb[2 * N + a] = (uint32_t)n.zp | ((uint32_t)n.zm << 16);
+    }
+
+    RankCtx R;
+    R.thr = thr; R.LTS = LTS; R.nT = nT;
+    R.z0 = P.z[0]; R.z1 = P.z[1]; R.z2 = P.z[2];
+    rank_ctx_key(R, A.K, bucket);
+    const uint32_t gw = P.w0 + (uint32_t)w;
+    const PhiloxQuad PQ = philox_quad_init((uint32_t)q, gw, A.rk);
+    cg::cluster_group cl = cg::this_cluster();
+    __syncthreads();
+    for (int kl = tid >> 5; kl < nk; kl += NT >> 5) build_mt(mt + (size_t)kl * MTS, lt + kl * LTS, trip, nT, lane);
+    if (C > 1) cl.sync(); else __syncthreads();   // every block's shared memory is initialised
+
+    uint32_t nswap = A.nswap0;
+    for (int it = 0; it < A.n_sweeps; ++it) {
+        const uint32_t g = A.g0 + (uint32_t)it;
+        const bool swap_now = A.swap_interval > 0 && ((uint64_t)g + 1) % (uint64_t)A.swap_interval == 0;
+        const bool need_E = swap_now || it == A.n_sweeps - 1;
+        Planes fin;
+        // ---------------- parity 0
+        for (int kl = sg; kl < nk; kl += G) {
+            if (!live) continue;
+            const uint4 rnd = philox_quad(PQ, g, (uint32_t)(k0 + kl), A.rk);
+            update_site_any<FAST, false>(sp + (size_t)kl * N, js, nb, lt + kl * LTS, mt + (size_t)kl * MTS, R, 0, j, Nh, N, pick(rnd, j & 3), fin);
+        }
+        __syncthreads();
+        // ---------------- parity 1 (+ satisfied-bond count of the finished sweep)
+        if (!need_E) {
+            for (int kl = sg; kl < nk; kl += G) {
+                if (!live) continue;
+                const uint4 rnd = philox_quad(PQ, g, (1u << 16) | (uint32_t)(k0 + kl), A.rk);
+                update_site_any<FAST, false>(sp + (size_t)kl * N, js, nb, lt + kl * LTS, mt + (size_t)kl * MTS, R, 1, j, Nh, N, pick(rnd, j & 3), fin);
+            }
+            __syncthreads();
+            continue;
+        }
+        for (int kb = sg; kb < S; kb += 4 * G) {     // batches of four slots: kb, kb+G, kb+2G, kb+3G
+            uint32_t en[4][3];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const int kl = kb + i * G;
+                if (kl < nk && live) {
+                    const uint4 rnd = philox_quad(PQ, g, (1u << 16) | (uint32_t)(k0 + kl), A.rk);
+                    update_site_any<FAST, true>(sp + (size_t)kl * N, js, nb, lt + kl * LTS, mt + (size_t)kl * MTS, R, 1, j, Nh, N, pick(rnd, j & 3), fin);
+                    en[i][0] = fin.b0; en[i][1] = fin.b1; en[i][2] = fin.b2;
+                } else {
+#pragma unroll
+                    for (int jj = 0; jj < 3; ++jj) en[i][jj] = 0;
+                }
+            }
+            uint32_t tot[8];
+            warp_sum4_t<3>(en, lane, tot);
+            const int i_mine = 2 * (lane >> 4) + ((lane >> 3) & 1);
+            const int kl = kb + i_mine * G;
+            if (kl < nk) add_counts_t<8>(tot, lane & 7, Eacc + kl * 32);
+        }
+        __syncthreads();
+        // ---- energies of my slots: E = 3N - 2 (satisfied bonds); pushed into every block of
+        //      the cluster (distributed shared memory), buffer chosen by the swap-round parity
+        int16_t *Ebuf = Eall + (nswap & 1u) * nT * 32;
+        for (int a = tid; a < nk * 32; a += NT) {
+            const int e = 3 * N - 2 * Eacc[a];
+            Eacc[a] = 0;
+            const int dst = k0 * 32 + a;
+            if (C > 1) {
+                for (int rr = 0; rr < C; ++rr) cl.map_shared_rank(Ebuf, rr)[dst] = (int16_t)e;
+            } else {
+                Ebuf[dst] = (int16_t)e;
+            }
+        }
+        if (!swap_now) { __syncthreads(); continue; }
+        if (C > 1) { cluster_arrive(); cluster_wait(); } else __syncthreads();
+        // ---- swap round: warp per temperature pair, lane = realization.  Every block of the
+        //      cluster computes all pairs of its word (identical results).
+        const int warp = tid >> 5, nwarp = NT >> 5;
+        for (int t = (int)(nswap & 1u) + 2 * warp; t + 1 < nT; t += 2 * nwarp) {
+            uint8_t *sg_ = sig8 + lane * nT, *ta_ = tau8 + lane * nT;
+            const int sa = sg_[t], sb = sg_[t + 1];
+            const int m = ((int)Ebuf[sa * 32 + lane] - (int)Ebuf[sb * 32 + lane]) / 4;
+            const uint4 v = philox_rk(g, (uint32_t)t, P.r0 + (uint32_t)(32 * w + lane), 2u << 16, A.rk);
+            const int lo = swm[4 * t], cnt = swm[4 * t + 1], kinds = swm[4 * t + 3];
+            bool acc;
+            if (m < lo) acc = kinds & 1;
+            else if (m >= lo + cnt) acc = (kinds >> 1) & 1;
+            else if (m >= -SW && m < 0) acc = v.x <= swwin[t * SW + m + SW];
+            else acc = v.x <= P.swp_val[swm[4 * t + 2] + (m - lo)];
+            if (acc) {
+                sg_[t] = (uint8_t)sb; sg_[t + 1] = (uint8_t)sa;
+                ta_[sa] = (uint8_t)(t + 1); ta_[sb] = (uint8_t)t;
+            }
+        }
+        ++nswap;
+        __syncthreads();
+        for (int kl = warp; kl < nk; kl += nwarp) {   // rank masks of my slots
+            const int t = tau8[lane * nT + k0 + kl];
+            const int pos = P.desc ? t : nT - 1 - t;
+#pragma unroll 8
+            for (int n = 0; n <= nT; ++n) {
+                const uint32_t mk = __ballot_sync(0xFFFFFFFFu, pos >= n);
+                if (lane == (n & 31)) lt[kl * LTS + n] = mk;
+            }
+            __syncwarp();
+            build_mt(mt + (size_t)kl * MTS, lt + kl * LTS, trip, nT, lane);
+        }
+        __syncthreads();
+    }
+    // the energies written last are in the buffer selected by the final nswap parity... the
+    // last sweep always computes them; which buffer depends on whether that sweep swapped
+    const bool last_swapped = A.swap_interval > 0 &&
+                              ((uint64_t)A.g0 + (uint64_t)A.n_sweeps) % (uint64_t)A.swap_interval == 0;
+    const int16_t *Elast = Eall + (((last_swapped ? nswap - 1 : nswap) & 1u) * nT * 32);
+    if (C > 1) cl.sync();                         // no block exits while others may still push to it
+
+    // ---- write back
+    for (int k = 0; k < nk; ++k) {
+        uint4 *dst = reinterpret_cast<uint4 *>(P.spin + ((size_t)(k0 + k) * P.W + w) * N);
+        const uint4 *src = reinterpret_cast<const uint4 *>(sp + (size_t)k * N);
+        for (int a = tid; a < N / 4; a += NT) dst[a] = src[a];
+        for (int a = tid; a < LTS; a += NT) P.lt[((size_t)w * nT + k0 + k) * LTS + a] = lt[k * LTS + a];
+        for (int a = tid; a < 32; a += NT) P.E[(size_t)(32 * w + a) * nT + k0 + k] = Elast[(k0 + k) * 32 + a];
+    }
+    if (rank == 0) {
+        for (int a = tid; a < 32 * nT; a += NT) {
+            P.tau[(size_t)32 * w * nT + a] = tau8[a];
+            P.sigma[(size_t)32 * w * nT + a] = sig8[a];
+        }
+    }
+}
+
+}  // namespace ea

@@ -33,12 +33,12 @@ def _assert_same(g, o, tag=""):
     assert st["sweeps"] == c["sweeps"] and st["swap_rounds"] == c["swap_rounds"]
 
 
-KERNELS = [1, 2, 3, 4]   # GENERIC, RESIDENT (L = 8, 16), TILED (L = 16, 32, 64), STREAM (L = 32, 64)
+KERNELS = [1, 2, 3, 4]   # GENERIC, RESIDENT (even L <= 12, 16), TILED (L = 16, 32, 64), STREAM (L = 32, 64)
 
 
 def _skip_unsupported(kernel, L):
-    if kernel == 2 and L not in (8, 16):
-        pytest.skip("resident kernel supports L = 8, 16")
+    if kernel == 2 and (L > 16 or L == 14):
+        pytest.skip("resident kernels support even L <= 12 and L = 16 (lattices in shared memory)")
     if kernel == 3 and L not in (16, 32, 64):
         pytest.skip("tiled kernel supports L = 16, 32, 64")
     if kernel == 4 and L not in (32, 64):
@@ -192,7 +192,11 @@ def test_auto_picks_resident_for_L16():
     g = EA(16, 4, 32, np.array([1.0, 0.9, 0.8, 0.7]), 1)
     assert g.get_kernel() == 2
     g.destroy()
-    g = EA(12, 4, 32, np.array([1.0, 0.9, 0.8, 0.7]), 1)
+    for L in (2, 4, 6, 12):            # run-time geometry, still shared-memory resident
+        g = EA(L, 4, 32, np.array([1.0, 0.9, 0.8, 0.7]), 1)
+        assert g.get_kernel() == 2
+        g.destroy()
+    g = EA(20, 4, 32, np.array([1.0, 0.9, 0.8, 0.7]), 1)
     assert g.get_kernel() == 1
     g.destroy()
     g = EA(32, 4, 32, np.array([1.0, 0.9, 0.8, 0.7]), 1)
