@@ -51,8 +51,11 @@ enum {
     EA_KERNEL_STREAM = 4,    /* L = 32, 64: one persistent cooperative launch for all sweeps; z-slab
                                 tiles streamed through shared memory by TMA bulk copies, two
                                 grid-wide barriers per sweep, PT decided redundantly per block */
-    EA_KERNEL_REPLICA = 5    /* the one kernel of EA_LAYOUT_REPLICA_BITS (ea_set_layout): reported by
+    EA_KERNEL_REPLICA = 5,   /* the one kernel of EA_LAYOUT_REPLICA_BITS (ea_set_layout): reported by
                                 ea_get_kernel, not selectable                                  */
+    EA_KERNEL_GENERIC_STEPWISE = 6   /* the generic kernels with one launch per half-sweep / energy /
+                                swap round: what EA_KERNEL_GENERIC falls back to when the
+                                cooperative launch is refused or the work exceeds one wave     */
 };
 
 /* Multispin coding (ea_set_layout).  Two workloads with the same model, tables, initial state and

@@ -11,6 +11,7 @@ _LIB_PATH = _PKG / "libea_b200.so"
 _lib = None
 
 EA_KERNEL_AUTO, EA_KERNEL_GENERIC, EA_KERNEL_RESIDENT, EA_KERNEL_TILED, EA_KERNEL_STREAM, EA_KERNEL_REPLICA = 0, 1, 2, 3, 4, 5
+EA_KERNEL_GENERIC_STEPWISE = 6
 EA_LAYOUT_REALIZATION_BITS, EA_LAYOUT_REPLICA_BITS = 0, 1
 
 _SYMBOLS = [

@@ -36,6 +36,15 @@ __global__ void k_identity_perm(Params P)
     P.sigma[tid] = k;
 }
 
+// energy[r][t] = E[r][sigma[r][t]] for the first R realizations (ea_energy: north_star (4), by temperature index)
+__global__ void k_energy_by_temp(Params P, int R, int32_t *out)
+{
+    const int tid = blockIdx.x * blockDim.x + threadIdx.x;
+    if (tid >= R * P.nT) return;
+    const int r = tid / P.nT;
+    out[tid] = P.E[(size_t)r * P.nT + P.sigma[tid]];
+}
+
 // sigma = inverse of tau, per realization (after tau was replaced: ea_set_state)
 __global__ void k_invert_perm(Params P)
 {

@@ -67,6 +67,10 @@ struct ea_handle {
     uint64_t *d_acc64 = nullptr;
     int ncube = 0, NW = 0;
     bool r_valid = true, t_valid = false;
+    // scratch for the host-buffer calls (packing inputs, overlaps, exported spins / couplings, energies
+    // by temperature): one allocation that only grows, instead of a cudaMalloc / cudaFree per call
+    char *d_scratch = nullptr;
+    size_t scratch_bytes = 0;
     int field = 0;
     char *d_field = nullptr;
     std::vector<uint64_t> accf, swpf;  // host copies: [nT][7][2], [nT-1][2 (3+|h|) N + 1]
@@ -355,6 +359,17 @@ static int upload_tables(ea_handle *h, const std::vector<uint64_t> &acc, const s
     return EA_OK;
 }
 
+// ---------------------------------------------------------------- scratch
+static char *scratch(ea_handle *h, size_t bytes)
+{
+    if (bytes <= h->scratch_bytes) return h->d_scratch;
+    if (h->d_scratch) { cudaStreamSynchronize(h->stream); cudaFree(h->d_scratch); h->d_scratch = nullptr; h->scratch_bytes = 0; }
+    const size_t want = (bytes + ((size_t)1 << 20)) & ~(((size_t)1 << 20) - 1);
+    if (cudaMalloc((void **)&h->d_scratch, want) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+    h->scratch_bytes = want;
+    return h->d_scratch;
+}
+
 // ---------------------------------------------------------------- second layout: which store is current
 static ea::ReplicaArgs replica_args(const ea_handle *h)
 {
@@ -532,6 +547,7 @@ extern "C" void ea_destroy(ea_handle *h)
     if (h->d_meas) cudaFree(h->d_meas);
     if (h->d_field) cudaFree(h->d_field);
     if (h->d_rep) cudaFree(h->d_rep);
+    if (h->d_scratch) cudaFree(h->d_scratch);
     delete h;
 }
 
@@ -555,8 +571,8 @@ static int pack_from_host(ea_handle *h, const int8_t *src, int n_outer, int mode
     const size_t n = (size_t)h->R * n_outer * h->N;
     const size_t nw = (size_t)n_outer * h->W * h->N;
     const size_t off_w = (n + 255) & ~(size_t)255, off_f = off_w + 4 * nw;
-    char *tmp = nullptr;
-    CUDA_TRY(h, cudaMalloc((void **)&tmp, off_f + 256));
+    char *tmp = scratch(h, off_f + 256);
+    if (!tmp) return fail(h, EA_ERR_ALLOC, "pack: cudaMalloc failed");
     int bad = 0;
     cudaError_t e = cudaMemcpyAsync(tmp, src, n, cudaMemcpyHostToDevice, h->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(tmp + off_f, 0, 4, h->stream);
@@ -572,9 +588,7 @@ static int pack_from_host(ea_handle *h, const int8_t *src, int n_outer, int mode
     if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
     if (e == cudaSuccess && !bad) {
         e = cudaMemcpyAsync(dst, tmp + off_w, 4 * nw, cudaMemcpyDeviceToDevice, h->stream);
-        if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
     }
-    cudaFree(tmp);
     if (e != cudaSuccess) return fail(h, EA_ERR_CUDA, std::string("pack: ") + cudaGetErrorString(e));
     if (bad) return fail(h, EA_ERR_INVALID_ARG, "values must be +1 or -1");
     return recompute_energy(h);
@@ -745,9 +759,8 @@ static cudaError_t launch_generic_persistent(ea_handle *h, int n_sweeps, int swa
 
 static int sweep_generic(ea_handle *h, int64_t n_sweeps, int swap_interval)
 {
-    // persistent path first (EA_GENERIC_STEPWISE=1 forces the one-launch-per-step path: tests)
-    const char *stepwise = std::getenv("EA_GENERIC_STEPWISE");
-    while (n_sweeps > 0 && !(stepwise && stepwise[0] == '1')) {
+    // persistent path first (EA_KERNEL_GENERIC_STEPWISE asks for the one-launch-per-step path)
+    while (n_sweeps > 0 && h->kernel_sel != EA_KERNEL_GENERIC_STEPWISE) {
         const int chunk = (int)std::min<int64_t>(n_sweeps, 1 << 30);
         const cudaError_t e = launch_generic_persistent(h, chunk, swap_interval);
         if (e == cudaErrorCooperativeLaunchTooLarge || e == cudaErrorNotSupported) { cudaGetLastError(); break; }
@@ -1107,7 +1120,7 @@ static int sweep_stream(ea_handle *h, int64_t n_sweeps, int swap_interval)
             A.rk[2 * r] = h->P.k0 + (uint32_t)r * 0x9E3779B9u;
             A.rk[2 * r + 1] = h->P.k1 + (uint32_t)r * 0xBB67AE85u;
         }
-        // debug aid: EA_STREAM_TRACE=<file> dumps per-block phase time stamps of the first 8 sweeps
+#ifdef EA_TRACE   // builder's aid (nvcc -DEA_TRACE): EA_STREAM_TRACE=<file> dumps per-block phase time stamps
         const char *trace_path = std::getenv("EA_STREAM_TRACE");
         unsigned long long *d_trace = nullptr;
         const size_t trace_n = (size_t)pg.grid * 64;
@@ -1115,10 +1128,12 @@ static int sweep_stream(ea_handle *h, int64_t n_sweeps, int swap_interval)
             cudaMemsetAsync(d_trace, 0, 8 * trace_n, h->stream);
             A.trace = d_trace;
         }
+#endif
         // counters and the grid-barrier word start from zero in every launch
         CUDA_TRY(h, cudaMemsetAsync(h->d_Ecnt, 0, 2 * 4 * (size_t)h->Rp * h->nT + 256, h->stream));
         const cudaError_t e = h->L == 32 ? launch_stream_t<32>(h, A, pg, h->fast_rank)
                                          : launch_stream_t<64>(h, A, pg, h->fast_rank);
+#ifdef EA_TRACE
         if (d_trace) {
             std::vector<unsigned long long> tr(trace_n);
             cudaMemcpyAsync(tr.data(), d_trace, 8 * trace_n, cudaMemcpyDeviceToHost, h->stream);
@@ -1126,6 +1141,7 @@ static int sweep_stream(ea_handle *h, int64_t n_sweeps, int swap_interval)
             if (FILE *f = std::fopen(trace_path, "wb")) { std::fwrite(tr.data(), 8, trace_n, f); std::fclose(f); }
             cudaFree(d_trace);
         }
+#endif
         if (e == cudaErrorCooperativeLaunchTooLarge && h->kernel_sel == EA_KERNEL_AUTO && w_off == 0) {
             // the SMs are not all free (another context holds some): same result, one launch per
             // half-sweep instead of one cooperative launch
@@ -1212,6 +1228,7 @@ static int sweep_replica(ea_handle *h, int64_t n_sweeps, int swap_interval)
 static int pick_kernel(const ea_handle *h)
 {
     if (h->layout == EA_LAYOUT_REPLICA_BITS) return EA_KERNEL_REPLICA;
+    if (h->kernel_sel == EA_KERNEL_GENERIC_STEPWISE) return EA_KERNEL_GENERIC_STEPWISE;
     if (h->field != 0) return EA_KERNEL_GENERIC;     // the fast kernels are zero-field only
     if (h->kernel_sel != EA_KERNEL_AUTO) return h->kernel_sel;
     if (plan_resident(h).ok) return EA_KERNEL_RESIDENT;
@@ -1225,7 +1242,7 @@ extern "C" int ea_set_kernel(ea_handle *h, int kernel)
     if (!h) return EA_ERR_INVALID_ARG;
     if (h->layout == EA_LAYOUT_REPLICA_BITS)
         return kernel == EA_KERNEL_AUTO ? EA_OK : fail(h, EA_ERR_UNSUPPORTED, "ea_set_kernel: the replica-bits layout has one kernel");
-    if (kernel == EA_KERNEL_AUTO || kernel == EA_KERNEL_GENERIC) { h->kernel_sel = kernel; return EA_OK; }
+    if (kernel == EA_KERNEL_AUTO || kernel == EA_KERNEL_GENERIC || kernel == EA_KERNEL_GENERIC_STEPWISE) { h->kernel_sel = kernel; return EA_OK; }
     if (h->field != 0) return fail(h, EA_ERR_UNSUPPORTED, "ea_set_kernel: only the generic kernel runs with a field");
     if (kernel == EA_KERNEL_RESIDENT && plan_resident(h).ok) { h->kernel_sel = kernel; return EA_OK; }
     if (kernel == EA_KERNEL_TILED && plan_tiled(h).ok) { h->kernel_sel = kernel; return EA_OK; }
@@ -1251,15 +1268,16 @@ extern "C" int ea_energy(ea_handle *h, int32_t *E)
 {
     if (!h || !E) return fail(h, EA_ERR_INVALID_ARG, "ea_energy: null argument");
     if (!h->energy_valid) { int rc = recompute_energy(h); if (rc != EA_OK) return rc; }
-    const size_t n = (size_t)h->Rp * h->nT;
-    std::vector<int32_t> Es(n);
-    std::vector<uint8_t> sg(n);
-    CUDA_TRY(h, cudaMemcpyAsync(Es.data(), h->P.E, 4 * n, cudaMemcpyDeviceToHost, h->stream));
-    CUDA_TRY(h, cudaMemcpyAsync(sg.data(), h->P.sigma, n, cudaMemcpyDeviceToHost, h->stream));
+    const size_t n = (size_t)h->R * h->nT;                 // energy[r][t] = E[r][sigma[r][t]], gathered on the device
+    int32_t *d = (int32_t *)scratch(h, 4 * n);
+    if (!d) return fail(h, EA_ERR_ALLOC, "ea_energy: cudaMalloc failed");
+    int grid;
+    launch_cfg((int64_t)n, 256, grid);
+    ea::k_energy_by_temp<<<grid, 256, 0, h->stream>>>(h->P, h->R, d);
+    h->launches++;
+    CUDA_TRY(h, cudaGetLastError());
+    CUDA_TRY(h, cudaMemcpyAsync(E, d, 4 * n, cudaMemcpyDeviceToHost, h->stream));
     CUDA_TRY(h, cudaStreamSynchronize(h->stream));
-    for (int r = 0; r < h->R; ++r)
-        for (int t = 0; t < h->nT; ++t)
-            E[(size_t)r * h->nT + t] = Es[(size_t)r * h->nT + sg[(size_t)r * h->nT + t]];
     return EA_OK;
 }
 
@@ -1271,9 +1289,9 @@ extern "C" int ea_overlap(ea_handle *h, const int32_t *pairs, int n_pairs, int32
             return fail(h, EA_ERR_INVALID_ARG, "ea_overlap: realization index out of range");
     if (n_pairs == 0) return EA_OK;
     { int rc = ensure_r(h); if (rc != EA_OK) return rc; }
-    int32_t *d = nullptr;
     const size_t nb_p = 8 * (size_t)n_pairs, nb_q = 4 * (size_t)n_pairs * h->nT;
-    CUDA_TRY(h, cudaMalloc((void **)&d, nb_p + nb_q));
+    int32_t *d = (int32_t *)scratch(h, nb_p + nb_q);
+    if (!d) return fail(h, EA_ERR_ALLOC, "ea_overlap: cudaMalloc failed");
     cudaError_t e = cudaMemcpyAsync(d, pairs, nb_p, cudaMemcpyHostToDevice, h->stream);
     if (e == cudaSuccess) {
         ea::k_overlap<<<n_pairs * h->nT, 256, 0, h->stream>>>(h->P, d, d + 2 * (size_t)n_pairs);
@@ -1282,7 +1300,6 @@ extern "C" int ea_overlap(ea_handle *h, const int32_t *pairs, int n_pairs, int32
     }
     if (e == cudaSuccess) e = cudaMemcpyAsync(Q, d + 2 * (size_t)n_pairs, nb_q, cudaMemcpyDeviceToHost, h->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
-    cudaFree(d);
     if (e != cudaSuccess) return fail(h, EA_ERR_CUDA, std::string("ea_overlap: ") + cudaGetErrorString(e));
     return EA_OK;
 }
@@ -1292,8 +1309,8 @@ extern "C" int ea_get_spins(ea_handle *h, int8_t *s)
     if (!h || !s) return fail(h, EA_ERR_INVALID_ARG, "ea_get_spins: null argument");
     { int rc = ensure_r(h); if (rc != EA_OK) return rc; }
     const size_t n = (size_t)h->R * h->nT * h->N;
-    int8_t *d = nullptr;
-    CUDA_TRY(h, cudaMalloc((void **)&d, n));
+    int8_t *d = (int8_t *)scratch(h, n);
+    if (!d) return fail(h, EA_ERR_ALLOC, "ea_get_spins: cudaMalloc failed");
     int grid;
     launch_cfg((int64_t)n, 256, grid);
     ea::k_unpack_spins<<<grid, 256, 0, h->stream>>>(h->P, h->R, 0, d);
@@ -1301,7 +1318,6 @@ extern "C" int ea_get_spins(ea_handle *h, int8_t *s)
     cudaError_t e = cudaGetLastError();
     if (e == cudaSuccess) e = cudaMemcpyAsync(s, d, n, cudaMemcpyDeviceToHost, h->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
-    cudaFree(d);
     if (e != cudaSuccess) return fail(h, EA_ERR_CUDA, std::string("ea_get_spins: ") + cudaGetErrorString(e));
     return EA_OK;
 }
@@ -1328,8 +1344,8 @@ extern "C" int ea_get_couplings(ea_handle *h, int8_t *J)
 {
     if (!h || !J) return fail(h, EA_ERR_INVALID_ARG, "ea_get_couplings: null argument");
     const size_t n = (size_t)h->R * 3 * h->N;
-    int8_t *d = nullptr;
-    CUDA_TRY(h, cudaMalloc((void **)&d, n));
+    int8_t *d = (int8_t *)scratch(h, n);
+    if (!d) return fail(h, EA_ERR_ALLOC, "ea_get_couplings: cudaMalloc failed");
     int grid;
     launch_cfg((int64_t)n, 256, grid);
     ea::k_unpack_couplings<<<grid, 256, 0, h->stream>>>(h->P, h->R, d);
@@ -1337,7 +1353,6 @@ extern "C" int ea_get_couplings(ea_handle *h, int8_t *J)
     cudaError_t e = cudaGetLastError();
     if (e == cudaSuccess) e = cudaMemcpyAsync(J, d, n, cudaMemcpyDeviceToHost, h->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
-    cudaFree(d);
     if (e != cudaSuccess) return fail(h, EA_ERR_CUDA, std::string("ea_get_couplings: ") + cudaGetErrorString(e));
     return EA_OK;
 }

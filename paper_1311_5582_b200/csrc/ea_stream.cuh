@@ -45,16 +45,23 @@ struct StreamArgs {
     int esm_off;             // byte offset (16 B aligned) of the swap-phase staging area in smem
     int batch_off;           // byte offset (16 B aligned) of the batch list in smem
     unsigned int *gbar;      // grid barrier word (zero before the first launch; self-resetting)
-    unsigned long long *trace;   // debug (EA_STREAM_TRACE): [block][8 sweeps][8] globaltimer stamps of the phases, or null
+#ifdef EA_TRACE
+    unsigned long long *trace;   // builder's aid: [block][8 sweeps][8] globaltimer stamps of the phases, or null
+#endif
 };
 
+// Phase time stamps exist only in builds with -DEA_TRACE; the product build compiles them away.
 __device__ __forceinline__ void trace_stamp(const StreamArgs &A, int it, int slot)
 {
+#ifdef EA_TRACE
     if (A.trace && threadIdx.x == 0 && it < 8) {
         unsigned long long t;
         asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
         A.trace[((size_t)blockIdx.x * 8 + it) * 8 + slot] = t;
     }
+#else
+    (void)A; (void)it; (void)slot;
+#endif
 }
 
 template <int L>

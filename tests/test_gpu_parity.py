@@ -212,14 +212,13 @@ def test_auto_picks_resident_for_L16():
     (16, 24, 640, 1, 5, 0),        # more work items than one wave: stepwise launches either way
     (4, 6, 40, 1, 9, 2),           # with a field
 ])
-def test_generic_stepwise_launches_equal_the_persistent_kernel(monkeypatch, L, nT, R, swap, ns, h):
+def test_generic_stepwise_launches_equal_the_persistent_kernel(L, nT, R, swap, ns, h):
     """EA_KERNEL_GENERIC runs as one cooperative launch per call (k_generic_persistent); if that
     launch is impossible it falls back to one launch per half-sweep / energy / swap round.
-    EA_GENERIC_STEPWISE=1 forces the fall-back: both must follow the oracle."""
+    EA_KERNEL_GENERIC_STEPWISE (6) asks for the fall-back: both must follow the oracle."""
     betas = 1.0 / temperature_ladder(nT, 0.6, 2.2)
     for stepwise in ("0", "1"):
-        monkeypatch.setenv("EA_GENERIC_STEPWISE", stepwise)
-        g, o = _pair(L, nT, R, betas, 77, 1)
+        g, o = _pair(L, nT, R, betas, 77, 6 if stepwise == "1" else 1)
         if h:
             g.set_field(h); o.set_field(h)
         n0 = g.launch_count()
