@@ -72,6 +72,10 @@ struct ea_handle {
     char *d_scratch = nullptr;
     size_t scratch_bytes = 0;
     int field = 0;
+    bool fast_field = false;           // |h| <= 2 and the four-column bucket table exists: the resident kernel runs
+    ea::RankKey KF{};
+    uint4 *d_bucketF = nullptr;
+    uchar4 *d_tripF = nullptr;
     char *d_field = nullptr;
     std::vector<uint64_t> accf, swpf;  // host copies: [nT][7][2], [nT-1][2 (3+|h|) N + 1]
     mutable std::string err;
@@ -173,7 +177,10 @@ struct KeyFn {
 };
 }  // namespace
 
-static bool build_bucket_table(const std::vector<uint32_t> &thr32, const int z[3], int nT,
+// NC = 3: the zero-field classes n_sat = 4, 5, 6, one 16-byte entry per bucket.  NC = 4: the four
+// threshold columns of a field |h| <= 2, 32-byte entries
+// { ~thr_a, n, ~thr_b, ~thr_c | ~thr_d, slow flag, 0, 0 }.
+static bool build_bucket_table(const std::vector<uint32_t> &thr32, const int *z, int nT, int NC,
                                std::vector<uint4> &tab, std::vector<uchar4> &trip, ea::RankKey &K)
 {
     auto rank_c = [&](int c, uint64_t u) {   // n_c(u) = z_c + #{i >= z_c : thr32[c][i] < u}
@@ -181,14 +188,15 @@ static bool build_bucket_table(const std::vector<uint32_t> &thr32, const int z[3
         for (int i = z[c]; i < nT; ++i) if ((uint64_t)thr32[(size_t)c * (nT + 1) + i] < u) n = i + 1;
         return n;
     };
-    trip.assign((size_t)3 * nT + 1, make_uchar4((unsigned char)nT, (unsigned char)nT, (unsigned char)nT, 0));
+    trip.assign((size_t)NC * nT + 1, make_uchar4((unsigned char)nT, (unsigned char)nT, (unsigned char)nT, (unsigned char)(NC == 4 ? nT : 0)));
     auto note = [&](uint64_t u) {
-        const int a = rank_c(0, u), b = rank_c(1, u), c = rank_c(2, u);
-        trip[(size_t)(a + b + c)] = make_uchar4((unsigned char)a, (unsigned char)b, (unsigned char)c, 0);
+        int r[4] = {0, 0, 0, 0}, sum = 0;
+        for (int c = 0; c < NC; ++c) { r[c] = rank_c(c, u); sum += r[c]; }
+        trip[(size_t)sum] = make_uchar4((unsigned char)r[0], (unsigned char)r[1], (unsigned char)r[2], (unsigned char)r[3]);
     };
     note(0);
     uint32_t tmax = 0;
-    for (int c = 0; c < 3; ++c)
+    for (int c = 0; c < NC; ++c)
         for (int i = z[c]; i < nT; ++i) {
             const uint32_t v = thr32[(size_t)c * (nT + 1) + i];
             note((uint64_t)v + 1);
@@ -196,12 +204,13 @@ static bool build_bucket_table(const std::vector<uint32_t> &thr32, const int z[3
         }
     int E = 9;
     while (E < 32 && (tmax >> E)) ++E;                     // 2^E > every threshold - 1
-    const uint32_t slow_row = (uint32_t)(3 * nT + 1);
+    const uint32_t slow_row = (uint32_t)(3 * nT + 1);      // NC = 3 only
+    const int BW = NC == 4 ? 2 : 1;
     for (int MB = 3; MB <= 6; ++MB) {
         const KeyFn key{E, MB};
         const int klo = key(0), khi = key(0xFFFFFFFFu);
         const int n = khi - klo + 1;
-        if (n > kMaxBucket) continue;
+        if (n * BW > kMaxBucket) continue;
         // first u of every bucket (2^32 for an empty bucket at the top)
         std::vector<uint64_t> first((size_t)n + 1);
         first[0] = 0;
@@ -214,15 +223,24 @@ static bool build_bucket_table(const std::vector<uint32_t> &thr32, const int z[3
             }
             first[(size_t)b] = lo;
         }
-        std::vector<uint4> t((size_t)n);
+        std::vector<uint4> t((size_t)n * BW);
+        auto put = [&](int b, bool slow, uint32_t nsum, const uint32_t *inb) {
+            if (NC == 3) {
+                t[(size_t)b] = slow ? make_uint4(0u, slow_row, 0u, 0u) : make_uint4(~inb[0], nsum, ~inb[1], ~inb[2]);
+            } else {
+                t[(size_t)2 * b] = slow ? make_uint4(0u, 0u, 0u, 0u) : make_uint4(~inb[0], nsum, ~inb[1], ~inb[2]);
+                t[(size_t)2 * b + 1] = slow ? make_uint4(0u, 0x80000000u, 0u, 0u) : make_uint4(~inb[3], 0u, 0u, 0u);
+            }
+        };
         double slow_mass = 0.0;
         for (int b = 0; b < n; ++b) {
             const uint64_t lo_u = first[(size_t)b], end_u = first[(size_t)b + 1];
-            if (end_u <= lo_u) { t[(size_t)b] = make_uint4(0u, slow_row, 0u, 0u); continue; }   // empty: never read
+            const uint32_t none[4] = {0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu};
+            if (end_u <= lo_u) { put(b, true, 0u, none); continue; }   // empty: never read
             const uint64_t hi_u = end_u - 1;
-            uint32_t nsum = 0, inb[3] = {0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu};
+            uint32_t nsum = 0, inb[4] = {0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu};
             bool slow = false;
-            for (int c = 0; c < 3; ++c) {
+            for (int c = 0; c < NC; ++c) {
                 const uint32_t *col = thr32.data() + (size_t)c * (nT + 1);
                 int nlo = z[c], cnt = 0;
                 for (int i = z[c]; i < nT; ++i) {
@@ -232,12 +250,8 @@ static bool build_bucket_table(const std::vector<uint32_t> &thr32, const int z[3
                 if (cnt > 1) slow = true;
                 nsum += (uint32_t)nlo;
             }
-            if (slow) {
-                slow_mass += (double)(hi_u - lo_u + 1) / 4294967296.0;
-                t[(size_t)b] = make_uint4(0u, slow_row, 0u, 0u);
-            } else {
-                t[(size_t)b] = make_uint4(~inb[0], nsum, ~inb[1], ~inb[2]);
-            }
+            if (slow) slow_mass += (double)(hi_u - lo_u + 1) / 4294967296.0;
+            put(b, slow, nsum, inb);
         }
         if (slow_mass < 1e-5 || MB == 6) {
             if (slow_mass > 1e-3) return false;
@@ -345,7 +359,7 @@ static int upload_tables(ea_handle *h, const std::vector<uint64_t> &acc, const s
     {
         std::vector<uint4> tab;
         std::vector<uchar4> trip;
-        h->fast_rank = build_bucket_table(thr32, z, nT, tab, trip, h->K);
+        h->fast_rank = build_bucket_table(thr32, z, nT, 3, tab, trip, h->K);
         if (!h->fast_rank) { h->K = ea::RankKey{}; h->K.c16 = 16u; }
         h->n_bucket = h->fast_rank ? (int)tab.size() : 0;
         CUDA_TRY(h, cudaMemcpyAsync(h->d_trip, trip.data(), 4 * trip.size(), cudaMemcpyHostToDevice, s));
@@ -641,6 +655,7 @@ extern "C" int ea_set_field(ea_handle *h, int field)
         if (h->field == 0) return EA_OK;
         CUDA_TRY(h, cudaStreamSynchronize(h->stream));
         h->field = 0;
+        h->fast_field = false; h->d_bucketF = nullptr; h->d_tripF = nullptr;
         h->P.h = 0; h->P.ediv = 4; h->P.thrF = nullptr; h->P.swp_val = h->d_swp_val;
         for (int c = 0; c < 18; ++c) h->P.zF[c] = -1;
         const std::vector<uint64_t> acc = h->acc, swp = h->swp;
@@ -693,19 +708,34 @@ extern "C" int ea_set_field(ea_handle *h, int field)
         }
     SwapTrim tr;
     { int rc = trim_swap_table(h, swpf.data(), nT, Mf, tr); if (rc != EA_OK) return rc; }
+    // |h| <= 2: the four columns also get a bucket table, and the resident kernel runs with the field
+    std::vector<uint4> tabF;
+    std::vector<uchar4> tripF;
+    ea::RankKey KF{};
+    bool fastF = false;
+    if (field >= -2 && field <= 2) {
+        std::vector<uint32_t> col(thrF.begin() + (size_t)14 * LTS, thrF.begin() + (size_t)18 * LTS);
+        fastF = build_bucket_table(col, zF + 14, nT, 4, tabF, tripF, KF);
+    }
     const size_t o_val = align256(4 * thrF.size());
+    const size_t o_tab = align256(o_val + 4 * (tr.val.size() + 1)), o_trip = align256(o_tab + 16 * tabF.size());
     char *d = nullptr;
-    if (cudaMalloc((void **)&d, o_val + 4 * (tr.val.size() + 1)) != cudaSuccess) {
+    if (cudaMalloc((void **)&d, o_trip + 4 * tripF.size() + 16) != cudaSuccess) {
         cudaGetLastError();
         return fail(h, EA_ERR_ALLOC, "ea_set_field: cudaMalloc failed");
     }
     cudaError_t e = cudaStreamSynchronize(h->stream);
     if (e == cudaSuccess) e = cudaMemcpyAsync(d, thrF.data(), 4 * thrF.size(), cudaMemcpyHostToDevice, h->stream);
+    if (e == cudaSuccess && fastF) e = cudaMemcpyAsync(d + o_tab, tabF.data(), 16 * tabF.size(), cudaMemcpyHostToDevice, h->stream);
+    if (e == cudaSuccess && fastF) e = cudaMemcpyAsync(d + o_trip, tripF.data(), 4 * tripF.size(), cudaMemcpyHostToDevice, h->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);       // the vectors live on this stack frame
     if (e != cudaSuccess) { cudaFree(d); return fail(h, EA_ERR_CUDA, std::string("ea_set_field: ") + cudaGetErrorString(e)); }
     { int rc = upload_swap_trim(h, tr, (uint32_t *)(d + o_val)); if (rc != EA_OK) { cudaFree(d); return rc; } }
     if (h->d_field) cudaFree(h->d_field);
     h->d_field = d;
     h->field = field;
+    h->fast_field = fastF; h->KF = KF;
+    h->d_bucketF = (uint4 *)(d + o_tab); h->d_tripF = (uchar4 *)(d + o_trip);
     h->P.h = field; h->P.ediv = 2; h->P.thrF = (const uint32_t *)d; h->P.swp_val = (const uint32_t *)(d + o_val);
     for (int c = 0; c < 18; ++c) h->P.zF[c] = zF[c];
     h->accf.swap(accf);
@@ -807,9 +837,11 @@ struct ResPlan { bool ok; int C, S, G, swap_win; size_t smem; bool any; int NQP;
 // shared memory of k_resident without the swap-threshold window (layout: ea_resident.cuh)
 size_t resident_smem(const ea_handle *h, int S)
 {
-    const size_t N = (size_t)h->N, nT = (size_t)h->nT, LTS = nT + 1, MTS = 3 * nT + 2;
-    return 16 * (size_t)h->n_bucket + 4 * (size_t)S * N + 16 * (size_t)S * MTS +
-           4 * ((size_t)S * LTS + 3 * LTS + MTS + (size_t)S * 32 + 4 * nT) +
+    const bool f = h->field != 0;                 // field: four columns, 32-byte bucket entries
+    const size_t N = (size_t)h->N, nT = (size_t)h->nT, LTS = nT + 1, NC = f ? 4 : 3, MTS = NC * nT + 2;
+    const size_t nb = f ? 2 * (size_t)h->KF.n_bucket : (size_t)h->K.n_bucket;
+    return 16 * nb + 4 * (size_t)S * N + 16 * (size_t)S * MTS +
+           4 * ((size_t)S * LTS + NC * LTS + MTS + (size_t)S * 32 + 4 * nT) +
            2 * (2 * nT * 32) + 64 * nT + 16;
 }
 
@@ -819,6 +851,7 @@ ResPlan plan_resident(const ea_handle *h)
     // run-time geometry: + the word's couplings (3 N words) and the neighbour table (3 words per site)
     const size_t extra = (h->L != 8 && h->L != 16) ? 24 * (size_t)h->N + 16 : 0;
     pl.any = h->L != 8 && h->L != 16;          // any other even L: run-time geometry (ea_small.cuh)
+    if (h->field != 0 && (pl.any || !h->fast_field)) return pl;   // field: |h| <= 2 on L = 8, 16
     if (pl.any && h->N / 2 > 1024) return pl;  // one thread per site of a parity: L <= 12
     const size_t cap = 227 * 1024;
     int C = 0;
@@ -850,7 +883,7 @@ ResPlan plan_resident(const ea_handle *h)
 template <int L, int G>
 cudaError_t launch_resident_t(const ea_handle *h, const ea::ResArgs &A, const ResPlan &pl, bool fast)
 {
-    auto kern = fast ? ea::k_resident<L, G, true> : ea::k_resident<L, G, false>;
+    auto kern = h->field != 0 ? ea::k_resident<L, G, true, 4> : fast ? ea::k_resident<L, G, true> : ea::k_resident<L, G, false>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem);
     if (e != cudaSuccess) return e;
     cudaLaunchConfig_t cfg{};
@@ -903,6 +936,7 @@ static int sweep_resident(ea_handle *h, int64_t n_sweeps, int swap_interval)
         A.nswap0 = (uint32_t)h->nswap;
         A.C = pl.C; A.S = pl.S;
         A.bucket = h->d_bucket; A.K = h->K; A.trip = h->d_trip;
+        if (h->field != 0) { A.bucket = h->d_bucketF; A.K = h->KF; A.trip = h->d_tripF; }
         A.swap_win = pl.swap_win;
         for (int r = 0; r < 10; ++r) {
             A.rk[2 * r] = h->P.k0 + (uint32_t)r * 0x9E3779B9u;
@@ -1229,7 +1263,9 @@ static int pick_kernel(const ea_handle *h)
 {
     if (h->layout == EA_LAYOUT_REPLICA_BITS) return EA_KERNEL_REPLICA;
     if (h->kernel_sel == EA_KERNEL_GENERIC_STEPWISE) return EA_KERNEL_GENERIC_STEPWISE;
-    if (h->field != 0) return EA_KERNEL_GENERIC;     // the fast kernels are zero-field only
+    if (h->field != 0)       // with a field: the resident kernel for |h| <= 2 on L = 8, 16, else the generic path
+        return (h->kernel_sel == EA_KERNEL_AUTO || h->kernel_sel == EA_KERNEL_RESIDENT) && plan_resident(h).ok
+                   ? EA_KERNEL_RESIDENT : EA_KERNEL_GENERIC;
     if (h->kernel_sel != EA_KERNEL_AUTO) return h->kernel_sel;
     if (plan_resident(h).ok) return EA_KERNEL_RESIDENT;
     if (plan_stream(h).ok) return EA_KERNEL_STREAM;
@@ -1243,7 +1279,8 @@ extern "C" int ea_set_kernel(ea_handle *h, int kernel)
     if (h->layout == EA_LAYOUT_REPLICA_BITS)
         return kernel == EA_KERNEL_AUTO ? EA_OK : fail(h, EA_ERR_UNSUPPORTED, "ea_set_kernel: the replica-bits layout has one kernel");
     if (kernel == EA_KERNEL_AUTO || kernel == EA_KERNEL_GENERIC || kernel == EA_KERNEL_GENERIC_STEPWISE) { h->kernel_sel = kernel; return EA_OK; }
-    if (h->field != 0) return fail(h, EA_ERR_UNSUPPORTED, "ea_set_kernel: only the generic kernel runs with a field");
+    if (h->field != 0 && !(kernel == EA_KERNEL_RESIDENT && plan_resident(h).ok))
+        return fail(h, EA_ERR_UNSUPPORTED, "ea_set_kernel: with a field only the generic kernel and, for |h| <= 2 on L = 8, 16, the resident one");
     if (kernel == EA_KERNEL_RESIDENT && plan_resident(h).ok) { h->kernel_sel = kernel; return EA_OK; }
     if (kernel == EA_KERNEL_TILED && plan_tiled(h).ok) { h->kernel_sel = kernel; return EA_OK; }
     if (kernel == EA_KERNEL_STREAM && plan_stream(h).ok) { h->kernel_sel = kernel; return EA_OK; }

@@ -53,6 +53,15 @@ __device__ __forceinline__ void build_mt(uint4 *mt, const uint32_t *lt, const uc
     }
     if (lane == 0) mt[3 * nT + 1] = make_uint4(0u, 0u, 0u, 0x80000000u);
 }
+// Field |h| <= 2 (four threshold columns): row n = the four rank masks of the
+// quadruple whose sum is n; the "use the exact search" flag travels in the bucket entry instead.
+__device__ __forceinline__ void build_mt4(uint4 *mt, const uint32_t *lt, const uchar4 *trip, int nT, int lane)
+{
+    for (int n = lane; n <= 4 * nT; n += 32) {
+        const uchar4 t = trip[n];
+        mt[n] = make_uint4(lt[t.x], lt[t.y], lt[t.z], lt[t.w]);
+    }
+}
 
 constexpr int kResPlanes = 10;   // planes of a warp's per-slot satisfied-bond count (<= 768)
 
@@ -197,12 +206,15 @@ struct RankCtx {
     int z0, z1, z2;
     float kscale, kadd;
     uint32_t kmul, c16;
+    int h, z3;               // field variant (four columns): field of Eq. 1, zero count of the fourth column
+    uint32_t c32;            // 32: its bucket entries are two 16-byte words
 };
 
 __device__ __forceinline__ void rank_ctx_key(RankCtx &R, const RankKey &K, const uint4 *bucket)
 {
     R.bucket0 = reinterpret_cast<const char *>(bucket) - 16 * (ptrdiff_t)K.key_lo;
     R.kscale = K.kscale; R.kadd = K.kadd; R.kmul = K.kmul; R.c16 = K.c16;
+    R.h = 0; R.z3 = 0; R.c32 = 2u * K.c16;
 }
 
 // n + (u + a overflows) + (u + b overflows) + (u + c overflows): three carries (IADD3 with a
@@ -247,6 +259,48 @@ __device__ __forceinline__ uint32_t accept_exact(const RankCtx &R, const uint32_
     return accept_mask(p, m4, m5, m6);
 }
 
+// ---- field |h| <= 2: four threshold columns (shifted class index, accept_mask_field), bucket
+// entries of 32 bytes { ~thr_a, n at the lower edge, ~thr_b, ~thr_c | ~thr_d, slow flag, -, - }
+__device__ __forceinline__ uint32_t accept_fast4(const RankCtx &R, const uint4 *mt, uint32_t u, const Planes &p,
+                                                 uint32_t s, uint32_t *flag)
+{
+    float g;
+    asm("fma.rn.sat.f32 %0, %1, %2, %3;" : "=f"(g) : "f"(__uint2float_rz(u)), "f"(R.kscale), "f"(R.kadd));
+    const uint32_t key = __umulhi(__float_as_uint(g), R.kmul);
+    const char *ep = R.bucket0 + mad_lo(key, R.c32, 0u);
+    const uint4 e = *reinterpret_cast<const uint4 *>(ep);
+    const uint2 f = *reinterpret_cast<const uint2 *>(ep + 16);
+    uint32_t n = add3_carries(u, e.y, e.x, e.z, e.w);
+    n = add3_carries(u, n, f.x, 0u, 0u);
+    const uint4 row = *reinterpret_cast<const uint4 *>(reinterpret_cast<const char *>(mt) + mad_lo(n, R.c16, 0u));
+    *flag |= f.y;
+    return accept_mask_field(p, s, R.h, row.x, row.y, row.z, row.w);
+}
+__device__ __forceinline__ uint32_t accept_exact4(const RankCtx &R, const uint32_t *lt, uint32_t u, const Planes &p,
+                                                  uint32_t s)
+{
+    const uint32_t m0 = lt[rank_of(u, R.thr, R.z0, R.nT)];
+    const uint32_t m1 = lt[rank_of(u, R.thr + R.LTS, R.z1, R.nT)];
+    const uint32_t m2 = lt[rank_of(u, R.thr + 2 * R.LTS, R.z2, R.nT)];
+    const uint32_t m3 = lt[rank_of(u, R.thr + 3 * R.LTS, R.z3, R.nT)];
+    return accept_mask_field(p, s, R.h, m0, m1, m2, m3);
+}
+
+// Number of set bits over eight words, per bit lane, as four planes (<= 8).
+__device__ __forceinline__ void count8(const uint32_t (&x)[8], uint32_t (&o)[4])
+{
+    const uint32_t s1 = xor3(x[0], x[1], x[2]), c1 = maj3(x[0], x[1], x[2]);
+    const uint32_t s2 = xor3(x[3], x[4], x[5]), c2 = maj3(x[3], x[4], x[5]);
+    const uint32_t s3 = x[6] ^ x[7], c3 = x[6] & x[7];
+    o[0] = xor3(s1, s2, s3);
+    const uint32_t c4 = maj3(s1, s2, s3);
+    const uint32_t s5 = xor3(c1, c2, c3), c5 = maj3(c1, c2, c3);
+    o[1] = s5 ^ c4;
+    const uint32_t c6 = s5 & c4;
+    o[2] = c5 ^ c6;
+    o[3] = c5 & c6;
+}
+
 }  // namespace ea
 
 namespace ea {
@@ -267,7 +321,7 @@ struct ResGeom {
 // New spin words of the four sites of quad q (parity p) of one slot's lattice `sp` (smem,
 // [2][Nh]); nothing is stored.  EXACT = false: ranks from the bucket table; *flag collects
 // bit 31 of the entries (set: the caller must redo the quad with EXACT = true).
-template <int L, bool EXACT, bool ENERGY, bool UNIS>
+template <int L, bool EXACT, bool ENERGY, bool UNIS, int NC = 3>
 __device__ __forceinline__ uint4 quad_core(const char *self_q, const char *oth_b, uint32_t ov, uint32_t oyp,
                                            uint32_t oym, uint32_t ozp, uint32_t ozm, int qx,
                                            const uint32_t *lt, const uint4 *mt, const RankCtx &R,
@@ -332,7 +386,8 @@ __device__ __forceinline__ uint4 quad_core(const char *self_q, const char *oth_b
                                       xor3(m[l], jys[l], a_yp[l]), xor3(m[l], jym[l], a_ym[l]),
                                       xor3(m[l], jzs[l], a_zp[l]), xor3(m[l], jzm[l], a_zm[l]));
         uint32_t acc;
-        if (EXACT) acc = accept_exact(R, lt, u[l], pl);
+        if (NC == 4) acc = EXACT ? accept_exact4(R, lt, u[l], pl, m[l]) : accept_fast4(R, mt, u[l], pl, m[l], &fl);
+        else if (EXACT) acc = accept_exact(R, lt, u[l], pl);
         else acc = accept_fast(R, mt, u[l], pl, &fl);
         out[l] = m[l] ^ acc;
         if (ENERGY) fin[l] = planes_after(pl, acc);
@@ -345,22 +400,22 @@ __device__ __forceinline__ uint4 quad_core(const char *self_q, const char *oth_b
 // quad in 10^7, and keeping it out of the hot loops saves their code size and registers.
 struct QuadOut { uint4 res; Planes fin[4]; };
 
-template <int L, bool ENERGY>
+template <int L, bool ENERGY, int NC = 3>
 __device__ __noinline__ QuadOut quad_exact(const char *self_q, const char *oth_b, uint32_t ov, uint32_t oyp,
                                            uint32_t oym, uint32_t ozp, uint32_t ozm, int qx, const uint32_t *lt,
                                            const RankCtx R, const QuadJ J, int s, const uint4 rnd)
 {
     QuadOut o;
     uint32_t flag;
-    o.res = quad_core<L, true, ENERGY, false>(self_q, oth_b, ov, oyp, oym, ozp, ozm, qx, lt, nullptr, R, J, s, rnd,
-                                              o.fin, &flag);
+    o.res = quad_core<L, true, ENERGY, false, NC>(self_q, oth_b, ov, oyp, oym, ozp, ozm, qx, lt, nullptr, R, J, s, rnd,
+                                                  o.fin, &flag);
     return o;
 }
 
 // New words of a quad (nothing is stored): fast rank path first; rare (or !FAST): the whole
 // quad again from memory with the exact search (OOL: through the out-of-line function; measured
 // +5 % for the resident kernel, -12 % for the streaming kernel, which then spills more).
-template <int L, bool FAST, bool ENERGY, bool UNIS, bool OOL>
+template <int L, bool FAST, bool ENERGY, bool UNIS, bool OOL, int NC = 3>
 __device__ __forceinline__ uint4 update_quad_mem(const char *self_q, const char *oth_b, uint32_t ov,
                                                  uint32_t oyp, uint32_t oym, uint32_t ozp, uint32_t ozm, int qx,
                                                  const uint32_t *lt, const uint4 *mt, const RankCtx &R,
@@ -368,11 +423,11 @@ __device__ __forceinline__ uint4 update_quad_mem(const char *self_q, const char 
 {
     uint32_t flag = 0x80000000u;
     uint4 res;
-    if (FAST) res = quad_core<L, false, ENERGY, UNIS>(self_q, oth_b, ov, oyp, oym, ozp, ozm, qx, lt, mt, R, J, s, rnd, fin, &flag);
+    if (FAST) res = quad_core<L, false, ENERGY, UNIS, NC>(self_q, oth_b, ov, oyp, oym, ozp, ozm, qx, lt, mt, R, J, s, rnd, fin, &flag);
     if (!OOL) {
-        if ((int)flag < 0) res = quad_core<L, true, ENERGY, UNIS>(self_q, oth_b, ov, oyp, oym, ozp, ozm, qx, lt, mt, R, J, s, rnd, fin, &flag);
+        if ((int)flag < 0) res = quad_core<L, true, ENERGY, UNIS, NC>(self_q, oth_b, ov, oyp, oym, ozp, ozm, qx, lt, mt, R, J, s, rnd, fin, &flag);
     } else if ((int)flag < 0) {
-        const QuadOut o = quad_exact<L, ENERGY>(self_q, oth_b, ov, oyp, oym, ozp, ozm, qx, lt, R, J, s, rnd);
+        const QuadOut o = quad_exact<L, ENERGY, NC>(self_q, oth_b, ov, oyp, oym, ozp, ozm, qx, lt, R, J, s, rnd);
         res = o.res;
         if (ENERGY) {
 #pragma unroll
@@ -383,7 +438,7 @@ __device__ __forceinline__ uint4 update_quad_mem(const char *self_q, const char 
 }
 
 // lattice `sp` = [2][Nh] words (resident and tiled kernels): update quad q of parity p in place
-template <int L, bool FAST, bool ENERGY, bool UNIS>
+template <int L, bool FAST, bool ENERGY, bool UNIS, int NC = 3>
 __device__ __forceinline__ void update_quad_off(uint32_t *sp, const uint32_t *lt, const uint4 *mt, const RankCtx &R,
                                                 const QuadJ &J, int p, int s, int q, uint32_t oyp,
                                                 uint32_t oym, uint32_t ozp, uint32_t ozm, const uint4 rnd,
@@ -392,8 +447,8 @@ __device__ __forceinline__ void update_quad_off(uint32_t *sp, const uint32_t *lt
     using Gm = ResGeom<L>;
     char *self_q = reinterpret_cast<char *>(sp + p * Gm::Nh) + 16 * q;
     const char *oth_b = reinterpret_cast<const char *>(sp + (1 - p) * Gm::Nh);
-    const uint4 res = update_quad_mem<L, FAST, ENERGY, UNIS, true>(self_q, oth_b, 16u * q, oyp, oym, ozp, ozm,
-                                                             q & (Gm::QR - 1), lt, mt, R, J, s, rnd, fin);
+    const uint4 res = update_quad_mem<L, FAST, ENERGY, UNIS, true, NC>(self_q, oth_b, 16u * q, oyp, oym, ozp, ozm,
+                                                                 q & (Gm::QR - 1), lt, mt, R, J, s, rnd, fin);
     *reinterpret_cast<uint4 *>(self_q) = res;
 }
 
@@ -564,7 +619,70 @@ __device__ __forceinline__ void add_counts(const uint32_t (&tot)[kResPlanes], in
     atomicAdd(acc_row + i + 24, (int)(hi >> 16));
 }
 
-template <int L, int G, bool FAST>
+// warp_sum4 for NP-plane counts: four slots in flight, two halving levels, three
+// plain ones; every lane of the 8-lane group 2 (lane>>4) + ((lane>>3)&1) ends with that slot's sum.
+template <int NP>
+__device__ __forceinline__ void warp_sum4_t(uint32_t (&en)[4][NP], int lane, uint32_t (&out)[NP + 5])
+{
+    const uint32_t hi16 = (lane & 16) ? 0xFFFFFFFFu : 0u, hi8 = (lane & 8) ? 0xFFFFFFFFu : 0u;
+    uint32_t a[2][NP + 1];
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+        uint32_t keep[NP], got[NP];
+#pragma unroll
+        for (int i = 0; i < NP; ++i) {
+            keep[i] = mux(en[h][i], en[2 + h][i], hi16);
+            got[i] = __shfl_xor_sync(0xFFFFFFFFu, mux(en[2 + h][i], en[h][i], hi16), 16);
+        }
+        vsum<NP>(keep, got, a[h]);
+    }
+    uint32_t b[NP + 2], c[NP + 3], d[NP + 4];
+    {
+        uint32_t keep[NP + 1], got[NP + 1];
+#pragma unroll
+        for (int i = 0; i < NP + 1; ++i) {
+            keep[i] = mux(a[0][i], a[1][i], hi8);
+            got[i] = __shfl_xor_sync(0xFFFFFFFFu, mux(a[1][i], a[0][i], hi8), 8);
+        }
+        vsum<NP + 1>(keep, got, b);
+    }
+    {
+        uint32_t got[NP + 2];
+#pragma unroll
+        for (int i = 0; i < NP + 2; ++i) got[i] = __shfl_xor_sync(0xFFFFFFFFu, b[i], 4);
+        vsum<NP + 2>(b, got, c);
+    }
+    {
+        uint32_t got[NP + 3];
+#pragma unroll
+        for (int i = 0; i < NP + 3; ++i) got[i] = __shfl_xor_sync(0xFFFFFFFFu, c[i], 2);
+        vsum<NP + 3>(c, got, d);
+    }
+    {
+        uint32_t got[NP + 4];
+#pragma unroll
+        for (int i = 0; i < NP + 4; ++i) got[i] = __shfl_xor_sync(0xFFFFFFFFu, d[i], 1);
+        vsum<NP + 4>(d, got, out);
+    }
+}
+
+// add_counts for NPL planes
+template <int NPL>
+__device__ __forceinline__ void add_counts_t(const uint32_t (&tot)[NPL], int i, int *acc_row)
+{
+    uint32_t lo = 0, hi = 0;
+#pragma unroll
+    for (int j = 0; j < NPL; ++j) {
+        lo += ((tot[j] >> i) & 0x00010001u) * (1u << j);
+        hi += ((tot[j] >> (i + 8)) & 0x00010001u) * (1u << j);
+    }
+    atomicAdd(acc_row + i, (int)(lo & 0xFFFFu));
+    atomicAdd(acc_row + i + 16, (int)(lo >> 16));
+    atomicAdd(acc_row + i + 8, (int)(hi & 0xFFFFu));
+    atomicAdd(acc_row + i + 24, (int)(hi >> 16));
+}
+
+template <int L, int G, bool FAST, int NC = 3>
 __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs A)
 {
     using Gm = ResGeom<L>;
@@ -588,13 +706,14 @@ __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs
     const int q = qx + QR * (y + L * z);
 
     // shared memory: the rank table first (fixed offset 0), lattices next (16 B aligned)
-    const int MTS = 3 * nT + 2, SW = A.swap_win;
-    uint4 *bucket = reinterpret_cast<uint4 *>(smem);                 // [n_bucket] 16 B entries
-    uint32_t *sp = smem + 4 * (size_t)A.K.n_bucket;                    // [S][2][Nh]
+    const int MTS = NC * nT + 2, SW = A.swap_win;
+    constexpr int BW = NC == 4 ? 2 : 1;                              // 16-byte words per bucket entry
+    uint4 *bucket = reinterpret_cast<uint4 *>(smem);                 // [n_bucket] 16 B (field: 32 B) entries
+    uint32_t *sp = smem + 4 * (size_t)BW * A.K.n_bucket;             // [S][2][Nh]
     uint4 *mt = reinterpret_cast<uint4 *>(sp + (size_t)S * N);       // [S][MTS] mask tables
     uint32_t *lt = reinterpret_cast<uint32_t *>(mt + (size_t)S * MTS);   // [S][LTS]
-    uint32_t *thr = lt + S * LTS;                                    // [3][LTS]
-    uchar4 *trip = reinterpret_cast<uchar4 *>(thr + 3 * LTS);        // [MTS]
+    uint32_t *thr = lt + S * LTS;                                    // [NC][LTS]
+    uchar4 *trip = reinterpret_cast<uchar4 *>(thr + NC * LTS);       // [MTS]
     int32_t *Eacc = (int32_t *)(trip + MTS);                         // [S][32] satisfied-bond counts
     int32_t *swm = Eacc + S * 32;                                    // [nT][4]: lo, cnt, off, kinds
     uint32_t *swwin = (uint32_t *)(swm + 4 * nT);                    // [nT][SW] thresholds - 1
@@ -624,8 +743,8 @@ __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs
     }
     for (int k = 0; k < nk; ++k)
         for (int a = tid; a < LTS; a += NT) lt[k * LTS + a] = P.lt[((size_t)w * nT + k0 + k) * LTS + a];
-    for (int a = tid; a < 3 * LTS; a += NT) thr[a] = P.thr32[a];
-    for (int a = tid; a < A.K.n_bucket; a += NT) bucket[a] = A.bucket[a];
+    for (int a = tid; a < NC * LTS; a += NT) thr[a] = NC == 4 ? P.thrF[14 * LTS + a] : P.thr32[a];
+    for (int a = tid; a < BW * A.K.n_bucket; a += NT) bucket[a] = A.bucket[a];
     for (int a = tid; a < 32 * nT; a += NT) {
         tau8[a] = P.tau[(size_t)32 * w * nT + a];
         sig8[a] = P.sigma[(size_t)32 * w * nT + a];
@@ -664,11 +783,15 @@ __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs
     R.thr = thr; R.LTS = LTS; R.nT = nT;
     R.z0 = P.z[0]; R.z1 = P.z[1]; R.z2 = P.z[2];
     rank_ctx_key(R, A.K, bucket);
+    if (NC == 4) {
+        R.z0 = P.zF[14]; R.z1 = P.zF[15]; R.z2 = P.zF[16]; R.z3 = P.zF[17]; R.h = P.h;
+        R.bucket0 = reinterpret_cast<const char *>(bucket) - 32 * (ptrdiff_t)A.K.key_lo;
+    }
     const uint32_t gw = P.w0 + (uint32_t)w;
     const PhiloxQuad PQ = philox_quad_init((uint32_t)q, gw, A.rk);
     cg::cluster_group cl = cg::this_cluster();
     __syncthreads();
-    for (int kl = tid >> 5; kl < nk; kl += NT >> 5) build_mt(mt + (size_t)kl * MTS, lt + kl * LTS, trip, nT, lane);
+    for (int kl = tid >> 5; kl < nk; kl += NT >> 5) (NC == 4 ? build_mt4 : build_mt)(mt + (size_t)kl * MTS, lt + kl * LTS, trip, nT, lane);
     if (C > 1) cl.sync(); else __syncthreads();   // every block's shared memory is initialised
 
     uint32_t nswap = A.nswap0;
@@ -680,46 +803,65 @@ __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs
         // ---------------- parity 0
         for (int kl = sg; kl < nk; kl += G) {
             const uint4 rnd = philox_quad(PQ, g, (uint32_t)(k0 + kl), A.rk);
-            update_quad_off<L, FAST, false, true>(sp + (size_t)kl * N, lt + kl * LTS, mt + (size_t)kl * MTS, R, J0, 0, s0, q, oyp, oym, ozp, ozm, rnd, fin);
+            update_quad_off<L, FAST, false, true, NC>(sp + (size_t)kl * N, lt + kl * LTS, mt + (size_t)kl * MTS, R, J0, 0, s0, q, oyp, oym, ozp, ozm, rnd, fin);
         }
         __syncthreads();
         // ---------------- parity 1 (+ satisfied-bond count of the finished sweep)
         if (!need_E) {
             for (int kl = sg; kl < nk; kl += G) {
                 const uint4 rnd = philox_quad(PQ, g, (1u << 16) | (uint32_t)(k0 + kl), A.rk);
-                update_quad_off<L, FAST, false, true>(sp + (size_t)kl * N, lt + kl * LTS, mt + (size_t)kl * MTS, R, J1, 1, 1 - s0, q,
+                update_quad_off<L, FAST, false, true, NC>(sp + (size_t)kl * N, lt + kl * LTS, mt + (size_t)kl * MTS, R, J1, 1, 1 - s0, q,
                                                       oyp, oym, ozp, ozm, rnd, fin);
             }
             __syncthreads();
             continue;
         }
         for (int kb = sg; kb < S; kb += 4 * G) {     // batches of four slots: kb, kb+G, kb+2G, kb+3G
-            uint32_t en[4][5];
+            constexpr int NPE = NC == 4 ? 6 : 5;
+            uint32_t en[4][NPE];
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
                 const int kl = kb + i * G;
                 if (kl < nk) {
                     const uint4 rnd = philox_quad(PQ, g, (1u << 16) | (uint32_t)(k0 + kl), A.rk);
-                    update_quad_off<L, FAST, true, true>(sp + (size_t)kl * N, lt + kl * LTS, mt + (size_t)kl * MTS, R, J1, 1, 1 - s0, q,
+                    update_quad_off<L, FAST, true, true, NC>(sp + (size_t)kl * N, lt + kl * LTS, mt + (size_t)kl * MTS, R, J1, 1, 1 - s0, q,
                                                          oyp, oym, ozp, ozm, rnd, fin);
-                    quad_sum(fin, en[i]);
+                    if constexpr (NC == 4) {
+                        // field: T = (satisfied bonds) + |h| (sites whose spin pays the field energy), over my
+                        // four parity-1 sites and the four parity-0 sites of the index-aligned quad, which
+                        // every thread of the lattice meets exactly once: E = (3 + |h|) N - 2 T
+                        uint32_t e5[5], x4[4], y5[5];
+                        quad_sum(fin, e5);
+                        const uint4 me4 = *reinterpret_cast<const uint4 *>(sp + (size_t)kl * N + Gm::Nh + 4 * q);
+                        const uint4 v4 = *reinterpret_cast<const uint4 *>(sp + (size_t)kl * N + 4 * q);
+                        const uint32_t inv = P.h > 0 ? 0xFFFFFFFFu : 0u;      // h > 0: down spins pay
+                        const uint32_t xs[8] = {me4.x ^ inv, me4.y ^ inv, me4.z ^ inv, me4.w ^ inv,
+                                                v4.x ^ inv, v4.y ^ inv, v4.z ^ inv, v4.w ^ inv};
+                        count8(xs, x4);
+                        const bool two = (P.h & 1) == 0;
+                        y5[0] = two ? 0u : x4[0]; y5[1] = two ? x4[0] : x4[1]; y5[2] = two ? x4[1] : x4[2];
+                        y5[3] = two ? x4[2] : x4[3]; y5[4] = two ? x4[3] : 0u;
+                        vsum<5>(e5, y5, en[i]);
+                    } else {
+                        quad_sum(fin, en[i]);
+                    }
                 } else {
 #pragma unroll
-                    for (int j = 0; j < 5; ++j) en[i][j] = 0;
+                    for (int j = 0; j < NPE; ++j) en[i][j] = 0;
                 }
             }
-            uint32_t tot[kResPlanes];
-            warp_sum4(en, lane, tot);
+            uint32_t tot[NPE + 5];
+            warp_sum4_t<NPE>(en, lane, tot);
             const int i_mine = 2 * (lane >> 4) + ((lane >> 3) & 1);
             const int kl = kb + i_mine * G;
-            if (kl < nk) add_counts(tot, lane & 7, Eacc + kl * 32);
+            if (kl < nk) add_counts_t<NPE + 5>(tot, lane & 7, Eacc + kl * 32);
         }
         __syncthreads();
         // ---- energies of my slots: E = 3N - 2 (satisfied bonds); pushed into every block of
         //      the cluster (distributed shared memory), buffer chosen by the swap-round parity
         int16_t *Ebuf = Eall + (nswap & 1u) * nT * 32;
         for (int a = tid; a < nk * 32; a += NT) {
-            const int e = 3 * N - 2 * Eacc[a];
+            const int e = (3 + (NC == 4 ? abs(P.h) : 0)) * N - 2 * Eacc[a];
             Eacc[a] = 0;
             const int dst = k0 * 32 + a;
             if (C > 1) {
@@ -736,7 +878,7 @@ __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs
         for (int t = (int)(nswap & 1u) + 2 * warp; t + 1 < nT; t += 2 * nwarp) {
             uint8_t *sg_ = sig8 + lane * nT, *ta_ = tau8 + lane * nT;
             const int sa = sg_[t], sb = sg_[t + 1];
-            const int m = ((int)Ebuf[sa * 32 + lane] - (int)Ebuf[sb * 32 + lane]) / 4;
+            const int m = ((int)Ebuf[sa * 32 + lane] - (int)Ebuf[sb * 32 + lane]) / (NC == 4 ? 2 : 4);
             const uint4 v = philox_rk(g, (uint32_t)t, P.r0 + (uint32_t)(32 * w + lane), 2u << 16, A.rk);
             const int lo = swm[4 * t], cnt = swm[4 * t + 1], kinds = swm[4 * t + 3];
             bool acc;
@@ -760,7 +902,7 @@ __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs
                 if (lane == (n & 31)) lt[kl * LTS + n] = mk;
             }
             __syncwarp();
-            build_mt(mt + (size_t)kl * MTS, lt + kl * LTS, trip, nT, lane);
+            (NC == 4 ? build_mt4 : build_mt)(mt + (size_t)kl * MTS, lt + kl * LTS, trip, nT, lane);
         }
         __syncthreads();
     }

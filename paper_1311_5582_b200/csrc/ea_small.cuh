@@ -54,69 +54,6 @@ __device__ __forceinline__ void update_site_any(uint32_t *sp, const uint32_t *js
     if (ENERGY) fin = planes_after(pl, acc);
 }
 
-// warp_sum4 (ea_resident.cuh) for NP-plane counts: four slots in flight, two halving levels, three
-// plain ones; every lane of the 8-lane group 2 (lane>>4) + ((lane>>3)&1) ends with that slot's sum.
-template <int NP>
-__device__ __forceinline__ void warp_sum4_t(uint32_t (&en)[4][NP], int lane, uint32_t (&out)[NP + 5])
-{
-    const uint32_t hi16 = (lane & 16) ? 0xFFFFFFFFu : 0u, hi8 = (lane & 8) ? 0xFFFFFFFFu : 0u;
-    uint32_t a[2][NP + 1];
-#pragma unroll
-    for (int h = 0; h < 2; ++h) {
-        uint32_t keep[NP], got[NP];
-#pragma unroll
-        for (int i = 0; i < NP; ++i) {
-            keep[i] = mux(en[h][i], en[2 + h][i], hi16);
-            got[i] = __shfl_xor_sync(0xFFFFFFFFu, mux(en[2 + h][i], en[h][i], hi16), 16);
-        }
-        vsum<NP>(keep, got, a[h]);
-    }
-    uint32_t b[NP + 2], c[NP + 3], d[NP + 4];
-    {
-        uint32_t keep[NP + 1], got[NP + 1];
-#pragma unroll
-        for (int i = 0; i < NP + 1; ++i) {
-            keep[i] = mux(a[0][i], a[1][i], hi8);
-            got[i] = __shfl_xor_sync(0xFFFFFFFFu, mux(a[1][i], a[0][i], hi8), 8);
-        }
-        vsum<NP + 1>(keep, got, b);
-    }
-    {
-        uint32_t got[NP + 2];
-#pragma unroll
-        for (int i = 0; i < NP + 2; ++i) got[i] = __shfl_xor_sync(0xFFFFFFFFu, b[i], 4);
-        vsum<NP + 2>(b, got, c);
-    }
-    {
-        uint32_t got[NP + 3];
-#pragma unroll
-        for (int i = 0; i < NP + 3; ++i) got[i] = __shfl_xor_sync(0xFFFFFFFFu, c[i], 2);
-        vsum<NP + 3>(c, got, d);
-    }
-    {
-        uint32_t got[NP + 4];
-#pragma unroll
-        for (int i = 0; i < NP + 4; ++i) got[i] = __shfl_xor_sync(0xFFFFFFFFu, d[i], 1);
-        vsum<NP + 4>(d, got, out);
-    }
-}
-
-// add_counts (ea_resident.cuh) for NPL planes
-template <int NPL>
-__device__ __forceinline__ void add_counts_t(const uint32_t (&tot)[NPL], int i, int *acc_row)
-{
-    uint32_t lo = 0, hi = 0;
-#pragma unroll
-    for (int j = 0; j < NPL; ++j) {
-        lo += ((tot[j] >> i) & 0x00010001u) * (1u << j);
-        hi += ((tot[j] >> (i + 8)) & 0x00010001u) * (1u << j);
-    }
-    atomicAdd(acc_row + i, (int)(lo & 0xFFFFu));
-    atomicAdd(acc_row + i + 16, (int)(lo >> 16));
-    atomicAdd(acc_row + i + 8, (int)(hi & 0xFFFFu));
-    atomicAdd(acc_row + i + 24, (int)(hi >> 16));
-}
-
 template <bool FAST>
 __global__ void __launch_bounds__(1024, 1) k_resident_any(const ResArgs A)
 {

@@ -43,7 +43,9 @@ def test_field_trajectory_matches_oracle(L, nT, R, h, swap, asc):
     o = Oracle(L, nT, R, betas, 19)
     g.set_field(h)
     o.set_field(h)
-    assert g.get_field() == h and g.get_kernel() == pkg.binding.EA_KERNEL_GENERIC
+    fast = abs(h) <= 2 and L in (8, 16)          # |h| <= 2 on the resident kernel's lattices, else the generic path
+    assert g.get_field() == h
+    assert g.get_kernel() == (pkg.binding.EA_KERNEL_RESIDENT if fast else pkg.binding.EA_KERNEL_GENERIC)
     ga, gs = g.get_field_tables()
     oa, os_ = o.field_tables()
     assert (ga == oa).all() and (gs == os_).all()          # both sides hold identical tables
@@ -66,6 +68,33 @@ def test_field_trajectory_matches_oracle(L, nT, R, h, swap, asc):
     g.destroy()
 
 
+@pytest.mark.parametrize("L,nT,R,h,swap,ns", [
+    (16, 24, 64, 1, 1, 6), (16, 24, 64, -1, 1, 6), (16, 7, 40, 2, 1, 5), (16, 12, 96, -2, 2, 7),
+    (8, 16, 32, 1, 1, 12), (8, 16, 40, -2, 1, 12), (8, 5, 64, 2, 3, 9), (8, 2, 32, -1, 1, 8),
+    (16, 24, 33, 1, 0, 4),
+])
+def test_field_on_the_resident_kernel_matches_oracle_and_the_generic_kernel(L, nT, R, h, swap, ns):
+    """Field |h| <= 2 in the shared-memory-resident kernel (four threshold columns of the shifted
+    class index, up/down-spin count fused into the energy pass): bit for bit against the oracle,
+    across several calls, and with the kernel switched in mid-run."""
+    pkg, Oracle = _mods()
+    betas = 1.0 / temperature_ladder(nT, 0.7, 2.2)
+    g = pkg.EA(L, nT, R, betas, 23)
+    o = Oracle(L, nT, R, betas, 23)
+    g.set_field(h); o.set_field(h)
+    assert g.get_kernel() == pkg.binding.EA_KERNEL_RESIDENT
+    for n in (1, ns, 2):
+        g.sweep(n, swap); o.sweep(n, swap)
+        _same_state(g, o, L, R)
+    g.set_kernel(pkg.binding.EA_KERNEL_GENERIC)
+    g.sweep(3, swap); o.sweep(3, swap)
+    _same_state(g, o, L, R)
+    g.set_kernel(pkg.binding.EA_KERNEL_RESIDENT)
+    g.sweep(3, swap); o.sweep(3, swap)
+    _same_state(g, o, L, R)
+    g.destroy()
+
+
 def test_field_restrictions_and_errors():
     pkg, _ = _mods()
     betas = 1.0 / temperature_ladder(4, 0.8, 2.0)
@@ -76,9 +105,18 @@ def test_field_restrictions_and_errors():
         g.get_field_tables()                                 # no field set
     with pytest.raises(pkg.EAError):
         g.set_field(65)
-    g.set_field(2)
+    g.set_field(3)                                           # |h| > 2: generic kernels only
+    assert g.get_kernel() == pkg.binding.EA_KERNEL_GENERIC
     with pytest.raises(pkg.EAError) as e:
         g.set_kernel(pkg.binding.EA_KERNEL_RESIDENT)
+    assert e.value.code == -5
+    g.set_field(2)                                           # |h| <= 2: the resident kernel runs
+    assert g.get_kernel() == pkg.binding.EA_KERNEL_RESIDENT
+    g.set_kernel(pkg.binding.EA_KERNEL_GENERIC)
+    assert g.get_kernel() == pkg.binding.EA_KERNEL_GENERIC
+    g.set_kernel(pkg.binding.EA_KERNEL_AUTO)
+    with pytest.raises(pkg.EAError) as e:
+        g.set_kernel(pkg.binding.EA_KERNEL_TILED)
     assert e.value.code == -5
     acc, swp = g.get_tables()                                # still the zero-field tables
     with pytest.raises(pkg.EAError) as e:
