@@ -259,10 +259,10 @@ __device__ __forceinline__ void stream_consume(const StreamArgs &A, const Stream
                 stream_release<L>(A, C, p, li, efill);
             }
         } else {
-            for (int i0 = 0; i0 < cnt; i0 += 2) {      // pairs of slots: few live registers
-                uint32_t en[2][5];
+            for (int i0 = 0; i0 < cnt; i0 += 4) {      // the batch's (up to four) slots share one butterfly
+                uint32_t en[4][5];
 #pragma unroll
-                for (int h = 0; h < 2; ++h) {
+                for (int h = 0; h < 4; ++h) {
                     const int i = i0 + h;
                     if (i < cnt) {
                         const int li = pos + i - C.i0, st = li % NST;
@@ -282,9 +282,9 @@ __device__ __forceinline__ void stream_consume(const StreamArgs &A, const Stream
                     }
                 }
                 uint32_t tot[kResPlanes];
-                warp_sum2(en, C.lane, tot);
-                const int i_mine = i0 + (C.lane >> 4);
-                if (i_mine < cnt && !(C.lane & 8)) add_counts(tot, C.lane & 7, C.Eacc + (pos + i_mine - C.i0) * 32);
+                warp_sum4(en, C.lane, tot);
+                const int i_mine = i0 + 2 * (C.lane >> 4) + ((C.lane >> 3) & 1);
+                if (i_mine < cnt) add_counts(tot, C.lane & 7, C.Eacc + (pos + i_mine - C.i0) * 32);
             }
         }
     }
