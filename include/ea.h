@@ -11,7 +11,11 @@
  *     the device state of a handle until ea_destroy (inside the caller's workspace if one
  *     was given to ea_create_ex).
  *   - Every call except ea_create* returns 0 (EA_OK) or a negative status.  On error the
- *     simulation state is unchanged.  ea_last_error() gives a message.
+ *     simulation state is unchanged, with one exception: a problem larger than one launch can
+ *     hold runs as several launches over groups of realization words, and if a LATER group's
+ *     launch fails (a CUDA error) the earlier groups have already advanced.  The handle then
+ *     refuses ea_sweep / ea_measure (EA_ERR_CUDA) until ea_set_state restores a state.
+ *     ea_last_error() gives a message.
  *   - Work is enqueued on the handle's CUDA stream.  ea_sweep returns after enqueueing
  *     (asynchronous); every call that fills a host buffer synchronizes the stream first.
  *   - One handle is not thread-safe; different handles are independent.
@@ -119,7 +123,8 @@ int ea_get_tables(ea_handle *h, uint64_t *acc, uint64_t *swp);
  * n_sweeps >= 0 full checkerboard sweeps (parity 0 then parity 1); a
  * parallel-tempering round (R4-R6) follows every sweep whose
  * 1-based GLOBAL index is a multiple of swap_interval; swap_interval = 0: no PT.
- * EA_ERR_RANGE if the global sweep counter would pass 2^32 - 1.  Asynchronous.
+ * EA_ERR_RANGE if the global sweep counter would pass 2^32 - 1.  Asynchronous.  Launch
+ * configurations of all word groups are checked before the first launch.
  */
 int ea_sweep(ea_handle *h, int64_t n_sweeps, int swap_interval);
 

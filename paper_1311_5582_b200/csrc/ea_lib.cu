@@ -47,6 +47,8 @@ struct ea_handle {
     uint64_t g = 0, nswap = 0;
     bool energy_valid = false;
     int kernel_sel = EA_KERNEL_AUTO;
+    bool poisoned = false;             // a launch failed between the word groups of one ea_sweep call: the words
+                                       // are no longer at the same sweep; ea_set_state brings the handle back
     int64_t launches = 0;
     int sm_count = 0;
     // measurement series (ea_measure_begin): own allocation, freed by ea_destroy / the next begin
@@ -1121,6 +1123,12 @@ static int sweep_stream(ea_handle *h, int64_t n_sweeps, int swap_interval)
 {
     const StreamPlan pl = plan_stream(h);
     if (!pl.ok) return fail(h, EA_ERR_UNSUPPORTED, "stream kernel: shape not supported");
+    // every word group must have a plan before the first one is launched (the last group may be smaller)
+    if (h->W % pl.Wn) {
+        const int Wl = h->W % pl.Wn;
+        const StreamPlan pt = h->L == 32 ? plan_stream_words<32>(h, Wl) : plan_stream_words<64>(h, Wl);
+        if (!pt.ok) return fail(h, EA_ERR_UNSUPPORTED, "stream kernel: word group does not fit");
+    }
     int64_t left = n_sweeps;
     while (left > 0) {
         const int chunk = (int)std::min<int64_t>(left, 1 << 30);
@@ -1182,7 +1190,13 @@ static int sweep_stream(ea_handle *h, int64_t n_sweeps, int swap_interval)
             cudaGetLastError();
             return sweep_tiled(h, left, swap_interval);
         }
-        if (e != cudaSuccess) return fail(h, EA_ERR_CUDA, std::string("stream launch: ") + cudaGetErrorString(e));
+        if (e != cudaSuccess) {
+            // a later group failed: the earlier groups of this chunk have already advanced, so the
+            // handle no longer holds ONE simulation state.  Refuse further work until ea_set_state.
+            if (w_off > 0) h->poisoned = true;
+            return fail(h, EA_ERR_CUDA, std::string("stream launch: ") + cudaGetErrorString(e) +
+                                            (w_off > 0 ? " (between word groups: state invalid, restore it with ea_set_state)" : ""));
+        }
         h->launches++;
       }
         if (swap_interval > 0) h->nswap += (h->g + (uint64_t)chunk) / (uint64_t)swap_interval - h->g / (uint64_t)swap_interval;
@@ -1293,6 +1307,7 @@ extern "C" int ea_sweep(ea_handle *h, int64_t n_sweeps, int swap_interval)
     if (!h || n_sweeps < 0 || swap_interval < 0) return fail(h, EA_ERR_INVALID_ARG, "ea_sweep: bad argument");
     if (h->g + (uint64_t)n_sweeps > 0xFFFFFFFFull) return fail(h, EA_ERR_RANGE, "ea_sweep: sweep counter would pass 2^32-1");
     if (n_sweeps == 0) return EA_OK;
+    if (h->poisoned) return fail(h, EA_ERR_CUDA, "ea_sweep: an earlier call failed between word groups; restore the state with ea_set_state");
     if (pick_kernel(h) == EA_KERNEL_REPLICA) return sweep_replica(h, n_sweeps, swap_interval);
     if (pick_kernel(h) == EA_KERNEL_RESIDENT) return sweep_resident(h, n_sweeps, swap_interval);
     if (pick_kernel(h) == EA_KERNEL_TILED) return sweep_tiled(h, n_sweeps, swap_interval);
@@ -1628,6 +1643,7 @@ extern "C" int ea_set_state(ea_handle *h, const uint32_t *spin_words, const uint
         }
     }
     h->r_valid = true; h->t_valid = false;
+    h->poisoned = false;
     CUDA_TRY(h, cudaMemcpyAsync(h->P.spin, spin_words, 4 * (size_t)nT * h->W * h->N, cudaMemcpyHostToDevice, h->stream));
     CUDA_TRY(h, cudaMemcpyAsync(h->P.tau, tau.data(), tau.size(), cudaMemcpyHostToDevice, h->stream));
     int grid;
