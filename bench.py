@@ -259,6 +259,19 @@ def time_steps(torch, sim, step, steps, flush_l2):
     return [e0.elapsed_time(e1) for e0, e1 in ev]
 
 
+def oracle_one_core(cfg):
+    """The oracle on ONE host core on this config's shape: one word (or the config's R if smaller),
+    about 1e8 attempts (~1 s)."""
+    from oracle import Oracle, build_oracle
+    build_oracle()
+    R = min(32, cfg.R)
+    sweeps = max(1, int(1.0e8 / (R * cfg.n_temps * cfg.N)))
+    o = Oracle(cfg.L, cfg.n_temps, R, betas_for(cfg), cfg.seed)
+    t = time.perf_counter()
+    o.sweep(sweeps, cfg.swap_interval)
+    return (time.perf_counter() - t) * 1e12 / (R * cfg.n_temps * cfg.N * sweeps)
+
+
 def per_config_block(torch, EA, flush_l2, lop3_peak, skip):
     """ps per attempt on every BASELINE config, outside the headline's timed region:
     3 steps of 1000 sweeps each (config 1: 333, its full length) on a fresh handle after one warm-up step,
@@ -282,6 +295,7 @@ def per_config_block(torch, EA, flush_l2, lop3_peak, skip):
                "alu_frac": ops / step_s / lop3_peak, "digest": check_digest(sim, cfg, cid, 3 * sps)}
         if sim.get_kernel() == 4:
             ent["hbm_view"] = hbm_view(cfg, sps, step_s)
+        ent["oracle_one_core_ps"] = oracle_one_core(cfg)
         out[str(cid)] = ent
         sim.destroy()
     return out
@@ -436,6 +450,7 @@ def run_cuda(a, cfg):
                    "us_per_sweep": step_s * 1e6 / sps, "ps_per_attempt": value, "alu_frac": roofline["frac"], "digest": digest}
             if kernel == 4:
                 ent["hbm_view"] = roofline["hbm_view"]
+            ent["oracle_one_core_ps"] = oracle_one_core(cfg)
             per_config[str(a.config)] = ent
 
     # ---- CPU oracle on the host cores: bounded samples of the same workload, all cores and one core
