@@ -1261,6 +1261,10 @@ static int sweep_replica(ea_handle *h, int64_t n_sweeps, int swap_interval)
         const int chunk = (int)std::min<int64_t>(left, 1 << 30);
         ea::ReplicaArgs A = replica_args(h);
         A.g0 = (uint32_t)h->g; A.n_sweeps = chunk; A.swap_interval = swap_interval; A.nswap0 = (uint32_t)h->nswap;
+        for (int r = 0; r < 10; ++r) {
+            A.rk[2 * r] = h->P.k0 + (uint32_t)r * 0x9E3779B9u;
+            A.rk[2 * r + 1] = h->P.k1 + (uint32_t)r * 0xBB67AE85u;
+        }
         ea::k_replica_sweep<<<h->Rp, 256, smem, h->stream>>>(A);
         CUDA_TRY(h, cudaGetLastError());
         h->launches++;

@@ -17,6 +17,7 @@
 // physical systems with different random numbers.
 #pragma once
 #include "ea_generic.cuh"
+#include "ea_resident.cuh"
 
 namespace ea {
 
@@ -29,6 +30,7 @@ struct ReplicaArgs {
     uint32_t g0;
     int n_sweeps, swap_interval;
     uint32_t nswap0;
+    uint32_t rk[20];          // Philox round keys (k0 + r*0x9E3779B9, k1 + r*0xBB67AE85), r = 0..9
 };
 
 __device__ __forceinline__ int replica_nw(int Nh) { return (Nh + 31) >> 5; }
@@ -98,7 +100,7 @@ __device__ __forceinline__ Planes replica_planes(const uint32_t *lat, const uint
 // Thread = quad of four sites (one Philox call per replica serves them); the lattice (N words per
 // cube) and the probability table stay in shared memory; energies by
 // bit-sliced counters over the parity-1 sites; one warp takes the swap decisions.
-__global__ void __launch_bounds__(256) k_replica_sweep(const ReplicaArgs A)
+__global__ void __launch_bounds__(256, 2) k_replica_sweep(const ReplicaArgs A)
 {
     extern __shared__ __align__(16) uint32_t smem[];
     const Params &P = A.P;
@@ -132,6 +134,9 @@ __global__ void __launch_bounds__(256) k_replica_sweep(const ReplicaArgs A)
         const bool need_E = swap_now || it == A.n_sweeps - 1;
         for (int p = 0; p < 2; ++p) {
             for (int q = tid; q < nq; q += NT) {
+                // counter (g, q, r, tag|k): q is the thread's, everything else the block's -- rounds 0-2 of
+                // Philox are partly per-thread constants, partly uniform (philox_quad, ea_resident.cuh)
+                const PhiloxQuad PQ = philox_quad_init((uint32_t)q, gr, A.rk);
                 for (int c = 0; c < ncube; ++c) {
                     uint32_t *lc = lat + (size_t)c * N;
                     Planes pl[4];
@@ -139,16 +144,28 @@ __global__ void __launch_bounds__(256) k_replica_sweep(const ReplicaArgs A)
 #pragma unroll
                     for (int l = 0; l < 4; ++l) pl[l] = replica_planes(lc, jb, p, 4 * q + l, L, Lh, Nh, NW, &s[l]);
                     const int kn = min(32, nT - 32 * c);
+                    // planes rotated so that replica kb's class bits land on bits 3, 4, 5 of a right
+                    // rotation by kb: (rot & 8) | (rot & 16) | (rot & 32) = 8 * n_sat = byte offset of
+                    // the 64-bit threshold in the replica's table row
+                    uint32_t r0[4], r1[4], r2[4];
+#pragma unroll
+                    for (int l = 0; l < 4; ++l) {
+                        r0[l] = __funnelshift_l(pl[l].b0, pl[l].b0, 3);
+                        r1[l] = __funnelshift_l(pl[l].b1, pl[l].b1, 4);
+                        r2[l] = __funnelshift_l(pl[l].b2, pl[l].b2, 5);
+                    }
                     for (int kb = 0; kb < kn; ++kb) {            // replica by replica ("AMSC1")
                         const int k = 32 * c + kb;
-                        const uint4 rnd = philox4x32_10(g, (uint32_t)q, gr, ((uint32_t)(6 + p) << 16) | (uint32_t)k, P.k0, P.k1);
-                        const uint64_t *row = acc + 7 * (int)tau[k];   // the replica's row of the table
+                        const uint4 rnd = philox_quad(PQ, g, ((uint32_t)(6 + p) << 16) | (uint32_t)k, A.rk);
+                        const char *row = reinterpret_cast<const char *>(acc + 7 * (int)tau[k]);   // the replica's row of the table
                         const uint32_t u[4] = {rnd.x, rnd.y, rnd.z, rnd.w};
+                        const uint32_t kmask = 1u << kb;
 #pragma unroll
                         for (int l = 0; l < 4; ++l) {
-                            const int cls = (int)((pl[l].b0 >> kb) & 1u) | ((int)((pl[l].b1 >> kb) & 1u) << 1) |
-                                            ((int)((pl[l].b2 >> kb) & 1u) << 2);
-                            flip[l] |= (uint32_t)((uint64_t)u[l] < row[cls]) << kb;
+                            const uint32_t a = __funnelshift_r(r0[l], r0[l], kb), b = __funnelshift_r(r1[l], r1[l], kb);
+                            const uint32_t d = __funnelshift_r(r2[l], r2[l], kb);
+                            const uint32_t off = (a & 8u) | (b & 16u) | (d & 32u);
+                            if ((uint64_t)u[l] < *reinterpret_cast<const uint64_t *>(row + off)) flip[l] |= kmask;
                         }
                     }
 #pragma unroll
