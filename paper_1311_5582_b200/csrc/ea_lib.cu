@@ -27,7 +27,8 @@ struct ea_handle {
     uint64_t seed = 0;
     std::vector<double> betas;
     bool desc = true;
-    std::vector<uint64_t> acc, swp;   // host copies of the full tables
+    std::vector<uint64_t> acc, swp;   // host copies: acc always; swp only when ea_set_tables gave one (else the
+                                      // table is a formula of betas and is written out on demand, ea_get_tables)
     cudaStream_t stream = nullptr;
     bool own_ws = false;
     char *ws = nullptr;
@@ -79,7 +80,7 @@ struct ea_handle {
     uint4 *d_bucketF = nullptr;
     uchar4 *d_tripF = nullptr;
     char *d_field = nullptr;
-    std::vector<uint64_t> accf, swpf;  // host copies: [nT][7][2], [nT-1][2 (3+|h|) N + 1]
+    std::vector<uint64_t> accf;        // host copy [nT][7][2]; the field swap table is a formula (ea_get_field_tables)
     mutable std::string err;
 };
 
@@ -308,6 +309,38 @@ static int trim_swap_table(ea_handle *h, const uint64_t *swp, int nT, int64_t M,
     }
     return EA_OK;
 }
+// The same trimmed form for a table given by its FORMULA f(t, m), m in [-M, M], without writing the
+// table out: every row is monotone in m and constant (0 or 2^32) outside one interval, whose two
+// ends are found by bisection; only the thresholds inside it are evaluated.  (A full table is
+// (n_temps - 1)(2 M + 1) exp() calls and 8 bytes each: 400 MB at L = 64, n_temps = 64.)
+template <class F>
+static void trim_swap_generated(int nT, int64_t M, const F &f, SwapTrim &o)
+{
+    o.lo.assign(nT, 0); o.cnt.assign(nT, 0); o.off.assign(nT, 0);
+    o.kind.assign((size_t)2 * nT, 0);
+    o.val.clear();
+    auto trivial = [](uint64_t v) { return v == 0 || v == kTwo32; };
+    for (int t = 0; t + 1 < nT; ++t) {
+        const uint64_t v_lo = f(t, -M), v_hi = f(t, M);
+        int64_t a = -M, b = M + 1;
+        if (trivial(v_lo)) {              // a = first m whose threshold differs from the left constant
+            int64_t lo = -M, hi = M + 1;
+            while (lo < hi) { const int64_t mid = lo + (hi - lo) / 2; if (f(t, mid) != v_lo) hi = mid; else lo = mid + 1; }
+            a = lo;
+        }
+        if (trivial(v_hi) && a <= M) {    // b = first m >= a whose threshold is the right constant
+            int64_t lo = a, hi = M + 1;
+            while (lo < hi) { const int64_t mid = lo + (hi - lo) / 2; if (f(t, mid) == v_hi) hi = mid; else lo = mid + 1; }
+            b = lo;
+        }
+        if (a > M) b = a;
+        o.lo[t] = (int32_t)a; o.cnt[t] = (int32_t)(b - a); o.off[t] = (int32_t)o.val.size();
+        o.kind[2 * t] = v_lo == kTwo32;
+        o.kind[2 * t + 1] = v_hi == kTwo32;
+        for (int64_t m = a; m < b; ++m) o.val.push_back((uint32_t)(f(t, m) - 1));
+    }
+}
+
 static int upload_swap_trim(ea_handle *h, const SwapTrim &o, uint32_t *d_val)
 {
     const int nT = h->nT;
@@ -322,7 +355,8 @@ static int upload_swap_trim(ea_handle *h, const SwapTrim &o, uint32_t *d_val)
     return EA_OK;
 }
 
-static int upload_tables(ea_handle *h, const std::vector<uint64_t> &acc, const std::vector<uint64_t> &swp)
+// swp == nullptr: the zero-field swap table of the handle's betas, from its formula
+static int upload_tables(ea_handle *h, const std::vector<uint64_t> &acc, const std::vector<uint64_t> *swp)
 {
     const int nT = h->nT, M = 3 * h->N / 2;
     for (int t = 0; t < nT; ++t)
@@ -352,7 +386,13 @@ static int upload_tables(ea_handle *h, const std::vector<uint64_t> &acc, const s
         z[c - 4] = zc;
     }
     SwapTrim tr;
-    { int rc = trim_swap_table(h, swp.data(), nT, M, tr); if (rc != EA_OK) return rc; }
+    if (swp) {
+        int rc = trim_swap_table(h, swp->data(), nT, M, tr);
+        if (rc != EA_OK) return rc;
+    } else {
+        const std::vector<double> &b = h->betas;
+        trim_swap_generated(nT, M, [&](int t, int64_t m) { return threshold_of((b[t] - b[t + 1]) * (double)(4 * m)); }, tr);
+    }
     if (tr.val.size() > h->swp_val_cap) return fail(h, EA_ERR_ALLOC, "swap table overflow");
     cudaStream_t s = h->stream;
     CUDA_TRY(h, cudaStreamSynchronize(s));
@@ -371,7 +411,7 @@ static int upload_tables(ea_handle *h, const std::vector<uint64_t> &acc, const s
     }
     for (int c = 0; c < 3; ++c) h->P.z[c] = z[c];
     h->acc = acc;
-    h->swp = swp;
+    if (swp) h->swp = *swp; else { h->swp.clear(); h->swp.shrink_to_fit(); }
     return EA_OK;
 }
 
@@ -528,14 +568,10 @@ extern "C" ea_handle *ea_create_ex(int L, int n_temps, int n_realizations, const
 
     // threshold tables in double on the host
     const int M = 3 * h->N / 2;
-    std::vector<uint64_t> acc((size_t)n_temps * 7), swp((size_t)(n_temps > 1 ? n_temps - 1 : 0) * (2 * M + 1));
+    std::vector<uint64_t> acc((size_t)n_temps * 7);
     for (int t = 0; t < n_temps; ++t)
         for (int c = 0; c < 7; ++c) acc[(size_t)t * 7 + c] = threshold_of(-(betas[t] * (double)(4 * c - 12)));
-    for (int t = 0; t + 1 < n_temps; ++t) {
-        const double db = betas[t] - betas[t + 1];
-        for (int m = -M; m <= M; ++m) swp[(size_t)t * (2 * M + 1) + (m + M)] = threshold_of(db * (double)(4 * m));
-    }
-    if (upload_tables(h, acc, swp) != EA_OK) return (ea_handle *)bail(EA_ERR_CUDA, "ea_create: tables: " + h->err);
+    if (upload_tables(h, acc, nullptr) != EA_OK) return (ea_handle *)bail(EA_ERR_CUDA, "ea_create: tables: " + h->err);
 
     int grid;
     launch_cfg((int64_t)h->W * h->N, 128, grid);
@@ -634,14 +670,22 @@ extern "C" int ea_set_tables(ea_handle *h, const uint64_t *acc, const uint64_t *
     std::vector<uint64_t> a(acc, acc + (size_t)h->nT * 7);
     std::vector<uint64_t> s;
     if (h->nT > 1) s.assign(swp, swp + (size_t)(h->nT - 1) * cols);
-    return upload_tables(h, a, s);
+    return upload_tables(h, a, &s);
 }
 
 extern "C" int ea_get_tables(ea_handle *h, uint64_t *acc, uint64_t *swp)
 {
     if (!h) return EA_ERR_INVALID_ARG;
     if (acc) std::memcpy(acc, h->acc.data(), 8 * h->acc.size());
-    if (swp && !h->swp.empty()) std::memcpy(swp, h->swp.data(), 8 * h->swp.size());
+    if (swp && !h->swp.empty()) {
+        std::memcpy(swp, h->swp.data(), 8 * h->swp.size());
+    } else if (swp) {                     // the default table, written out from its formula
+        const int64_t M = 3 * (int64_t)h->N / 2;
+        for (int t = 0; t + 1 < h->nT; ++t) {
+            const double db = h->betas[t] - h->betas[t + 1];
+            for (int64_t m = -M; m <= M; ++m) swp[(size_t)t * (size_t)(2 * M + 1) + (size_t)(m + M)] = threshold_of(db * (double)(4 * m));
+        }
+    }
     return EA_OK;
 }
 
@@ -661,26 +705,22 @@ extern "C" int ea_set_field(ea_handle *h, int field)
         h->P.h = 0; h->P.ediv = 4; h->P.thrF = nullptr; h->P.swp_val = h->d_swp_val;
         for (int c = 0; c < 18; ++c) h->P.zF[c] = -1;
         const std::vector<uint64_t> acc = h->acc, swp = h->swp;
-        int rc = upload_tables(h, acc, swp);                  // the zero-field swap table again
+        int rc = upload_tables(h, acc, swp.empty() ? nullptr : &swp);      // the zero-field swap table again
         if (rc != EA_OK) return rc;
         if (h->d_field) { cudaFree(h->d_field); h->d_field = nullptr; }
-        h->accf.clear(); h->swpf.clear();
+        h->accf.clear();
         return recompute_energy(h);
     }
     // tables in double on the host, same formulas as at h = 0 (R21)
     const int64_t Mf = (int64_t)(3 + std::abs(field)) * h->N, cols = 2 * Mf + 1;
-    std::vector<uint64_t> accf((size_t)nT * 14), swpf((size_t)(nT > 1 ? nT - 1 : 0) * (size_t)cols);
+    std::vector<uint64_t> accf((size_t)nT * 14);
+    (void)cols;
     for (int t = 0; t < nT; ++t)
         for (int c = 0; c < 7; ++c)
             for (int up = 0; up < 2; ++up) {
                 const double dE = (double)(4 * c - 12 - 2 * field * (2 * up - 1));
                 accf[((size_t)t * 7 + c) * 2 + up] = threshold_of(-(h->betas[t] * dE));
             }
-    for (int t = 0; t + 1 < nT; ++t) {
-        const double db = h->betas[t] - h->betas[t + 1];
-        for (int64_t d2 = -Mf; d2 <= Mf; ++d2)
-            swpf[(size_t)t * (size_t)cols + (size_t)(d2 + Mf)] = threshold_of(db * (double)(2 * d2));
-    }
     // class thresholds in pos order (coldest first), as (threshold - 1); classes with dE <= 0 flip always
     std::vector<uint32_t> thrF((size_t)18 * LTS, 0xFFFFFFFFu);
     int zF[18];
@@ -709,7 +749,10 @@ extern "C" int ea_set_field(ea_handle *h, int field)
             zF[cls] = zc;
         }
     SwapTrim tr;
-    { int rc = trim_swap_table(h, swpf.data(), nT, Mf, tr); if (rc != EA_OK) return rc; }
+    {   // swpf[t][d2 + Mf] = thr((beta_t - beta_{t+1}) 2 d2), trimmed from the formula
+        const std::vector<double> &bt = h->betas;
+        trim_swap_generated(nT, Mf, [&](int t, int64_t d2) { return threshold_of((bt[t] - bt[t + 1]) * (double)(2 * d2)); }, tr);
+    }
     // |h| <= 2: the four columns also get a bucket table, and the resident kernel runs with the field
     std::vector<uint4> tabF;
     std::vector<uchar4> tripF;
@@ -741,7 +784,6 @@ extern "C" int ea_set_field(ea_handle *h, int field)
     h->P.h = field; h->P.ediv = 2; h->P.thrF = (const uint32_t *)d; h->P.swp_val = (const uint32_t *)(d + o_val);
     for (int c = 0; c < 18; ++c) h->P.zF[c] = zF[c];
     h->accf.swap(accf);
-    h->swpf.swap(swpf);
     return recompute_energy(h);
 }
 
@@ -752,7 +794,14 @@ extern "C" int ea_get_field_tables(ea_handle *h, uint64_t *accf, uint64_t *swpf)
     if (!h) return EA_ERR_INVALID_ARG;
     if (h->field == 0) return fail(h, EA_ERR_INVALID_ARG, "ea_get_field_tables: no field is set");
     if (accf) std::memcpy(accf, h->accf.data(), 8 * h->accf.size());
-    if (swpf && !h->swpf.empty()) std::memcpy(swpf, h->swpf.data(), 8 * h->swpf.size());
+    if (swpf) {                           // written out from its formula on demand
+        const int64_t Mf = (int64_t)(3 + std::abs(h->field)) * h->N;
+        for (int t = 0; t + 1 < h->nT; ++t) {
+            const double db = h->betas[t] - h->betas[t + 1];
+            for (int64_t d2 = -Mf; d2 <= Mf; ++d2)
+                swpf[(size_t)t * (size_t)(2 * Mf + 1) + (size_t)(d2 + Mf)] = threshold_of(db * (double)(2 * d2));
+        }
+    }
     return EA_OK;
 }
 
