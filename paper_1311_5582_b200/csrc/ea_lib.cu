@@ -213,7 +213,7 @@ static bool build_bucket_table(const std::vector<uint32_t> &thr32, const int *z,
         const KeyFn key{E, MB};
         const int klo = key(0), khi = key(0xFFFFFFFFu);
         const int n = khi - klo + 1;
-        if (n * BW > kMaxBucket) continue;
+        if (n > kMaxBucket) continue;      // entries (the field table has its own allocation: 32 B each)
         // first u of every bucket (2^32 for an empty bucket at the top)
         std::vector<uint64_t> first((size_t)n + 1);
         first[0] = 0;
@@ -1112,9 +1112,11 @@ StreamPlan plan_stream_words(const ea_handle *h, int Wn)
     pl.MS = (int)((T + pl.grid - 1) / pl.grid);
     const long long per_w = (long long)Sg::NSLAB * h->nT;
     pl.MW = (int)((pl.MS + per_w - 2) / per_w) + 1;
-    const size_t nT = (size_t)h->nT, LTS = nT + 1, MTS = 3 * nT + 2;
-    size_t base = Sg::MBAR_BYTES + 16 * (size_t)h->n_bucket + (size_t)Sg::NST * Sg::BUF_BYTES + 16 * (size_t)pl.MS * MTS +
-                  4 * ((size_t)pl.MS * LTS + 3 * LTS + MTS + (size_t)pl.MS * 32) + 2 * (size_t)pl.MW * 32 * nT;
+    const bool f = h->field != 0;                 // field |h| <= 2: four columns, 32-byte bucket entries
+    const size_t nT = (size_t)h->nT, LTS = nT + 1, NC = f ? 4 : 3, MTS = NC * nT + 2;
+    const size_t nbk = f ? 2 * (size_t)h->KF.n_bucket : (size_t)h->n_bucket;
+    size_t base = Sg::MBAR_BYTES + 16 * nbk + (size_t)Sg::NST * Sg::BUF_BYTES + 16 * (size_t)pl.MS * MTS +
+                  4 * ((size_t)pl.MS * LTS + NC * LTS + MTS + (size_t)pl.MS * 32) + 2 * (size_t)pl.MW * 32 * nT;
     pl.esm_off = (base + 15) & ~(size_t)15;
     pl.batch_off = pl.esm_off + 4 * (size_t)pl.MW * 32 * nT;
     base = pl.batch_off + 16 * (size_t)pl.MS + 12 * nT;
@@ -1147,6 +1149,7 @@ StreamPlan plan_stream(const ea_handle *h)
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
     if (!coop) return StreamPlan{false, 0, 0, 0, 0, 0, 0, 0, 0};
+    if (h->field != 0 && !h->fast_field) return StreamPlan{false, 0, 0, 0, 0, 0, 0, 0, 0};   // field: |h| <= 2 only
     if (h->L == 32) return plan_stream_t<32>(h);
     if (h->L == 64) return plan_stream_t<64>(h);
     return StreamPlan{false, 0, 0, 0, 0, 0, 0, 0, 0};
@@ -1155,7 +1158,7 @@ StreamPlan plan_stream(const ea_handle *h)
 template <int L>
 cudaError_t launch_stream_t(const ea_handle *h, ea::StreamArgs &A, const StreamPlan &pl, bool fast)
 {
-    void (*kern)(const ea::StreamArgs) = fast ? ea::k_stream<L, true> : ea::k_stream<L, false>;
+    void (*kern)(const ea::StreamArgs) = h->field != 0 ? ea::k_stream<L, true, 4> : fast ? ea::k_stream<L, true> : ea::k_stream<L, false>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem);
     if (e != cudaSuccess) return e;
     int per_sm = 0;
@@ -1206,6 +1209,7 @@ static int sweep_stream(ea_handle *h, int64_t n_sweeps, int swap_interval)
         A.Ecnt = h->d_Ecnt + (size_t)32 * w_off * h->nT;
         A.gbar = (unsigned int *)(h->d_Ecnt + 2 * (size_t)h->Rp * h->nT);
         A.bucket = h->d_bucket; A.K = h->K; A.trip = h->d_trip;
+        if (h->field != 0) { A.bucket = h->d_bucketF; A.K = h->KF; A.trip = h->d_tripF; }
         A.MS = pg.MS; A.MW = pg.MW; A.swap_win = pg.swap_win; A.esm_off = (int)pg.esm_off; A.batch_off = (int)pg.batch_off;
         for (int r = 0; r < 10; ++r) {
             A.rk[2 * r] = h->P.k0 + (uint32_t)r * 0x9E3779B9u;
@@ -1237,7 +1241,7 @@ static int sweep_stream(ea_handle *h, int64_t n_sweeps, int swap_interval)
             // the SMs are not all free (another context holds some): same result, one launch per
             // half-sweep instead of one cooperative launch
             cudaGetLastError();
-            return sweep_tiled(h, left, swap_interval);
+            return h->field != 0 ? sweep_generic(h, left, swap_interval) : sweep_tiled(h, left, swap_interval);
         }
         if (e != cudaSuccess) {
             // a later group failed: the earlier groups of this chunk have already advanced, so the
@@ -1330,9 +1334,12 @@ static int pick_kernel(const ea_handle *h)
 {
     if (h->layout == EA_LAYOUT_REPLICA_BITS) return EA_KERNEL_REPLICA;
     if (h->kernel_sel == EA_KERNEL_GENERIC_STEPWISE) return EA_KERNEL_GENERIC_STEPWISE;
-    if (h->field != 0)       // with a field: the resident kernel for |h| <= 2 on L = 8, 16, else the generic path
-        return (h->kernel_sel == EA_KERNEL_AUTO || h->kernel_sel == EA_KERNEL_RESIDENT) && plan_resident(h).ok
-                   ? EA_KERNEL_RESIDENT : EA_KERNEL_GENERIC;
+    if (h->field != 0) {     // with a field: |h| <= 2 on the resident (L = 8, 16) and streaming (L = 32, 64) kernels,
+                             // else the generic path
+        if ((h->kernel_sel == EA_KERNEL_AUTO || h->kernel_sel == EA_KERNEL_RESIDENT) && plan_resident(h).ok) return EA_KERNEL_RESIDENT;
+        if ((h->kernel_sel == EA_KERNEL_AUTO || h->kernel_sel == EA_KERNEL_STREAM) && plan_stream(h).ok) return EA_KERNEL_STREAM;
+        return EA_KERNEL_GENERIC;
+    }
     if (h->kernel_sel != EA_KERNEL_AUTO) return h->kernel_sel;
     if (plan_resident(h).ok) return EA_KERNEL_RESIDENT;
     if (plan_stream(h).ok) return EA_KERNEL_STREAM;
@@ -1346,8 +1353,8 @@ extern "C" int ea_set_kernel(ea_handle *h, int kernel)
     if (h->layout == EA_LAYOUT_REPLICA_BITS)
         return kernel == EA_KERNEL_AUTO ? EA_OK : fail(h, EA_ERR_UNSUPPORTED, "ea_set_kernel: the replica-bits layout has one kernel");
     if (kernel == EA_KERNEL_AUTO || kernel == EA_KERNEL_GENERIC || kernel == EA_KERNEL_GENERIC_STEPWISE) { h->kernel_sel = kernel; return EA_OK; }
-    if (h->field != 0 && !(kernel == EA_KERNEL_RESIDENT && plan_resident(h).ok))
-        return fail(h, EA_ERR_UNSUPPORTED, "ea_set_kernel: with a field only the generic kernel and, for |h| <= 2 on L = 8, 16, the resident one");
+    if (h->field != 0 && !(kernel == EA_KERNEL_RESIDENT && plan_resident(h).ok) && !(kernel == EA_KERNEL_STREAM && plan_stream(h).ok))
+        return fail(h, EA_ERR_UNSUPPORTED, "ea_set_kernel: with a field only the generic kernel and, for |h| <= 2, the resident (L = 8, 16) and streaming (L = 32, 64) ones");
     if (kernel == EA_KERNEL_RESIDENT && plan_resident(h).ok) { h->kernel_sel = kernel; return EA_OK; }
     if (kernel == EA_KERNEL_TILED && plan_tiled(h).ok) { h->kernel_sel = kernel; return EA_OK; }
     if (kernel == EA_KERNEL_STREAM && plan_stream(h).ok) { h->kernel_sel = kernel; return EA_OK; }

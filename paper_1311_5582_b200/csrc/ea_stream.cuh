@@ -215,7 +215,7 @@ __device__ __forceinline__ void stream_release(const StreamArgs &A, const Stream
 
 // One half-sweep (parity p) over the block's batches; the first NST items are in flight
 // (stream_prime).  ENERGY: also count the satisfied bonds of the updated (parity-1) sites.
-template <int L, bool FAST, bool ENERGY>
+template <int L, bool FAST, bool ENERGY, int NC = 3>
 __device__ __forceinline__ void stream_consume(const StreamArgs &A, const StreamCtx<L> &C, int p, uint32_t g,
                                                uint32_t &phase, uint32_t &efill)
 {
@@ -252,7 +252,7 @@ __device__ __forceinline__ void stream_consume(const StreamArgs &A, const Stream
                 mbar_wait(&C.full[st], (phase >> st) & 1u);
                 phase ^= 1u << st;
                 const char *buf = reinterpret_cast<const char *>(C.bufs + (size_t)st * Sg::BUF_BYTES);
-                const uint4 res = update_quad_mem<L, FAST, false, false, false>(
+                const uint4 res = update_quad_mem<L, FAST, false, false, false, NC>(
                     buf + 16 * tid, buf + Sg::OWN_BYTES, C.ov, C.oyp, C.oym, C.ozp, C.ozm, C.qx, C.lt + li * C.LTS,
                     C.mt + (size_t)li * C.MTS, C.R, J, s, rnd, fin);
                 reinterpret_cast<uint4 *>(P.spin + ((size_t)(k0 + i) * P.W + w) * N + p * Nh)[q] = res;
@@ -260,7 +260,8 @@ __device__ __forceinline__ void stream_consume(const StreamArgs &A, const Stream
             }
         } else {
             for (int i0 = 0; i0 < cnt; i0 += 4) {      // the batch's (up to four) slots share one butterfly
-                uint32_t en[4][5];
+                constexpr int NPE = NC == 4 ? 6 : 5;
+                uint32_t en[4][NPE];
 #pragma unroll
                 for (int h = 0; h < 4; ++h) {
                     const int i = i0 + h;
@@ -270,21 +271,39 @@ __device__ __forceinline__ void stream_consume(const StreamArgs &A, const Stream
                         mbar_wait(&C.full[st], (phase >> st) & 1u);
                         phase ^= 1u << st;
                         const char *buf = reinterpret_cast<const char *>(C.bufs + (size_t)st * Sg::BUF_BYTES);
-                        const uint4 res = update_quad_mem<L, FAST, true, false, false>(
+                        const uint4 res = update_quad_mem<L, FAST, true, false, false, NC>(
                             buf + 16 * tid, buf + Sg::OWN_BYTES, C.ov, C.oyp, C.oym, C.ozp, C.ozm, C.qx,
                             C.lt + li * C.LTS, C.mt + (size_t)li * C.MTS, C.R, J, s, rnd, fin);
                         reinterpret_cast<uint4 *>(P.spin + ((size_t)(k0 + i) * P.W + w) * N + p * Nh)[q] = res;
-                        stream_release<L>(A, C, p, li, efill);
-                        quad_sum(fin, en[h]);
+                        if constexpr (NC == 4) {
+                            // field: T = (satisfied bonds) + |h| (spins that pay the field energy) over my four
+                            // parity-1 sites (new words) and the four parity-0 sites of the index-aligned quad
+                            // of the tile (every quad of the slab is met once): E = (3 + |h|) N - 2 T
+                            const uint4 v4 = *reinterpret_cast<const uint4 *>(buf + Sg::OWN_BYTES + C.ov);
+                            stream_release<L>(A, C, p, li, efill);
+                            uint32_t e5[5], x4[4], y5[5];
+                            quad_sum(fin, e5);
+                            const uint32_t inv = P.h > 0 ? 0xFFFFFFFFu : 0u;      // h > 0: down spins pay
+                            const uint32_t xs[8] = {res.x ^ inv, res.y ^ inv, res.z ^ inv, res.w ^ inv,
+                                                    v4.x ^ inv, v4.y ^ inv, v4.z ^ inv, v4.w ^ inv};
+                            count8(xs, x4);
+                            const bool two = (P.h & 1) == 0;
+                            y5[0] = two ? 0u : x4[0]; y5[1] = two ? x4[0] : x4[1]; y5[2] = two ? x4[1] : x4[2];
+                            y5[3] = two ? x4[2] : x4[3]; y5[4] = two ? x4[3] : 0u;
+                            vsum<5>(e5, y5, en[h]);
+                        } else {
+                            stream_release<L>(A, C, p, li, efill);
+                            quad_sum(fin, en[h]);
+                        }
                     } else {
 #pragma unroll
-                        for (int j = 0; j < 5; ++j) en[h][j] = 0;
+                        for (int j = 0; j < NPE; ++j) en[h][j] = 0;
                     }
                 }
-                uint32_t tot[kResPlanes];
-                warp_sum4(en, C.lane, tot);
+                uint32_t tot[NPE + 5];
+                warp_sum4_t<NPE>(en, C.lane, tot);
                 const int i_mine = i0 + 2 * (C.lane >> 4) + ((C.lane >> 3) & 1);
-                if (i_mine < cnt) add_counts(tot, C.lane & 7, C.Eacc + (pos + i_mine - C.i0) * 32);
+                if (i_mine < cnt) add_counts_t<NPE + 5>(tot, C.lane & 7, C.Eacc + (pos + i_mine - C.i0) * 32);
             }
         }
     }
@@ -331,7 +350,7 @@ __device__ __forceinline__ void stream_grid_sync(unsigned int *bar)
     __syncthreads();
 }
 
-template <int L, bool FAST>
+template <int L, bool FAST, int NC = 3>
 __global__ void __launch_bounds__(StreamGeom<L>::NTHR, 1) k_stream(const StreamArgs A)
 {
     using Gm = ResGeom<L>;
@@ -340,7 +359,8 @@ __global__ void __launch_bounds__(StreamGeom<L>::NTHR, 1) k_stream(const StreamA
     constexpr int NSLAB = Sg::NSLAB;
     extern __shared__ __align__(128) unsigned char smraw[];
     const Params &P = A.P;
-    const int nT = P.nT, LTS = P.LTS, MTS = 3 * nT + 2, MS = A.MS, MW = A.MW;
+    const int nT = P.nT, LTS = P.LTS, MTS = NC * nT + 2, MS = A.MS, MW = A.MW;
+    constexpr int BW = NC == 4 ? 2 : 1;          // 16-byte words per bucket entry (field: 32-byte entries)
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarp = NT >> 5;
     constexpr int NTA = NT;
 
@@ -354,11 +374,11 @@ __global__ void __launch_bounds__(StreamGeom<L>::NTHR, 1) k_stream(const StreamA
     // shared memory
     uint64_t *mbar = reinterpret_cast<uint64_t *>(smraw);                        // full[NST], empty[NST], number of batches
     uint4 *bucket = reinterpret_cast<uint4 *>(smraw + Sg::MBAR_BYTES);           // [n_bucket]
-    unsigned char *bufs = reinterpret_cast<unsigned char *>(bucket + A.K.n_bucket);   // [NST][BUF_BYTES]
+    unsigned char *bufs = reinterpret_cast<unsigned char *>(bucket + BW * A.K.n_bucket);   // [NST][BUF_BYTES]
     uint4 *mt = reinterpret_cast<uint4 *>(bufs + (size_t)NST * Sg::BUF_BYTES);      // [MS][MTS]
     uint32_t *lt = reinterpret_cast<uint32_t *>(mt + (size_t)MS * MTS);          // [MS][LTS]
     uint32_t *thr = lt + MS * LTS;                                               // [3][LTS]
-    uchar4 *trip = reinterpret_cast<uchar4 *>(thr + 3 * LTS);                    // [MTS]
+    uchar4 *trip = reinterpret_cast<uchar4 *>(thr + NC * LTS);                   // [MTS]
     int32_t *Eacc = reinterpret_cast<int32_t *>(trip + MTS);                     // [MS][32]
     uint8_t *tau8 = reinterpret_cast<uint8_t *>(Eacc + MS * 32);                 // [MW][32][nT]
     uint8_t *sig8 = tau8 + (size_t)MW * 32 * nT;                                 // [MW][32][nT]
@@ -370,8 +390,8 @@ __global__ void __launch_bounds__(StreamGeom<L>::NTHR, 1) k_stream(const StreamA
     int *swhi = swlo + nT;                                                       // [nT] one past its last m
     int *swk = swhi + nT;                                                        // [nT] decisions left | right << 1 of the range
 
-    for (int a = tid; a < A.K.n_bucket; a += NTA) bucket[a] = A.bucket[a];
-    for (int a = tid; a < 3 * LTS; a += NTA) thr[a] = P.thr32[a];
+    for (int a = tid; a < BW * A.K.n_bucket; a += NTA) bucket[a] = A.bucket[a];
+    for (int a = tid; a < NC * LTS; a += NTA) thr[a] = NC == 4 ? P.thrF[14 * LTS + a] : P.thr32[a];
     for (int a = tid; a < MTS - 1; a += NTA) trip[a] = A.trip[a];
     for (int a = tid; a < (nT - 1) * SW; a += NTA) {         // window m = -SW + i of row t
         const int t = a / SW, m = -SW + a % SW;
@@ -412,7 +432,7 @@ __global__ void __launch_bounds__(StreamGeom<L>::NTHR, 1) k_stream(const StreamA
                 if (lane == (n & 31)) lt[li * LTS + n] = mk;
             }
             __syncwarp();
-            build_mt(mt + (size_t)li * MTS, lt + li * LTS, trip, nT, lane);
+            (NC == 4 ? build_mt4 : build_mt)(mt + (size_t)li * MTS, lt + li * LTS, trip, nT, lane);
         }
     };
     rebuild_tables();
@@ -433,6 +453,10 @@ __global__ void __launch_bounds__(StreamGeom<L>::NTHR, 1) k_stream(const StreamA
     C.R.thr = thr; C.R.LTS = LTS; C.R.nT = nT;
     rank_ctx_key(C.R, A.K, bucket);
     C.R.z0 = P.z[0]; C.R.z1 = P.z[1]; C.R.z2 = P.z[2];
+    if (NC == 4) {
+        C.R.z0 = P.zF[14]; C.R.z1 = P.zF[15]; C.R.z2 = P.zF[16]; C.R.z3 = P.zF[17]; C.R.h = P.h;
+        C.R.bucket0 = reinterpret_cast<const char *>(bucket) - 32 * (ptrdiff_t)A.K.key_lo;
+    }
     __syncthreads();
 
     uint32_t nswap = A.nswap0, phase = 0, efill = 0;
@@ -444,17 +468,17 @@ __global__ void __launch_bounds__(StreamGeom<L>::NTHR, 1) k_stream(const StreamA
         const bool swap_now = A.swap_interval > 0 && ((uint64_t)g + 1) % (uint64_t)A.swap_interval == 0;
         const bool need_E = swap_now || it == A.n_sweeps - 1;
         trace_stamp(A, it, 0);
-        stream_consume<L, FAST, false>(A, C, 0, g, phase, efill);
+        stream_consume<L, FAST, false, NC>(A, C, 0, g, phase, efill);
         trace_stamp(A, it, 1);
         stream_grid_sync(A.gbar);
         __syncwarp();   // thread 0 spins inside grid.sync: make its warp converge again before the hot loop
         stream_prime<L>(A, C, 1, efill);
         trace_stamp(A, it, 2);
         if (need_E) {
-            stream_consume<L, FAST, true>(A, C, 1, g, phase, efill);
+            stream_consume<L, FAST, true, NC>(A, C, 1, g, phase, efill);
             stream_flush_counts<L>(A, C, ebuf);
         } else {
-            stream_consume<L, FAST, false>(A, C, 1, g, phase, efill);
+            stream_consume<L, FAST, false, NC>(A, C, 1, g, phase, efill);
         }
         trace_stamp(A, it, 3);
         stream_grid_sync(A.gbar);
@@ -475,7 +499,8 @@ __global__ void __launch_bounds__(StreamGeom<L>::NTHR, 1) k_stream(const StreamA
                 const int32_t *er = Esm + (size_t)(wl * 32 + lane) * nT;
                 for (int t = (int)(nswap & 1u) + 2 * warp; t + 1 < nT; t += 2 * nwarp) {
                     const int sa = sg_[t], sb = sg_[t + 1];
-                    const int m = (er[sb] - er[sa]) / 2;
+                    // counts c: E = E0 - 2 c; h = 0: m = (E_a - E_b) / 4 = (c_b - c_a) / 2; field: (E_a - E_b) / 2 = c_b - c_a
+                    const int m = NC == 4 ? er[sb] - er[sa] : (er[sb] - er[sa]) / 2;
                     const uint4 v = philox_rk(g, (uint32_t)t, P.r0 + (uint32_t)r, 2u << 16, A.rk);
                     bool acc;           // everything but the far tail of the stored range is in shared memory
                     if (m < swlo[t]) acc = swk[t] & 1;
@@ -499,7 +524,7 @@ __global__ void __launch_bounds__(StreamGeom<L>::NTHR, 1) k_stream(const StreamA
             if (it == A.n_sweeps - 1) {
                 for (int a = tid; a < 32 * nT; a += NT) {
                     const size_t idx = (size_t)32 * w * nT + a;
-                    P.E[idx] = 3 * N - 2 * Esm[(size_t)wl * 32 * nT + a];
+                    P.E[idx] = (3 + (NC == 4 ? abs(P.h) : 0)) * N - 2 * Esm[(size_t)wl * 32 * nT + a];
                     P.tau[idx] = tau8[(size_t)wl * 32 * nT + a];
                     P.sigma[idx] = sig8[(size_t)wl * 32 * nT + a];
                 }

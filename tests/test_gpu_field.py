@@ -46,6 +46,7 @@ def test_field_trajectory_matches_oracle(L, nT, R, h, swap, asc):
     fast = abs(h) <= 2 and L in (8, 16)          # |h| <= 2 on the resident kernel's lattices, else the generic path
     assert g.get_field() == h
     assert g.get_kernel() == (pkg.binding.EA_KERNEL_RESIDENT if fast else pkg.binding.EA_KERNEL_GENERIC)
+    assert L < 32
     ga, gs = g.get_field_tables()
     oa, os_ = o.field_tables()
     assert (ga == oa).all() and (gs == os_).all()          # both sides hold identical tables
@@ -91,6 +92,27 @@ def test_field_on_the_resident_kernel_matches_oracle_and_the_generic_kernel(L, n
     _same_state(g, o, L, R)
     g.set_kernel(pkg.binding.EA_KERNEL_RESIDENT)
     g.sweep(3, swap); o.sweep(3, swap)
+    _same_state(g, o, L, R)
+    g.destroy()
+
+
+@pytest.mark.parametrize("L,nT,R,h,swap,ns", [
+    (32, 8, 32, 1, 1, 4), (32, 5, 40, -2, 1, 3), (32, 32, 32, 2, 2, 3), (32, 6, 64, -1, 0, 3), (64, 3, 32, 1, 1, 2),
+])
+def test_field_on_the_streaming_kernel_matches_oracle(L, nT, R, h, swap, ns):
+    """Field |h| <= 2 in the streaming kernel (L = 32, 64): the same four-column route as in the
+    resident kernel, the paying spins counted from the tile's index-aligned quad."""
+    pkg, Oracle = _mods()
+    betas = 1.0 / temperature_ladder(nT, 0.9, 2.2)
+    g = pkg.EA(L, nT, R, betas, 29)
+    o = Oracle(L, nT, R, betas, 29)
+    g.set_field(h); o.set_field(h)
+    assert g.get_kernel() == pkg.binding.EA_KERNEL_STREAM
+    for n in (1, ns):
+        g.sweep(n, swap); o.sweep(n, swap)
+        _same_state(g, o, L, R)
+    g.set_kernel(pkg.binding.EA_KERNEL_GENERIC)
+    g.sweep(2, swap); o.sweep(2, swap)
     _same_state(g, o, L, R)
     g.destroy()
 
