@@ -232,10 +232,12 @@ int ea_get_binder(ea_handle *h, double *g /* [n_temps] */);
  * dE = 4 n_sat - 12 - 2 h s_i, so the acceptance table has the paper's 14 columns (7 local energies
  * x 2 spins).  h is an integer, |h| <= 64 (R21: H stays an exact
  * integer; the swap table is then indexed by (E_a - E_b)/2).  Tables are rebuilt on the host in
- * double from betas, energies are recomputed, the sweep counter is kept.  With h != 0 only
- * EA_KERNEL_GENERIC runs (ea_set_kernel(other) -> EA_ERR_UNSUPPORTED, ea_set_tables ->
- * EA_ERR_UNSUPPORTED, ea_get_tables keeps returning the zero-field tables); h = 0 restores the
- * zero-field path.
+ * double from betas, energies are recomputed, the sweep counter is kept.  With 1 <= |h| <= 2 the
+ * resident (L = 8, 16) and streaming (L = 32, 64) kernels run (four threshold columns of the
+ * shifted class index); every other case runs on EA_KERNEL_GENERIC.
+ * ea_set_kernel of a kernel that cannot run the field -> EA_ERR_UNSUPPORTED; ea_set_tables ->
+ * EA_ERR_UNSUPPORTED; ea_get_tables keeps returning the zero-field tables; h = 0 restores the
+ * zero-field path.  Not available in EA_LAYOUT_REPLICA_BITS.
  */
 int ea_set_field(ea_handle *h, int field);
 int ea_get_field(ea_handle *h);
