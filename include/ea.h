@@ -48,8 +48,9 @@ enum {
     EA_KERNEL_AUTO = 0,
     EA_KERNEL_GENERIC = 1,   /* any even L, global memory: one cooperative launch per call when
                                 the work fits one wave, else one launch per half-sweep       */
-    EA_KERNEL_RESIDENT = 2,  /* L in {8,16}: lattices resident in shared memory, one launch
-                                for all sweeps of the call, PT inside a thread-block cluster */
+    EA_KERNEL_RESIDENT = 2,  /* every even L <= 12 and L = 16: lattices resident in shared memory,
+                                one launch for all sweeps of the call, PT inside a thread-block
+                                cluster (L = 8, 16: quad vectors; other L: run-time geometry)   */
     EA_KERNEL_TILED = 3,     /* L = 16, 32, 64: z-slab tiles, one launch per half-sweep, lattice
                                 read in place from global memory (L1/L2)                     */
     EA_KERNEL_STREAM = 4,    /* L = 32, 64: one persistent cooperative launch for all sweeps; z-slab
@@ -233,7 +234,7 @@ int ea_get_binder(ea_handle *h, double *g /* [n_temps] */);
  * x 2 spins).  h is an integer, |h| <= 64 (R21: H stays an exact
  * integer; the swap table is then indexed by (E_a - E_b)/2).  Tables are rebuilt on the host in
  * double from betas, energies are recomputed, the sweep counter is kept.  With 1 <= |h| <= 2 the
- * resident (L = 8, 16) and streaming (L = 32, 64) kernels run (four threshold columns of the
+ * resident (even L <= 12, L = 16) and streaming (L = 32, 64) kernels run (four threshold columns of the
  * shifted class index); every other case runs on EA_KERNEL_GENERIC.
  * ea_set_kernel of a kernel that cannot run the field -> EA_ERR_UNSUPPORTED; ea_set_tables ->
  * EA_ERR_UNSUPPORTED; ea_get_tables keeps returning the zero-field tables; h = 0 restores the

@@ -902,7 +902,7 @@ ResPlan plan_resident(const ea_handle *h)
     // run-time geometry: + the word's couplings (3 N words) and the neighbour table (3 words per site)
     const size_t extra = (h->L != 8 && h->L != 16) ? 24 * (size_t)h->N + 16 : 0;
     pl.any = h->L != 8 && h->L != 16;          // any other even L: run-time geometry (ea_small.cuh)
-    if (h->field != 0 && (pl.any || !h->fast_field)) return pl;   // field: |h| <= 2 on L = 8, 16
+    if (h->field != 0 && !h->fast_field) return pl;   // field: |h| <= 2 only
     if (pl.any && h->N / 2 > 1024) return pl;  // one thread per site of a parity: L <= 12
     const size_t cap = 227 * 1024;
     int C = 0;
@@ -953,7 +953,7 @@ cudaError_t launch_resident_t(const ea_handle *h, const ea::ResArgs &A, const Re
 }
 cudaError_t launch_resident_any(const ea_handle *h, const ea::ResArgs &A, const ResPlan &pl, bool fast)
 {
-    auto kern = fast ? ea::k_resident_any<true> : ea::k_resident_any<false>;
+    auto kern = h->field != 0 ? ea::k_resident_any<true, 4> : fast ? ea::k_resident_any<true> : ea::k_resident_any<false>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem);
     if (e != cudaSuccess) return e;
     cudaLaunchConfig_t cfg{};
@@ -1334,7 +1334,7 @@ static int pick_kernel(const ea_handle *h)
 {
     if (h->layout == EA_LAYOUT_REPLICA_BITS) return EA_KERNEL_REPLICA;
     if (h->kernel_sel == EA_KERNEL_GENERIC_STEPWISE) return EA_KERNEL_GENERIC_STEPWISE;
-    if (h->field != 0) {     // with a field: |h| <= 2 on the resident (L = 8, 16) and streaming (L = 32, 64) kernels,
+    if (h->field != 0) {     // with a field: |h| <= 2 on the resident (even L <= 12, 16) and streaming (L = 32, 64) kernels,
                              // else the generic path
         if ((h->kernel_sel == EA_KERNEL_AUTO || h->kernel_sel == EA_KERNEL_RESIDENT) && plan_resident(h).ok) return EA_KERNEL_RESIDENT;
         if ((h->kernel_sel == EA_KERNEL_AUTO || h->kernel_sel == EA_KERNEL_STREAM) && plan_stream(h).ok) return EA_KERNEL_STREAM;
@@ -1354,7 +1354,7 @@ extern "C" int ea_set_kernel(ea_handle *h, int kernel)
         return kernel == EA_KERNEL_AUTO ? EA_OK : fail(h, EA_ERR_UNSUPPORTED, "ea_set_kernel: the replica-bits layout has one kernel");
     if (kernel == EA_KERNEL_AUTO || kernel == EA_KERNEL_GENERIC || kernel == EA_KERNEL_GENERIC_STEPWISE) { h->kernel_sel = kernel; return EA_OK; }
     if (h->field != 0 && !(kernel == EA_KERNEL_RESIDENT && plan_resident(h).ok) && !(kernel == EA_KERNEL_STREAM && plan_stream(h).ok))
-        return fail(h, EA_ERR_UNSUPPORTED, "ea_set_kernel: with a field only the generic kernel and, for |h| <= 2, the resident (L = 8, 16) and streaming (L = 32, 64) ones");
+        return fail(h, EA_ERR_UNSUPPORTED, "ea_set_kernel: with a field only the generic kernel and, for |h| <= 2, the resident (even L <= 12, L = 16) and streaming (L = 32, 64) ones");
     if (kernel == EA_KERNEL_RESIDENT && plan_resident(h).ok) { h->kernel_sel = kernel; return EA_OK; }
     if (kernel == EA_KERNEL_TILED && plan_tiled(h).ok) { h->kernel_sel = kernel; return EA_OK; }
     if (kernel == EA_KERNEL_STREAM && plan_stream(h).ok) { h->kernel_sel = kernel; return EA_OK; }

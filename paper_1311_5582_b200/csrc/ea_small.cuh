@@ -41,20 +41,25 @@ __device__ __forceinline__ Planes site_planes_tab(const uint32_t *sp, const uint
 
 // New word of site (p, j) of lattice `sp` for the draw u.  FAST: ranks from the bucket table; the
 // rare flagged site is redone with the exact search.
-template <bool FAST, bool ENERGY>
+template <bool FAST, bool ENERGY, int NC = 3>
 __device__ __forceinline__ void update_site_any(uint32_t *sp, const uint32_t *js, const uint32_t *nb, const uint32_t *lt,
                                                 const uint4 *mt, const RankCtx &R, int p, int j, int Nh, int N,
                                                 uint32_t u, Planes &fin)
 {
     uint32_t s, flag = FAST ? 0u : 0x80000000u, acc = 0u;
     const Planes pl = site_planes_tab(sp, js, nb, p, j, Nh, N, &s);
-    if (FAST) acc = accept_fast(R, mt, u, pl, &flag);
-    if ((int)flag < 0) acc = accept_exact(R, lt, u, pl);
+    if (NC == 4) {                       // field |h| <= 2: four threshold columns, the spin enters the class
+        if (FAST) acc = accept_fast4(R, mt, u, pl, s, &flag);
+        if ((int)flag < 0) acc = accept_exact4(R, lt, u, pl, s);
+    } else {
+        if (FAST) acc = accept_fast(R, mt, u, pl, &flag);
+        if ((int)flag < 0) acc = accept_exact(R, lt, u, pl);
+    }
     sp[p * Nh + j] = s ^ acc;
     if (ENERGY) fin = planes_after(pl, acc);
 }
 
-template <bool FAST>
+template <bool FAST, int NC = 3>
 __global__ void __launch_bounds__(1024, 1) k_resident_any(const ResArgs A)
 {
     const int L = A.P.L, Lh = A.P.Lh, N = A.P.N, Nh = A.P.Nh, NSP = A.NQP, G = A.G, NT = NSP * G;
@@ -73,13 +78,14 @@ __global__ void __launch_bounds__(1024, 1) k_resident_any(const ResArgs A)
     const bool live = j < Nh;
 
     // shared memory: the rank table first (fixed offset 0), lattices next (16 B aligned)
-    const int MTS = 3 * nT + 2, SW = A.swap_win;
-    uint4 *bucket = reinterpret_cast<uint4 *>(smem);                 // [n_bucket] 16 B entries
-    uint32_t *sp = smem + 4 * (size_t)A.K.n_bucket;                    // [S][2][Nh]
+    const int MTS = NC * nT + 2, SW = A.swap_win;
+    constexpr int BW = NC == 4 ? 2 : 1;                              // 16-byte words per bucket entry
+    uint4 *bucket = reinterpret_cast<uint4 *>(smem);                 // [n_bucket] 16 B (field: 32 B) entries
+    uint32_t *sp = smem + 4 * (size_t)BW * A.K.n_bucket;             // [S][2][Nh]
     uint4 *mt = reinterpret_cast<uint4 *>(sp + (size_t)S * N);       // [S][MTS] mask tables
     uint32_t *lt = reinterpret_cast<uint32_t *>(mt + (size_t)S * MTS);   // [S][LTS]
     uint32_t *thr = lt + S * LTS;                                    // [3][LTS]
-    uchar4 *trip = reinterpret_cast<uchar4 *>(thr + 3 * LTS);        // [MTS]
+    uchar4 *trip = reinterpret_cast<uchar4 *>(thr + NC * LTS);       // [MTS]
     int32_t *Eacc = (int32_t *)(trip + MTS);                         // [S][32] satisfied-bond counts
     int32_t *swm = Eacc + S * 32;                                    // [nT][4]: lo, cnt, off, kinds
     uint32_t *swwin = (uint32_t *)(swm + 4 * nT);                    // [nT][SW] thresholds - 1
@@ -111,8 +117,8 @@ __global__ void __launch_bounds__(1024, 1) k_resident_any(const ResArgs A)
     }
     for (int k = 0; k < nk; ++k)
         for (int a = tid; a < LTS; a += NT) lt[k * LTS + a] = P.lt[((size_t)w * nT + k0 + k) * LTS + a];
-    for (int a = tid; a < 3 * LTS; a += NT) thr[a] = P.thr32[a];
-    for (int a = tid; a < A.K.n_bucket; a += NT) bucket[a] = A.bucket[a];
+    for (int a = tid; a < NC * LTS; a += NT) thr[a] = NC == 4 ? P.thrF[14 * LTS + a] : P.thr32[a];
+    for (int a = tid; a < BW * A.K.n_bucket; a += NT) bucket[a] = A.bucket[a];
     for (int a = tid; a < 32 * nT; a += NT) {
         tau8[a] = P.tau[(size_t)32 * w * nT + a];
         sig8[a] = P.sigma[(size_t)32 * w * nT + a];
@@ -148,11 +154,15 @@ __global__ void __launch_bounds__(1024, 1) k_resident_any(const ResArgs A)
     R.thr = thr; R.LTS = LTS; R.nT = nT;
     R.z0 = P.z[0]; R.z1 = P.z[1]; R.z2 = P.z[2];
     rank_ctx_key(R, A.K, bucket);
+    if (NC == 4) {
+        R.z0 = P.zF[14]; R.z1 = P.zF[15]; R.z2 = P.zF[16]; R.z3 = P.zF[17]; R.h = P.h;
+        R.bucket0 = reinterpret_cast<const char *>(bucket) - 32 * (ptrdiff_t)A.K.key_lo;
+    }
     const uint32_t gw = P.w0 + (uint32_t)w;
     const PhiloxQuad PQ = philox_quad_init((uint32_t)q, gw, A.rk);
     cg::cluster_group cl = cg::this_cluster();
     __syncthreads();
-    for (int kl = tid >> 5; kl < nk; kl += NT >> 5) build_mt(mt + (size_t)kl * MTS, lt + kl * LTS, trip, nT, lane);
+    for (int kl = tid >> 5; kl < nk; kl += NT >> 5) (NC == 4 ? build_mt4 : build_mt)(mt + (size_t)kl * MTS, lt + kl * LTS, trip, nT, lane);
     if (C > 1) cl.sync(); else __syncthreads();   // every block's shared memory is initialised
 
     uint32_t nswap = A.nswap0;
@@ -165,7 +175,7 @@ __global__ void __launch_bounds__(1024, 1) k_resident_any(const ResArgs A)
         for (int kl = sg; kl < nk; kl += G) {
             if (!live) continue;
             const uint4 rnd = philox_quad(PQ, g, (uint32_t)(k0 + kl), A.rk);
-            update_site_any<FAST, false>(sp + (size_t)kl * N, js, nb, lt + kl * LTS, mt + (size_t)kl * MTS, R, 0, j, Nh, N, pick(rnd, j & 3), fin);
+            update_site_any<FAST, false, NC>(sp + (size_t)kl * N, js, nb, lt + kl * LTS, mt + (size_t)kl * MTS, R, 0, j, Nh, N, pick(rnd, j & 3), fin);
         }
         __syncthreads();
         // ---------------- parity 1 (+ satisfied-bond count of the finished sweep)
@@ -173,37 +183,50 @@ __global__ void __launch_bounds__(1024, 1) k_resident_any(const ResArgs A)
             for (int kl = sg; kl < nk; kl += G) {
                 if (!live) continue;
                 const uint4 rnd = philox_quad(PQ, g, (1u << 16) | (uint32_t)(k0 + kl), A.rk);
-                update_site_any<FAST, false>(sp + (size_t)kl * N, js, nb, lt + kl * LTS, mt + (size_t)kl * MTS, R, 1, j, Nh, N, pick(rnd, j & 3), fin);
+                update_site_any<FAST, false, NC>(sp + (size_t)kl * N, js, nb, lt + kl * LTS, mt + (size_t)kl * MTS, R, 1, j, Nh, N, pick(rnd, j & 3), fin);
             }
             __syncthreads();
             continue;
         }
         for (int kb = sg; kb < S; kb += 4 * G) {     // batches of four slots: kb, kb+G, kb+2G, kb+3G
-            uint32_t en[4][3];
+            constexpr int NPE = NC == 4 ? 4 : 3;
+            uint32_t en[4][NPE];
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
                 const int kl = kb + i * G;
                 if (kl < nk && live) {
                     const uint4 rnd = philox_quad(PQ, g, (1u << 16) | (uint32_t)(k0 + kl), A.rk);
-                    update_site_any<FAST, true>(sp + (size_t)kl * N, js, nb, lt + kl * LTS, mt + (size_t)kl * MTS, R, 1, j, Nh, N, pick(rnd, j & 3), fin);
-                    en[i][0] = fin.b0; en[i][1] = fin.b1; en[i][2] = fin.b2;
+                    update_site_any<FAST, true, NC>(sp + (size_t)kl * N, js, nb, lt + kl * LTS, mt + (size_t)kl * MTS, R, 1, j, Nh, N, pick(rnd, j & 3), fin);
+                    if constexpr (NC == 4) {
+                        // field: T = (satisfied bonds) + |h| (spins that pay the field energy) over my parity-1
+                        // site and the parity-0 site with the same index (each met once): E = (3 + |h|) N - 2 T
+                        const uint32_t inv = P.h > 0 ? 0xFFFFFFFFu : 0u;      // h > 0: down spins pay
+                        const uint32_t x1 = sp[(size_t)kl * N + Nh + j] ^ inv, x0 = sp[(size_t)kl * N + j] ^ inv;
+                        const uint32_t c0 = x0 ^ x1, c1 = x0 & x1;              // 0..2 paying spins
+                        const bool two = (P.h & 1) == 0;
+                        const uint32_t a3[3] = {fin.b0, fin.b1, fin.b2};
+                        const uint32_t b3[3] = {two ? 0u : c0, two ? c0 : c1, two ? c1 : 0u};
+                        vsum<3>(a3, b3, en[i]);
+                    } else {
+                        en[i][0] = fin.b0; en[i][1] = fin.b1; en[i][2] = fin.b2;
+                    }
                 } else {
 #pragma unroll
-                    for (int jj = 0; jj < 3; ++jj) en[i][jj] = 0;
+                    for (int jj = 0; jj < NPE; ++jj) en[i][jj] = 0;
                 }
             }
-            uint32_t tot[8];
-            warp_sum4_t<3>(en, lane, tot);
+            uint32_t tot[NPE + 5];
+            warp_sum4_t<NPE>(en, lane, tot);
             const int i_mine = 2 * (lane >> 4) + ((lane >> 3) & 1);
             const int kl = kb + i_mine * G;
-            if (kl < nk) add_counts_t<8>(tot, lane & 7, Eacc + kl * 32);
+            if (kl < nk) add_counts_t<NPE + 5>(tot, lane & 7, Eacc + kl * 32);
         }
         __syncthreads();
         // ---- energies of my slots: E = 3N - 2 (satisfied bonds); pushed into every block of
         //      the cluster (distributed shared memory), buffer chosen by the swap-round parity
         int16_t *Ebuf = Eall + (nswap & 1u) * nT * 32;
         for (int a = tid; a < nk * 32; a += NT) {
-            const int e = 3 * N - 2 * Eacc[a];
+            const int e = (3 + (NC == 4 ? abs(P.h) : 0)) * N - 2 * Eacc[a];
             Eacc[a] = 0;
             const int dst = k0 * 32 + a;
             if (C > 1) {
@@ -220,7 +243,7 @@ __global__ void __launch_bounds__(1024, 1) k_resident_any(const ResArgs A)
         for (int t = (int)(nswap & 1u) + 2 * warp; t + 1 < nT; t += 2 * nwarp) {
             uint8_t *sg_ = sig8 + lane * nT, *ta_ = tau8 + lane * nT;
             const int sa = sg_[t], sb = sg_[t + 1];
-            const int m = ((int)Ebuf[sa * 32 + lane] - (int)Ebuf[sb * 32 + lane]) / 4;
+            const int m = ((int)Ebuf[sa * 32 + lane] - (int)Ebuf[sb * 32 + lane]) / (NC == 4 ? 2 : 4);
             const uint4 v = philox_rk(g, (uint32_t)t, P.r0 + (uint32_t)(32 * w + lane), 2u << 16, A.rk);
             const int lo = swm[4 * t], cnt = swm[4 * t + 1], kinds = swm[4 * t + 3];
             bool acc;
@@ -244,7 +267,7 @@ __global__ void __launch_bounds__(1024, 1) k_resident_any(const ResArgs A)
                 if (lane == (n & 31)) lt[kl * LTS + n] = mk;
             }
             __syncwarp();
-            build_mt(mt + (size_t)kl * MTS, lt + kl * LTS, trip, nT, lane);
+            (NC == 4 ? build_mt4 : build_mt)(mt + (size_t)kl * MTS, lt + kl * LTS, trip, nT, lane);
         }
         __syncthreads();
     }

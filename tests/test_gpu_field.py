@@ -43,7 +43,7 @@ def test_field_trajectory_matches_oracle(L, nT, R, h, swap, asc):
     o = Oracle(L, nT, R, betas, 19)
     g.set_field(h)
     o.set_field(h)
-    fast = abs(h) <= 2 and L in (8, 16)          # |h| <= 2 on the resident kernel's lattices, else the generic path
+    fast = abs(h) <= 2 and L <= 16               # |h| <= 2 on the resident kernels' lattices, else the generic path
     assert g.get_field() == h
     assert g.get_kernel() == (pkg.binding.EA_KERNEL_RESIDENT if fast else pkg.binding.EA_KERNEL_GENERIC)
     assert L < 32
@@ -73,6 +73,7 @@ def test_field_trajectory_matches_oracle(L, nT, R, h, swap, asc):
     (16, 24, 64, 1, 1, 6), (16, 24, 64, -1, 1, 6), (16, 7, 40, 2, 1, 5), (16, 12, 96, -2, 2, 7),
     (8, 16, 32, 1, 1, 12), (8, 16, 40, -2, 1, 12), (8, 5, 64, 2, 3, 9), (8, 2, 32, -1, 1, 8),
     (16, 24, 33, 1, 0, 4),
+    (12, 20, 64, 1, 2, 6), (12, 7, 33, -2, 1, 5), (4, 16, 40, 2, 1, 20), (6, 5, 70, -1, 1, 9), (2, 3, 5, 1, 1, 12),
 ])
 def test_field_on_the_resident_kernel_matches_oracle_and_the_generic_kernel(L, nT, R, h, swap, ns):
     """Field |h| <= 2 in the shared-memory-resident kernel (four threshold columns of the shifted
