@@ -27,7 +27,10 @@
  *                 <E>(T) with PT == without PT
  *   replica draws (eao_set_draw_mode 1, the paper's coding): beta = 0 complement, gauge
  *                 covariance, incremental == recomputed, 2^3 enumeration with and without PT,
- *                 composition, independence of realizations (tests/test_oracle_replica.py)
+ *                 composition, independence of realizations (tests/test_oracle_replica.py / test_oracle_couplings.py)
+ *   bond concentration (eao_seed_couplings): p = 0, 1 closed forms, bond and frustrated-plaquette
+ *                 fractions against p and (1 - (2p-1)^4)/2, independent Python Philox
+ *                 (tests/test_oracle_replica.py / test_oracle_couplings.py)
  *   field h     : flip-and-recompute dE, incremental == recomputed, exact
  *                 (s -> -s, h -> -h) symmetry, Boltzmann stationarity on the
  *                 2^3 lattice, saturation at large |h| (tests/test_oracle_field.py)
@@ -301,6 +304,29 @@ int eao_set_couplings(eao *o, const int8_t *J)
         for (int d = 0; d < 3; ++d)
             for (int i = 0; i < o->N; ++i)
                 J_(o, d, i, r) = J[((size_t)r * 3 + d) * o->N + i];
+    recompute_all_energies(o);
+    return 0;
+}
+
+/* Other bimodal coupling distributions ("other distributions of the couplings";
+ * PAPER.md:44 fixes only the mean): the +-J model with bond concentration p_plus = P(J = +1),
+ * each bond independently (R25).  p_plus = 1/2 is the paper's distribution in law (not
+ * the same sample as the default seeding), 1 the ferromagnet, 0 the antiferromagnet.
+ *   J_d(i) of realization r = +1  iff  PX(0, i, r0 + r, (5<<16)|d)[0] < floor(2^32 p_plus)
+ * (64-bit compare, so p_plus = 1 gives +1 everywhere).  Spins, permutation, counters are kept;
+ * energies are recomputed. */
+int eao_seed_couplings(eao *o, double p_plus)
+{
+    if (!(p_plus >= 0.0 && p_plus <= 1.0)) return -1;
+    uint64_t thr = (uint64_t)floor(ldexp(p_plus, 32));
+    uint32_t out[4];
+    for (int r = 0; r < o->R; ++r)
+        for (int d = 0; d < 3; ++d)
+            for (int i = 0; i < o->N; ++i) {
+                eao_philox4x32_10(0u, (uint32_t)i, (uint32_t)(o->r0 + r), (5u << 16) | (uint32_t)d,
+                                  o->k0, o->k1, out);
+                J_(o, d, i, r) = (uint64_t)out[0] < thr ? 1 : -1;
+            }
     recompute_all_energies(o);
     return 0;
 }

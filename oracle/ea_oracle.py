@@ -69,6 +69,8 @@ def _load():
     lib.eao_set_state.argtypes = [vp, vp, vp, u64, u64]
     lib.eao_set_field.restype = i32
     lib.eao_set_field.argtypes = [vp, i32]
+    lib.eao_seed_couplings.restype = i32
+    lib.eao_seed_couplings.argtypes = [vp, C.c_double]
     lib.eao_set_draw_mode.restype = i32
     lib.eao_set_draw_mode.argtypes = [vp, i32]
     lib.eao_get_draw_mode.restype = i32
@@ -148,6 +150,11 @@ class Oracle:
         rc = self.lib.eao_set_state(self.h, _ptr(s), _ptr(t), int(sweeps), int(swap_rounds))
         if rc != 0:
             raise ValueError(f"eao_set_state -> {rc}")
+
+    def seed_couplings(self, p_plus):
+        """+-J couplings with bond concentration p_plus = P(J = +1), from the Philox seed (R25)."""
+        if self.lib.eao_seed_couplings(self.h, float(p_plus)) != 0:
+            raise ValueError("p_plus must lie in [0, 1]")
 
     def set_draw_mode(self, mode):
         """0: one draw per (site, word, slot) (default); 1: one per (site, realization, slot) --
