@@ -248,6 +248,13 @@ int ea_get_field(ea_handle *h);
 int ea_get_field_tables(ea_handle *h, uint64_t *accf /* [n_temps][7][2] */,
                         uint64_t *swpf /* [n_temps-1][2 (3+|h|) N + 1] */);
 
+/* Other bimodal coupling distributions (R25):
+ * replace the couplings by +-J bonds with concentration p_plus = P(J = +1), 0 <= p_plus <= 1,
+ * drawn independently per bond from the handle's seed (p_plus = 1: ferromagnet, as used for the
+ * Ising check of PAPER.md:329).  Spins, permutation and counters are kept, energies recomputed.
+ * Any other +-1 disorder can be given explicitly with ea_set_couplings. */
+int ea_seed_couplings(ea_handle *h, double p_plus);
+
 /* Switch the multispin coding of the handle (EA_LAYOUT_*).  The physical state (spins, couplings,
  * permutation, energies, counters) is kept: only the random numbers consumed by later sweeps
  * follow the other convention, so ea_set_layout is normally called right after ea_create.

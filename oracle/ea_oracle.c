@@ -27,10 +27,10 @@
  *                 <E>(T) with PT == without PT
  *   replica draws (eao_set_draw_mode 1, the paper's coding): beta = 0 complement, gauge
  *                 covariance, incremental == recomputed, 2^3 enumeration with and without PT,
- *                 composition, independence of realizations (tests/test_oracle_replica.py / test_oracle_couplings.py)
+ *                 composition, independence of realizations (tests/test_oracle_replica.py)
  *   bond concentration (eao_seed_couplings): p = 0, 1 closed forms, bond and frustrated-plaquette
  *                 fractions against p and (1 - (2p-1)^4)/2, independent Python Philox
- *                 (tests/test_oracle_replica.py / test_oracle_couplings.py)
+ *                 (tests/test_oracle_couplings.py)
  *   field h     : flip-and-recompute dE, incremental == recomputed, exact
  *                 (s -> -s, h -> -h) symmetry, Boltzmann stationarity on the
  *                 2^3 lattice, saturation at large |h| (tests/test_oracle_field.py)

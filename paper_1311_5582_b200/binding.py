@@ -22,7 +22,7 @@ _SYMBOLS = [
     "ea_get_couplings", "ea_pair_couplings", "ea_measure_begin", "ea_measure", "ea_get_moments",
     "ea_get_binder", "ea_set_field", "ea_get_field", "ea_get_field_tables",
     "ea_get_round_trips", "ea_get_correlation", "ea_get_correlation_length", "ea_set_state",
-    "ea_set_layout", "ea_get_layout",
+    "ea_set_layout", "ea_get_layout", "ea_seed_couplings",
 ]
 
 
@@ -74,6 +74,8 @@ def lib():
         f = getattr(l, name)
         f.restype = i32
         f.argtypes = args
+    l.ea_seed_couplings.restype = i32
+    l.ea_seed_couplings.argtypes = [vp, C.c_double]
     l.ea_set_state.restype = i32
     l.ea_set_state.argtypes = [vp, vp, vp, u64, u64]
     l.ea_launch_count.restype = i64
@@ -263,6 +265,9 @@ class EA:
 
     def get_kernel(self):
         return int(self._l.ea_get_kernel(self.h))
+
+    def seed_couplings(self, p_plus):
+        self._chk(self._l.ea_seed_couplings(self.h, float(p_plus)))
 
     def set_layout(self, layout):
         self._chk(self._l.ea_set_layout(self.h, int(layout)))

@@ -27,6 +27,25 @@ __global__ void k_seed(Params P)
     }
 }
 
+// +-J couplings with bond concentration p (ea_seed_couplings, R25): bit b of coupling word
+// (d, i, w) = [PX(0, i, r, (5<<16)|d)[0] < thr], r = global realization 32 w + b, thr = floor(2^32 p)
+// (64-bit compare: p = 1 sets every bit).  One thread per (w, d, canonical site i), 32 draws each.
+__global__ void k_seed_couplings(Params P, unsigned long long thr)
+{
+    const int64_t tid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (tid >= (int64_t)P.W * 3 * P.N) return;
+    const int i = (int)(tid % P.N), d = (int)((tid / P.N) % 3), w = (int)(tid / ((int64_t)3 * P.N));
+    const int x = i % P.L, y = (i / P.L) % P.L, z = i / (P.L * P.L);
+    const int p = (x + y + z) & 1;
+    const int j = (x >> 1) + P.Lh * (y + P.L * z);
+    uint32_t word = 0;
+    for (int b = 0; b < 32; ++b) {
+        const uint4 c = philox4x32_10(0u, (uint32_t)i, P.r0 + (uint32_t)(32 * w + b), (5u << 16) | (uint32_t)d, P.k0, P.k1);
+        word |= (uint32_t)((unsigned long long)c.x < thr) << b;
+    }
+    P.coup[(size_t)w * 3 * P.N + (size_t)d * P.N + p * P.Nh + j] = word;
+}
+
 __global__ void k_identity_perm(Params P)
 {
     const int tid = blockIdx.x * blockDim.x + threadIdx.x;

@@ -1469,6 +1469,20 @@ extern "C" int ea_get_couplings(ea_handle *h, int8_t *J)
     return EA_OK;
 }
 
+extern "C" int ea_seed_couplings(ea_handle *h, double p_plus)
+{
+    if (!h || !(p_plus >= 0.0 && p_plus <= 1.0)) return fail(h, EA_ERR_INVALID_ARG, "ea_seed_couplings: p_plus must lie in [0, 1]");
+    { int rc = ensure_r(h); if (rc != EA_OK) return rc; }
+    h->t_valid = false;
+    const unsigned long long thr = (unsigned long long)std::floor(std::ldexp(p_plus, 32));
+    int grid;
+    launch_cfg((int64_t)h->W * 3 * h->N, 128, grid);
+    ea::k_seed_couplings<<<grid, 128, 0, h->stream>>>(h->P, thr);
+    h->launches++;
+    CUDA_TRY(h, cudaGetLastError());
+    return recompute_energy(h);
+}
+
 extern "C" int ea_pair_couplings(ea_handle *h)
 {
     if (!h) return EA_ERR_INVALID_ARG;

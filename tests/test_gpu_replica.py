@@ -89,3 +89,21 @@ def test_unsupported_combinations_are_refused():
     with pytest.raises(EAError):
         g.set_kernel(1)
     g.destroy()
+
+
+@pytest.mark.parametrize("L,nT,R,p,layout", [(4, 6, 40, 0.3, 0), (8, 8, 33, 0.9, 0), (16, 5, 64, 0.5, 0), (32, 3, 32, 0.75, 0),
+                                             (12, 4, 7, 1.0, 0), (6, 6, 5, 0.2, 1)])
+def test_seeded_bond_concentration_matches_oracle(L, nT, R, p, layout):
+    """+-J couplings with bond concentration p (ea_seed_couplings, R25) are the
+    oracle's bit for bit, on a sharded handle too, and the trajectories that follow agree."""
+    from paper_1311_5582_b200 import EA
+    betas = 1.0 / temperature_ladder(nT, 0.7, 2.2)
+    g = EA(L, nT, R, betas, 41, first_realization=64)
+    o = Oracle(L, nT, R, betas, 41, r0=64)
+    g.set_layout(layout); o.set_draw_mode(layout)
+    g.seed_couplings(p); o.seed_couplings(p)
+    assert (g.get_couplings() == o.couplings()).all()
+    _same(g, o, L, R)
+    g.sweep(6, 1); o.sweep(6, 1)
+    _same(g, o, L, R)
+    g.destroy()
