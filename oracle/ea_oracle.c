@@ -31,6 +31,9 @@
  *   bond concentration (eao_seed_couplings): p = 0, 1 closed forms, bond and frustrated-plaquette
  *                 fractions against p and (1 - (2p-1)^4)/2, independent Python Philox
  *                 (tests/test_oracle_couplings.py)
+ *   moving swaps (eao_set_swap_mode 1): beta = 0 closed form of the slot permutation, agreement with
+ *                 the index-permuting mode through the first swap round, multiset conservation,
+ *                 2^3 enumeration (tests/test_oracle_swapmove.py)
  *   field h     : flip-and-recompute dE, incremental == recomputed, exact
  *                 (s -> -s, h -> -h) symmetry, Boltzmann stationarity on the
  *                 2^3 lattice, saturation at large |h| (tests/test_oracle_field.py)
@@ -88,6 +91,9 @@ typedef struct eao {
     int draw_mode;       /* 0: one draw per (site, word, slot) shared by the word's 32 realizations (R11);
                             1: one draw per (site, realization, slot) -- the paper's own coding, in which the
                             bits of a word are the temperature replicas of one realization (eao_set_draw_mode) */
+    int swap_mode;       /* 0: an accepted swap exchanges temperature indices, lattices stay (north_star);
+                            1: it exchanges the two lattices, temperatures stay with their slots -- the
+                            data-moving swap of the paper's discussion, R26 */
     int check;           /* recompute-and-compare energies every sweep */
     int64_t check_failures;
     int64_t n_attempt, n_accept, n_swap_attempt, n_swap_accept;
@@ -448,6 +454,15 @@ int eao_set_draw_mode(eao *o, int mode)
 }
 int eao_get_draw_mode(const eao *o) { return o->draw_mode; }
 
+/* 0: swaps permute temperature indices; 1: swaps move the lattices (R26). */
+int eao_set_swap_mode(eao *o, int mode)
+{
+    if (mode != 0 && mode != 1) return -1;
+    o->swap_mode = mode;
+    return 0;
+}
+int eao_get_swap_mode(const eao *o) { return o->swap_mode; }
+
 /* One parallel-tempering round (temperatures
  * (table rows) are exchanged, lattices stay where they are).  Round n pairs
  * temperature indices (t, t+1) for t = n&1, n&1 + 2, ... (R4);
@@ -474,9 +489,17 @@ static void swap_round(eao *o, uint64_t g_done)
                 int64_t Mf = (int64_t)(3 + abs(o->h)) * o->N;
                 thr = o->swpf[(size_t)t * (size_t)(2 * Mf + 1) + (size_t)(dE / 2 + Mf)];
             }
-            if (v < thr) {
+            if (v < thr && o->swap_mode == 0) {
                 sg[t] = b; sg[t + 1] = a;
                 ta[a] = t + 1; ta[b] = t;
+                o->n_swap_accept++;
+            } else if (v < thr) {        /* R26: the configurations change places, tau stays as it is */
+                for (int i = 0; i < o->N; ++i) {
+                    int8_t x = S_(o, a, i, r);
+                    S_(o, a, i, r) = S_(o, b, i, r);
+                    S_(o, b, i, r) = x;
+                }
+                int32_t e = E[a]; E[a] = E[b]; E[b] = e;
                 o->n_swap_accept++;
             }
         }

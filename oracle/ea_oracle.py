@@ -75,6 +75,10 @@ def _load():
     lib.eao_set_draw_mode.argtypes = [vp, i32]
     lib.eao_get_draw_mode.restype = i32
     lib.eao_get_draw_mode.argtypes = [vp]
+    lib.eao_set_swap_mode.restype = i32
+    lib.eao_set_swap_mode.argtypes = [vp, i32]
+    lib.eao_get_swap_mode.restype = i32
+    lib.eao_get_swap_mode.argtypes = [vp]
     lib.eao_get_field.restype = i32
     lib.eao_get_field.argtypes = [vp]
     lib.eao_get_field_tables.restype = i32
@@ -164,6 +168,15 @@ class Oracle:
 
     def draw_mode(self) -> int:
         return int(self.lib.eao_get_draw_mode(self.h))
+
+    def set_swap_mode(self, mode):
+        """0: an accepted swap exchanges temperature indices (default); 1: it exchanges the two
+        lattices and their energies, temperatures stay with the slots (R26)."""
+        if self.lib.eao_set_swap_mode(self.h, int(mode)) != 0:
+            raise ValueError("swap mode must be 0 or 1")
+
+    def swap_mode(self) -> int:
+        return int(self.lib.eao_get_swap_mode(self.h))
 
     def set_field(self, h):
         """Constant external field h of Eq. 1 (integer); energies are recomputed."""
