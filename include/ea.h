@@ -264,6 +264,21 @@ int ea_seed_couplings(ea_handle *h, double p_plus);
 int ea_set_layout(ea_handle *h, int layout);
 int ea_get_layout(ea_handle *h);
 
+/* What an accepted parallel-tempering swap exchanges.  EA_SWAP_PERMUTE (default, north_star): the
+ * temperature indices of the two slots; lattices stay ("swap rows, not lattices").
+ * EA_SWAP_MOVE: the two lattices (per realization: the masked bits of every word of the two slots)
+ * and their energies; slot k keeps temperature index k for every realization, so the 32 realizations
+ * of a word are always at the same temperature.  The draws keep their counters (flip: by slot;
+ * swap: by temperature pair), which makes MOVE a different, equally valid, Markov chain: its oracle
+ * is the oracle's swap mode 1 (R26).  Allowed only while the permutation is the identity
+ * (before the first swap round, or after ea_set_state with identity temp_of_slot) and in the
+ * REALIZATION_BITS layout: else EA_ERR_UNSUPPORTED and nothing changes.  ea_get_round_trips counts
+ * movements of temperature indices and therefore stays at zero in MOVE mode. */
+#define EA_SWAP_PERMUTE 0
+#define EA_SWAP_MOVE 1
+int ea_set_swap_mode(ea_handle *h, int mode);
+int ea_get_swap_mode(ea_handle *h);
+
 /* Select the sweep implementation (EA_KERNEL_*); EA_ERR_UNSUPPORTED if it cannot run this shape. */
 int ea_set_kernel(ea_handle *h, int kernel);
 /* The implementation ea_sweep would use now (EA_KERNEL_GENERIC/RESIDENT/TILED/STREAM). */

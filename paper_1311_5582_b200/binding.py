@@ -13,6 +13,7 @@ _lib = None
 EA_KERNEL_AUTO, EA_KERNEL_GENERIC, EA_KERNEL_RESIDENT, EA_KERNEL_TILED, EA_KERNEL_STREAM, EA_KERNEL_REPLICA = 0, 1, 2, 3, 4, 5
 EA_KERNEL_GENERIC_STEPWISE = 6
 EA_LAYOUT_REALIZATION_BITS, EA_LAYOUT_REPLICA_BITS = 0, 1
+EA_SWAP_PERMUTE, EA_SWAP_MOVE = 0, 1
 
 _SYMBOLS = [
     "ea_create", "ea_workspace_bytes", "ea_create_ex", "ea_destroy", "ea_set_couplings",
@@ -22,7 +23,7 @@ _SYMBOLS = [
     "ea_get_couplings", "ea_pair_couplings", "ea_measure_begin", "ea_measure", "ea_get_moments",
     "ea_get_binder", "ea_set_field", "ea_get_field", "ea_get_field_tables",
     "ea_get_round_trips", "ea_get_correlation", "ea_get_correlation_length", "ea_set_state",
-    "ea_set_layout", "ea_get_layout", "ea_seed_couplings",
+    "ea_set_layout", "ea_get_layout", "ea_seed_couplings", "ea_set_swap_mode", "ea_get_swap_mode",
 ]
 
 
@@ -70,7 +71,8 @@ def lib():
                        ("ea_set_field", [vp, i32]), ("ea_get_field", [vp]),
                        ("ea_get_field_tables", [vp, vp, vp]), ("ea_get_round_trips", [vp, vp]),
                        ("ea_get_correlation", [vp, vp]), ("ea_get_correlation_length", [vp, vp]),
-                       ("ea_set_layout", [vp, i32]), ("ea_get_layout", [vp])):
+                       ("ea_set_layout", [vp, i32]), ("ea_get_layout", [vp]),
+                       ("ea_set_swap_mode", [vp, i32]), ("ea_get_swap_mode", [vp])):
         f = getattr(l, name)
         f.restype = i32
         f.argtypes = args
@@ -274,6 +276,12 @@ class EA:
 
     def get_layout(self):
         return int(self._l.ea_get_layout(self.h))
+
+    def set_swap_mode(self, mode):
+        self._chk(self._l.ea_set_swap_mode(self.h, int(mode)))
+
+    def get_swap_mode(self):
+        return int(self._l.ea_get_swap_mode(self.h))
 
     def launch_count(self):
         return int(self._l.ea_launch_count(self.h))

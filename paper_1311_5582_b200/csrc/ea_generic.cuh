@@ -329,6 +329,39 @@ __global__ void __launch_bounds__(256) k_pt_swap(Params P, uint32_t g_done, uint
     pt_swap_word(P, blockIdx.x, g_done, round);
 }
 
+// Data-moving swap (ea_set_swap_mode, R26): block = (word, pair of this round).  Warp 0
+// takes the 32 decisions of the word (lane = realization), the ballot is the exchange mask, then the
+// whole block exchanges the masked bits of the two lattices: x = (a ^ b) & m, a ^= x, b ^= x.
+// tau stays the identity, so the rank masks never change.
+__global__ void __launch_bounds__(256) k_swap_move(Params P, uint32_t g_done, uint32_t round)
+{
+    __shared__ uint32_t s_mask;
+    const int w = blockIdx.x, t = (int)(round & 1u) + 2 * (int)blockIdx.y;
+    if (t + 1 >= P.nT) return;
+    if (threadIdx.x < 32) {
+        const int lane = threadIdx.x, r = 32 * w + lane;
+        int32_t *E = P.E + (size_t)r * P.nT;
+        const int ea = E[t], eb = E[t + 1];
+        const uint4 v = philox4x32_10(g_done, (uint32_t)t, P.r0 + (uint32_t)r, 2u << 16, P.k0, P.k1);
+        const bool acc = swap_accept(P, t, (ea - eb) / P.ediv, v.x);
+        if (acc) { E[t] = eb; E[t + 1] = ea; }
+        const uint32_t m = __ballot_sync(0xFFFFFFFFu, acc);
+        if (lane == 0) s_mask = m;
+    }
+    __syncthreads();
+    const uint32_t m = s_mask;
+    if (m == 0u) return;
+    uint4 *A = reinterpret_cast<uint4 *>(P.spin + ((size_t)t * P.W + w) * P.N);
+    uint4 *B = reinterpret_cast<uint4 *>(P.spin + ((size_t)(t + 1) * P.W + w) * P.N);
+    for (int i = threadIdx.x; i < P.N / 4; i += blockDim.x) {
+        uint4 a = A[i], b = B[i];
+        const uint4 x = make_uint4((a.x ^ b.x) & m, (a.y ^ b.y) & m, (a.z ^ b.z) & m, (a.w ^ b.w) & m);
+        a.x ^= x.x; a.y ^= x.y; a.z ^= x.z; a.w ^= x.w;
+        b.x ^= x.x; b.y ^= x.y; b.z ^= x.z; b.w ^= x.w;
+        A[i] = a; B[i] = b;
+    }
+}
+
 // ------------------------------------------------------------------ persistent generic path
 // All sweeps of a call in ONE cooperative launch for lattices that have no shared-memory path
 // (L = 2, 4, 6, 12, ... and every L with a field): the same work items as the kernels above,

@@ -48,6 +48,7 @@ struct ea_handle {
     uint64_t g = 0, nswap = 0;
     bool energy_valid = false;
     int kernel_sel = EA_KERNEL_AUTO;
+    int swap_mode = EA_SWAP_PERMUTE;   // ea_set_swap_mode
     bool poisoned = false;             // a launch failed between the word groups of one ea_sweep call: the words
                                        // are no longer at the same sweep; ea_set_state brings the handle back
     int64_t launches = 0;
@@ -1276,6 +1277,8 @@ extern "C" int ea_set_layout(ea_handle *h, int layout)
     if (!h || (layout != EA_LAYOUT_REALIZATION_BITS && layout != EA_LAYOUT_REPLICA_BITS))
         return fail(h, EA_ERR_INVALID_ARG, "ea_set_layout: bad argument");
     if (layout == h->layout) return EA_OK;
+    if (h->swap_mode != EA_SWAP_PERMUTE)
+        return fail(h, EA_ERR_UNSUPPORTED, "ea_set_layout: the replica-bits layout has no moving swaps (ea_set_swap_mode)");
     if (layout == EA_LAYOUT_REALIZATION_BITS) {
         { int rc = ensure_r(h); if (rc != EA_OK) return rc; }
         h->layout = layout;
@@ -1362,18 +1365,60 @@ extern "C" int ea_set_kernel(ea_handle *h, int kernel)
 }
 extern "C" int ea_get_kernel(ea_handle *h) { return h ? pick_kernel(h) : EA_ERR_INVALID_ARG; }
 
+static int sweep_dispatch(ea_handle *h, int64_t n_sweeps, int swap_interval)
+{
+    const int k = pick_kernel(h);
+    if (k == EA_KERNEL_REPLICA) return sweep_replica(h, n_sweeps, swap_interval);
+    if (k == EA_KERNEL_RESIDENT) return sweep_resident(h, n_sweeps, swap_interval);
+    if (k == EA_KERNEL_TILED) return sweep_tiled(h, n_sweeps, swap_interval);
+    if (k == EA_KERNEL_STREAM) return sweep_stream(h, n_sweeps, swap_interval);
+    return sweep_generic(h, n_sweeps, swap_interval);
+}
+
 extern "C" int ea_sweep(ea_handle *h, int64_t n_sweeps, int swap_interval)
 {
     if (!h || n_sweeps < 0 || swap_interval < 0) return fail(h, EA_ERR_INVALID_ARG, "ea_sweep: bad argument");
     if (h->g + (uint64_t)n_sweeps > 0xFFFFFFFFull) return fail(h, EA_ERR_RANGE, "ea_sweep: sweep counter would pass 2^32-1");
     if (n_sweeps == 0) return EA_OK;
     if (h->poisoned) return fail(h, EA_ERR_CUDA, "ea_sweep: an earlier call failed between word groups; restore the state with ea_set_state");
-    if (pick_kernel(h) == EA_KERNEL_REPLICA) return sweep_replica(h, n_sweeps, swap_interval);
-    if (pick_kernel(h) == EA_KERNEL_RESIDENT) return sweep_resident(h, n_sweeps, swap_interval);
-    if (pick_kernel(h) == EA_KERNEL_TILED) return sweep_tiled(h, n_sweeps, swap_interval);
-    if (pick_kernel(h) == EA_KERNEL_STREAM) return sweep_stream(h, n_sweeps, swap_interval);
-    return sweep_generic(h, n_sweeps, swap_interval);
+    if (h->swap_mode == EA_SWAP_MOVE && swap_interval > 0) {
+        // sweeps up to the next swap point on the selected kernel (no swap inside), then the exchange
+        while (n_sweeps > 0) {
+            const int64_t chunk = std::min<int64_t>(n_sweeps, (int64_t)((uint64_t)swap_interval - h->g % (uint64_t)swap_interval));
+            int rc = sweep_dispatch(h, chunk, 0);
+            if (rc != EA_OK) return rc;
+            n_sweeps -= chunk;
+            if (h->g % (uint64_t)swap_interval != 0) continue;
+            if (!h->energy_valid && (rc = recompute_energy(h)) != EA_OK) return rc;
+            ea::k_swap_move<<<dim3((unsigned)h->W, (unsigned)(h->nT / 2)), 256, 0, h->stream>>>(
+                h->P, (uint32_t)(h->g - 1), (uint32_t)(h->nswap & 1u));
+            CUDA_TRY(h, cudaGetLastError());
+            h->launches++;
+            h->nswap++;
+        }
+        return EA_OK;
+    }
+    return sweep_dispatch(h, n_sweeps, swap_interval);
 }
+
+extern "C" int ea_set_swap_mode(ea_handle *h, int mode)
+{
+    if (!h || (mode != EA_SWAP_PERMUTE && mode != EA_SWAP_MOVE)) return fail(h, EA_ERR_INVALID_ARG, "ea_set_swap_mode: bad argument");
+    if (mode == h->swap_mode) return EA_OK;
+    if (h->layout != EA_LAYOUT_REALIZATION_BITS)
+        return fail(h, EA_ERR_UNSUPPORTED, "ea_set_swap_mode: only in the realization-bits layout");
+    if (h->nT < 2) return fail(h, EA_ERR_UNSUPPORTED, "ea_set_swap_mode: needs at least two temperatures");
+    // both directions need slot == temperature index for every realization (moving swaps keep it so)
+    std::vector<uint8_t> tau((size_t)h->Rp * h->nT);
+    CUDA_TRY(h, cudaMemcpyAsync(tau.data(), h->P.tau, tau.size(), cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    for (size_t a = 0; a < tau.size(); ++a)
+        if (tau[a] != (uint8_t)(a % (size_t)h->nT))
+            return fail(h, EA_ERR_UNSUPPORTED, "ea_set_swap_mode: the temperature permutation is not the identity (call it before the first swap round)");
+    h->swap_mode = mode;
+    return EA_OK;
+}
+extern "C" int ea_get_swap_mode(ea_handle *h) { return h ? h->swap_mode : EA_ERR_INVALID_ARG; }
 
 // ---------------------------------------------------------------- observables
 extern "C" int ea_energy(ea_handle *h, int32_t *E)
@@ -1712,6 +1757,8 @@ extern "C" int ea_set_state(ea_handle *h, const uint32_t *spin_words, const uint
             const int t = r < h->R ? temp_of_slot[(size_t)r * nT + k] : k;   // padding realizations: identity
             if (t >= nT || ((seen >> t) & 1u))
                 return fail(h, EA_ERR_INVALID_ARG, "ea_set_state: temp_of_slot is not a permutation");
+            if (h->swap_mode == EA_SWAP_MOVE && t != k)
+                return fail(h, EA_ERR_INVALID_ARG, "ea_set_state: with moving swaps temp_of_slot must be the identity");
             seen |= (uint64_t)1 << t;
             tau[(size_t)r * nT + k] = (uint8_t)t;
         }
