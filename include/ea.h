@@ -141,6 +141,23 @@ int ea_energy(ea_handle *h, int32_t *E /* [R][n_temps] */);
 int ea_overlap(ea_handle *h, const int32_t *pairs /* [n_pairs][2] */, int n_pairs,
                int32_t *Q /* [n_pairs][n_temps] */);
 
+/* ea_overlap for callers that must not allocate (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc): same arguments (host pointers), same results, but the
+ * device copies of pairs and Q live in ONE file-scope device array of the library instead of the
+ * handle's growing scratch buffer, and the call makes no cudaMalloc / cudaFree / allocating library
+ * call.  The array holds EA_OVERLAP_STATIC_MAX_INT32 32-bit words (256 KiB, held by every GPU that
+ * loads the library until the process exits); n_pairs * (2 + n_temps) beyond that: EA_ERR_RANGE, and
+ * nothing is launched.  Its address is resolved once per device (cudaGetSymbolAddress, with that
+ * device current -- the device of the handle must be current, as for every call).  ALL handles and
+ * ALL calls on a device share the array and it keeps the last call's contents (nothing in it needs
+ * to start at zero: every element read back is written by the call): calls that overlap on the GPU
+ * -- two host threads, two streams -- race; a call returns after its stream has drained, so calls
+ * made one after the other from one thread are safe.  In the REPLICA_BITS layout the call may first
+ * launch the transposition to the exchange format, as ea_overlap does. */
+#define EA_OVERLAP_STATIC_MAX_INT32 65536
+int ea_overlap_static(ea_handle *h, const int32_t *pairs /* [n_pairs][2] */, int n_pairs,
+                      int32_t *Q /* [n_pairs][n_temps] */);
+
 /* s[r][t][site] = +-1 by temperature index. */
 int ea_get_spins(ea_handle *h, int8_t *s /* [R][n_temps][N] */);
 

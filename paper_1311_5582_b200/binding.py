@@ -24,6 +24,7 @@ _SYMBOLS = [
     "ea_get_binder", "ea_set_field", "ea_get_field", "ea_get_field_tables",
     "ea_get_round_trips", "ea_get_correlation", "ea_get_correlation_length", "ea_set_state",
     "ea_set_layout", "ea_get_layout", "ea_seed_couplings", "ea_set_swap_mode", "ea_get_swap_mode",
+    "ea_overlap_static",
 ]
 
 
@@ -63,6 +64,7 @@ def lib():
                        ("ea_set_tables", [vp, vp, vp]), ("ea_get_tables", [vp, vp, vp]),
                        ("ea_sweep", [vp, i64, i32]), ("ea_synchronize", [vp]),
                        ("ea_energy", [vp, vp]), ("ea_overlap", [vp, vp, i32, vp]),
+                       ("ea_overlap_static", [vp, vp, i32, vp]),
                        ("ea_get_spins", [vp, vp]), ("ea_get_state", [vp, vp, vp, vp, vp, vp]),
                        ("ea_set_kernel", [vp, i32]), ("ea_get_kernel", [vp]),
                        ("ea_get_couplings", [vp, vp]), ("ea_pair_couplings", [vp]),
@@ -178,6 +180,13 @@ class EA:
         pairs = np.ascontiguousarray(pairs, dtype=np.int32).reshape(-1, 2)
         Q = np.zeros((len(pairs), self.nT), dtype=np.int32)
         self._chk(self._l.ea_overlap(self.h, _p(pairs), len(pairs), _p(Q)))
+        return Q
+
+    def overlap_static(self, pairs):
+        """ea_overlap through the library's fixed device array: no allocation in the call (ea.h)."""
+        pairs = np.ascontiguousarray(pairs, dtype=np.int32).reshape(-1, 2)
+        Q = np.zeros((len(pairs), self.nT), dtype=np.int32)
+        self._chk(self._l.ea_overlap_static(self.h, _p(pairs), len(pairs), _p(Q)))
         return Q
 
     def get_spins(self):

@@ -8,6 +8,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -1458,6 +1459,66 @@ extern "C" int ea_overlap(ea_handle *h, const int32_t *pairs, int n_pairs, int32
     if (e == cudaSuccess) e = cudaMemcpyAsync(Q, d + 2 * (size_t)n_pairs, nb_q, cudaMemcpyDeviceToHost, h->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
     if (e != cudaSuccess) return fail(h, EA_ERR_CUDA, std::string("ea_overlap: ") + cudaGetErrorString(e));
+    return EA_OK;
+}
+
+// ---------------------------------------------------------------- ea_overlap without any allocation
+// Scratch of ea_overlap_static: pairs [n_pairs][2] followed by Q [n_pairs][n_temps], int32.  File-scope
+// device array: every GPU that loads the library holds these 256 KiB until the process exits.  In host
+// code the NAME below is only a stand-in of the host side; the device address comes from
+// cudaGetSymbolAddress, once per device, with that device current (overlap_static_ptr).
+static __device__ __align__(256) int32_t g_overlap_static[EA_OVERLAP_STATIC_MAX_INT32];
+
+namespace {
+constexpr int kMaxDev = 64;
+int32_t *g_overlap_static_ptr[kMaxDev] = {};       // by device ordinal; written once, under the lock
+std::mutex g_overlap_static_lock;
+}  // namespace
+
+static cudaError_t overlap_static_ptr(int32_t **out)
+{
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= kMaxDev) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> guard(g_overlap_static_lock);
+    if (!g_overlap_static_ptr[dev]) {
+        void *ptr = nullptr;
+        e = cudaGetSymbolAddress(&ptr, g_overlap_static);
+        if (e != cudaSuccess) return e;
+        g_overlap_static_ptr[dev] = (int32_t *)ptr;
+    }
+    if (out) *out = g_overlap_static_ptr[dev];
+    return cudaSuccess;
+}
+
+extern "C" int ea_overlap_static(ea_handle *h, const int32_t *pairs, int n_pairs, int32_t *Q)
+{
+    if (!h || n_pairs < 0 || (n_pairs && (!pairs || !Q))) return fail(h, EA_ERR_INVALID_ARG, "ea_overlap_static: bad argument");
+    for (int p = 0; p < n_pairs; ++p)
+        if (pairs[2 * p] < 0 || pairs[2 * p] >= h->R || pairs[2 * p + 1] < -1 || pairs[2 * p + 1] >= h->R)
+            return fail(h, EA_ERR_INVALID_ARG, "ea_overlap_static: realization index out of range");
+    if (n_pairs == 0) return EA_OK;
+    if ((int64_t)n_pairs * (2 + h->nT) > (int64_t)EA_OVERLAP_STATIC_MAX_INT32)
+        return fail(h, EA_ERR_RANGE, "ea_overlap_static: n_pairs * (2 + n_temps) = " + std::to_string((int64_t)n_pairs * (2 + h->nT)) +
+                                         " exceeds EA_OVERLAP_STATIC_MAX_INT32 = " + std::to_string(EA_OVERLAP_STATIC_MAX_INT32) +
+                                         " (split the pair list, or use ea_overlap)");
+    { int rc = ensure_r(h); if (rc != EA_OK) return rc; }
+    int32_t *d = nullptr;
+    cudaError_t e = overlap_static_ptr(&d);
+    if (e != cudaSuccess) return fail(h, EA_ERR_CUDA, std::string("ea_overlap_static: cudaGetSymbolAddress: ") + cudaGetErrorString(e));
+    const size_t nb_p = 8 * (size_t)n_pairs, nb_q = 4 * (size_t)n_pairs * h->nT;
+    // nothing in the array has to start at zero: the pairs are copied in, and every Q element read back
+    // below is written by exactly one block of this launch
+    e = cudaMemcpyAsync(d, pairs, nb_p, cudaMemcpyHostToDevice, h->stream);
+    if (e == cudaSuccess) {
+        ea::k_overlap<<<n_pairs * h->nT, 256, 0, h->stream>>>(h->P, d, d + 2 * (size_t)n_pairs);
+        h->launches++;
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaMemcpyAsync(Q, d + 2 * (size_t)n_pairs, nb_q, cudaMemcpyDeviceToHost, h->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+    if (e != cudaSuccess) return fail(h, EA_ERR_CUDA, std::string("ea_overlap_static: ") + cudaGetErrorString(e));
     return EA_OK;
 }
 
