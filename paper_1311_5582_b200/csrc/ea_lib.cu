@@ -1876,3 +1876,12 @@ extern "C" int ea_measure_int_peak(void *cuda_stream, double *out)
     cudaFree(d);
     return e == cudaSuccess ? EA_OK : EA_ERR_CUDA;
 }
+
+// examples/resident_phases.py: cycles per phase of k_resident summed by block 0 (reset != 0: clear)
+#ifdef EA_TRACE
+extern "C" int ea_debug_res_trace(unsigned long long *out, int reset)
+{
+    if (reset) { unsigned long long z[8] = {}; return (int)cudaMemcpyToSymbol(ea::g_res_trace, z, sizeof z); }
+    return (int)cudaMemcpyFromSymbol(out, ea::g_res_trace, 8 * sizeof(unsigned long long));
+}
+#endif

@@ -682,9 +682,22 @@ __device__ __forceinline__ void add_counts_t(const uint32_t (&tot)[NPL], int i, 
     atomicAdd(acc_row + i + 24, (int)(hi >> 16));
 }
 
+// Phase clocks of k_resident, only in the -DEA_TRACE build of examples/resident_phases.py (the product
+// library has none): thread 0 of block 0 adds the SM cycles between consecutive stamps of a sweep to
+// g_res_trace[phase]; ea_debug_res_trace (ea_lib.cu, same build only) reads and clears the sums.
+#ifdef EA_TRACE
+__device__ unsigned long long g_res_trace[8];
+#define RES_STAMP(i) do { if (threadIdx.x == 0 && blockIdx.x == 0) { const long long t_ = clock64(); g_res_trace[i] += (unsigned long long)(t_ - t_last); t_last = t_; } } while (0)
+#else
+#define RES_STAMP(i) do { } while (0)
+#endif
+
 template <int L, int G, bool FAST, int NC = 3>
 __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs A)
 {
+#ifdef EA_TRACE
+    long long t_last = clock64();
+#endif
     using Gm = ResGeom<L>;
     constexpr int N = Gm::N, NQ = Gm::NQ, QR = Gm::QR, NT = NQ * G;
     extern __shared__ __align__(16) uint32_t smem[];
@@ -806,6 +819,7 @@ __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs
             update_quad_off<L, FAST, false, true, NC>(sp + (size_t)kl * N, lt + kl * LTS, mt + (size_t)kl * MTS, R, J0, 0, s0, q, oyp, oym, ozp, ozm, rnd, fin);
         }
         __syncthreads();
+        RES_STAMP(0);
         // ---------------- parity 1 (+ satisfied-bond count of the finished sweep)
         if (!need_E) {
             for (int kl = sg; kl < nk; kl += G) {
@@ -814,6 +828,7 @@ __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs
                                                       oyp, oym, ozp, ozm, rnd, fin);
             }
             __syncthreads();
+            RES_STAMP(5);
             continue;
         }
         for (int kb = sg; kb < S; kb += 4 * G) {     // batches of four slots: kb, kb+G, kb+2G, kb+3G
@@ -857,6 +872,7 @@ __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs
             if (kl < nk) add_counts_t<NPE + 5>(tot, lane & 7, Eacc + kl * 32);
         }
         __syncthreads();
+        RES_STAMP(1);
         // ---- energies of my slots: E = 3N - 2 (satisfied bonds); pushed into every block of
         //      the cluster (distributed shared memory), buffer chosen by the swap-round parity
         int16_t *Ebuf = Eall + (nswap & 1u) * nT * 32;
@@ -872,6 +888,7 @@ __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs
         }
         if (!swap_now) { __syncthreads(); continue; }
         if (C > 1) { cluster_arrive(); cluster_wait(); } else __syncthreads();
+        RES_STAMP(2);
         // ---- swap round: warp per temperature pair, lane = realization.  Every block of the
         //      cluster computes all pairs of its word (identical results).
         const int warp = tid >> 5, nwarp = NT >> 5;
@@ -893,6 +910,7 @@ __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs
         }
         ++nswap;
         __syncthreads();
+        RES_STAMP(3);
         for (int kl = warp; kl < nk; kl += nwarp) {   // rank masks of my slots
             const int t = tau8[lane * nT + k0 + kl];
             const int pos = P.desc ? t : nT - 1 - t;
@@ -905,6 +923,7 @@ __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs
             (NC == 4 ? build_mt4 : build_mt)(mt + (size_t)kl * MTS, lt + kl * LTS, trip, nT, lane);
         }
         __syncthreads();
+        RES_STAMP(4);
     }
     // the energies written last are in the buffer selected by the final nswap parity... the
     // last sweep always computes them; which buffer depends on whether that sweep swapped
