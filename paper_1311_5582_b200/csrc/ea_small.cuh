@@ -236,39 +236,50 @@ __global__ void __launch_bounds__(1024, 1) k_resident_any(const ResArgs A)
             }
         }
         if (!swap_now) { __syncthreads(); continue; }
-        if (C > 1) { cluster_arrive(); cluster_wait(); } else __syncthreads();
         // ---- swap round: warp per temperature pair, lane = realization.  Every block of the
-        //      cluster computes all pairs of its word (identical results).
+        //      cluster computes all pairs of its word (identical results).  What does not depend on
+        //      the energies (the slots of the pair, the draw) is fetched while the barrier completes.
         const int warp = tid >> 5, nwarp = NT >> 5;
-        for (int t = (int)(nswap & 1u) + 2 * warp; t + 1 < nT; t += 2 * nwarp) {
-            uint8_t *sg_ = sig8 + lane * nT, *ta_ = tau8 + lane * nT;
-            const int sa = sg_[t], sb = sg_[t + 1];
+        const int t0 = (int)(nswap & 1u) + 2 * warp;
+        uint8_t *sg_ = sig8 + lane * nT, *ta_ = tau8 + lane * nT;
+        if (C > 1) cluster_arrive();
+        int sa0 = 0, sb0 = 0;
+        uint32_t v0 = 0;
+        if (t0 + 1 < nT) {
+            sa0 = sg_[t0]; sb0 = sg_[t0 + 1];
+            v0 = philox_rk(g, (uint32_t)t0, P.r0 + (uint32_t)(32 * w + lane), 2u << 16, A.rk).x;
+        }
+        if (C > 1) cluster_wait(); else __syncthreads();
+        for (int t = t0; t + 1 < nT; t += 2 * nwarp) {
+            int sa = sa0, sb = sb0;
+            uint32_t vx = v0;
+            if (t != t0) {
+                sa = sg_[t]; sb = sg_[t + 1];
+                vx = philox_rk(g, (uint32_t)t, P.r0 + (uint32_t)(32 * w + lane), 2u << 16, A.rk).x;
+            }
             const int m = ((int)Ebuf[sa * 32 + lane] - (int)Ebuf[sb * 32 + lane]) / (NC == 4 ? 2 : 4);
-            const uint4 v = philox_rk(g, (uint32_t)t, P.r0 + (uint32_t)(32 * w + lane), 2u << 16, A.rk);
             const int lo = swm[4 * t], cnt = swm[4 * t + 1], kinds = swm[4 * t + 3];
             bool acc;
             if (m < lo) acc = kinds & 1;
             else if (m >= lo + cnt) acc = (kinds >> 1) & 1;
-            else if (m >= -SW && m < 0) acc = v.x <= swwin[t * SW + m + SW];
-            else acc = v.x <= P.swp_val[swm[4 * t + 2] + (m - lo)];
+            else if (m >= -SW && m < 0) acc = vx <= swwin[t * SW + m + SW];
+            else acc = vx <= P.swp_val[swm[4 * t + 2] + (m - lo)];
             if (acc) {
                 sg_[t] = (uint8_t)sb; sg_[t + 1] = (uint8_t)sa;
                 ta_[sa] = (uint8_t)(t + 1); ta_[sb] = (uint8_t)t;
+                // rank masks: lt[slot][n] bit r = (pos_r >= n).  The position of a goes from p to p + 1
+                // and that of b from p + 1 to p (descending betas; the other way round for ascending),
+                // so exactly bit r of row rho toggles in both slots; row rho belongs to this pair alone
+                const int rho = P.desc ? t + 1 : nT - 1 - t;
+                const int la = sa - k0, lb = sb - k0;
+                if ((unsigned)la < (unsigned)nk) atomicXor(&lt[la * LTS + rho], 1u << lane);
+                if ((unsigned)lb < (unsigned)nk) atomicXor(&lt[lb * LTS + rho], 1u << lane);
             }
         }
         ++nswap;
         __syncthreads();
-        for (int kl = warp; kl < nk; kl += nwarp) {   // rank masks of my slots
-            const int t = tau8[lane * nT + k0 + kl];
-            const int pos = P.desc ? t : nT - 1 - t;
-#pragma unroll 8
-            for (int n = 0; n <= nT; ++n) {
-                const uint32_t mk = __ballot_sync(0xFFFFFFFFu, pos >= n);
-                if (lane == (n & 31)) lt[kl * LTS + n] = mk;
-            }
-            __syncwarp();
+        for (int kl = warp; kl < nk; kl += nwarp)     // mask tables of my slots from their rank masks
             (NC == 4 ? build_mt4 : build_mt)(mt + (size_t)kl * MTS, lt + kl * LTS, trip, nT, lane);
-        }
         __syncthreads();
     }
     // the energies written last are in the buffer selected by the final nswap parity... the
