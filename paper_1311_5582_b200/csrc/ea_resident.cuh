@@ -808,6 +808,7 @@ __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs
     if (C > 1) cl.sync(); else __syncthreads();   // every block's shared memory is initialised
 
     uint32_t nswap = A.nswap0;
+    RES_STAMP(6);                                 // prologue
     for (int it = 0; it < A.n_sweeps; ++it) {
         const uint32_t g = A.g0 + (uint32_t)it;
         const bool swap_now = A.swap_interval > 0 && ((uint64_t)g + 1) % (uint64_t)A.swap_interval == 0;
@@ -957,6 +958,7 @@ __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs
             P.sigma[(size_t)32 * w * nT + a] = sig8[a];
         }
     }
+    RES_STAMP(7);                                 // epilogue (issue of the write-back)
 }
 
 }  // namespace ea

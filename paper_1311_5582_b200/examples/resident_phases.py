@@ -58,6 +58,7 @@ def main():
     for n, v in zip(names, out[:6]):
         print(f"  {n:32s} {v / ns:9.1f}  {100 * v / tot:5.1f} %")
     print(f"  {'whole sweep':32s} {tot / ns:9.1f}")
+    print(f"  per launch: prologue (state and tables into shared memory) {out[6]} cycles, epilogue (write-back issued) {out[7]} cycles")
 
 
 if __name__ == "__main__":
