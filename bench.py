@@ -8,6 +8,7 @@ through the C ABI of libea_b200.so.
   python bench.py --impl reference ...      # the CPU oracle, as it stands, on the host cores
   python bench.py --field 1                 # the same workload with h = 1 (generic kernel)
   python bench.py --measure-every 10        # two-copy overlap/energy moments every 10 sweeps
+  python bench.py --swap-mode move                         # swaps that move the lattices
   python bench.py --layout replica --sweeps-per-step 200   # the paper's own coding (bits = temperature
                                             # replicas of one realization, one random number per replica)
 
@@ -325,7 +326,8 @@ def run_cuda(a, cfg):
     me = a.measure_every
     # the golden digests describe the BASELINE config itself, as rank 0 simulates it
     replica = a.layout == "replica"
-    plain = not (a.field or me or a.realizations is not None or a.swap_interval is not None or replica)
+    moving = a.swap_mode == "move"
+    plain = not (a.field or me or a.realizations is not None or a.swap_interval is not None or replica or moving)
 
     def make():
         # weak scaling: every rank owns cfg.R realizations; rank r simulates global words r*W..
@@ -335,6 +337,9 @@ def run_cuda(a, cfg):
         if replica:
             from paper_1311_5582_b200 import EA_LAYOUT_REPLICA_BITS
             sim.set_layout(EA_LAYOUT_REPLICA_BITS)
+        if moving:
+            from paper_1311_5582_b200 import EA_SWAP_MOVE
+            sim.set_swap_mode(EA_SWAP_MOVE)
         if me:
             # two copies of every disorder realization (words w and w + W/2), overlap and energy
             # moments accumulated on the device every `me` sweeps (ea_measure)
@@ -468,7 +473,7 @@ def run_cuda(a, cfg):
         "dtype": "u32 bit-sliced words (32 realizations each), u32 Philox draws", "data": "synthetic",
         "config": {"workload": cfg.name, "L": cfg.L, "n_temps": cfg.n_temps, "realizations_per_gpu": cfg.R,
                    "swap_interval": cfg.swap_interval, "sweeps_per_step": sps, "seed": cfg.seed,
-                   "field": a.field, "measure_every": me, "layout": a.layout,
+                   "field": a.field, "measure_every": me, "layout": a.layout, "swap_mode": a.swap_mode,
                    "kernel": KERNEL_NAMES.get(kernel, str(kernel)),
                    "l2": "flushed between timed steps (256 MiB write); state is re-read from HBM each step",
                    "parallelism": f"shard by realization word x{world}, no collective"},
@@ -521,6 +526,9 @@ def main():
     ap.add_argument("--layout", default="realization", choices=["realization", "replica"],
                     help="multispin coding: bits = realizations (BASELINE configs) or the paper's own bits = temperature "
                          "replicas with one random number per replica (SURVEY 8(f3), ea_set_layout)")
+    ap.add_argument("--swap-mode", default="permute", choices=["permute", "move"],
+                    help="an accepted swap exchanges temperature indices (BASELINE configs) or moves the two lattices "
+                         "(SURVEY 8(f3), ea_set_swap_mode)")
     ap.add_argument("--no-per-config", dest="per_config", action="store_false",
                     help="skip the per_config block (ps per attempt of the other BASELINE configs)")
     ap.add_argument("--ref-cores", type=int, default=0, help="--impl reference: processes to use (default: all cores)")

@@ -290,7 +290,9 @@ int ea_get_layout(ea_handle *h);
  * is the oracle's swap mode 1 (R26).  Allowed only while the permutation is the identity
  * (before the first swap round, or after ea_set_state with identity temp_of_slot) and in the
  * REALIZATION_BITS layout: else EA_ERR_UNSUPPORTED and nothing changes.  ea_get_round_trips counts
- * movements of temperature indices and therefore stays at zero in MOVE mode. */
+ * movements of temperature indices and therefore stays at zero in MOVE mode.  The resident kernels
+ * exchange inside shared memory (one launch per ea_sweep, as in PERMUTE mode); the other kernels are
+ * launched once per swap round, followed by an exchange kernel. */
 #define EA_SWAP_PERMUTE 0
 #define EA_SWAP_MOVE 1
 int ea_set_swap_mode(ea_handle *h, int mode);

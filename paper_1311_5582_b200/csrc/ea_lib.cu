@@ -895,7 +895,7 @@ size_t resident_smem(const ea_handle *h, int S)
     const size_t nb = f ? 2 * (size_t)h->KF.n_bucket : (size_t)h->K.n_bucket;
     return 16 * nb + 4 * (size_t)S * N + 16 * (size_t)S * MTS +
            4 * ((size_t)S * LTS + NC * LTS + MTS + (size_t)S * 32 + 4 * nT) +
-           2 * (2 * nT * 32) + 64 * nT + 16;
+           2 * (2 * nT * 32) + 64 * nT + 4 * nT + 16;
 }
 
 ResPlan plan_resident(const ea_handle *h)
@@ -998,6 +998,7 @@ static int sweep_resident(ea_handle *h, int64_t n_sweeps, int swap_interval)
         cudaError_t e = cudaErrorInvalidValue;
         const bool fast = h->fast_rank;
         A.NQP = pl.NQP; A.G = pl.G; A.any_off = (int)pl.any_off;
+        A.swap_move = h->swap_mode == EA_SWAP_MOVE;
         if (pl.any) e = launch_resident_any(h, A, pl, fast);
         else if (h->L == 16) e = launch_resident_t<16, 1>(h, A, pl, fast);
         else if (pl.G == 8) e = launch_resident_t<8, 8>(h, A, pl, fast);
@@ -1382,6 +1383,8 @@ extern "C" int ea_sweep(ea_handle *h, int64_t n_sweeps, int swap_interval)
     if (h->g + (uint64_t)n_sweeps > 0xFFFFFFFFull) return fail(h, EA_ERR_RANGE, "ea_sweep: sweep counter would pass 2^32-1");
     if (n_sweeps == 0) return EA_OK;
     if (h->poisoned) return fail(h, EA_ERR_CUDA, "ea_sweep: an earlier call failed between word groups; restore the state with ea_set_state");
+    if (h->swap_mode == EA_SWAP_MOVE && swap_interval > 0 && pick_kernel(h) == EA_KERNEL_RESIDENT)
+        return sweep_resident(h, n_sweeps, swap_interval);      // the resident kernels exchange in shared memory
     if (h->swap_mode == EA_SWAP_MOVE && swap_interval > 0) {
         // sweeps up to the next swap point on the selected kernel (no swap inside), then the exchange
         while (n_sweeps > 0) {

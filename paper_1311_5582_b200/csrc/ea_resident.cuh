@@ -41,6 +41,7 @@ struct ResArgs {
     int swap_win;             // swap thresholds for m in [-swap_win, -1] are staged in smem
     int NQP, G;               // k_resident_any (ea_small.cuh): quads per parity padded to whole warps, slot groups
     int any_off;              // ... byte offset (16 B aligned) of its coupling copy and neighbour table in smem
+    int swap_move;            // != 0: an accepted swap exchanges the two lattices (EA_SWAP_MOVE), tau stays the identity
 };
 
 // Mask table of one slot from its rank masks (one warp): row n = { lt[n4], lt[n5], lt[n6], 0 },
@@ -733,6 +734,7 @@ __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs
     int16_t *Eall = (int16_t *)(swwin + nT * SW);                    // [2][nT][32], by swap-round parity
     uint8_t *tau8 = (uint8_t *)(Eall + 2 * nT * 32);                 // [32][nT]
     uint8_t *sig8 = tau8 + 32 * nT;                                  // [32][nT]
+    uint32_t *mvmask = reinterpret_cast<uint32_t *>(sig8 + 32 * nT);   // [nT] moving swaps: who exchanges in pair t
 
     // ---- load state: lattices of my slots, tables, permutation of my 32 realizations
     {   // lattices: eight independent 128-bit loads in flight per thread before the first store
@@ -917,7 +919,18 @@ __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs
             else if (m >= lo + cnt) acc = (kinds >> 1) & 1;
             else if (m >= -SW && m < 0) acc = vx <= swwin[t * SW + m + SW];
             else acc = vx <= P.swp_val[swm[4 * t + 2] + (m - lo)];
-            if (acc) {
+            if (A.swap_move) {
+                // data-moving swap (ea_set_swap_mode, R26): slots keep their temperatures
+                // (sa = t, sb = t + 1 for ever), the accepting realizations exchange their lattices
+                // below and their energies here
+                const uint32_t mk = __ballot_sync(0xFFFFFFFFu, acc);
+                if (acc) {
+                    const int16_t x = Ebuf[sa * 32 + lane];
+                    Ebuf[sa * 32 + lane] = Ebuf[sb * 32 + lane];
+                    Ebuf[sb * 32 + lane] = x;
+                }
+                if (lane == 0) mvmask[t] = mk;
+            } else if (acc) {
                 sg_[t] = (uint8_t)sb; sg_[t + 1] = (uint8_t)sa;
                 ta_[sa] = (uint8_t)(t + 1); ta_[sb] = (uint8_t)t;
                 // rank masks: lt[slot][n] bit r = (pos_r >= n).  The position of a goes from p to p + 1
@@ -932,9 +945,33 @@ __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs
         ++nswap;
         __syncthreads();
         RES_STAMP(3);
-        for (int kl = warp; kl < nk; kl += nwarp)     // mask tables of my slots from their rank masks
-            (NC == 4 ? build_mt4 : build_mt)(mt + (size_t)kl * MTS, lt + kl * LTS, trip, nT, lane);
-        __syncthreads();
+        if (A.swap_move) {
+            // pairs (t, t + 1) of this round whose lower slot is mine: x = (a ^ b) & mask, a ^= x, b ^= x on
+            // every word of the two lattices; the upper slot may be the first one of the next block
+            // of the cluster (distributed shared memory), which does not touch it meanwhile
+            const int par = (int)((nswap - 1u) & 1u);
+            for (int kl = 0; kl < nk; ++kl) {
+                const int t = k0 + kl;
+                if ((t & 1) != par || t + 1 >= nT) continue;
+                const uint32_t mk = mvmask[t];
+                if (mk == 0u) continue;
+                uint4 *pa = reinterpret_cast<uint4 *>(sp + (size_t)kl * N);
+                uint4 *pb = kl + 1 < nk ? reinterpret_cast<uint4 *>(sp + (size_t)(kl + 1) * N)
+                                        : reinterpret_cast<uint4 *>(cl.map_shared_rank(sp, rank + 1));
+                for (int i = tid; i < N / 4; i += NT) {
+                    uint4 a = pa[i], b = pb[i];
+                    const uint4 x = make_uint4((a.x ^ b.x) & mk, (a.y ^ b.y) & mk, (a.z ^ b.z) & mk, (a.w ^ b.w) & mk);
+                    a.x ^= x.x; a.y ^= x.y; a.z ^= x.z; a.w ^= x.w;
+                    b.x ^= x.x; b.y ^= x.y; b.z ^= x.z; b.w ^= x.w;
+                    pa[i] = a; pb[i] = b;
+                }
+            }
+            if (C > 1) cl.sync(); else __syncthreads();
+        } else {
+            for (int kl = warp; kl < nk; kl += nwarp)     // mask tables of my slots from their rank masks
+                (NC == 4 ? build_mt4 : build_mt)(mt + (size_t)kl * MTS, lt + kl * LTS, trip, nT, lane);
+            __syncthreads();
+        }
         RES_STAMP(4);
     }
     // the energies written last are in the buffer selected by the final nswap parity... the
