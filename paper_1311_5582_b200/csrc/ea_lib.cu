@@ -937,6 +937,8 @@ template <int L, int G>
 cudaError_t launch_resident_t(const ea_handle *h, const ea::ResArgs &A, const ResPlan &pl, bool fast)
 {
     auto kern = h->field != 0 ? ea::k_resident<L, G, true, 4> : fast ? ea::k_resident<L, G, true> : ea::k_resident<L, G, false>;
+    if (h->swap_mode == EA_SWAP_MOVE && (h->field != 0 || fast))     // moving swaps inside the kernel: FAST variants only
+        kern = h->field != 0 ? ea::k_resident<L, G, true, 4, true> : ea::k_resident<L, G, true, 3, true>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem);
     if (e != cudaSuccess) return e;
     cudaLaunchConfig_t cfg{};
@@ -956,6 +958,8 @@ cudaError_t launch_resident_t(const ea_handle *h, const ea::ResArgs &A, const Re
 cudaError_t launch_resident_any(const ea_handle *h, const ea::ResArgs &A, const ResPlan &pl, bool fast)
 {
     auto kern = h->field != 0 ? ea::k_resident_any<true, 4> : fast ? ea::k_resident_any<true> : ea::k_resident_any<false>;
+    if (h->swap_mode == EA_SWAP_MOVE && (h->field != 0 || fast))
+        kern = h->field != 0 ? ea::k_resident_any<true, 4, true> : ea::k_resident_any<true, 3, true>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pl.smem);
     if (e != cudaSuccess) return e;
     cudaLaunchConfig_t cfg{};
@@ -998,7 +1002,6 @@ static int sweep_resident(ea_handle *h, int64_t n_sweeps, int swap_interval)
         cudaError_t e = cudaErrorInvalidValue;
         const bool fast = h->fast_rank;
         A.NQP = pl.NQP; A.G = pl.G; A.any_off = (int)pl.any_off;
-        A.swap_move = h->swap_mode == EA_SWAP_MOVE;
         if (pl.any) e = launch_resident_any(h, A, pl, fast);
         else if (h->L == 16) e = launch_resident_t<16, 1>(h, A, pl, fast);
         else if (pl.G == 8) e = launch_resident_t<8, 8>(h, A, pl, fast);
@@ -1383,7 +1386,7 @@ extern "C" int ea_sweep(ea_handle *h, int64_t n_sweeps, int swap_interval)
     if (h->g + (uint64_t)n_sweeps > 0xFFFFFFFFull) return fail(h, EA_ERR_RANGE, "ea_sweep: sweep counter would pass 2^32-1");
     if (n_sweeps == 0) return EA_OK;
     if (h->poisoned) return fail(h, EA_ERR_CUDA, "ea_sweep: an earlier call failed between word groups; restore the state with ea_set_state");
-    if (h->swap_mode == EA_SWAP_MOVE && swap_interval > 0 && pick_kernel(h) == EA_KERNEL_RESIDENT)
+    if (h->swap_mode == EA_SWAP_MOVE && swap_interval > 0 && pick_kernel(h) == EA_KERNEL_RESIDENT && (h->field != 0 || h->fast_rank))
         return sweep_resident(h, n_sweeps, swap_interval);      // the resident kernels exchange in shared memory
     if (h->swap_mode == EA_SWAP_MOVE && swap_interval > 0) {
         // sweeps up to the next swap point on the selected kernel (no swap inside), then the exchange

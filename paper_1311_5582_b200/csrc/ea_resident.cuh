@@ -41,7 +41,6 @@ struct ResArgs {
     int swap_win;             // swap thresholds for m in [-swap_win, -1] are staged in smem
     int NQP, G;               // k_resident_any (ea_small.cuh): quads per parity padded to whole warps, slot groups
     int any_off;              // ... byte offset (16 B aligned) of its coupling copy and neighbour table in smem
-    int swap_move;            // != 0: an accepted swap exchanges the two lattices (EA_SWAP_MOVE), tau stays the identity
 };
 
 // Mask table of one slot from its rank masks (one warp): row n = { lt[n4], lt[n5], lt[n6], 0 },
@@ -693,7 +692,7 @@ __device__ unsigned long long g_res_trace[8];
 #define RES_STAMP(i) do { } while (0)
 #endif
 
-template <int L, int G, bool FAST, int NC = 3>
+template <int L, int G, bool FAST, int NC = 3, bool MOVE = false>
 __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs A)
 {
 #ifdef EA_TRACE
@@ -919,7 +918,7 @@ __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs
             else if (m >= lo + cnt) acc = (kinds >> 1) & 1;
             else if (m >= -SW && m < 0) acc = vx <= swwin[t * SW + m + SW];
             else acc = vx <= P.swp_val[swm[4 * t + 2] + (m - lo)];
-            if (A.swap_move) {
+            if (MOVE) {
                 // data-moving swap (ea_set_swap_mode, R26): slots keep their temperatures
                 // (sa = t, sb = t + 1 for ever), the accepting realizations exchange their lattices
                 // below and their energies here
@@ -945,7 +944,7 @@ __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs
         ++nswap;
         __syncthreads();
         RES_STAMP(3);
-        if (A.swap_move) {
+        if (MOVE) {
             // pairs (t, t + 1) of this round whose lower slot is mine: x = (a ^ b) & mask, a ^= x, b ^= x on
             // every word of the two lattices; the upper slot may be the first one of the next block
             // of the cluster (distributed shared memory), which does not touch it meanwhile

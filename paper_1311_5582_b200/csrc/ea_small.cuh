@@ -59,7 +59,7 @@ __device__ __forceinline__ void update_site_any(uint32_t *sp, const uint32_t *js
     if (ENERGY) fin = planes_after(pl, acc);
 }
 
-template <bool FAST, int NC = 3>
+template <bool FAST, int NC = 3, bool MOVE = false>
 __global__ void __launch_bounds__(1024, 1) k_resident_any(const ResArgs A)
 {
     const int L = A.P.L, Lh = A.P.Lh, N = A.P.N, Nh = A.P.Nh, NSP = A.NQP, G = A.G, NT = NSP * G;
@@ -265,7 +265,7 @@ __global__ void __launch_bounds__(1024, 1) k_resident_any(const ResArgs A)
             else if (m >= lo + cnt) acc = (kinds >> 1) & 1;
             else if (m >= -SW && m < 0) acc = vx <= swwin[t * SW + m + SW];
             else acc = vx <= P.swp_val[swm[4 * t + 2] + (m - lo)];
-            if (A.swap_move) {
+            if (MOVE) {
                 // data-moving swap (ea_set_swap_mode, R26): slots keep their temperatures
                 // (sa = t, sb = t + 1 for ever), the accepting realizations exchange their lattices
                 // below and their energies here
@@ -290,7 +290,7 @@ __global__ void __launch_bounds__(1024, 1) k_resident_any(const ResArgs A)
         }
         ++nswap;
         __syncthreads();
-        if (A.swap_move) {
+        if (MOVE) {
             // pairs (t, t + 1) of this round whose lower slot is mine: x = (a ^ b) & mask, a ^= x, b ^= x on
             // every word of the two lattices; the upper slot may be the first one of the next block
             // of the cluster (distributed shared memory), which does not touch it meanwhile
