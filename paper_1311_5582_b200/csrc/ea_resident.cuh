@@ -169,12 +169,15 @@ __device__ __forceinline__ void quad_sum(const Planes (&f)[4], uint32_t (&o)[5])
 }
 
 // n_sat of a site AFTER its update: a flipped spin turns every bond around it, n -> 6 - n.
+// Three LOP3 written out (ptxas, given the plain expressions, spent six per site here):
+// 6 - n >= 4 iff n <= 2, and n >= 3 = b2 | (b1 & b0).
 __device__ __forceinline__ Planes planes_after(const Planes &p, uint32_t acc)
 {
     Planes f;
     f.b0 = p.b0;
-    f.b1 = mux(p.b1, ~(p.b1 ^ p.b0), acc);
-    f.b2 = mux(p.b2, ~p.b2 & ~(p.b1 & p.b0), acc);
+    f.b1 = lop3<0xD2>(p.b1, p.b0, acc);                     // acc ? ~(b1 ^ b0) : b1
+    const uint32_t ge3 = lop3<0xF8>(p.b2, p.b1, p.b0);      // b2 | (b1 & b0)
+    f.b2 = lop3<0x3A>(acc, ge3, p.b2);                      // acc ? ~ge3 : b2
     return f;
 }
 
