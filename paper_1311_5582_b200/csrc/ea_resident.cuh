@@ -669,20 +669,21 @@ __device__ __forceinline__ void warp_sum4_t(uint32_t (&en)[4][NP], int lane, uin
     }
 }
 
-// add_counts for NPL planes
+// Lane i (0..7) of a slot's eight lanes adds the counts of realizations i, i + 8, i + 16, i + 24 (all eight
+// lanes hold the same NPL-plane totals) to the slot's row: the four bits of a plane are gathered as
+// four bytes, planes 0..7 weighted into one word (a byte holds up to 255) and the rest into a second.
 template <int NPL>
 __device__ __forceinline__ void add_counts_t(const uint32_t (&tot)[NPL], int i, int *acc_row)
 {
+    static_assert(NPL <= 16, "two byte-packed accumulators");
     uint32_t lo = 0, hi = 0;
 #pragma unroll
-    for (int j = 0; j < NPL; ++j) {
-        lo += ((tot[j] >> i) & 0x00010001u) * (1u << j);
-        hi += ((tot[j] >> (i + 8)) & 0x00010001u) * (1u << j);
-    }
-    atomicAdd(acc_row + i, (int)(lo & 0xFFFFu));
-    atomicAdd(acc_row + i + 16, (int)(lo >> 16));
-    atomicAdd(acc_row + i + 8, (int)(hi & 0xFFFFu));
-    atomicAdd(acc_row + i + 24, (int)(hi >> 16));
+    for (int j = 0; j < (NPL < 8 ? NPL : 8); ++j) lo += ((tot[j] >> i) & 0x01010101u) * (1u << j);
+#pragma unroll
+    for (int j = 8; j < NPL; ++j) hi += ((tot[j] >> i) & 0x01010101u) * (1u << (j - 8));
+#pragma unroll
+    for (int b = 0; b < 4; ++b)
+        atomicAdd(acc_row + i + 8 * b, (int)(((lo >> (8 * b)) & 0xFFu) + (((hi >> (8 * b)) & 0xFFu) << 8)));
 }
 
 // Phase clocks of k_resident, only in the -DEA_TRACE build of examples/resident_phases.py (the product
