@@ -321,6 +321,13 @@ struct ResGeom {
     static_assert(Lh % 4 == 0 && (QR & (QR - 1)) == 0 && QR <= 8, "needs L in {8,16,32,64}");
 };
 
+__device__ __forceinline__ uint4 lds128(uint32_t addr)
+{
+    uint4 v;
+    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr) : "memory");
+    return v;
+}
+
 // New spin words of the four sites of quad q (parity p) of one slot's lattice `sp` (smem,
 // [2][Nh]); nothing is stored.  EXACT = false: ranks from the bucket table; *flag collects
 // bit 31 of the entries (set: the caller must redo the quad with EXACT = true).
@@ -334,12 +341,23 @@ __device__ __forceinline__ uint4 quad_core(const char *self_q, const char *oth_b
     using Gm = ResGeom<L>;
     // self_q: address of the quad's own four words; oth_b: base of the other parity's words;
     // ov, oyp..ozm: byte offsets in oth_b of the index-aligned quad and of the +-y / +-z quads
-    const uint4 me = *reinterpret_cast<const uint4 *>(self_q);
-    const uint4 v = *reinterpret_cast<const uint4 *>(oth_b + ov);
-    const uint4 yp = *reinterpret_cast<const uint4 *>(oth_b + oyp);
-    const uint4 ym = *reinterpret_cast<const uint4 *>(oth_b + oym);
-    const uint4 zp = *reinterpret_cast<const uint4 *>(oth_b + ozp);
-    const uint4 zm = *reinterpret_cast<const uint4 *>(oth_b + ozm);
+    uint4 me, v, yp, ym, zp, zm;
+    if (UNIS && !EXACT) {
+        // resident kernel: the lattice is this block's own shared memory; shared-state-space loads at
+        // (uniform slot base) + (per-thread offset) let ptxas use the [R + UR] form instead of adding
+        // the cluster window base and the slot base to every one of the six addresses
+        const uint32_t ob = (uint32_t)__cvta_generic_to_shared(oth_b);
+        me = lds128((uint32_t)__cvta_generic_to_shared(self_q));
+        v = lds128(ob + ov); yp = lds128(ob + oyp); ym = lds128(ob + oym);
+        zp = lds128(ob + ozp); zm = lds128(ob + ozm);
+    } else {
+        me = *reinterpret_cast<const uint4 *>(self_q);
+        v = *reinterpret_cast<const uint4 *>(oth_b + ov);
+        yp = *reinterpret_cast<const uint4 *>(oth_b + oyp);
+        ym = *reinterpret_cast<const uint4 *>(oth_b + oym);
+        zp = *reinterpret_cast<const uint4 *>(oth_b + ozp);
+        zm = *reinterpret_cast<const uint4 *>(oth_b + ozm);
+    }
     const uint32_t m[4] = {me.x, me.y, me.z, me.w};
     const uint32_t jb[4] = {J.jb.x, J.jb.y, J.jb.z, J.jb.w};
     // x neighbour that is not index-aligned: x+1 if s, x-1 otherwise; the word beyond the quad
