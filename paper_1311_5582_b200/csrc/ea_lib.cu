@@ -895,7 +895,7 @@ size_t resident_smem(const ea_handle *h, int S)
     const size_t nb = f ? 2 * (size_t)h->KF.n_bucket : (size_t)h->K.n_bucket;
     return 16 * nb + 4 * (size_t)S * N + 16 * (size_t)S * MTS +
            4 * ((size_t)S * LTS + NC * LTS + MTS + (size_t)S * 32 + 4 * nT) +
-           2 * (2 * nT * 32) + 64 * nT + 4 * nT + 16;
+           2 * (2 * nT * 32) + 64 * nT + 4 * nT + 48;
 }
 
 ResPlan plan_resident(const ea_handle *h)

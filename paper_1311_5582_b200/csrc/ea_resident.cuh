@@ -704,6 +704,52 @@ __device__ __forceinline__ void add_counts_t(const uint32_t (&tot)[NPL], int i, 
         atomicAdd(acc_row + i + 8 * b, (int)(((lo >> (8 * b)) & 0xFFu) + (((hi >> (8 * b)) & 0xFFu) << 8)));
 }
 
+// ------------------------------------------------------------------ mbarrier / TMA bulk copy
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.global;" ::: "memory"); }
+// Remote 16-byte store into the shared memory of block `rank` of the cluster that also counts its
+// bytes on that block's mbarrier (st.async): the receiver waits on its own barrier, no cluster-wide
+// barrier and no fence on the sender's side.
+__device__ __forceinline__ void st_async_v4(void *local_dst, uint4 v, uint64_t *local_bar, int rank)
+{
+    uint32_t ra, rb;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(ra) : "r"(smem_u32(local_dst)), "r"(rank));
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(rb) : "r"(smem_u32(local_bar)), "r"(rank));
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v4.b32 [%0], {%1, %2, %3, %4}, [%5];"
+                 ::"r"(ra), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w), "r"(rb) : "memory");
+}
+
 // Phase clocks of k_resident, only in the -DEA_TRACE build of examples/resident_phases.py (the product
 // library has none): thread 0 of block 0 adds the SM cycles between consecutive stamps of a sweep to
 // g_res_trace[phase]; ea_debug_res_trace (ea_lib.cu, same build only) reads and clears the sums.
@@ -752,10 +798,17 @@ __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs
     int32_t *Eacc = (int32_t *)(trip + MTS);                         // [S][32] satisfied-bond counts
     int32_t *swm = Eacc + S * 32;                                    // [nT][4]: lo, cnt, off, kinds
     uint32_t *swwin = (uint32_t *)(swm + 4 * nT);                    // [nT][SW] thresholds - 1
-    int16_t *Eall = (int16_t *)(swwin + nT * SW);                    // [2][nT][32], by swap-round parity
+    int16_t *Eall = (int16_t *)((reinterpret_cast<uintptr_t>(swwin + nT * SW) + 15) & ~(uintptr_t)15);   // [2][nT][32], by swap-round parity; 16 B aligned (st.async.v4)
     uint8_t *tau8 = (uint8_t *)(Eall + 2 * nT * 32);                 // [32][nT]
     uint8_t *sig8 = tau8 + 32 * nT;                                  // [32][nT]
     uint32_t *mvmask = reinterpret_cast<uint32_t *>(sig8 + 32 * nT);   // [nT] moving swaps: who exchanges in pair t
+    // the other blocks' energies of a swap round arrive by st.async and are counted here
+    uint64_t *ebar = reinterpret_cast<uint64_t *>((reinterpret_cast<uintptr_t>(mvmask + nT) + 7) & ~(uintptr_t)7);
+    if (tid == 0) {
+        mbar_init(ebar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    uint32_t ephase = 0;
 
     // ---- load state: lattices of my slots, tables, permutation of my 32 realizations
     {   // lattices: eight independent 128-bit loads in flight per thread before the first store
@@ -900,15 +953,23 @@ __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs
         // ---- energies of my slots: E = 3N - 2 (satisfied bonds); pushed into every block of
         //      the cluster (distributed shared memory), buffer chosen by the swap-round parity
         int16_t *Ebuf = Eall + (nswap & 1u) * nT * 32;
-        for (int a = tid; a < nk * 32; a += NT) {
-            const int e = (3 + (NC == 4 ? abs(P.h) : 0)) * N - 2 * Eacc[a];
-            Eacc[a] = 0;
-            const int dst = k0 * 32 + a;
-            if (C > 1) {
-                for (int rr = 0; rr < C; ++rr) cl.map_shared_rank(Ebuf, rr)[dst] = (int16_t)e;
-            } else {
-                Ebuf[dst] = (int16_t)e;
-            }
+        if (C > 1 && swap_now && tid == 0) mbar_expect_tx(ebar, (uint32_t)(nT - nk) * 64u);   // 32 x int16 per foreign slot
+        for (int a = NT - 1 - tid; a < nk * 4; a += NT) {    // eight energies = 16 bytes per thread; the last warps do it: with
+                                                             // n_T / 2 < NT / 32 they have no pair to prepare below
+            const int E0 = (3 + (NC == 4 ? abs(P.h) : 0)) * N;
+            int *src = Eacc + 8 * a;
+            const int4 c0 = make_int4(src[0], src[1], src[2], src[3]), c1 = make_int4(src[4], src[5], src[6], src[7]);
+#pragma unroll
+            for (int i = 0; i < 8; ++i) src[i] = 0;
+            const uint32_t e0 = (uint32_t)(E0 - 2 * c0.x) & 0xFFFFu, e1 = (uint32_t)(E0 - 2 * c0.y), e2 = (uint32_t)(E0 - 2 * c0.z) & 0xFFFFu,
+                           e3 = (uint32_t)(E0 - 2 * c0.w), e4 = (uint32_t)(E0 - 2 * c1.x) & 0xFFFFu, e5 = (uint32_t)(E0 - 2 * c1.y),
+                           e6 = (uint32_t)(E0 - 2 * c1.z) & 0xFFFFu, e7 = (uint32_t)(E0 - 2 * c1.w);
+            const uint4 v = make_uint4(e0 | (e1 << 16), e2 | (e3 << 16), e4 | (e5 << 16), e6 | (e7 << 16));
+            uint4 *dst = reinterpret_cast<uint4 *>(Ebuf + k0 * 32) + a;
+            *dst = v;
+            if (C > 1 && swap_now)                            // (the last sweep of a call without a swap: own slots only)
+                for (int rr = 0; rr < C; ++rr)
+                    if (rr != rank) st_async_v4(dst, v, ebar, rr);
         }
         if (!swap_now) { __syncthreads(); continue; }
         // ---- swap round: warp per temperature pair, lane = realization.  Every block of the
@@ -917,14 +978,14 @@ __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs
         const int warp = tid >> 5, nwarp = NT >> 5;
         const int t0 = (int)(nswap & 1u) + 2 * warp;
         uint8_t *sg_ = sig8 + lane * nT, *ta_ = tau8 + lane * nT;
-        if (C > 1) cluster_arrive();
         int sa0 = 0, sb0 = 0;
         uint32_t v0 = 0;
         if (t0 + 1 < nT) {
             sa0 = sg_[t0]; sb0 = sg_[t0 + 1];
             v0 = philox_rk(g, (uint32_t)t0, P.r0 + (uint32_t)(32 * w + lane), 2u << 16, A.rk).x;
         }
-        if (C > 1) cluster_wait(); else __syncthreads();
+        __syncthreads();                                      // my own energies are in Ebuf
+        if (C > 1) { mbar_wait(ebar, ephase); ephase ^= 1u; }   // ... and those of the other blocks
         RES_STAMP(2);
         for (int t = t0; t + 1 < nT; t += 2 * nwarp) {
             int sa = sa0, sb = sb0;
