@@ -953,8 +953,24 @@ __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs
         // ---- energies of my slots: E = 3N - 2 (satisfied bonds); pushed into every block of
         //      the cluster (distributed shared memory), buffer chosen by the swap-round parity
         int16_t *Ebuf = Eall + (nswap & 1u) * nT * 32;
-        if (C > 1 && swap_now && tid == 0) mbar_expect_tx(ebar, (uint32_t)(nT - nk) * 64u);   // 32 x int16 per foreign slot
-        for (int a = NT - 1 - tid; a < nk * 4; a += NT) {    // eight energies = 16 bytes per thread; the last warps do it: with
+        // L = 16 (few large blocks per cluster): st.async + the receiver's mbarrier; L = 8 (clusters of up
+        // to eight blocks of a few warps): plain DSMEM stores + barrier.cluster, which measured faster there
+        // (config 2: 2.77 against 2.85 us per sweep)
+        constexpr bool ASYNC = L == 16;
+        if (!ASYNC) {
+            for (int a = tid; a < nk * 32; a += NT) {
+                const int e = (3 + (NC == 4 ? abs(P.h) : 0)) * N - 2 * Eacc[a];
+                Eacc[a] = 0;
+                const int dst = k0 * 32 + a;
+                if (C > 1) {
+                    for (int rr = 0; rr < C; ++rr) cl.map_shared_rank(Ebuf, rr)[dst] = (int16_t)e;
+                } else {
+                    Ebuf[dst] = (int16_t)e;
+                }
+            }
+        }
+        if (ASYNC && C > 1 && swap_now && tid == 0) mbar_expect_tx(ebar, (uint32_t)(nT - nk) * 64u);   // 32 x int16 per foreign slot
+        for (int a = NT - 1 - tid; ASYNC && a < nk * 4; a += NT) {    // eight energies = 16 bytes per thread; the last warps do it: with
                                                              // n_T / 2 < NT / 32 they have no pair to prepare below
             const int E0 = (3 + (NC == 4 ? abs(P.h) : 0)) * N;
             int *src = Eacc + 8 * a;
@@ -984,8 +1000,14 @@ __global__ void __launch_bounds__(ResGeom<L>::NQ *G, 1) k_resident(const ResArgs
             sa0 = sg_[t0]; sb0 = sg_[t0 + 1];
             v0 = philox_rk(g, (uint32_t)t0, P.r0 + (uint32_t)(32 * w + lane), 2u << 16, A.rk).x;
         }
-        __syncthreads();                                      // my own energies are in Ebuf
-        if (C > 1) { mbar_wait(ebar, ephase); ephase ^= 1u; }   // ... and those of the other blocks
+        if (ASYNC) {
+            __syncthreads();                                      // my own energies are in Ebuf
+            if (C > 1) { mbar_wait(ebar, ephase); ephase ^= 1u; }   // ... and those of the other blocks
+        } else if (C > 1) {
+            cluster_arrive(); cluster_wait();
+        } else {
+            __syncthreads();
+        }
         RES_STAMP(2);
         for (int t = t0; t + 1 < nT; t += 2 * nwarp) {
             int sa = sa0, sb = sb0;
