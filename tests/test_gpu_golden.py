@@ -5,8 +5,8 @@ oracle has stored, and compared with the digests it wrote ahead of time
 100, 200, 500, 1000, 2000, 5000, 10^4, 2 10^4, ..., 10^5.  A digest covers the word's packed spins,
 temperature permutation and integer energies, so equality is bit-exactness.  Coverage (recorded in
 each JSON file, stated in DESIGN.md section 7): configs 1-3 every word to the config's full length;
-config 4 words 0, 5, 20, 31, 40 and 63 to the full 10^5 sweeps; config 5 words 3
-and 6 to the full 10^4 sweeps.  test_full_length_is_covered fails if a config's
+config 4 words 0, 5, 20, 31, 40 and 63 to the full 10^5 sweeps; config 5 words 0,
+3, 6 and 7 to the full 10^4 sweeps.  test_full_length_is_covered fails if a config's
 longest stored checkpoint is shorter than the config."""
 import glob
 import json
